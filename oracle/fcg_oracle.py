@@ -1,0 +1,395 @@
+"""CPU oracle for FCGRAFT KV-cache grafting.  TEST INFRASTRUCTURE ONLY.
+
+This file is the plain, slow, obviously-correct statement of what the hot path
+computes.  It is imported only by ``tests/``, ``__graft_entry__.smoke()`` and the
+``cpu_baseline`` / ``--impl reference`` legs of ``bench.py``.  The product
+(``paper_2606_13097_b200``) never imports it, and it never imports the product:
+the two share no code, no tables, no helpers.
+
+Everything is numpy, fp64, one rounding (fp64 -> bf16, round-to-nearest-even)
+at the very end of each step that stores bf16.  K/V/q are carried around as
+``uint16`` arrays holding bf16 bit patterns, so "bit-exact" means integer
+equality of those arrays.
+
+What the paper fixes and what it leaves open (``PAPER.md`` = /root/reference/PAPER.md,
+not needed at run time; DESIGN.md "Readings" lists every choice R1..R14):
+
+* segment library  = the KV half of the two-tier code cache H=(I,C), Eq. (2),
+  PAPER.md:66-79: per function a K/V state that can be re-injected "without
+  being tied to fixed prefix positions".
+* cache-stitching  = Eq. (4): cached KV states are
+  "concatenated and injected ... as additional context", each module
+  "preserving its internal token order during composition".
+* cache-patching   = Eq. (6): prefix KV reused, only
+  the middle span recomputed, suffix kept.
+* The paper never says how positions are reconciled; BASELINE.json's north_star
+  fixes it: keys are re-rotated by the integer position delta (RoPE group law),
+  values are untouched (R1).  Pair layout: HF half-split (R2).
+
+Pinned by tests/test_oracle_pins.py (group law, identity, synthetic one-layer
+model, brute-force attention, closed forms, torch SDPA special case ...).  No
+function here is "parity unpinned".
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+
+import numpy as np
+
+# ----------------------------------------------------------------------------
+# status codes (values are part of the C ABI contract in include/fcg.h; the
+# oracle restates them so that plan-rejection behaviour can be compared)
+# ----------------------------------------------------------------------------
+FCG_OK = 0
+FCG_ERR_INVALID_ARG = -1
+FCG_ERR_BAD_SEGMENT = -2
+FCG_ERR_RANGE = -3
+FCG_ERR_OVERLAP = -4
+FCG_ERR_UNFILLED = -5
+FCG_ERR_OUT_OF_PAGES = -6
+FCG_ERR_OUT_OF_ARENA = -7
+FCG_ERR_CUDA = -8
+FCG_ERR_BAD_TASK = -9
+
+
+class OracleError(Exception):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"status {status}: {msg}")
+        self.status = status
+
+
+# ----------------------------------------------------------------------------
+# 1. bf16 <-> fp64                                   (DESIGN R4)
+# ----------------------------------------------------------------------------
+def bf16_to_f64(bits) -> np.ndarray:
+    """bf16 bit patterns (uint16) -> float64, exact (bf16 is a prefix of fp32)."""
+    b = np.ascontiguousarray(bits, dtype=np.uint16)
+    with np.errstate(invalid="ignore"):            # signalling-NaN patterns widen to NaN, quietly
+        return (b.astype(np.uint32) << np.uint32(16)).view(np.float32).astype(np.float64)
+
+
+def f64_to_bf16(x) -> np.ndarray:
+    """float64 -> bf16 bit patterns, ONE direct round-to-nearest-even.
+
+    bf16 has 8 significant bits and fp32's exponent range.  For x in
+    [2^E, 2^(E+1)) with E >= -126 the bf16 grid has spacing q = 2^(E-7); below
+    2^-126 (subnormals) the spacing stays 2^-133.  x/q is exact (power of two),
+    np.rint rounds half to even, so r = rint(x/q)*q is the correctly rounded
+    bf16 value; it is exactly representable in fp32, whose top 16 bits are the
+    answer.  |r| >= 2^128 becomes inf; NaN stays NaN.  Never goes through fp32
+    rounding of the *unrounded* value (no double rounding).
+    """
+    x = np.asarray(x, dtype=np.float64)
+    _, e = np.frexp(x)                     # |x| = m * 2^e, m in [0.5, 1)  =>  floor(log2|x|) = e - 1
+    E = np.maximum(e - 1, -126)
+    q = np.ldexp(1.0, E - 7)
+    with np.errstate(over="ignore", invalid="ignore"):
+        r = np.rint(x / q) * q
+        r32 = r.astype(np.float32)         # exact unless |r| >= 2^128 -> inf (what bf16 RNE overflow gives)
+    return (r32.view(np.uint32) >> np.uint32(16)).astype(np.uint16)
+
+
+# ----------------------------------------------------------------------------
+# 2. RoPE delta rotation                              (DESIGN R1-R4)
+# ----------------------------------------------------------------------------
+def rope_inv_freq(head_dim: int, base: float) -> np.ndarray:
+    """theta_j = base^(-2j/D), j in [0, D/2), fp64 pow."""
+    j = np.arange(head_dim // 2, dtype=np.float64)
+    return np.power(np.float64(base), -2.0 * j / np.float64(head_dim))
+
+
+def rope_rotate_f64(x: np.ndarray, delta, inv_freq: np.ndarray) -> np.ndarray:
+    """Rotate x[..., D] (fp64) by the position delta; result fp64, NOT rounded.
+
+    Half-split pairs (a, b) = (x[j], x[j + D/2]) (HF convention, DESIGN R2):
+        phi_j  = delta * theta_j
+        out[j]       = a cos(phi_j) - b sin(phi_j)
+        out[j + D/2] = b cos(phi_j) + a sin(phi_j)
+    ``delta`` is an integer, or an array broadcastable against x[..., :1]
+    (one delta per row).
+    """
+    x = np.asarray(x, dtype=np.float64)
+    D = x.shape[-1]
+    half = D // 2
+    phi = np.asarray(delta, dtype=np.float64)[..., None] * inv_freq     # scalar delta -> [D/2]; per-row -> [..., D/2]
+    c, s = np.cos(phi), np.sin(phi)
+    a, b = x[..., :half], x[..., half:]
+    out = np.empty_like(x)
+    out[..., :half] = a * c - b * s
+    out[..., half:] = b * c + a * s
+    return out
+
+
+def rope_shift_bf16(k_bits: np.ndarray, delta, inv_freq: np.ndarray) -> np.ndarray:
+    """bf16 keys -> bf16 keys rotated by ``delta``: fp64 arithmetic, one RNE."""
+    return f64_to_bf16(rope_rotate_f64(bf16_to_f64(k_bits), delta, inv_freq))
+
+
+# ----------------------------------------------------------------------------
+# 3. page pool                                         (DESIGN R9)
+# ----------------------------------------------------------------------------
+class PagePool:
+    """Deterministic LIFO page allocator: a fresh pool hands out 0, 1, 2, ...
+
+    ``release`` pushes pages back so that the *next* allocation returns them in
+    the order they are listed (i.e. a released task's pages are re-issued in
+    ascending logical order).
+    """
+
+    def __init__(self, n_pages: int):
+        self.n_pages = int(n_pages)
+        self._stack = list(range(self.n_pages - 1, -1, -1))   # pop() -> 0, 1, 2, ...
+
+    def available(self) -> int:
+        return len(self._stack)
+
+    def allocate(self, n: int) -> list[int]:
+        if n > len(self._stack):
+            raise OracleError(FCG_ERR_OUT_OF_PAGES, f"need {n} pages, {len(self._stack)} free")
+        return [self._stack.pop() for _ in range(n)]
+
+    def release(self, pages: list[int]) -> None:
+        for p in reversed(pages):
+            self._stack.append(p)
+
+
+# ----------------------------------------------------------------------------
+# 4. library / plans / tasks
+# ----------------------------------------------------------------------------
+@dataclass
+class Segment:
+    k: np.ndarray            # [L][Hkv][n][D] uint16 (bf16 bits), owned copy
+    v: np.ndarray
+    n_tokens: int
+    orig_start: int          # position at which token 0's key was RoPE-encoded
+
+
+@dataclass
+class PlanEntry:
+    seg_id: int
+    src_begin: int
+    n_tokens: int
+    dst_offset: int
+
+
+@dataclass
+class Hole:
+    begin: int
+    n_tokens: int
+
+
+@dataclass
+class Plan:
+    task_id: int
+    entries: list
+    holes: list = field(default_factory=list)
+    capacity_tokens: int = 0       # 0 -> max end of entries/holes
+
+
+@dataclass
+class Task:
+    page_table: list          # logical page -> physical page id
+    capacity: int
+    n_tokens: int             # T: max filled-or-declared end
+    filled: np.ndarray        # bool[capacity]
+    k: np.ndarray             # logical cache [L][Hkv][capacity][D] uint16
+    v: np.ndarray
+    deltas: list              # per entry, for inspection
+
+
+class OracleLibrary:
+    """Plain restatement of the library state machine behind the C ABI."""
+
+    def __init__(self, n_layers, n_q_heads, n_kv_heads, head_dim, page_size=16,
+                 rope_mode=1, rope_base=1e4, inv_freq=None, max_segments=1 << 16,
+                 max_tasks=1 << 16, n_pages=1 << 20):
+        if head_dim % 8 or head_dim <= 0 or n_q_heads % n_kv_heads or page_size <= 0:
+            raise OracleError(FCG_ERR_INVALID_ARG, "bad geometry")
+        self.L, self.Hq, self.Hkv, self.D, self.P = n_layers, n_q_heads, n_kv_heads, head_dim, page_size
+        self.G = n_q_heads // n_kv_heads
+        self.rope_mode = rope_mode
+        self.inv_freq = (np.asarray(inv_freq, dtype=np.float64) if inv_freq is not None
+                         else rope_inv_freq(head_dim, rope_base))
+        self.max_segments, self.max_tasks = max_segments, max_tasks
+        self.pool = PagePool(n_pages)
+        self.segments: dict[int, Segment] = {}
+        self.tasks: dict[int, Task] = {}
+        self._next_seg = 0
+
+    # -- S1 ------------------------------------------------------------------
+    def segment_register(self, k_bits, v_bits, orig_start: int) -> int:
+        """Keep the K/V bits, orig_start and n."""
+        k = np.array(k_bits, dtype=np.uint16, copy=True)
+        v = np.array(v_bits, dtype=np.uint16, copy=True)
+        if k.shape != v.shape or k.ndim != 4 or k.shape[0] != self.L or k.shape[1] != self.Hkv \
+                or k.shape[3] != self.D or k.shape[2] <= 0 or orig_start < 0:
+            raise OracleError(FCG_ERR_INVALID_ARG, "segment shape must be [L][Hkv][n][D], n > 0, orig_start >= 0")
+        # lowest free id (ids of released segments are reused, smallest first)
+        sid = 0
+        while sid in self.segments:
+            sid += 1
+        if sid >= self.max_segments:
+            raise OracleError(FCG_ERR_OUT_OF_ARENA, "segment table full")
+        self.segments[sid] = Segment(k, v, k.shape[2], int(orig_start))
+        return sid
+
+    def segment_release(self, seg_id: int) -> None:
+        if seg_id not in self.segments:
+            raise OracleError(FCG_ERR_BAD_SEGMENT, f"unknown segment {seg_id}")
+        del self.segments[seg_id]
+
+    # -- S2 ------------------------------------------------------------------
+    def validate_plan(self, plan: Plan):
+        """Returns (capacity, T, deltas).  Raises OracleError; changes no state.
+
+        Rules (DESIGN R5-R7): 0 <= src_begin, n > 0,
+        src_begin + n <= n_seg, dst_offset >= 0, end <= capacity; entries and
+        holes pairwise disjoint; delta_e = dst_offset - orig_start - src_begin.
+        """
+        if plan.task_id < 0 or plan.task_id >= self.max_tasks:
+            raise OracleError(FCG_ERR_BAD_TASK, "task id out of range")
+        if plan.task_id in self.tasks:
+            raise OracleError(FCG_ERR_BAD_TASK, "task id already live")
+        if len(plan.entries) + len(plan.holes) == 0:
+            raise OracleError(FCG_ERR_INVALID_ARG, "empty plan")
+        spans, deltas = [], []
+        for e in plan.entries:
+            if e.seg_id not in self.segments:
+                raise OracleError(FCG_ERR_BAD_SEGMENT, f"unknown segment {e.seg_id}")
+            seg = self.segments[e.seg_id]
+            if e.n_tokens <= 0 or e.src_begin < 0 or e.src_begin + e.n_tokens > seg.n_tokens or e.dst_offset < 0:
+                raise OracleError(FCG_ERR_RANGE, "entry source/destination range")
+            spans.append((e.dst_offset, e.dst_offset + e.n_tokens))
+            deltas.append(e.dst_offset - seg.orig_start - e.src_begin)
+        for h in plan.holes:
+            if h.n_tokens <= 0 or h.begin < 0:
+                raise OracleError(FCG_ERR_RANGE, "hole range")
+            spans.append((h.begin, h.begin + h.n_tokens))
+        T = max(end for _, end in spans)
+        capacity = plan.capacity_tokens if plan.capacity_tokens > 0 else T
+        if T > capacity:
+            raise OracleError(FCG_ERR_RANGE, "plan exceeds capacity_tokens")
+        srt = sorted(spans)
+        for (b0, e0), (b1, e1) in zip(srt, srt[1:]):
+            if b1 < e0:
+                raise OracleError(FCG_ERR_OVERLAP, "entries/holes overlap")
+        return capacity, T, deltas
+
+    # -- S2 + S3 -------------------------------------------------------------
+    def stitch(self, plans: list) -> None:
+        """Build page tables and gather + RoPE-shift (Eq. 4).
+
+        All plans are validated and all pages reserved before any state
+        changes (allocate-then-commit): a failing batch leaves the library as
+        it was.
+        """
+        checked = []
+        seen = set()
+        need = 0
+        for plan in plans:
+            if plan.task_id in seen:
+                raise OracleError(FCG_ERR_BAD_TASK, "task id repeated in batch")
+            seen.add(plan.task_id)
+            cap, T, deltas = self.validate_plan(plan)
+            n_pg = -(-cap // self.P)
+            need += n_pg
+            checked.append((plan, cap, T, deltas, n_pg))
+        if need > self.pool.available():
+            raise OracleError(FCG_ERR_OUT_OF_PAGES, f"need {need} pages, {self.pool.available()} free")
+        for plan, cap, T, deltas, n_pg in checked:
+            table = self.pool.allocate(n_pg)           # plans in array order, pages in ascending logical order
+            kc = np.zeros((self.L, self.Hkv, cap, self.D), np.uint16)
+            vc = np.zeros_like(kc)
+            filled = np.zeros(cap, bool)
+            for e, delta in zip(plan.entries, deltas):
+                seg = self.segments[e.seg_id]
+                src = slice(e.src_begin, e.src_begin + e.n_tokens)
+                dst = slice(e.dst_offset, e.dst_offset + e.n_tokens)
+                if self.rope_mode == 0:
+                    kc[:, :, dst] = seg.k[:, :, src]                       # pure gather
+                else:
+                    kc[:, :, dst] = rope_shift_bf16(seg.k[:, :, src], delta, self.inv_freq)
+                vc[:, :, dst] = seg.v[:, :, src]                           # V: bit copy
+                filled[dst] = True
+            self.tasks[plan.task_id] = Task(table, cap, T, filled, kc, vc, deltas)
+
+    # -- S4 + S5/S6 ----------------------------------------------------------
+    def check_patch(self, task_id: int, positions) -> None:
+        if task_id not in self.tasks:
+            raise OracleError(FCG_ERR_BAD_TASK, f"unknown task {task_id}")
+        t = self.tasks[task_id]
+        pos = np.asarray(positions, dtype=np.int64)
+        if pos.ndim != 1 or pos.size == 0:
+            raise OracleError(FCG_ERR_INVALID_ARG, "positions must be a non-empty 1-d array")
+        if np.any(np.diff(pos) <= 0):
+            raise OracleError(FCG_ERR_INVALID_ARG, "positions must be strictly increasing")
+        if pos[0] < 0 or pos[-1] >= t.capacity:
+            raise OracleError(FCG_ERR_RANGE, "position outside task capacity")
+        f = t.filled.copy()
+        f[pos] = True
+        if not np.all(f[: pos[-1] + 1]):
+            raise OracleError(FCG_ERR_UNFILLED, "a patch query would attend over an unfilled position")
+
+    def patch(self, task_id: int, layer_begin: int, q_bits, k_bits, v_bits, positions) -> np.ndarray:
+        """Scatter then causal patch attention (Eq. 6).
+
+        q_bits [nl][n][Hq][D], k_bits/v_bits [nl][n][Hkv][D] (uint16 bf16 bits,
+        already position-encoded by the caller, DESIGN R13).  Returns the
+        attention output as float64 [nl][n][Hq][D], NOT rounded.
+        Query i at position p_i sees cache positions x <= p_i (DESIGN R12).
+        """
+        self.check_patch(task_id, positions)
+        t = self.tasks[task_id]
+        pos = np.asarray(positions, dtype=np.int64)
+        q_bits = np.asarray(q_bits, np.uint16)
+        k_bits = np.asarray(k_bits, np.uint16)
+        v_bits = np.asarray(v_bits, np.uint16)
+        nl, n = q_bits.shape[0], pos.size
+        if layer_begin < 0 or nl <= 0 or layer_begin + nl > self.L \
+                or q_bits.shape != (nl, n, self.Hq, self.D) or k_bits.shape != (nl, n, self.Hkv, self.D) \
+                or v_bits.shape != k_bits.shape:
+            raise OracleError(FCG_ERR_INVALID_ARG, "patch tensor shapes / layer range")
+        out = np.empty((nl, n, self.Hq, self.D), np.float64)
+        for li in range(nl):
+            layer = layer_begin + li
+            # S4: scatter (bit copy) -- happens before this layer's attention
+            t.k[layer][:, pos, :] = np.transpose(k_bits[li], (1, 0, 2))
+            t.v[layer][:, pos, :] = np.transpose(v_bits[li], (1, 0, 2))
+            out[li] = patch_attention(t.k[layer], t.v[layer], q_bits[li], pos, self.G)
+        t.filled[pos] = True
+        t.n_tokens = max(t.n_tokens, int(pos[-1]) + 1)
+        return out
+
+    def task_release(self, task_id: int) -> None:
+        if task_id not in self.tasks:
+            raise OracleError(FCG_ERR_BAD_TASK, f"unknown task {task_id}")
+        self.pool.release(self.tasks.pop(task_id).page_table)
+
+
+# ----------------------------------------------------------------------------
+# 5. patch attention, the definition                 (DESIGN R11-R12)
+# ----------------------------------------------------------------------------
+def patch_attention(k_cache, v_cache, q_bits, positions, group: int) -> np.ndarray:
+    """k_cache, v_cache: [Hkv][cap][D] bf16 bits (one layer, logical order);
+    q_bits [n][Hq][D]; returns float64 [n][Hq][D].
+
+        g = h // G                      (HF repeat_kv head mapping)
+        s_x = q_{i,h} . K[x,g] / sqrt(D)      for x = 0 .. p_i
+        o   = sum_x softmax(s)_x V[x,g]
+    All in fp64; max-subtraction only for range safety.
+    """
+    kf = bf16_to_f64(k_cache)
+    vf = bf16_to_f64(v_cache)
+    qf = bf16_to_f64(q_bits)
+    n, Hq, D = qf.shape
+    out = np.empty((n, Hq, D), np.float64)
+    inv_sqrt_d = 1.0 / math.sqrt(D)
+    for i in range(n):
+        vis = int(positions[i]) + 1
+        for h in range(Hq):
+            g = h // group
+            s = (kf[g, :vis] @ qf[i, h]) * inv_sqrt_d
+            w = np.exp(s - s.max())
+            out[i, h] = (w @ vf[g, :vis]) / w.sum()
+    return out
