@@ -1,0 +1,200 @@
+/* fcg.h -- C ABI of the B200-native FCGRAFT KV-cache grafting library (libfcg.so).
+ *
+ * What the calls compute is defined by the paper (PAPER.md = the text of arxiv/paper_2606_13097)
+ * and, where the paper is silent, by the readings R1..R16 in DESIGN.md:
+ *
+ *   segment library   the KV half of the two-tier code cache H = (I, C), Eq. (2), PAPER.md:66-79:
+ *                     per function a cached K/V state that can be re-injected "without being tied
+ *                     to fixed prefix positions".
+ *   cache-stitching   Eq. (4): cached KV states are "concatenated and
+ *                     injected ... as additional context", each module "preserving its internal
+ *                     token order during composition".  Keys are re-rotated by the
+ *                     integer position delta (RoPE group law, R1), values are bit-copied.
+ *   cache-patching    Eq. (6): the prefix KV is reused, only the middle span
+ *                     is recomputed; its fresh K/V are scattered into the cache and the patch
+ *                     queries attend causally over the stitched cache (R12).
+ *
+ * Conventions
+ *   - Plain C, no exceptions cross the boundary.  Every call returns an fcg_status_t; on a non-OK
+ *     status fcg_last_error() holds a message and the library state is unchanged (host-side
+ *     validation happens before any allocation or launch: allocate-then-commit).
+ *   - "device" pointers are CUDA device pointers valid on the library's device; "host" pointers are
+ *     ordinary host memory read only during the call (unless stated otherwise).
+ *   - All device work is enqueued on the given `stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream).  Calls return after enqueueing.  Calls on one library must come from
+ *     one thread at a time, and work on one task must be issued on one stream (or externally ordered).
+ *   - bf16 everywhere for K, V, q, out (2 bytes/element, the bit layout of __nv_bfloat16).
+ *   - The library owns everything inside `arena` (page pool, page tables, segments, workspace); the
+ *     caller owns the arena allocation itself and all q/k/v/out buffers.
+ *   - There is no CPU fallback and no other backend: without a CUDA device every compute call fails
+ *     with FCG_ERR_CUDA.
+ */
+#ifndef FCG_H_
+#define FCG_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fcg_library fcg_library_t; /* opaque */
+typedef int32_t fcg_status_t;
+
+enum {
+  FCG_OK = 0,
+  FCG_ERR_INVALID_ARG = -1,  /* null pointer, bad geometry, bad shape, positions not increasing */
+  FCG_ERR_BAD_SEGMENT = -2,  /* unknown / released segment id */
+  FCG_ERR_RANGE = -3,        /* source or destination token range out of bounds */
+  FCG_ERR_OVERLAP = -4,      /* plan entries / holes overlap */
+  FCG_ERR_UNFILLED = -5,     /* a patch query would attend over a position nobody has filled */
+  FCG_ERR_OUT_OF_PAGES = -6, /* page pool (or per-task page-table stride) exhausted */
+  FCG_ERR_OUT_OF_ARENA = -7, /* arena / segment table / workspace too small */
+  FCG_ERR_CUDA = -8,         /* a CUDA runtime call failed; message has the CUDA error string */
+  FCG_ERR_BAD_TASK = -9      /* task id out of range, already live (stitch) or not live (patch) */
+};
+
+enum { FCG_ROPE_NONE = 0, FCG_ROPE_HALF_SPLIT = 1 };
+
+/* Geometry and capacities, fixed at create time.
+ * Arena layout (all offsets 256-byte aligned, reported by fcg_pool_info):
+ *   K pool  [n_layers][n_pages][n_kv_heads][page_size][head_dim] bf16   ("HND" pages: one head's
+ *   V pool  same shape                                                   slice of a page is contiguous)
+ *   page tables  int32 [max_tasks][ceil(max_task_tokens / page_size)]
+ *   workspace    workspace_bytes (split-KV partials, host-call staging, plan blobs)
+ *   segments     the rest, first-fit; a segment is K [n_layers][n_kv_heads][n][head_dim] then V. */
+typedef struct {
+  int32_t n_layers;
+  int32_t n_q_heads;       /* multiple of n_kv_heads */
+  int32_t n_kv_heads;
+  int32_t head_dim;        /* 64 or 128 */
+  int32_t page_size;       /* tokens per page: 8, 16, 32 or 64 */
+  int32_t rope_mode;       /* FCG_ROPE_NONE: stitch is a pure gather; FCG_ROPE_HALF_SPLIT: pairs (j, j + head_dim/2) (R2) */
+  double rope_base;        /* theta_j = rope_base^(-2j/head_dim) (R3); ignored if inv_freq != NULL */
+  const double *inv_freq;  /* host, optional [head_dim/2] override (scaled RoPE); copied at create */
+  void *arena;             /* device */
+  uint64_t arena_bytes;
+  int32_t max_segments;
+  int32_t max_tasks;
+  int32_t max_task_tokens; /* largest capacity a single task may have */
+  uint32_t n_pages;        /* pages in the pool, shared by all live tasks */
+  uint64_t workspace_bytes;/* 0 -> 256 MiB */
+  int32_t device;          /* CUDA device ordinal the arena lives on */
+} fcg_config_t;
+
+/* Bytes of arena needed for a configuration that must hold `segment_tokens` library tokens in total
+ * (host-only arithmetic, works without a GPU).  Returns 0 on a bad configuration. */
+uint64_t fcg_arena_bytes_required(const fcg_config_t *cfg, uint64_t segment_tokens);
+
+/* Creates a library over cfg->arena.  Fails with INVALID_ARG (geometry), OUT_OF_ARENA (arena too small
+ * for pool + tables + workspace) or CUDA. */
+fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out);
+/* Synchronises the device, then frees host state.  The arena is the caller's. */
+fcg_status_t fcg_library_destroy(fcg_library_t *lib);
+
+/* S1 (Eq. 2).  Copies n_tokens of K and V into the library.  k, v: device bf16, logical shape
+ * [n_layers][n_kv_heads][n_tokens][head_dim]; strides in ELEMENTS for those four axes (NULL =
+ * contiguous; strides[3] must be 1).  orig_start >= 0 is the position at which token 0's key was
+ * RoPE-encoded.  The caller may free k/v once `stream` has passed this call.  The id returned is the
+ * smallest id not in use. */
+fcg_status_t fcg_segment_register(fcg_library_t *lib, const void *k, const void *v, int32_t n_tokens,
+                                  int32_t orig_start, const int64_t *strides, void *stream,
+                                  int32_t *seg_id_out);
+/* The caller guarantees no enqueued stitch still reads the segment. */
+fcg_status_t fcg_segment_release(fcg_library_t *lib, int32_t seg_id);
+
+typedef struct { int32_t seg_id, src_begin, n_tokens, dst_offset; } fcg_plan_entry_t;
+typedef struct { int32_t begin, n_tokens; } fcg_hole_t;            /* ranges left for patches */
+typedef struct {
+  int32_t task_id;                  /* chosen by the caller in [0, max_tasks); must not be live */
+  const fcg_plan_entry_t *entries;  /* host */
+  int32_t n_entries;
+  const fcg_hole_t *holes;          /* host; may be NULL if n_holes == 0 */
+  int32_t n_holes;
+  int32_t capacity_tokens;          /* 0 -> max end of entries/holes; pages are reserved for the capacity */
+} fcg_plan_t;
+
+/* S2 + S3 (Eq. 4).  For every plan: validates it (R5-R7: 0 <= src_begin, n > 0, src_begin + n <= n_seg,
+ * dst_offset >= 0, end <= capacity <= max_task_tokens; entries and holes pairwise disjoint), computes
+ * delta_e = dst_offset - orig_start - src_begin, reserves ceil(capacity / page_size) pages (plans in
+ * array order, pages in ascending logical order, from a LIFO pool that initially hands out 0, 1, 2, ...;
+ * R9), writes the page table, and launches ONE fused kernel over all plans:
+ *     K_out[dst + i][j]       = bf16(a cos(delta theta_j) - b sin(delta theta_j))
+ *     K_out[dst + i][j + D/2] = bf16(b cos(delta theta_j) + a sin(delta theta_j)),  (a, b) = K_seg[src + i][j, j + D/2]
+ *     V_out[dst + i] = V_seg[src + i]   (bits)
+ * Entries with delta 0 (and rope_mode NONE) are bit copies.  Any failing plan fails the whole batch
+ * with nothing changed.  Unused tail slots of the last page are never written nor read (R10). */
+fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_plans, void *stream);
+
+/* S4 + S5/S6 (Eq. 6).  q [n_layers][n][n_q_heads][head_dim], k, v [n_layers][n][n_kv_heads][head_dim],
+ * out [n_layers][n][n_q_heads][head_dim]: device bf16, contiguous, for cache layers
+ * [layer_begin, layer_begin + n_layers).  k (and q) are already position-encoded by the caller (R13).
+ * positions: host int32[n], strictly increasing, < capacity.  For each layer the n fresh K/V rows are
+ * written to the slots of `positions` (bit copy), then for each patch token i and q-head h
+ *     out[i][h] = softmax_{x <= positions[i]}(q[i][h] . K[x][h / G] / sqrt(head_dim)) V[x][h / G],   G = n_q_heads / n_kv_heads
+ * with fp32 softmax/accumulation, bf16 result.  Every x <= positions[n-1] must be filled (stitched, or
+ * patched by this or an earlier call), else UNFILLED.  Rows per KV head R = n * G selects the kernel:
+ * split-KV warp-MMA path, or tcgen05/TMEM tiles for large R. */
+fcg_status_t fcg_patch(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers,
+                       const void *q, const void *k, const void *v, const int32_t *positions, int32_t n,
+                       void *out, void *stream);
+
+/* Same as fcg_patch with q, k, v, out in HOST memory (pinned for true asynchrony): the call enqueues the
+ * host->device copies, the kernels and the device->host copy of `out` on `stream`; out is valid once the
+ * stream has been synchronised.  Staging comes from the workspace (OUT_OF_ARENA if it does not fit). */
+fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers,
+                            const void *q, const void *k, const void *v, const int32_t *positions, int32_t n,
+                            void *out, void *stream);
+
+/* Batched patching (independent tasks, one launch): task_ids host int32[n_tasks] (distinct, live);
+ * n_per_task host int32[n_tasks]; positions host int32[sum n], the tasks' position lists back to back;
+ * q/k/v/out device bf16 [n_layers][sum n][heads][head_dim]. */
+fcg_status_t fcg_patch_batch(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task,
+                             int32_t n_tasks, int32_t layer_begin, int32_t n_layers, const void *q,
+                             const void *k, const void *v, const int32_t *positions, void *out, void *stream);
+
+/* Device pointer to the task's page table (int32[n_pages], logical page -> physical page id), its page
+ * count and current token count T (max end of stitched/declared/patched ranges).  Token x lives at
+ * (table[x / page_size], x % page_size). */
+fcg_status_t fcg_task_page_table(fcg_library_t *lib, int32_t task_id, const int32_t **dev_table,
+                                 int32_t *n_pages, int32_t *n_tokens);
+/* Host copy of the same table (no device access): writes min(n_pages, cap) entries to `out`. */
+fcg_status_t fcg_task_page_table_host(fcg_library_t *lib, int32_t task_id, int32_t *out, int32_t cap,
+                                      int32_t *n_pages);
+/* Returns the task's pages to the pool (pushed so that they are re-issued in ascending logical order). */
+fcg_status_t fcg_task_release(fcg_library_t *lib, int32_t task_id);
+
+/* Gathers logical tokens [begin, begin + n) of one layer of a task's cache into contiguous device
+ * buffers k_out, v_out [n_kv_heads][n][head_dim] (bit copy through the page table; for tests and for
+ * callers that need a dense view). */
+fcg_status_t fcg_task_read(fcg_library_t *lib, int32_t task_id, int32_t layer, int32_t begin, int32_t n,
+                           void *k_out, void *v_out, void *stream);
+
+typedef struct {
+  uint64_t k_pool_offset, v_pool_offset;  /* byte offsets into the arena */
+  uint64_t pool_bytes;                    /* bytes of ONE pool */
+  uint64_t page_table_offset, workspace_offset, segments_offset;
+  uint64_t segments_bytes_free;
+  uint32_t n_pages, n_pages_free;
+  int32_t n_segments_live, n_tasks_live;
+} fcg_pool_info_t;
+fcg_status_t fcg_pool_info(fcg_library_t *lib, fcg_pool_info_t *out);
+
+/* Launch statistics since create (kernels launched by this library; bench.py reports them). */
+typedef struct {
+  uint64_t stitch_launches, register_launches, scatter_launches, attn_split_launches, attn_combine_launches,
+      attn_tc_launches, read_launches;
+  int32_t last_attn_path;   /* 0 none, 1 split-KV warp-MMA, 2 tcgen05 */
+  int32_t last_attn_splits;
+} fcg_stats_t;
+fcg_status_t fcg_stats(fcg_library_t *lib, fcg_stats_t *out);
+
+/* Message for the last non-OK status returned on this thread (never NULL). */
+const char *fcg_last_error(void);
+/* "x.y.z sm_100a" */
+const char *fcg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FCG_H_ */

@@ -203,7 +203,7 @@ class OracleLibrary:
 
     def __init__(self, n_layers, n_q_heads, n_kv_heads, head_dim, page_size=16,
                  rope_mode=1, rope_base=1e4, inv_freq=None, max_segments=1 << 16,
-                 max_tasks=1 << 16, n_pages=1 << 20):
+                 max_tasks=1 << 16, n_pages=1 << 20, max_task_tokens=1 << 30):
         if head_dim % 8 or head_dim <= 0 or n_q_heads % n_kv_heads or page_size <= 0:
             raise OracleError(FCG_ERR_INVALID_ARG, "bad geometry")
         self.L, self.Hq, self.Hkv, self.D, self.P = n_layers, n_q_heads, n_kv_heads, head_dim, page_size
@@ -211,7 +211,7 @@ class OracleLibrary:
         self.rope_mode = rope_mode
         self.inv_freq = (np.asarray(inv_freq, dtype=np.float64) if inv_freq is not None
                          else rope_inv_freq(head_dim, rope_base))
-        self.max_segments, self.max_tasks = max_segments, max_tasks
+        self.max_segments, self.max_tasks, self.max_task_tokens = max_segments, max_tasks, max_task_tokens
         self.pool = PagePool(n_pages)
         self.segments: dict[int, Segment] = {}
         self.tasks: dict[int, Task] = {}
@@ -270,6 +270,8 @@ class OracleLibrary:
         capacity = plan.capacity_tokens if plan.capacity_tokens > 0 else T
         if T > capacity:
             raise OracleError(FCG_ERR_RANGE, "plan exceeds capacity_tokens")
+        if capacity > self.max_task_tokens:
+            raise OracleError(FCG_ERR_RANGE, "capacity exceeds max_task_tokens")
         srt = sorted(spans)
         for (b0, e0), (b1, e1) in zip(srt, srt[1:]):
             if b1 < e0:

@@ -1,0 +1,366 @@
+"""ctypes binding of libfcg.so (include/fcg.h).  Argument marshalling only: every step of the hot
+path (gather + RoPE shift, scatter, patch attention) runs in the CUDA kernels behind the C ABI.
+
+The functions ``fcg_*`` mirror the C entry points one to one and take raw pointers / ints (or torch
+tensors, whose ``data_ptr()`` is passed).  ``FcgLibrary`` is a small convenience wrapper over them.
+PyTorch is used for device memory and streams only.  There is no CPU fallback: if libfcg.so has not
+been built, importing works but the first call raises ``FcgError`` telling how to build it.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfcg.so")
+
+FCG_OK = 0
+FCG_ERR_INVALID_ARG = -1
+FCG_ERR_BAD_SEGMENT = -2
+FCG_ERR_RANGE = -3
+FCG_ERR_OVERLAP = -4
+FCG_ERR_UNFILLED = -5
+FCG_ERR_OUT_OF_PAGES = -6
+FCG_ERR_OUT_OF_ARENA = -7
+FCG_ERR_CUDA = -8
+FCG_ERR_BAD_TASK = -9
+
+FCG_ROPE_NONE = 0
+FCG_ROPE_HALF_SPLIT = 1
+
+
+class FcgError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"fcg status {status}: {msg}")
+        self.status = status
+
+
+class fcg_config_t(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32),
+                ("head_dim", C.c_int32), ("page_size", C.c_int32), ("rope_mode", C.c_int32),
+                ("rope_base", C.c_double), ("inv_freq", C.POINTER(C.c_double)),
+                ("arena", C.c_void_p), ("arena_bytes", C.c_uint64),
+                ("max_segments", C.c_int32), ("max_tasks", C.c_int32), ("max_task_tokens", C.c_int32),
+                ("n_pages", C.c_uint32), ("workspace_bytes", C.c_uint64), ("device", C.c_int32)]
+
+
+class fcg_plan_entry_t(C.Structure):
+    _fields_ = [("seg_id", C.c_int32), ("src_begin", C.c_int32), ("n_tokens", C.c_int32), ("dst_offset", C.c_int32)]
+
+
+class fcg_hole_t(C.Structure):
+    _fields_ = [("begin", C.c_int32), ("n_tokens", C.c_int32)]
+
+
+class fcg_plan_t(C.Structure):
+    _fields_ = [("task_id", C.c_int32), ("entries", C.POINTER(fcg_plan_entry_t)), ("n_entries", C.c_int32),
+                ("holes", C.POINTER(fcg_hole_t)), ("n_holes", C.c_int32), ("capacity_tokens", C.c_int32)]
+
+
+class fcg_pool_info_t(C.Structure):
+    _fields_ = [("k_pool_offset", C.c_uint64), ("v_pool_offset", C.c_uint64), ("pool_bytes", C.c_uint64),
+                ("page_table_offset", C.c_uint64), ("workspace_offset", C.c_uint64), ("segments_offset", C.c_uint64),
+                ("segments_bytes_free", C.c_uint64), ("n_pages", C.c_uint32), ("n_pages_free", C.c_uint32),
+                ("n_segments_live", C.c_int32), ("n_tasks_live", C.c_int32)]
+
+
+class fcg_stats_t(C.Structure):
+    _fields_ = [("stitch_launches", C.c_uint64), ("register_launches", C.c_uint64), ("scatter_launches", C.c_uint64),
+                ("attn_split_launches", C.c_uint64), ("attn_combine_launches", C.c_uint64),
+                ("attn_tc_launches", C.c_uint64), ("read_launches", C.c_uint64),
+                ("last_attn_path", C.c_int32), ("last_attn_splits", C.c_int32)]
+
+
+# every symbol include/fcg.h declares: name -> (restype, argtypes)
+_P = C.c_void_p
+_I = C.c_int32
+_PI = C.POINTER(C.c_int32)
+SYMBOLS = {
+    "fcg_arena_bytes_required": (C.c_uint64, [C.POINTER(fcg_config_t), C.c_uint64]),
+    "fcg_library_create": (_I, [C.POINTER(fcg_config_t), C.POINTER(_P)]),
+    "fcg_library_destroy": (_I, [_P]),
+    "fcg_segment_register": (_I, [_P, _P, _P, _I, _I, C.POINTER(C.c_int64), _P, _PI]),
+    "fcg_segment_release": (_I, [_P, _I]),
+    "fcg_stitch": (_I, [_P, C.POINTER(fcg_plan_t), _I, _P]),
+    "fcg_patch": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
+    "fcg_patch_host": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
+    "fcg_patch_batch": (_I, [_P, _PI, _PI, _I, _I, _I, _P, _P, _P, _PI, _P, _P]),
+    "fcg_task_page_table": (_I, [_P, _I, C.POINTER(_P), _PI, _PI]),
+    "fcg_task_page_table_host": (_I, [_P, _I, _PI, _I, _PI]),
+    "fcg_task_release": (_I, [_P, _I]),
+    "fcg_task_read": (_I, [_P, _I, _I, _I, _I, _P, _P, _P]),
+    "fcg_pool_info": (_I, [_P, C.POINTER(fcg_pool_info_t)]),
+    "fcg_stats": (_I, [_P, C.POINTER(fcg_stats_t)]),
+    "fcg_last_error": (C.c_char_p, []),
+    "fcg_version": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """dlopen libfcg.so (once).  Fails loudly when it has not been built -- there is no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FcgError(FCG_ERR_CUDA, f"{LIB_PATH} is missing: build it with "
+                                         "`python -m paper_2606_13097_b200.build` (or __graft_entry__.build()); "
+                                         "there is no CPU fallback")
+        lib = C.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+def _check(status: int):
+    if status != FCG_OK:
+        raise FcgError(status, load().fcg_last_error().decode())
+
+
+def _ptr(x) -> int:
+    if x is None:
+        return None
+    if isinstance(x, torch.Tensor):
+        return x.data_ptr()
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    return int(x)
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, torch.cuda.Stream):
+        return stream.cuda_stream
+    return int(stream)
+
+
+def _i32(a) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+
+
+# ------------------------------------------------------------------------------------------------
+# 1:1 functions
+# ------------------------------------------------------------------------------------------------
+def fcg_version() -> str:
+    return load().fcg_version().decode()
+
+
+def fcg_last_error() -> str:
+    return load().fcg_last_error().decode()
+
+
+def make_config(*, n_layers, n_q_heads, n_kv_heads, head_dim, page_size=16, rope_mode=FCG_ROPE_HALF_SPLIT,
+                rope_base=1e4, inv_freq=None, arena=0, arena_bytes=0, max_segments=64, max_tasks=8,
+                max_task_tokens=8192, n_pages=1024, workspace_bytes=0, device=0):
+    cfg = fcg_config_t()
+    cfg.n_layers, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim = n_layers, n_q_heads, n_kv_heads, head_dim
+    cfg.page_size, cfg.rope_mode, cfg.rope_base = page_size, rope_mode, float(rope_base)
+    keep = None
+    if inv_freq is not None:
+        keep = np.ascontiguousarray(np.asarray(inv_freq, dtype=np.float64))
+        cfg.inv_freq = keep.ctypes.data_as(C.POINTER(C.c_double))
+    cfg.arena, cfg.arena_bytes = _ptr(arena), int(arena_bytes)
+    cfg.max_segments, cfg.max_tasks, cfg.max_task_tokens = max_segments, max_tasks, max_task_tokens
+    cfg.n_pages, cfg.workspace_bytes, cfg.device = n_pages, workspace_bytes, device
+    cfg._keepalive = keep
+    return cfg
+
+
+def fcg_arena_bytes_required(cfg: fcg_config_t, segment_tokens: int) -> int:
+    return int(load().fcg_arena_bytes_required(C.byref(cfg), int(segment_tokens)))
+
+
+def fcg_library_create(cfg: fcg_config_t) -> int:
+    h = _P()
+    _check(load().fcg_library_create(C.byref(cfg), C.byref(h)))
+    return h.value
+
+
+def fcg_library_destroy(handle: int) -> None:
+    _check(load().fcg_library_destroy(handle))
+
+
+def fcg_segment_register(handle, k, v, n_tokens, orig_start, strides=None, stream=None) -> int:
+    sid = C.c_int32(-1)
+    st = None
+    if strides is not None:
+        st = (C.c_int64 * 4)(*[int(s) for s in strides])
+    _check(load().fcg_segment_register(handle, _ptr(k), _ptr(v), int(n_tokens), int(orig_start), st,
+                                       _stream(stream), C.byref(sid)))
+    return sid.value
+
+
+def fcg_segment_release(handle, seg_id) -> None:
+    _check(load().fcg_segment_release(handle, int(seg_id)))
+
+
+def _marshal_plans(plans):
+    """plans: iterable of dicts {task_id, entries=[(seg, src_begin, n, dst)], holes=[(begin, n)], capacity_tokens}."""
+    arr = (fcg_plan_t * len(plans))()
+    keep = []
+    for i, p in enumerate(plans):
+        ents = p.get("entries", [])
+        holes = p.get("holes", [])
+        e_arr = (fcg_plan_entry_t * max(1, len(ents)))(*[fcg_plan_entry_t(*map(int, e)) for e in ents])
+        h_arr = (fcg_hole_t * max(1, len(holes)))(*[fcg_hole_t(*map(int, h)) for h in holes])
+        keep += [e_arr, h_arr]
+        arr[i].task_id = int(p["task_id"])
+        arr[i].entries = C.cast(e_arr, C.POINTER(fcg_plan_entry_t))
+        arr[i].n_entries = len(ents)
+        arr[i].holes = C.cast(h_arr, C.POINTER(fcg_hole_t))
+        arr[i].n_holes = len(holes)
+        arr[i].capacity_tokens = int(p.get("capacity_tokens", 0))
+    return arr, keep
+
+
+def fcg_stitch(handle, plans, stream=None) -> None:
+    arr, _keep = _marshal_plans(list(plans))
+    _check(load().fcg_stitch(handle, arr, len(arr), _stream(stream)))
+
+
+def fcg_patch(handle, task_id, layer_begin, n_layers, q, k, v, positions, out, stream=None) -> None:
+    pos = _i32(positions)
+    _check(load().fcg_patch(handle, int(task_id), int(layer_begin), int(n_layers), _ptr(q), _ptr(k), _ptr(v),
+                            pos.ctypes.data_as(_PI), int(pos.size), _ptr(out), _stream(stream)))
+
+
+def fcg_patch_host(handle, task_id, layer_begin, n_layers, q, k, v, positions, out, stream=None) -> None:
+    pos = _i32(positions)
+    _check(load().fcg_patch_host(handle, int(task_id), int(layer_begin), int(n_layers), _ptr(q), _ptr(k), _ptr(v),
+                                 pos.ctypes.data_as(_PI), int(pos.size), _ptr(out), _stream(stream)))
+
+
+def fcg_patch_batch(handle, task_ids, n_per_task, layer_begin, n_layers, q, k, v, positions, out, stream=None) -> None:
+    ids, npt, pos = _i32(task_ids), _i32(n_per_task), _i32(positions)
+    _check(load().fcg_patch_batch(handle, ids.ctypes.data_as(_PI), npt.ctypes.data_as(_PI), int(ids.size),
+                                  int(layer_begin), int(n_layers), _ptr(q), _ptr(k), _ptr(v),
+                                  pos.ctypes.data_as(_PI), _ptr(out), _stream(stream)))
+
+
+def fcg_task_page_table(handle, task_id):
+    """-> (device pointer of int32 table, n_pages, n_tokens)"""
+    p, n_pages, n_tokens = _P(), C.c_int32(), C.c_int32()
+    _check(load().fcg_task_page_table(handle, int(task_id), C.byref(p), C.byref(n_pages), C.byref(n_tokens)))
+    return p.value, n_pages.value, n_tokens.value
+
+
+def fcg_task_page_table_host(handle, task_id) -> np.ndarray:
+    n = C.c_int32()
+    _check(load().fcg_task_page_table_host(handle, int(task_id), None, 0, C.byref(n)))
+    out = np.empty(n.value, np.int32)
+    _check(load().fcg_task_page_table_host(handle, int(task_id), out.ctypes.data_as(_PI), n.value, C.byref(n)))
+    return out
+
+
+def fcg_task_release(handle, task_id) -> None:
+    _check(load().fcg_task_release(handle, int(task_id)))
+
+
+def fcg_task_read(handle, task_id, layer, begin, n, k_out, v_out, stream=None) -> None:
+    _check(load().fcg_task_read(handle, int(task_id), int(layer), int(begin), int(n), _ptr(k_out), _ptr(v_out),
+                                _stream(stream)))
+
+
+def fcg_pool_info(handle) -> dict:
+    info = fcg_pool_info_t()
+    _check(load().fcg_pool_info(handle, C.byref(info)))
+    return {f: getattr(info, f) for f, _ in fcg_pool_info_t._fields_}
+
+
+def fcg_stats(handle) -> dict:
+    st = fcg_stats_t()
+    _check(load().fcg_stats(handle, C.byref(st)))
+    return {f: getattr(st, f) for f, _ in fcg_stats_t._fields_}
+
+
+# ------------------------------------------------------------------------------------------------
+# convenience wrapper
+# ------------------------------------------------------------------------------------------------
+class FcgLibrary:
+    """Owns a torch uint8 arena on ``device`` and a library handle over it."""
+
+    def __init__(self, *, n_layers, n_q_heads, n_kv_heads, head_dim, page_size=16, rope_mode=FCG_ROPE_HALF_SPLIT,
+                 rope_base=1e4, inv_freq=None, max_segments=64, max_tasks=8, max_task_tokens=8192, n_pages=1024,
+                 workspace_bytes=0, segment_tokens=0, device=0):
+        self.n_layers, self.n_q_heads, self.n_kv_heads, self.head_dim = n_layers, n_q_heads, n_kv_heads, head_dim
+        self.page_size = page_size
+        self.device = torch.device("cuda", device)
+        cfg = make_config(n_layers=n_layers, n_q_heads=n_q_heads, n_kv_heads=n_kv_heads, head_dim=head_dim,
+                          page_size=page_size, rope_mode=rope_mode, rope_base=rope_base, inv_freq=inv_freq,
+                          max_segments=max_segments, max_tasks=max_tasks, max_task_tokens=max_task_tokens,
+                          n_pages=n_pages, workspace_bytes=workspace_bytes, device=device)
+        need = fcg_arena_bytes_required(cfg, segment_tokens)
+        if need == 0:
+            raise FcgError(FCG_ERR_INVALID_ARG, "bad configuration")
+        self.arena = torch.empty(need, dtype=torch.uint8, device=self.device)
+        cfg.arena, cfg.arena_bytes = self.arena.data_ptr(), need
+        self.handle = fcg_library_create(cfg)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            fcg_library_destroy(self.handle)
+            self.handle = None
+            self.arena = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def segment_register(self, k: torch.Tensor, v: torch.Tensor, orig_start: int, stream=None) -> int:
+        assert k.dtype == torch.bfloat16 and v.dtype == torch.bfloat16 and k.is_cuda and v.is_cuda
+        assert k.shape == v.shape and k.stride() == v.stride()
+        return fcg_segment_register(self.handle, k, v, k.shape[2], orig_start, k.stride(), stream)
+
+    def segment_release(self, seg_id):
+        fcg_segment_release(self.handle, seg_id)
+
+    def stitch(self, plans, stream=None):
+        fcg_stitch(self.handle, plans, stream)
+
+    def patch(self, task_id, layer_begin, q, k, v, positions, out=None, stream=None) -> torch.Tensor:
+        assert q.is_cuda and q.is_contiguous() and k.is_contiguous() and v.is_contiguous()
+        if out is None:
+            out = torch.empty_like(q)
+        fcg_patch(self.handle, task_id, layer_begin, q.shape[0], q, k, v, positions, out, stream)
+        return out
+
+    def patch_host(self, task_id, layer_begin, q, k, v, positions, out, stream=None) -> torch.Tensor:
+        assert not q.is_cuda and q.is_contiguous() and k.is_contiguous() and v.is_contiguous() and out.is_contiguous()
+        fcg_patch_host(self.handle, task_id, layer_begin, q.shape[0], q, k, v, positions, out, stream)
+        return out
+
+    def patch_batch(self, task_ids, n_per_task, layer_begin, q, k, v, positions, out=None, stream=None) -> torch.Tensor:
+        if out is None:
+            out = torch.empty_like(q)
+        fcg_patch_batch(self.handle, task_ids, n_per_task, layer_begin, q.shape[0], q, k, v, positions, out, stream)
+        return out
+
+    def task_page_table(self, task_id):
+        return fcg_task_page_table(self.handle, task_id)
+
+    def task_page_table_host(self, task_id) -> np.ndarray:
+        return fcg_task_page_table_host(self.handle, task_id)
+
+    def task_read(self, task_id, layer, begin, n, stream=None):
+        k = torch.empty((self.n_kv_heads, n, self.head_dim), dtype=torch.bfloat16, device=self.device)
+        v = torch.empty_like(k)
+        fcg_task_read(self.handle, task_id, layer, begin, n, k, v, stream)
+        return k, v
+
+    def task_release(self, task_id):
+        fcg_task_release(self.handle, task_id)
+
+    def pool_info(self) -> dict:
+        return fcg_pool_info(self.handle)
+
+    def stats(self) -> dict:
+        return fcg_stats(self.handle)

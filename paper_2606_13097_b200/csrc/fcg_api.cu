@@ -1,0 +1,858 @@
+// Host side of libfcg.so: the C ABI of include/fcg.h -- segment library (S1), stitch-plan builder and
+// page allocator (S2), and the launch logic for S3-S6.  Everything here is integer bookkeeping plus
+// the fp64 evaluation of the per-entry RoPE table; all K/V/q arithmetic runs in the kernels.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <map>
+#include <string>
+#include <vector>
+
+#include "../../include/fcg.h"
+#include "fcg_internal.h"
+
+namespace {
+
+thread_local std::string g_err = "";
+
+fcg_status_t fail(fcg_status_t st, const char *fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return st;
+}
+
+#define FCG_CUDA(expr)                                                                         \
+  do {                                                                                         \
+    cudaError_t e__ = (expr);                                                                  \
+    if (e__ != cudaSuccess) return fail(FCG_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e__)); \
+  } while (0)
+
+constexpr uint64_t ALIGN = 256;
+constexpr int BLOB_SLOTS = 16;
+constexpr uint64_t BLOB_BYTES = 1ull << 20;
+constexpr int KV_TILE = 64;          // tokens per attention tile (fcg_attn_split.cu BN)
+constexpr int N_SMS = 148;
+
+uint64_t align_up(uint64_t x, uint64_t a = ALIGN) { return (x + a - 1) / a * a; }
+
+struct SegmentRec {
+  bool live = false;
+  uint64_t offset = 0, bytes = 0;   // in the arena; K then V
+  int32_t n_tokens = 0, orig_start = 0;
+};
+
+struct TaskRec {
+  bool live = false;
+  std::vector<int32_t> pages;
+  int32_t capacity = 0, n_tokens = 0;
+  std::vector<uint8_t> filled;
+  int32_t filled_prefix = 0;        // every x < filled_prefix is filled
+};
+
+struct BlobSlot {
+  unsigned char *host = nullptr;    // pinned
+  unsigned char *dev = nullptr;     // inside the workspace
+  cudaEvent_t ev = nullptr;
+  bool in_flight = false;
+};
+
+struct FreeRange {
+  uint64_t off, bytes;
+};
+
+}  // namespace
+
+struct fcg_library {
+  fcg_config_t cfg;
+  std::vector<double> inv_freq;
+  unsigned char *arena = nullptr;
+  uint64_t k_pool_off = 0, v_pool_off = 0, pool_bytes = 0, table_off = 0, ws_off = 0, seg_off = 0, seg_bytes = 0;
+  uint64_t scratch_off = 0, scratch_bytes = 0;   // workspace after the blob slots
+  int32_t pages_per_task = 0;
+  std::vector<int32_t> page_stack;               // LIFO: back() is handed out next
+  std::vector<SegmentRec> segments;
+  std::vector<FreeRange> seg_free;               // sorted by offset
+  std::vector<TaskRec> tasks;
+  BlobSlot slots[BLOB_SLOTS];
+  int next_slot = 0;
+  fcg_stats_t stats;
+  int n_segments_live = 0, n_tasks_live = 0;
+
+  uint16_t *k_pool() const { return reinterpret_cast<uint16_t *>(arena + k_pool_off); }
+  uint16_t *v_pool() const { return reinterpret_cast<uint16_t *>(arena + v_pool_off); }
+  int32_t *tables() const { return reinterpret_cast<int32_t *>(arena + table_off); }
+  uint64_t kv_row_bytes() const { return (uint64_t)cfg.head_dim * 2; }
+  uint64_t seg_bytes_for(int64_t n) const {
+    return 2 * align_up((uint64_t)cfg.n_layers * cfg.n_kv_heads * (uint64_t)n * kv_row_bytes());
+  }
+};
+
+namespace {
+
+bool geometry_ok(const fcg_config_t *c) {
+  if (!c) return false;
+  if (c->n_layers <= 0 || c->n_kv_heads <= 0 || c->n_q_heads <= 0 || c->n_q_heads % c->n_kv_heads) return false;
+  if (c->head_dim != 64 && c->head_dim != 128) return false;
+  if (c->page_size != 8 && c->page_size != 16 && c->page_size != 32 && c->page_size != 64) return false;
+  if (c->rope_mode != FCG_ROPE_NONE && c->rope_mode != FCG_ROPE_HALF_SPLIT) return false;
+  if (c->rope_mode == FCG_ROPE_HALF_SPLIT && !c->inv_freq && !(c->rope_base > 0.0)) return false;
+  if (c->max_segments <= 0 || c->max_tasks <= 0 || c->max_task_tokens <= 0 || c->n_pages == 0) return false;
+  return true;
+}
+
+struct Layout {
+  uint64_t k_pool_off, v_pool_off, pool_bytes, table_off, ws_off, ws_bytes, seg_off;
+  int32_t pages_per_task;
+};
+
+Layout layout_of(const fcg_config_t *c) {
+  Layout l;
+  l.pool_bytes = align_up((uint64_t)c->n_layers * c->n_pages * c->n_kv_heads * c->page_size * c->head_dim * 2);
+  l.k_pool_off = 0;
+  l.v_pool_off = l.pool_bytes;
+  l.table_off = 2 * l.pool_bytes;
+  l.pages_per_task = (c->max_task_tokens + c->page_size - 1) / c->page_size;
+  l.ws_off = l.table_off + align_up((uint64_t)c->max_tasks * l.pages_per_task * 4);
+  l.ws_bytes = align_up(c->workspace_bytes ? c->workspace_bytes : (256ull << 20));
+  l.seg_off = l.ws_off + l.ws_bytes;
+  return l;
+}
+
+// acquire a blob slot whose previous consumer kernels have finished
+fcg_status_t acquire_slot(fcg_library *lib, BlobSlot **out) {
+  BlobSlot &s = lib->slots[lib->next_slot];
+  lib->next_slot = (lib->next_slot + 1) % BLOB_SLOTS;
+  if (s.in_flight) {
+    FCG_CUDA(cudaEventSynchronize(s.ev));
+    s.in_flight = false;
+  }
+  *out = &s;
+  return FCG_OK;
+}
+
+struct BlobWriter {
+  unsigned char *base;
+  uint64_t used = 0, cap;
+  BlobWriter(unsigned char *b, uint64_t c) : base(b), cap(c) {}
+  // returns the byte offset of `bytes` reserved bytes (16-byte aligned) or UINT64_MAX
+  uint64_t reserve(uint64_t bytes) {
+    uint64_t off = align_up(used, 16);
+    if (off + bytes > cap) return UINT64_MAX;
+    used = off + bytes;
+    return off;
+  }
+};
+
+}  // namespace
+
+extern "C" {
+
+const char *fcg_last_error(void) { return g_err.c_str(); }
+const char *fcg_version(void) { return "0.1.0 sm_100a"; }
+
+uint64_t fcg_arena_bytes_required(const fcg_config_t *cfg, uint64_t segment_tokens) {
+  if (!geometry_ok(cfg)) return 0;
+  Layout l = layout_of(cfg);
+  const uint64_t per_tok = (uint64_t)cfg->n_layers * cfg->n_kv_heads * cfg->head_dim * 2 * 2;
+  return l.seg_off + segment_tokens * per_tok + (uint64_t)cfg->max_segments * 2 * ALIGN + 4096;
+}
+
+fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
+  if (!out) return fail(FCG_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  if (!geometry_ok(cfg))
+    return fail(FCG_ERR_INVALID_ARG,
+                "bad configuration (head_dim must be 64/128, page_size 8/16/32/64, n_q_heads %% n_kv_heads == 0, "
+                "capacities > 0)");
+  if (!cfg->arena || ((uintptr_t)cfg->arena % ALIGN)) return fail(FCG_ERR_INVALID_ARG, "arena must be a 256-byte aligned device pointer");
+  Layout l = layout_of(cfg);
+  if (l.ws_bytes < (uint64_t)BLOB_SLOTS * BLOB_BYTES + (16ull << 20))
+    return fail(FCG_ERR_INVALID_ARG, "workspace_bytes must be at least %llu", (unsigned long long)((uint64_t)BLOB_SLOTS * BLOB_BYTES + (16ull << 20)));
+  if (l.seg_off > cfg->arena_bytes)
+    return fail(FCG_ERR_OUT_OF_ARENA, "arena of %llu bytes cannot hold pools + tables + workspace (%llu bytes)",
+                (unsigned long long)cfg->arena_bytes, (unsigned long long)l.seg_off);
+  int n_dev = 0;
+  FCG_CUDA(cudaGetDeviceCount(&n_dev));
+  if (cfg->device < 0 || cfg->device >= n_dev) return fail(FCG_ERR_INVALID_ARG, "device %d out of range", cfg->device);
+  FCG_CUDA(cudaSetDevice(cfg->device));
+
+  fcg_library *lib = new fcg_library();
+  lib->cfg = *cfg;
+  lib->cfg.workspace_bytes = l.ws_bytes;
+  const int half = cfg->head_dim / 2;
+  lib->inv_freq.resize(half);
+  for (int j = 0; j < half; ++j)
+    lib->inv_freq[j] = cfg->inv_freq ? cfg->inv_freq[j] : pow(cfg->rope_base, -2.0 * (double)j / (double)cfg->head_dim);
+  lib->cfg.inv_freq = nullptr;
+  lib->arena = static_cast<unsigned char *>(cfg->arena);
+  lib->k_pool_off = l.k_pool_off;
+  lib->v_pool_off = l.v_pool_off;
+  lib->pool_bytes = l.pool_bytes;
+  lib->table_off = l.table_off;
+  lib->ws_off = l.ws_off;
+  lib->seg_off = l.seg_off;
+  lib->seg_bytes = cfg->arena_bytes - l.seg_off;
+  lib->pages_per_task = l.pages_per_task;
+  lib->scratch_off = l.ws_off + (uint64_t)BLOB_SLOTS * BLOB_BYTES;
+  lib->scratch_bytes = l.ws_bytes - (uint64_t)BLOB_SLOTS * BLOB_BYTES;
+  lib->page_stack.resize(cfg->n_pages);
+  for (uint32_t i = 0; i < cfg->n_pages; ++i) lib->page_stack[i] = (int32_t)(cfg->n_pages - 1 - i);  // back() == 0
+  lib->segments.resize(cfg->max_segments);
+  lib->tasks.resize(cfg->max_tasks);
+  if (lib->seg_bytes) lib->seg_free.push_back({lib->seg_off, lib->seg_bytes});
+  memset(&lib->stats, 0, sizeof lib->stats);
+  for (int i = 0; i < BLOB_SLOTS; ++i) {
+    cudaError_t e = cudaHostAlloc((void **)&lib->slots[i].host, BLOB_BYTES, cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->slots[i].ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+      for (int j = 0; j <= i; ++j) {
+        if (lib->slots[j].host) cudaFreeHost(lib->slots[j].host);
+        if (lib->slots[j].ev) cudaEventDestroy(lib->slots[j].ev);
+      }
+      delete lib;
+      return fail(FCG_ERR_CUDA, "blob slot allocation: %s", cudaGetErrorString(e));
+    }
+    lib->slots[i].dev = lib->arena + l.ws_off + (uint64_t)i * BLOB_BYTES;
+  }
+  *out = lib;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_library_destroy(fcg_library_t *lib) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  cudaSetDevice(lib->cfg.device);
+  cudaDeviceSynchronize();
+  for (int i = 0; i < BLOB_SLOTS; ++i) {
+    if (lib->slots[i].host) cudaFreeHost(lib->slots[i].host);
+    if (lib->slots[i].ev) cudaEventDestroy(lib->slots[i].ev);
+  }
+  delete lib;
+  return FCG_OK;
+}
+
+// ------------------------------------------------------------------------------------------ S1
+fcg_status_t fcg_segment_register(fcg_library_t *lib, const void *k, const void *v, int32_t n_tokens,
+                                  int32_t orig_start, const int64_t *strides, void *stream, int32_t *seg_id_out) {
+  if (!lib || !k || !v || !seg_id_out) return fail(FCG_ERR_INVALID_ARG, "NULL argument");
+  if (n_tokens <= 0 || orig_start < 0) return fail(FCG_ERR_INVALID_ARG, "n_tokens must be > 0 and orig_start >= 0");
+  const fcg_config_t &c = lib->cfg;
+  int64_t st[4] = {(int64_t)c.n_kv_heads * n_tokens * c.head_dim, (int64_t)n_tokens * c.head_dim, c.head_dim, 1};
+  if (strides) {
+    if (strides[3] != 1) return fail(FCG_ERR_INVALID_ARG, "strides[3] must be 1 (contiguous head_dim)");
+    for (int i = 0; i < 3; ++i) {
+      if (strides[i] % 8) return fail(FCG_ERR_INVALID_ARG, "strides must be multiples of 8 elements (16-byte rows)");
+      st[i] = strides[i];
+    }
+  }
+  if (((uintptr_t)k % 16) || ((uintptr_t)v % 16)) return fail(FCG_ERR_INVALID_ARG, "k and v must be 16-byte aligned");
+  int32_t sid = -1;
+  for (int32_t i = 0; i < c.max_segments; ++i)
+    if (!lib->segments[i].live) {
+      sid = i;
+      break;
+    }
+  if (sid < 0) return fail(FCG_ERR_OUT_OF_ARENA, "segment table full (%d)", c.max_segments);
+  const uint64_t bytes = lib->seg_bytes_for(n_tokens);
+  size_t fi = lib->seg_free.size();
+  for (size_t i = 0; i < lib->seg_free.size(); ++i)
+    if (lib->seg_free[i].bytes >= bytes) {
+      fi = i;
+      break;
+    }
+  if (fi == lib->seg_free.size())
+    return fail(FCG_ERR_OUT_OF_ARENA, "no free arena range of %llu bytes for a %d-token segment", (unsigned long long)bytes, n_tokens);
+  const uint64_t off = lib->seg_free[fi].off;
+
+  fcg::RegisterParams rp;
+  rp.k_src = static_cast<const uint16_t *>(k);
+  rp.v_src = static_cast<const uint16_t *>(v);
+  rp.k_dst = reinterpret_cast<uint16_t *>(lib->arena + off);
+  rp.v_dst = reinterpret_cast<uint16_t *>(lib->arena + off + bytes / 2);
+  rp.s_layer = st[0];
+  rp.s_head = st[1];
+  rp.s_tok = st[2];
+  rp.n_layers = c.n_layers;
+  rp.n_kv_heads = c.n_kv_heads;
+  rp.n_tokens = n_tokens;
+  rp.head_dim = c.head_dim;
+  FCG_CUDA(cudaSetDevice(c.device));
+  FCG_CUDA(fcg::launch_register_copy(rp, static_cast<cudaStream_t>(stream)));
+  lib->stats.register_launches++;
+
+  // commit
+  if (lib->seg_free[fi].bytes == bytes)
+    lib->seg_free.erase(lib->seg_free.begin() + fi);
+  else {
+    lib->seg_free[fi].off += bytes;
+    lib->seg_free[fi].bytes -= bytes;
+  }
+  SegmentRec &s = lib->segments[sid];
+  s.live = true;
+  s.offset = off;
+  s.bytes = bytes;
+  s.n_tokens = n_tokens;
+  s.orig_start = orig_start;
+  lib->n_segments_live++;
+  *seg_id_out = sid;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_segment_release(fcg_library_t *lib, int32_t seg_id) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  if (seg_id < 0 || seg_id >= lib->cfg.max_segments || !lib->segments[seg_id].live)
+    return fail(FCG_ERR_BAD_SEGMENT, "unknown segment %d", seg_id);
+  SegmentRec &s = lib->segments[seg_id];
+  FreeRange fr{s.offset, s.bytes};
+  auto it = std::lower_bound(lib->seg_free.begin(), lib->seg_free.end(), fr,
+                             [](const FreeRange &a, const FreeRange &b) { return a.off < b.off; });
+  it = lib->seg_free.insert(it, fr);
+  // coalesce with the next, then with the previous
+  if (it + 1 != lib->seg_free.end() && it->off + it->bytes == (it + 1)->off) {
+    it->bytes += (it + 1)->bytes;
+    lib->seg_free.erase(it + 1);
+  }
+  if (it != lib->seg_free.begin() && (it - 1)->off + (it - 1)->bytes == it->off) {
+    (it - 1)->bytes += it->bytes;
+    lib->seg_free.erase(it);
+  }
+  s.live = false;
+  lib->n_segments_live--;
+  return FCG_OK;
+}
+
+// ------------------------------------------------------------------------------------- S2 + S3
+namespace {
+struct CheckedPlan {
+  int32_t capacity, T, n_pages;
+  std::vector<int32_t> deltas;
+};
+
+fcg_status_t validate_plan(fcg_library *lib, const fcg_plan_t &pl, CheckedPlan &cp) {
+  const fcg_config_t &c = lib->cfg;
+  if (pl.task_id < 0 || pl.task_id >= c.max_tasks) return fail(FCG_ERR_BAD_TASK, "task id %d out of range", pl.task_id);
+  if (lib->tasks[pl.task_id].live) return fail(FCG_ERR_BAD_TASK, "task %d is already live", pl.task_id);
+  if (pl.n_entries < 0 || pl.n_holes < 0 || (pl.n_entries > 0 && !pl.entries) || (pl.n_holes > 0 && !pl.holes))
+    return fail(FCG_ERR_INVALID_ARG, "plan arrays");
+  if (pl.n_entries + pl.n_holes == 0) return fail(FCG_ERR_INVALID_ARG, "empty plan");
+  std::vector<std::pair<int64_t, int64_t>> spans;
+  spans.reserve(pl.n_entries + pl.n_holes);
+  cp.deltas.clear();
+  for (int i = 0; i < pl.n_entries; ++i) {
+    const fcg_plan_entry_t &e = pl.entries[i];
+    if (e.seg_id < 0 || e.seg_id >= c.max_segments || !lib->segments[e.seg_id].live)
+      return fail(FCG_ERR_BAD_SEGMENT, "entry %d: unknown segment %d", i, e.seg_id);
+    const SegmentRec &s = lib->segments[e.seg_id];
+    if (e.n_tokens <= 0 || e.src_begin < 0 || (int64_t)e.src_begin + e.n_tokens > s.n_tokens || e.dst_offset < 0)
+      return fail(FCG_ERR_RANGE, "entry %d: source/destination range", i);
+    spans.push_back({e.dst_offset, (int64_t)e.dst_offset + e.n_tokens});
+    cp.deltas.push_back(e.dst_offset - s.orig_start - e.src_begin);
+  }
+  for (int i = 0; i < pl.n_holes; ++i) {
+    const fcg_hole_t &h = pl.holes[i];
+    if (h.n_tokens <= 0 || h.begin < 0) return fail(FCG_ERR_RANGE, "hole %d: range", i);
+    spans.push_back({h.begin, (int64_t)h.begin + h.n_tokens});
+  }
+  int64_t T = 0;
+  for (auto &s : spans) T = std::max(T, s.second);
+  const int64_t cap = pl.capacity_tokens > 0 ? pl.capacity_tokens : T;
+  if (T > cap) return fail(FCG_ERR_RANGE, "plan ends at %lld, beyond capacity_tokens %lld", (long long)T, (long long)cap);
+  if (cap > c.max_task_tokens) return fail(FCG_ERR_RANGE, "capacity %lld exceeds max_task_tokens %d", (long long)cap, c.max_task_tokens);
+  std::sort(spans.begin(), spans.end());
+  for (size_t i = 1; i < spans.size(); ++i)
+    if (spans[i].first < spans[i - 1].second) return fail(FCG_ERR_OVERLAP, "entries/holes overlap at token %lld", (long long)spans[i].first);
+  cp.capacity = (int32_t)cap;
+  cp.T = (int32_t)T;
+  cp.n_pages = (int32_t)((cap + c.page_size - 1) / c.page_size);
+  return FCG_OK;
+}
+}  // namespace
+
+fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_plans, void *stream_) {
+  if (!lib || !plans || n_plans <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty plan array");
+  const fcg_config_t &c = lib->cfg;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  std::vector<CheckedPlan> checked(n_plans);
+  int64_t need_pages = 0;
+  for (int i = 0; i < n_plans; ++i) {
+    for (int j = 0; j < i; ++j)
+      if (plans[j].task_id == plans[i].task_id) return fail(FCG_ERR_BAD_TASK, "task id %d repeated in the batch", plans[i].task_id);
+    fcg_status_t st = validate_plan(lib, plans[i], checked[i]);
+    if (st != FCG_OK) return st;
+    need_pages += checked[i].n_pages;
+  }
+  if (need_pages > (int64_t)lib->page_stack.size())
+    return fail(FCG_ERR_OUT_OF_PAGES, "need %lld pages, %zu free", (long long)need_pages, lib->page_stack.size());
+
+  // ---- build the plan blob (host) --------------------------------------------------------------
+  FCG_CUDA(cudaSetDevice(c.device));
+  BlobSlot *slot = nullptr;
+  fcg_status_t st = acquire_slot(lib, &slot);
+  if (st != FCG_OK) return st;
+  const int P = c.page_size, half = c.head_dim / 2;
+  int64_t n_entries_total = 0, n_chunks_total = 0, n_table_pages = 0;
+  for (int i = 0; i < n_plans; ++i) {
+    n_entries_total += plans[i].n_entries;
+    n_table_pages += checked[i].n_pages;
+    for (int e = 0; e < plans[i].n_entries; ++e) {
+      const fcg_plan_entry_t &pe = plans[i].entries[e];
+      n_chunks_total += (pe.dst_offset + pe.n_tokens - 1) / P - pe.dst_offset / P + 1;
+    }
+  }
+  BlobWriter bw(slot->host, BLOB_BYTES);
+  const uint64_t off_entries = bw.reserve(n_entries_total * sizeof(fcg::StitchEntryDev));
+  const uint64_t off_chunks = bw.reserve(n_chunks_total * sizeof(fcg::StitchChunkDev));
+  const uint64_t off_pages = bw.reserve(n_table_pages * sizeof(int32_t));
+  const uint64_t off_table = bw.reserve(0);
+  if (off_entries == UINT64_MAX || off_chunks == UINT64_MAX || off_pages == UINT64_MAX || off_table == UINT64_MAX)
+    return fail(FCG_ERR_OUT_OF_ARENA, "stitch plan blob exceeds %llu bytes", (unsigned long long)BLOB_BYTES);
+  auto *entries = reinterpret_cast<fcg::StitchEntryDev *>(slot->host + off_entries);
+  auto *chunks = reinterpret_cast<fcg::StitchChunkDev *>(slot->host + off_chunks);
+  auto *pages = reinterpret_cast<int32_t *>(slot->host + off_pages);
+  auto *table = reinterpret_cast<float4 *>(slot->host + off_table);
+  const uint64_t table_cap = (BLOB_BYTES - off_table) / sizeof(float4);
+
+  // page ids are taken from a COPY of the stack; committed only when everything has been enqueued
+  std::vector<int32_t> stack = lib->page_stack;
+  std::map<int32_t, int32_t> table_of_delta;
+  uint64_t table_used = 0;
+  int64_t ei = 0, ci = 0, pi = 0;
+  std::vector<int64_t> plan_page_base(n_plans);
+  for (int i = 0; i < n_plans; ++i) {
+    plan_page_base[i] = pi;
+    for (int k = 0; k < checked[i].n_pages; ++k) {
+      pages[pi++] = stack.back();
+      stack.pop_back();
+    }
+    const int32_t *ptab = pages + plan_page_base[i];
+    for (int e = 0; e < plans[i].n_entries; ++e, ++ei) {
+      const fcg_plan_entry_t &pe = plans[i].entries[e];
+      const SegmentRec &s = lib->segments[pe.seg_id];
+      const int32_t delta = checked[i].deltas[e];
+      fcg::StitchEntryDev &de = entries[ei];
+      de.k_src = (uint64_t)(uintptr_t)(lib->arena + s.offset);
+      de.v_src = (uint64_t)(uintptr_t)(lib->arena + s.offset + s.bytes / 2);
+      de.seg_n = s.n_tokens;
+      de.pad0 = de.pad1 = 0;
+      if (c.rope_mode == FCG_ROPE_NONE || delta == 0) {
+        de.table_off = -1;
+      } else {
+        auto it = table_of_delta.find(delta);
+        if (it != table_of_delta.end()) {
+          de.table_off = it->second;
+        } else {
+          if (table_used + half > table_cap)
+            return fail(FCG_ERR_OUT_OF_ARENA, "stitch plan blob exceeds %llu bytes (rope tables)", (unsigned long long)BLOB_BYTES);
+          de.table_off = (int32_t)table_used;
+          table_of_delta[delta] = de.table_off;
+          for (int j = 0; j < half; ++j) {
+            const double phi = (double)delta * lib->inv_freq[j];
+            const double cs = cos(phi), sn = sin(phi);
+            // hi part: 16 significant bits, so that (bf16 x hi) is exact in fp32; lo: the remainder
+            auto split = [](double x, float &hi, float &lo) {
+              float f = (float)x;
+              uint32_t b;
+              memcpy(&b, &f, 4);
+              b = (b + 0x80u) & 0xffffff00u;
+              memcpy(&hi, &b, 4);
+              lo = (float)(x - (double)hi);
+            };
+            float4 t;
+            split(cs, t.x, t.y);
+            split(sn, t.z, t.w);
+            table[table_used + j] = t;
+          }
+          table_used += half;
+        }
+      }
+      // chunks: one per destination page touched
+      int32_t done = 0;
+      while (done < pe.n_tokens) {
+        const int32_t dst = pe.dst_offset + done;
+        const int32_t slot0 = dst % P;
+        const int32_t n = std::min(P - slot0, pe.n_tokens - done);
+        fcg::StitchChunkDev &dc = chunks[ci++];
+        dc.entry = (int32_t)ei;
+        dc.page = ptab[dst / P];
+        dc.src_tok = pe.src_begin + done;
+        dc.slot_ntok = slot0 | (n << 16);
+        done += n;
+      }
+    }
+  }
+  const uint64_t blob_used = off_table + table_used * sizeof(float4);
+
+  // ---- enqueue: blob, page tables, kernel -----------------------------------------------------
+  FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, blob_used, cudaMemcpyHostToDevice, stream));
+  for (int i = 0; i < n_plans; ++i) {
+    int32_t *dst = lib->tables() + (int64_t)plans[i].task_id * lib->pages_per_task;
+    FCG_CUDA(cudaMemcpyAsync(dst, slot->dev + off_pages + plan_page_base[i] * sizeof(int32_t),
+                             (size_t)checked[i].n_pages * sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
+  }
+  fcg::StitchParams sp;
+  sp.entries = reinterpret_cast<const fcg::StitchEntryDev *>(slot->dev + off_entries);
+  sp.chunks = reinterpret_cast<const fcg::StitchChunkDev *>(slot->dev + off_chunks);
+  sp.table = reinterpret_cast<const float4 *>(slot->dev + off_table);
+  sp.k_pool = lib->k_pool();
+  sp.v_pool = lib->v_pool();
+  sp.n_chunks = (int32_t)n_chunks_total;
+  sp.n_layers = c.n_layers;
+  sp.n_kv_heads = c.n_kv_heads;
+  sp.page_size = P;
+  sp.n_pages = c.n_pages;
+  if (n_chunks_total > 0) {
+    FCG_CUDA(fcg::launch_stitch(sp, c.head_dim, stream));
+    lib->stats.stitch_launches++;
+  }
+  FCG_CUDA(cudaEventRecord(slot->ev, stream));
+  slot->in_flight = true;
+
+  // ---- commit ------------------------------------------------------------------------------------
+  lib->page_stack.swap(stack);
+  for (int i = 0; i < n_plans; ++i) {
+    TaskRec &t = lib->tasks[plans[i].task_id];
+    t.live = true;
+    t.capacity = checked[i].capacity;
+    t.n_tokens = checked[i].T;
+    t.pages.assign(pages + plan_page_base[i], pages + plan_page_base[i] + checked[i].n_pages);
+    t.filled.assign(t.capacity, 0);
+    for (int e = 0; e < plans[i].n_entries; ++e) {
+      const fcg_plan_entry_t &pe = plans[i].entries[e];
+      std::fill(t.filled.begin() + pe.dst_offset, t.filled.begin() + pe.dst_offset + pe.n_tokens, (uint8_t)1);
+    }
+    t.filled_prefix = 0;
+    while (t.filled_prefix < t.capacity && t.filled[t.filled_prefix]) t.filled_prefix++;
+    lib->n_tasks_live++;
+  }
+  return FCG_OK;
+}
+
+// ------------------------------------------------------------------------------------ S4 + S5/S6
+namespace {
+
+// choose the number of KV splits for `base` CTAs per split so that waves on the GPU are well filled
+// without paying much for fp32 partials.
+int choose_splits(int64_t base_ctas, int tiles, int rows, int head_dim, int ctas_per_sm) {
+  if (tiles <= 1) return 1;
+  const double slots = (double)N_SMS * ctas_per_sm;
+  double best_cost = 1e30;
+  int best = 1;
+  const int max_s = std::min(tiles, 64);
+  for (int s = 1; s <= max_s; ++s) {
+    const int tiles_per = (tiles + s - 1) / s;
+    const int s_eff = (tiles + tiles_per - 1) / tiles_per;
+    if (s_eff != s) continue;
+    const double ctas = (double)base_ctas * s;
+    const double waves = ceil(ctas / slots);
+    // time ~ waves * (tiles per CTA) in units of one tile of streaming, plus partial traffic
+    const double kv_bytes = (double)tiles_per * KV_TILE * head_dim * 4.0;
+    const double part_bytes = s > 1 ? 2.0 * rows * (head_dim + 2) * 4.0 : 0.0;
+    const double per_cta = kv_bytes + part_bytes + 6000.0 /* fixed per-CTA latency in byte-equivalents */;
+    const double cost = waves * per_cta;
+    if (cost < best_cost * 0.999) {
+      best_cost = cost;
+      best = s;
+    }
+  }
+  return best;
+}
+
+struct PatchCall {
+  const int32_t *task_ids;
+  const int32_t *n_per_task;
+  int32_t n_tasks;
+  int32_t layer_begin, n_layers;
+  const void *q, *k, *v;
+  const int32_t *positions;
+  void *out;
+  cudaStream_t stream;
+};
+
+fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
+  const fcg_config_t &c = lib->cfg;
+  if (!pc.q || !pc.k || !pc.v || !pc.out || !pc.positions || !pc.task_ids || !pc.n_per_task || pc.n_tasks <= 0)
+    return fail(FCG_ERR_INVALID_ARG, "NULL / empty argument");
+  if (pc.layer_begin < 0 || pc.n_layers <= 0 || pc.layer_begin + pc.n_layers > c.n_layers)
+    return fail(FCG_ERR_INVALID_ARG, "layer range [%d, %d) outside [0, %d)", pc.layer_begin, pc.layer_begin + pc.n_layers, c.n_layers);
+  // ---- validate every task before touching anything ------------------------------------------
+  int64_t n_total = 0;
+  for (int t = 0; t < pc.n_tasks; ++t) {
+    const int32_t id = pc.task_ids[t];
+    if (id < 0 || id >= c.max_tasks || !lib->tasks[id].live) return fail(FCG_ERR_BAD_TASK, "unknown task %d", id);
+    for (int u = 0; u < t; ++u)
+      if (pc.task_ids[u] == id) return fail(FCG_ERR_BAD_TASK, "task %d repeated in the batch", id);
+    const int32_t n = pc.n_per_task[t];
+    if (n <= 0) return fail(FCG_ERR_INVALID_ARG, "task %d: n must be > 0", id);
+    const int32_t *pos = pc.positions + n_total;
+    for (int i = 1; i < n; ++i)
+      if (pos[i] <= pos[i - 1]) return fail(FCG_ERR_INVALID_ARG, "task %d: positions must be strictly increasing", id);
+    const TaskRec &tr = lib->tasks[id];
+    if (pos[0] < 0 || pos[n - 1] >= tr.capacity) return fail(FCG_ERR_RANGE, "task %d: position outside capacity %d", id, tr.capacity);
+    // every x <= pos[n-1] must be filled by earlier work or by this call
+    int pi = 0;
+    for (int32_t x = tr.filled_prefix; x <= pos[n - 1]; ++x) {
+      while (pi < n && pos[pi] < x) ++pi;
+      if (!tr.filled[x] && !(pi < n && pos[pi] == x))
+        return fail(FCG_ERR_UNFILLED, "task %d: position %d is visible to a patch query but was never filled", id, x);
+    }
+    n_total += n;
+  }
+  if (n_total > (1 << 20)) return fail(FCG_ERR_INVALID_ARG, "too many patch tokens in one call");
+
+  // ---- blob: positions, per-token table offsets / split counts, task descriptors --------------
+  FCG_CUDA(cudaSetDevice(c.device));
+  BlobSlot *slot = nullptr;
+  fcg_status_t st = acquire_slot(lib, &slot);
+  if (st != FCG_OK) return st;
+  BlobWriter bw(slot->host, BLOB_BYTES);
+  const uint64_t off_pos = bw.reserve(n_total * 4), off_toff = bw.reserve(n_total * 4), off_tspl = bw.reserve(n_total * 4);
+  const uint64_t off_tasks = bw.reserve((uint64_t)pc.n_tasks * sizeof(fcg::AttnTaskDev));
+  if (off_pos == UINT64_MAX || off_toff == UINT64_MAX || off_tspl == UINT64_MAX || off_tasks == UINT64_MAX)
+    return fail(FCG_ERR_OUT_OF_ARENA, "patch blob exceeds %llu bytes", (unsigned long long)BLOB_BYTES);
+  auto *h_pos = reinterpret_cast<int32_t *>(slot->host + off_pos);
+  auto *h_toff = reinterpret_cast<int32_t *>(slot->host + off_toff);
+  auto *h_tspl = reinterpret_cast<int32_t *>(slot->host + off_tspl);
+  auto *h_tasks = reinterpret_cast<fcg::AttnTaskDev *>(slot->host + off_tasks);
+  memcpy(h_pos, pc.positions, (size_t)n_total * 4);
+
+  const int G = c.n_q_heads / c.n_kv_heads;
+  int max_rows = 0;
+  for (int t = 0; t < pc.n_tasks; ++t) max_rows = std::max(max_rows, pc.n_per_task[t] * G);
+  const int rows_per_cta = max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64);
+  const int max_row_groups = (max_rows + rows_per_cta - 1) / rows_per_cta;
+  const int ctas_per_sm = fcg::attn_split_ctas_per_sm(c.head_dim);
+  int max_splits = 1;
+  int64_t tok_off = 0;
+  for (int t = 0; t < pc.n_tasks; ++t) {
+    const int32_t n = pc.n_per_task[t];
+    const int32_t kv_len = pc.positions[tok_off + n - 1] + 1;
+    const int tiles = (kv_len + KV_TILE - 1) / KV_TILE;
+    const int rg = (n * G + rows_per_cta - 1) / rows_per_cta;
+    const int64_t base = (int64_t)rg * c.n_kv_heads * pc.n_layers * pc.n_tasks;
+    const int ns = choose_splits(base, tiles, std::min(n * G, rows_per_cta), c.head_dim, ctas_per_sm);
+    const int tiles_per = (tiles + ns - 1) / ns;
+    fcg::AttnTaskDev &d = h_tasks[t];
+    d.table_off = pc.task_ids[t] * lib->pages_per_task;
+    d.n = n;
+    d.tok_off = (int32_t)tok_off;
+    d.kv_len = kv_len;
+    d.n_splits = ns;
+    d.split_len = tiles_per * KV_TILE;
+    d.pad0 = d.pad1 = 0;
+    max_splits = std::max(max_splits, ns);
+    for (int i = 0; i < n; ++i) {
+      h_toff[tok_off + i] = d.table_off;
+      h_tspl[tok_off + i] = ns;
+    }
+    tok_off += n;
+  }
+  // partials live at the start of the scratch area
+  const uint64_t part_rows = (uint64_t)pc.n_layers * max_splits * n_total * c.n_q_heads;
+  const uint64_t part_o_bytes = max_splits > 1 ? align_up(part_rows * c.head_dim * 4) : 0;
+  const uint64_t part_ml_bytes = max_splits > 1 ? align_up(part_rows * 2 * 4) : 0;
+  if (part_o_bytes + part_ml_bytes > lib->scratch_bytes)
+    return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for %d-way split partials (%llu bytes)", max_splits,
+                (unsigned long long)(part_o_bytes + part_ml_bytes));
+
+  FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, bw.used, cudaMemcpyHostToDevice, pc.stream));
+
+  fcg::ScatterParams sp;
+  sp.k_new = static_cast<const uint16_t *>(pc.k);
+  sp.v_new = static_cast<const uint16_t *>(pc.v);
+  sp.k_pool = lib->k_pool();
+  sp.v_pool = lib->v_pool();
+  sp.tables = lib->tables();
+  sp.positions = reinterpret_cast<const int32_t *>(slot->dev + off_pos);
+  sp.tok_table_off = reinterpret_cast<const int32_t *>(slot->dev + off_toff);
+  sp.n_layers = pc.n_layers;
+  sp.layer_begin = pc.layer_begin;
+  sp.n_total = (int32_t)n_total;
+  sp.n_kv_heads = c.n_kv_heads;
+  sp.head_dim = c.head_dim;
+  sp.page_size = c.page_size;
+  sp.n_pages = c.n_pages;
+  FCG_CUDA(fcg::launch_scatter(sp, pc.stream));
+  lib->stats.scatter_launches++;
+
+  fcg::AttnParams ap;
+  ap.q = static_cast<const uint16_t *>(pc.q);
+  ap.out = static_cast<uint16_t *>(pc.out);
+  ap.k_pool = lib->k_pool();
+  ap.v_pool = lib->v_pool();
+  ap.tables = lib->tables();
+  ap.positions = sp.positions;
+  ap.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(slot->dev + off_tasks);
+  ap.tok_splits = reinterpret_cast<const int32_t *>(slot->dev + off_tspl);
+  ap.part_o = reinterpret_cast<float *>(lib->arena + lib->scratch_off);
+  ap.part_ml = reinterpret_cast<float *>(lib->arena + lib->scratch_off + part_o_bytes);
+  ap.n_total = (int32_t)n_total;
+  ap.n_layers = pc.n_layers;
+  ap.layer_begin = pc.layer_begin;
+  ap.n_q_heads = c.n_q_heads;
+  ap.n_kv_heads = c.n_kv_heads;
+  ap.group = G;
+  ap.page_size = c.page_size;
+  ap.n_tasks = pc.n_tasks;
+  ap.max_splits = max_splits;
+  ap.max_row_groups = max_row_groups;
+  ap.n_pages = c.n_pages;
+  ap.scale_log2 = (float)(1.4426950408889634 / sqrt((double)c.head_dim));
+  FCG_CUDA(fcg::launch_attn_split(ap, c.head_dim, rows_per_cta, pc.stream));
+  lib->stats.attn_split_launches++;
+  lib->stats.last_attn_path = 1;
+  lib->stats.last_attn_splits = max_splits;
+  if (max_splits > 1) {
+    FCG_CUDA(fcg::launch_attn_combine(ap, c.head_dim, pc.stream));
+    lib->stats.attn_combine_launches++;
+  }
+  FCG_CUDA(cudaEventRecord(slot->ev, pc.stream));
+  slot->in_flight = true;
+
+  // ---- commit fill state ---------------------------------------------------------------------
+  tok_off = 0;
+  for (int t = 0; t < pc.n_tasks; ++t) {
+    TaskRec &tr = lib->tasks[pc.task_ids[t]];
+    const int32_t n = pc.n_per_task[t];
+    for (int i = 0; i < n; ++i) tr.filled[pc.positions[tok_off + i]] = 1;
+    while (tr.filled_prefix < tr.capacity && tr.filled[tr.filled_prefix]) tr.filled_prefix++;
+    tr.n_tokens = std::max(tr.n_tokens, pc.positions[tok_off + n - 1] + 1);
+    tok_off += n;
+  }
+  return FCG_OK;
+}
+
+}  // namespace
+
+fcg_status_t fcg_patch(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers, const void *q,
+                       const void *k, const void *v, const int32_t *positions, int32_t n, void *out, void *stream) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  PatchCall pc{&task_id, &n, 1, layer_begin, n_layers, q, k, v, positions, out, static_cast<cudaStream_t>(stream)};
+  return patch_common(lib, pc);
+}
+
+fcg_status_t fcg_patch_batch(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task, int32_t n_tasks,
+                             int32_t layer_begin, int32_t n_layers, const void *q, const void *k, const void *v,
+                             const int32_t *positions, void *out, void *stream) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  PatchCall pc{task_ids, n_per_task, n_tasks, layer_begin, n_layers, q, k, v, positions, out, static_cast<cudaStream_t>(stream)};
+  return patch_common(lib, pc);
+}
+
+fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers, const void *q,
+                            const void *k, const void *v, const int32_t *positions, int32_t n, void *out, void *stream_) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  if (!q || !k || !v || !out || n <= 0 || n_layers <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty argument");
+  const fcg_config_t &c = lib->cfg;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  const uint64_t q_bytes = (uint64_t)n_layers * n * c.n_q_heads * c.head_dim * 2;
+  const uint64_t kv_bytes = (uint64_t)n_layers * n * c.n_kv_heads * c.head_dim * 2;
+  const uint64_t need = 2 * align_up(q_bytes) + 2 * align_up(kv_bytes);
+  // staging sits at the END of the scratch area; split partials grow from its start
+  if (need > lib->scratch_bytes / 2) return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small to stage %llu bytes", (unsigned long long)need);
+  unsigned char *base = lib->arena + lib->scratch_off + lib->scratch_bytes - need;
+  unsigned char *dq = base, *dk = dq + align_up(q_bytes), *dv = dk + align_up(kv_bytes), *dout = dv + align_up(kv_bytes);
+  FCG_CUDA(cudaSetDevice(c.device));
+  FCG_CUDA(cudaMemcpyAsync(dq, q, q_bytes, cudaMemcpyHostToDevice, stream));
+  FCG_CUDA(cudaMemcpyAsync(dk, k, kv_bytes, cudaMemcpyHostToDevice, stream));
+  FCG_CUDA(cudaMemcpyAsync(dv, v, kv_bytes, cudaMemcpyHostToDevice, stream));
+  // partials must not collide with the staging area: temporarily shrink the scratch
+  const uint64_t saved = lib->scratch_bytes;
+  lib->scratch_bytes = saved - need;
+  PatchCall pc{&task_id, &n, 1, layer_begin, n_layers, dq, dk, dv, positions, dout, stream};
+  fcg_status_t st = patch_common(lib, pc);
+  lib->scratch_bytes = saved;
+  if (st != FCG_OK) return st;
+  FCG_CUDA(cudaMemcpyAsync(out, dout, q_bytes, cudaMemcpyDeviceToHost, stream));
+  return FCG_OK;
+}
+
+// ------------------------------------------------------------------------------- task utilities
+fcg_status_t fcg_task_page_table(fcg_library_t *lib, int32_t task_id, const int32_t **dev_table, int32_t *n_pages,
+                                 int32_t *n_tokens) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  if (task_id < 0 || task_id >= lib->cfg.max_tasks || !lib->tasks[task_id].live) return fail(FCG_ERR_BAD_TASK, "unknown task %d", task_id);
+  const TaskRec &t = lib->tasks[task_id];
+  if (dev_table) *dev_table = lib->tables() + (int64_t)task_id * lib->pages_per_task;
+  if (n_pages) *n_pages = (int32_t)t.pages.size();
+  if (n_tokens) *n_tokens = t.n_tokens;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_task_page_table_host(fcg_library_t *lib, int32_t task_id, int32_t *out, int32_t cap, int32_t *n_pages) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  if (task_id < 0 || task_id >= lib->cfg.max_tasks || !lib->tasks[task_id].live) return fail(FCG_ERR_BAD_TASK, "unknown task %d", task_id);
+  const TaskRec &t = lib->tasks[task_id];
+  if (n_pages) *n_pages = (int32_t)t.pages.size();
+  if (out && cap > 0) memcpy(out, t.pages.data(), sizeof(int32_t) * std::min<size_t>(cap, t.pages.size()));
+  return FCG_OK;
+}
+
+fcg_status_t fcg_task_release(fcg_library_t *lib, int32_t task_id) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  if (task_id < 0 || task_id >= lib->cfg.max_tasks || !lib->tasks[task_id].live) return fail(FCG_ERR_BAD_TASK, "unknown task %d", task_id);
+  TaskRec &t = lib->tasks[task_id];
+  for (auto it = t.pages.rbegin(); it != t.pages.rend(); ++it) lib->page_stack.push_back(*it);
+  t = TaskRec();
+  lib->n_tasks_live--;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_task_read(fcg_library_t *lib, int32_t task_id, int32_t layer, int32_t begin, int32_t n, void *k_out,
+                           void *v_out, void *stream) {
+  if (!lib || !k_out || !v_out) return fail(FCG_ERR_INVALID_ARG, "NULL argument");
+  const fcg_config_t &c = lib->cfg;
+  if (task_id < 0 || task_id >= c.max_tasks || !lib->tasks[task_id].live) return fail(FCG_ERR_BAD_TASK, "unknown task %d", task_id);
+  const TaskRec &t = lib->tasks[task_id];
+  if (layer < 0 || layer >= c.n_layers) return fail(FCG_ERR_INVALID_ARG, "layer out of range");
+  if (begin < 0 || n <= 0 || (int64_t)begin + n > t.capacity) return fail(FCG_ERR_RANGE, "token range outside capacity");
+  fcg::ReadParams rp;
+  rp.k_pool = lib->k_pool();
+  rp.v_pool = lib->v_pool();
+  rp.k_out = static_cast<uint16_t *>(k_out);
+  rp.v_out = static_cast<uint16_t *>(v_out);
+  rp.table = lib->tables() + (int64_t)task_id * lib->pages_per_task;
+  rp.layer = layer;
+  rp.begin = begin;
+  rp.n = n;
+  rp.n_kv_heads = c.n_kv_heads;
+  rp.head_dim = c.head_dim;
+  rp.page_size = c.page_size;
+  rp.n_pages = c.n_pages;
+  FCG_CUDA(cudaSetDevice(c.device));
+  FCG_CUDA(fcg::launch_task_read(rp, static_cast<cudaStream_t>(stream)));
+  lib->stats.read_launches++;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_pool_info(fcg_library_t *lib, fcg_pool_info_t *out) {
+  if (!lib || !out) return fail(FCG_ERR_INVALID_ARG, "NULL argument");
+  out->k_pool_offset = lib->k_pool_off;
+  out->v_pool_offset = lib->v_pool_off;
+  out->pool_bytes = lib->pool_bytes;
+  out->page_table_offset = lib->table_off;
+  out->workspace_offset = lib->ws_off;
+  out->segments_offset = lib->seg_off;
+  uint64_t fr = 0;
+  for (auto &r : lib->seg_free) fr += r.bytes;
+  out->segments_bytes_free = fr;
+  out->n_pages = lib->cfg.n_pages;
+  out->n_pages_free = (uint32_t)lib->page_stack.size();
+  out->n_segments_live = lib->n_segments_live;
+  out->n_tasks_live = lib->n_tasks_live;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_stats(fcg_library_t *lib, fcg_stats_t *out) {
+  if (!lib || !out) return fail(FCG_ERR_INVALID_ARG, "NULL argument");
+  *out = lib->stats;
+  return FCG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,109 @@
+// Internal declarations shared by the host side (fcg_api.cu) and the kernels of libfcg.so.
+// Not part of the public ABI (that is include/fcg.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace fcg {
+
+// ---------------------------------------------------------------------------------------------
+// S3: fused gather + RoPE-shift.  One work item ("chunk") = the tokens of one plan entry that land
+// in one destination page; the kernel grid is (chunk, layer) and warps stride over kv heads.
+// ---------------------------------------------------------------------------------------------
+struct StitchEntryDev {  // 32 B
+  uint64_t k_src;        // device address of the segment's K  [L][Hkv][seg_n][D]
+  uint64_t v_src;        // device address of the segment's V
+  int32_t seg_n;         // tokens in the segment (= head stride in tokens)
+  int32_t table_off;     // first float4 of this entry's rope table; -1 -> bit copy (delta 0 / rope off)
+  int32_t pad0, pad1;
+};
+
+struct StitchChunkDev {  // 16 B
+  int32_t entry;         // index into the entry array
+  int32_t page;          // physical destination page
+  int32_t src_tok;       // token index inside the segment of the chunk's first token
+  int32_t slot_ntok;     // first slot in the page | (number of tokens << 16)
+};
+
+struct StitchParams {
+  const StitchEntryDev *entries;
+  const StitchChunkDev *chunks;
+  const float4 *table;   // per (entry, j): {c_hi, c_lo, s_hi, s_lo}; c_hi/s_hi have <= 16 significant bits
+  uint16_t *k_pool;
+  uint16_t *v_pool;
+  int32_t n_chunks, n_layers, n_kv_heads, page_size;
+  uint32_t n_pages;
+};
+
+cudaError_t launch_stitch(const StitchParams &p, int head_dim, cudaStream_t stream);
+
+// ---------------------------------------------------------------------------------------------
+// S1 (register copy), S4 (scatter), task read
+// ---------------------------------------------------------------------------------------------
+struct RegisterParams {
+  const uint16_t *k_src, *v_src;
+  uint16_t *k_dst, *v_dst;   // contiguous [L][Hkv][n][D]
+  int64_t s_layer, s_head, s_tok;  // source strides in elements
+  int32_t n_layers, n_kv_heads, n_tokens, head_dim;
+};
+cudaError_t launch_register_copy(const RegisterParams &p, cudaStream_t stream);
+
+struct ScatterParams {
+  const uint16_t *k_new, *v_new;  // [n_layers][n_total][Hkv][D]
+  uint16_t *k_pool, *v_pool;
+  const int32_t *tables;          // page-table region
+  const int32_t *positions;       // [n_total]
+  const int32_t *tok_table_off;   // [n_total] page-table offset of the token's task
+  int32_t n_layers, layer_begin, n_total, n_kv_heads, head_dim, page_size;
+  uint32_t n_pages;
+};
+cudaError_t launch_scatter(const ScatterParams &p, cudaStream_t stream);
+
+struct ReadParams {
+  const uint16_t *k_pool, *v_pool;
+  uint16_t *k_out, *v_out;        // [Hkv][n][D]
+  const int32_t *table;
+  int32_t layer, begin, n, n_kv_heads, head_dim, page_size;
+  uint32_t n_pages;
+};
+cudaError_t launch_task_read(const ReadParams &p, cudaStream_t stream);
+
+// ---------------------------------------------------------------------------------------------
+// S5 / S6: patch attention
+// ---------------------------------------------------------------------------------------------
+struct AttnTaskDev {     // 32 B, one per task of a (batched) patch call
+  int32_t table_off;     // int32 index of the task's page table inside the table region
+  int32_t n;             // patch tokens of this task
+  int32_t tok_off;       // first row of this task in q/k/v/out/positions
+  int32_t kv_len;        // positions[n-1] + 1
+  int32_t n_splits;      // KV splits for this task (<= max_splits)
+  int32_t split_len;     // tokens per split, multiple of the KV tile
+  int32_t pad0, pad1;
+};
+
+struct AttnParams {
+  const uint16_t *q;         // [n_layers][n_total][Hq][D]
+  uint16_t *out;             // same shape
+  const uint16_t *k_pool, *v_pool;
+  const int32_t *tables;
+  const int32_t *positions;  // [n_total]
+  const AttnTaskDev *tasks;
+  const int32_t *tok_splits; // [n_total] n_splits of the token's task (combine kernel)
+  float *part_o;             // [n_layers][max_splits][n_total][Hq][D]   unnormalised
+  float *part_ml;            // [n_layers][max_splits][n_total][Hq][2]   (m in log2 units, l)
+  int32_t n_total, n_layers, layer_begin, n_q_heads, n_kv_heads, group, page_size, n_tasks;
+  int32_t max_splits, max_row_groups;
+  uint32_t n_pages;
+  float scale_log2;          // log2(e) / sqrt(D)
+};
+
+// split-KV warp-MMA (mma.sync m16n8k16) path; rows_per_cta in {16, 32, 64}
+cudaError_t launch_attn_split(const AttnParams &p, int head_dim, int rows_per_cta, cudaStream_t stream);
+cudaError_t launch_attn_combine(const AttnParams &p, int head_dim, cudaStream_t stream);
+int attn_split_ctas_per_sm(int head_dim);
+
+// tcgen05 / TMEM path (128-row tiles); returns cudaErrorNotSupported if not built
+cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, cudaStream_t stream);
+
+}  // namespace fcg

@@ -1,0 +1,151 @@
+// S3: fused gather + RoPE-shift (cache-stitching, Eq. 4).
+//
+// HBM-bound streaming kernel: every K/V byte of a stitched segment is read once and written once.
+// Work item = (chunk, layer): the tokens of one plan entry that land in one destination page, for
+// one layer; the 4 warps of a CTA stride over the kv heads.  A lane owns one 16-byte column of the
+// low half of a key row AND the matching 16-byte column of the high half, i.e. 8 complete rotation
+// pairs (j, j + D/2) -- no shuffles.  The delta is constant per plan entry, so cos/sin depend only on
+// (entry, j): 8 table entries per lane, loaded once per CTA.  No trigonometry on the device.
+//
+// Arithmetic (fp32 registers, error-free split of the table):
+//   cos = c_hi + c_lo, sin = s_hi + s_lo with c_hi, s_hi carrying <= 16 significant bits, so the
+//   products of an 8-bit bf16 input with c_hi / s_hi are EXACT in fp32.
+//     x = fma(a, c_hi, -(b * s_hi))        one rounding of the exact a*c_hi - b*s_hi  (no cancellation loss)
+//     x += fma(a, c_lo, -(b * s_lo))       correction, ~2^-16 of the operands
+//   and likewise y = b cos + a sin.  The fp32 result is within ~2^-23 relative of the exact value;
+//   RNE to bf16 then differs from the fp64 oracle by at most 1 bf16 ulp (double rounding only).
+#include <cuda_bf16.h>
+
+#include "fcg_internal.h"
+
+namespace fcg {
+namespace {
+
+__device__ __forceinline__ uint4 ldg_stream(const void *p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+
+__device__ __forceinline__ void stg_16(void *p, const uint4 &v) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+               "r"(v.w)
+               : "memory");
+}
+
+__device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
+
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  __nv_bfloat162 r = __floats2bfloat162_rn(lo, hi);  // .x = lo (low 16 bits), .y = hi
+  return *reinterpret_cast<uint32_t *>(&r);
+}
+
+// rotate one pair: (a, b) -> (a cos - b sin, b cos + a sin)
+__device__ __forceinline__ void rot_pair(float a, float b, const float4 &t, float &x, float &y) {
+  // t = {c_hi, c_lo, s_hi, s_lo}
+  const float bs = __fmul_rn(b, t.z);                 // exact
+  const float as = __fmul_rn(a, t.z);                 // exact
+  const float x0 = __fmaf_rn(a, t.x, -bs);            // round(a*c_hi - b*s_hi)
+  const float y0 = __fmaf_rn(b, t.x, as);             // round(b*c_hi + a*s_hi)
+  const float xr = __fmaf_rn(a, t.y, -__fmul_rn(b, t.w));
+  const float yr = __fmaf_rn(b, t.y, __fmul_rn(a, t.w));
+  x = __fadd_rn(x0, xr);
+  y = __fadd_rn(y0, yr);
+}
+
+__device__ __forceinline__ void rot_word(uint32_t wa, uint32_t wb, const float4 &t0, const float4 &t1, uint32_t &oa,
+                                         uint32_t &ob) {
+  float x0, y0, x1, y1;
+  rot_pair(bf16_lo(wa), bf16_lo(wb), t0, x0, y0);
+  rot_pair(bf16_hi(wa), bf16_hi(wb), t1, x1, y1);
+  oa = pack_bf16(x0, x1);
+  ob = pack_bf16(y0, y1);
+}
+
+template <int D>
+__global__ void __launch_bounds__(128, 4) stitch_kernel(const StitchParams p) {
+  constexpr int LPT = D / 16;      // lanes per token: one 16-byte column of each half per lane
+  constexpr int TPS = 32 / LPT;    // tokens per warp step
+  constexpr int STEPS = 4;         // steps in flight per batch (4 x 64 B per lane)
+  constexpr int ROW_BYTES = D * 2;
+
+  const StitchChunkDev ch = p.chunks[blockIdx.x];
+  const StitchEntryDev en = p.entries[ch.entry];
+  const int layer = blockIdx.y;
+  const int lane = threadIdx.x & 31;
+  const int warp = threadIdx.x >> 5;
+  const int col = lane % LPT;
+  const int tl = lane / LPT;
+  const int slot0 = ch.slot_ntok & 0xffff;
+  const int ntok = ch.slot_ntok >> 16;
+  const bool rotate = en.table_off >= 0;
+
+  float4 tab[8];
+  if (rotate) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) tab[i] = __ldg(p.table + en.table_off + col * 8 + i);
+  }
+
+  const int Hkv = p.n_kv_heads;
+  for (int g = warp; g < Hkv; g += 4) {
+    const size_t src_row = ((size_t)layer * Hkv + g) * (size_t)en.seg_n + (size_t)ch.src_tok;
+    const size_t dst_row = (((size_t)layer * p.n_pages + (size_t)ch.page) * Hkv + g) * (size_t)p.page_size + slot0;
+    const char *ksrc = reinterpret_cast<const char *>(en.k_src) + src_row * ROW_BYTES + col * 16;
+    const char *vsrc = reinterpret_cast<const char *>(en.v_src) + src_row * ROW_BYTES + col * 16;
+    char *kdst = reinterpret_cast<char *>(p.k_pool) + dst_row * ROW_BYTES + col * 16;
+    char *vdst = reinterpret_cast<char *>(p.v_pool) + dst_row * ROW_BYTES + col * 16;
+
+    for (int t0 = 0; t0 < ntok; t0 += TPS * STEPS) {
+      uint4 klo[STEPS], khi[STEPS], vlo[STEPS], vhi[STEPS];
+#pragma unroll
+      for (int s = 0; s < STEPS; ++s) {
+        const int t = t0 + s * TPS + tl;
+        if (t < ntok) {
+          const size_t off = (size_t)t * ROW_BYTES;
+          klo[s] = ldg_stream(ksrc + off);
+          khi[s] = ldg_stream(ksrc + off + D);
+          vlo[s] = ldg_stream(vsrc + off);
+          vhi[s] = ldg_stream(vsrc + off + D);
+        }
+      }
+#pragma unroll
+      for (int s = 0; s < STEPS; ++s) {
+        const int t = t0 + s * TPS + tl;
+        if (t < ntok) {
+          const size_t off = (size_t)t * ROW_BYTES;
+          uint4 olo = klo[s], ohi = khi[s];
+          if (rotate) {
+            rot_word(klo[s].x, khi[s].x, tab[0], tab[1], olo.x, ohi.x);
+            rot_word(klo[s].y, khi[s].y, tab[2], tab[3], olo.y, ohi.y);
+            rot_word(klo[s].z, khi[s].z, tab[4], tab[5], olo.z, ohi.z);
+            rot_word(klo[s].w, khi[s].w, tab[6], tab[7], olo.w, ohi.w);
+          }
+          stg_16(kdst + off, olo);
+          stg_16(kdst + off + D, ohi);
+          stg_16(vdst + off, vlo[s]);
+          stg_16(vdst + off + D, vhi[s]);
+        }
+      }
+    }
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_stitch(const StitchParams &p, int head_dim, cudaStream_t stream) {
+  if (p.n_chunks <= 0) return cudaSuccess;
+  dim3 grid((unsigned)p.n_chunks, (unsigned)p.n_layers, 1);
+  dim3 block(128, 1, 1);
+  if (head_dim == 128)
+    stitch_kernel<128><<<grid, block, 0, stream>>>(p);
+  else if (head_dim == 64)
+    stitch_kernel<64><<<grid, block, 0, stream>>>(p);
+  else
+    return cudaErrorInvalidValue;
+  return cudaGetLastError();
+}
+
+}  // namespace fcg
