@@ -1,0 +1,386 @@
+"""bench.py -- one "step" = one pass of the whole grafting hot path (S2 plan -> S3 fused gather +
+RoPE-shift -> S4 scatter -> S5/S6 patch attention, all layers) over one synthetic batch.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl reference]
+
+Prints ONE JSON line (rank 0).  metric = BASELINE.json's: graft latency (ms_per_step) and achieved
+algorithmic HBM GB/s (value) against the roofline on a B200.  Multi-GPU: the path shards by task
+(independent grafting tasks, no collective): every rank grafts its own copy of the workload
+("scaling": "weak").  --impl reference times the CPU oracle (the only reference this paper has).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2606_13097_b200 import synth  # noqa: E402
+
+METRIC = "graft latency ms + HBM GB/s (stitch+RoPE shift, patch attn) vs roofline, 1 B200"
+FALLBACK_HBM_GBS = 6650.0          # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json, torch copy_ read+write)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# --------------------------------------------------------------------------------------------------
+# algorithmic bytes
+# --------------------------------------------------------------------------------------------------
+def stitch_bytes(cfg, wl) -> int:
+    """every stitched K/V byte is read once and written once: T_stitched * L * Hkv * D * 2 B * 2 (K,V) * 2 (r+w)."""
+    return wl.stitched_tokens * cfg.kv_bytes_per_token * 2
+
+
+def attn_bytes(cfg, wl) -> int:
+    """visible K+V read once per kv head: sum over tasks of L * kv_len * Hkv * D * 4 B (q/out/partials < 1 %)."""
+    total = 0
+    for t in wl.tasks:
+        kv_len = int(t.positions[-1]) + 1
+        total += cfg.n_layers * kv_len * cfg.n_kv_heads * cfg.head_dim * 4
+    return total
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])), smax.append(float(r[2]))
+            except Exception:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------------------------------
+# the CUDA arm
+# --------------------------------------------------------------------------------------------------
+def build_library(cfg, wl, seed, device_index):
+    from paper_2606_13097_b200 import binding
+    total_pages = sum(-(-t.capacity // cfg.page_size) for t in wl.tasks)
+    seg_tokens = int(wl.seg_lens.sum())
+    lib = binding.FcgLibrary(n_layers=cfg.n_layers, n_q_heads=cfg.n_q_heads, n_kv_heads=cfg.n_kv_heads,
+                             head_dim=cfg.head_dim, page_size=cfg.page_size, rope_base=cfg.rope_base,
+                             max_segments=cfg.n_segments, max_tasks=max(cfg.n_tasks, 1),
+                             max_task_tokens=max(t.capacity for t in wl.tasks), n_pages=total_pages + 16,
+                             workspace_bytes=1 << 30, segment_tokens=seg_tokens, device=device_index)
+    dev = torch.device("cuda", device_index)
+    for s in range(cfg.n_segments):
+        k, v = synth.segment_kv(cfg, s, int(wl.seg_lens[s]), seed, dev)
+        sid = lib.segment_register(k, v, int(wl.orig_starts[s]))
+        assert sid == s
+        del k, v
+    torch.cuda.synchronize(dev)
+    return lib
+
+
+def plans_for(wl):
+    return [{"task_id": t.task_id, "entries": t.entries, "holes": t.holes, "capacity_tokens": t.capacity} for t in wl.tasks]
+
+
+def run_cuda(args, cfg, wl, seed):
+    from paper_2606_13097_b200 import binding
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    lib = build_library(cfg, wl, seed, local)
+    plans = plans_for(wl)
+    ids = [t.task_id for t in wl.tasks]
+    npt = [len(t.positions) for t in wl.tasks]
+    pos = np.concatenate([t.positions for t in wl.tasks]).astype(np.int32)
+    n_total = int(pos.size)
+    qs = [synth.patch_qkv(cfg, t.task_id, len(t.positions), seed, dev) for t in wl.tasks]
+    q = torch.cat([x[0] for x in qs], dim=1).contiguous()
+    k = torch.cat([x[1] for x in qs], dim=1).contiguous()
+    v = torch.cat([x[2] for x in qs], dim=1).contiguous()
+    out = torch.empty_like(q)
+    del qs
+    live = [False]
+
+    def step_device(ev=None):
+        if live[0]:
+            for tid in ids:
+                lib.task_release(tid)
+        if ev:
+            ev[0].record()
+        lib.stitch(plans)
+        live[0] = True
+        if ev:
+            ev[1].record()
+        if len(ids) == 1:
+            lib.patch(ids[0], 0, q, k, v, pos, out)
+        else:
+            lib.patch_batch(ids, npt, 0, q, k, v, pos, out)
+        if ev:
+            ev[2].record()
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        step_device()
+    barrier()
+    s0 = lib.stats()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_begin.record()
+    for i in range(args.steps):
+        step_device(evs[i])
+    t_end.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    s1 = lib.stats()
+    total_ms = t_begin.elapsed_time(t_end)
+    stitch_ms = [e[0].elapsed_time(e[1]) for e in evs]
+    patch_ms = [e[1].elapsed_time(e[2]) for e in evs]
+    if world > 1:
+        import torch.distributed as dist
+        tt = torch.tensor([total_ms], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / args.steps
+    launches = sum(s1[f] - s0[f] for f in s1 if f.endswith("_launches"))
+
+    # ---- e2e: same step through the C ABI with HOST buffers (H2D of q/k/v, D2H of out inside) ----
+    single = len(ids) == 1
+    e2e = None
+    if single:
+        qh, kh, vh = [x.cpu().contiguous().pin_memory() for x in (q, k, v)]
+        oh = torch.empty_like(qh).pin_memory()
+
+        def step_host():
+            lib.task_release(ids[0])
+            lib.stitch(plans)
+            lib.patch_host(ids[0], 0, qh, kh, vh, pos, oh)
+            torch.cuda.synchronize(dev)          # the caller reads `out` on the host every step
+
+        for _ in range(min(args.warmup, 3)):
+            step_host()
+        barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(args.steps):
+            step_host()
+        b.record()
+        barrier()
+        e2e_ms = a.elapsed_time(b) / args.steps
+        if world > 1:
+            import torch.distributed as dist
+            tt = torch.tensor([e2e_ms], device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            e2e_ms = float(tt.item())
+        h2d = int(qh.numel() + kh.numel() + vh.numel()) * 2
+        d2h = int(oh.numel()) * 2
+        e2e = (e2e_ms, h2d, d2h)
+        assert torch.equal(oh, out.cpu()), "host-buffer call and device call disagree"
+
+    sb, ab = stitch_bytes(cfg, wl), attn_bytes(cfg, wl)
+    peak, peak_src = peaks()
+    res = {
+        "metric": METRIC, "value": world * (sb + ab) / (ms_per_step * 1e-3) / 1e9, "unit": "GB/s (algorithmic, whole graft)",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": f"{cfg.name} ({args.config}): L={cfg.n_layers} Hq={cfg.n_q_heads} Hkv={cfg.n_kv_heads} "
+                               f"D={cfg.head_dim} page={cfg.page_size} base={cfg.rope_base:g}; library {cfg.n_segments} segments "
+                               f"({int(wl.seg_lens.sum())} tokens); {len(wl.tasks)} task(s), {wl.stitched_tokens} stitched + "
+                               f"{wl.patch_tokens} patch tokens; layout seed {seed}",
+                   "l2": "inputs larger than L2 (each step streams >= 1 GiB; no flush needed)" if sb > 4 * 126e6
+                   else "working set fits L2: latency only, no roofline claim",
+                   "stitch_ms": float(np.mean(stitch_ms)), "stitch_ms_min": float(np.min(stitch_ms)),
+                   "patch_ms": float(np.mean(patch_ms)), "patch_ms_min": float(np.min(patch_ms)),
+                   "stitch_GBps": sb / (np.mean(stitch_ms) * 1e-3) / 1e9, "patch_attn_GBps": ab / (np.mean(patch_ms) * 1e-3) / 1e9,
+                   "stitch_bytes": sb, "attn_bytes": ab, "attn_path": s1["last_attn_path"], "attn_splits": s1["last_attn_splits"],
+                   "parallelism": f"task-replica x{world}"},
+        "gpu_launches": int(launches),
+        "roofline": {"kernel": "stitch_kernel (fused gather + RoPE-shift)", "bound": "hbm",
+                     "achieved": sb / (np.mean(stitch_ms) * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": sb / (np.mean(stitch_ms) * 1e-3) / 1e9 / peak, "peak_source": peak_src,
+                     "frac_of_8TBps": sb / (np.mean(stitch_ms) * 1e-3) / 1e9 / 8000.0, "traffic": args.traffic,
+                     "patch_attention": {"bound": "hbm", "achieved": ab / (np.mean(patch_ms) * 1e-3) / 1e9,
+                                         "frac": ab / (np.mean(patch_ms) * 1e-3) / 1e9 / peak}},
+        "clocks": clocks,
+    }
+    if e2e:
+        res["e2e"] = {"value": world * (sb + ab) / (e2e[0] * 1e-3) / 1e9, "unit": "GB/s (algorithmic, whole graft)",
+                      "ms_per_step": e2e[0], "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2]}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        res["cpu_baseline"] = cpu_baseline(cfg, wl, seed, lib_segments=lambda s: synth.segment_kv(cfg, s, int(wl.seg_lens[s]), seed, dev))
+    lib.close()
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return res if rank == 0 else None
+
+
+# --------------------------------------------------------------------------------------------------
+# the oracle arm (cpu_baseline and --impl reference)
+# --------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, wl, seed, lib_segments, layers=1, kv_heads=None):
+    """Time the CPU oracle, as it stands, on a bounded sample of task 0 of the workload: `layers` layer(s),
+    the first `kv_heads` kv heads (and their q heads), all stitched tokens, all patch tokens.
+    `lib_segments(s)` returns the (K, V) tensors of library segment s.
+    Returns (seconds, algorithmic bytes of the sample, description)."""
+    from oracle import fcg_oracle as O
+    hk = kv_heads or cfg.n_kv_heads
+    G = cfg.n_q_heads // cfg.n_kv_heads
+    sub = synth.scaled(cfg, n_layers=layers, n_kv_heads=hk, n_q_heads=hk * G)
+    task = wl.tasks[0]
+    orc = O.OracleLibrary(layers, hk * G, hk, cfg.head_dim, page_size=cfg.page_size, rope_base=cfg.rope_base)
+    used = sorted({s for (s, _, _, _) in task.entries})
+    ids = {}
+    for s in used:
+        k, v = lib_segments(s)
+        ids[s] = orc.segment_register(synth.to_bits(k[:layers, :hk]), synth.to_bits(v[:layers, :hk]), int(wl.orig_starts[s]))
+    q, k, v = synth.patch_qkv(sub, task.task_id, len(task.positions), seed, "cpu")
+    qb, kb, vb = synth.to_bits(q), synth.to_bits(k), synth.to_bits(v)
+    plan = O.Plan(0, [O.PlanEntry(ids[s], b, n, d) for (s, b, n, d) in task.entries], [O.Hole(*h) for h in task.holes], task.capacity)
+    t0 = time.perf_counter()
+    orc.stitch([plan])
+    t1 = time.perf_counter()
+    orc.patch(0, 0, qb, kb, vb, task.positions)
+    t2 = time.perf_counter()
+    n_st = sum(n for (_, _, n, _) in task.entries)
+    sb = n_st * sub.kv_bytes_per_token * 2
+    ab = layers * (int(task.positions[-1]) + 1) * hk * cfg.head_dim * 4
+    desc = (f"task 0 of {cfg.name}, {layers} of {cfg.n_layers} layer(s) x {hk} of {cfg.n_kv_heads} kv heads: stitch {n_st} tokens "
+            f"({t1 - t0:.2f} s) + patch attention of {len(task.positions)} tokens ({t2 - t1:.2f} s)")
+    return t2 - t0, sb + ab, desc
+
+
+def blas_threads() -> int:
+    try:
+        from threadpoolctl import threadpool_info
+        return max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    except Exception:
+        return 1
+
+
+def sample_shape(cfg, wl, seed, lib_segments, budget_s):
+    """(layers, kv_heads) of a sample the oracle finishes in about `budget_s` seconds (probe: 1 layer x 2 heads)."""
+    probe_heads = min(2, cfg.n_kv_heads)
+    secs, _, _ = oracle_sample(cfg, wl, seed, lib_segments, 1, probe_heads)
+    units = max(1.0, budget_s / (secs / probe_heads))          # (layer, kv head) units that fit
+    if units >= cfg.n_kv_heads:
+        return int(min(cfg.n_layers, units // cfg.n_kv_heads)), cfg.n_kv_heads
+    return 1, int(units)
+
+
+def cpu_baseline(cfg, wl, seed, lib_segments, budget_s=15.0):
+    layers, heads = sample_shape(cfg, wl, seed, lib_segments, budget_s)
+    secs, nbytes, desc = oracle_sample(cfg, wl, seed, lib_segments, layers, heads)
+    return {"value": nbytes / secs / 1e9, "unit": "GB/s (algorithmic, whole graft)", "cores": blas_threads(),
+            "host_cpus": os.cpu_count(), "kind": "oracle", "seconds": secs,
+            "sample": desc + "; numpy fp64 (elementwise single-threaded, BLAS matvec multi-threaded)"}
+
+
+def run_reference(args, cfg, wl, seed):
+    """--impl reference: the oracle IS the reference for this paper.  Rank 0 only.  Each of the K steps is the
+    same bounded sample, sized so that warmup + K steps take about two minutes."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return None
+    cache = {}
+
+    def segs(s):
+        if s not in cache:
+            cache[s] = synth.segment_kv(cfg, s, int(wl.seg_lens[s]), seed, "cpu")
+        return cache[s]
+
+    budget = 120.0 / (args.steps + args.warmup)
+    layers, heads = sample_shape(cfg, wl, seed, segs, budget)
+    times, nbytes, desc = [], 0, ""
+    for i in range(args.warmup + args.steps):
+        secs, nbytes, desc = oracle_sample(cfg, wl, seed, segs, layers, heads)
+        if i >= args.warmup:
+            times.append(secs)
+    ms = float(np.mean(times)) * 1e3
+    val = nbytes / (ms * 1e-3) / 1e9
+    unit = "GB/s (algorithmic, whole graft)"
+    cb = {"value": val, "unit": unit, "cores": blas_threads(), "host_cpus": os.cpu_count(),
+          "kind": "oracle", "sample": "each step = " + desc}
+    return {"impl": "reference", "metric": METRIC, "value": val, "unit": unit,
+            "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg.name} ({args.config}); CPU oracle, each step = {layers} layer(s) x {heads} kv head(s) of task 0"},
+            "cpu_baseline": cb, "e2e": {"value": val, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per stitch launch, if known (profiles/)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    cfg = synth.CONFIGS[args.config]
+    wl = synth.make_workload(cfg, args.seed)
+    if args.impl == "reference":
+        res = run_reference(args, cfg, wl, args.seed)
+    else:
+        res = run_cuda(args, cfg, wl, args.seed)
+    if res is not None:
+        print(json.dumps(res))
+
+
+if __name__ == "__main__":
+    main()

@@ -307,7 +307,7 @@ def test_p14_rejections_match_oracle_and_leave_state_unchanged():
         torch.cuda.synchronize()
 
         class _DevView:      # zero-copy view of the library's device table
-            __cuda_array_interface__ = {"shape": (n_pages,), "typestr": "<i4", "data": (ptr, True), "version": 3}
+            __cuda_array_interface__ = {"shape": (n_pages,), "typestr": "<i4", "data": (ptr, False), "version": 3}
         dev = torch.as_tensor(_DevView(), device="cuda")
         assert np.array_equal(dev.cpu().numpy(), host)
         ids += host.tolist()
