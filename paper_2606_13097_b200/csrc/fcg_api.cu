@@ -85,6 +85,7 @@ struct fcg_library {
   int next_slot = 0;
   fcg_stats_t stats;
   int n_segments_live = 0, n_tasks_live = 0;
+  int32_t tc_min_rows = 64;                      // rows per kv head from which the tcgen05 path is used
 
   uint16_t *k_pool() const { return reinterpret_cast<uint16_t *>(arena + k_pool_off); }
   uint16_t *v_pool() const { return reinterpret_cast<uint16_t *>(arena + v_pool_off); }
@@ -625,9 +626,10 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
   const int G = c.n_q_heads / c.n_kv_heads;
   int max_rows = 0;
   for (int t = 0; t < pc.n_tasks; ++t) max_rows = std::max(max_rows, pc.n_per_task[t] * G);
-  const int rows_per_cta = max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64);
+  const bool use_tc = c.head_dim == 128 && max_rows >= lib->tc_min_rows;
+  const int rows_per_cta = use_tc ? 128 : (max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64));
   const int max_row_groups = (max_rows + rows_per_cta - 1) / rows_per_cta;
-  const int ctas_per_sm = fcg::attn_split_ctas_per_sm(c.head_dim);
+  const int ctas_per_sm = use_tc ? 1 : fcg::attn_split_ctas_per_sm(c.head_dim);
   int max_splits = 1;
   int64_t tok_off = 0;
   for (int t = 0; t < pc.n_tasks; ++t) {
@@ -704,9 +706,15 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
   ap.max_row_groups = max_row_groups;
   ap.n_pages = c.n_pages;
   ap.scale_log2 = (float)(1.4426950408889634 / sqrt((double)c.head_dim));
-  FCG_CUDA(fcg::launch_attn_split(ap, c.head_dim, rows_per_cta, pc.stream));
-  lib->stats.attn_split_launches++;
-  lib->stats.last_attn_path = 1;
+  if (use_tc) {
+    FCG_CUDA(fcg::launch_attn_tc(ap, c.head_dim, pc.stream));
+    lib->stats.attn_tc_launches++;
+    lib->stats.last_attn_path = 2;
+  } else {
+    FCG_CUDA(fcg::launch_attn_split(ap, c.head_dim, rows_per_cta, pc.stream));
+    lib->stats.attn_split_launches++;
+    lib->stats.last_attn_path = 1;
+  }
   lib->stats.last_attn_splits = max_splits;
   if (max_splits > 1) {
     FCG_CUDA(fcg::launch_attn_combine(ap, c.head_dim, pc.stream));
@@ -846,6 +854,12 @@ fcg_status_t fcg_pool_info(fcg_library_t *lib, fcg_pool_info_t *out) {
   out->n_pages_free = (uint32_t)lib->page_stack.size();
   out->n_segments_live = lib->n_segments_live;
   out->n_tasks_live = lib->n_tasks_live;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_set_attn_policy(fcg_library_t *lib, int32_t tc_min_rows) {
+  if (!lib || tc_min_rows < 0) return fail(FCG_ERR_INVALID_ARG, "NULL library or negative threshold");
+  lib->tc_min_rows = tc_min_rows;
   return FCG_OK;
 }
 

@@ -354,3 +354,24 @@ def test_segment_release_reuses_ids_and_arena():
     wl.tasks[0].task_id = 0
     T.compare_stitched(orc, lib, wl)
     lib.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# both attention kernels against the oracle on the same inputs (policy forced either way)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,Hq,Hkv,ctx", [(64, 4, 4, 700), (16, 2, 2, 300), (48, 8, 2, 1000), (128, 4, 1, 2100), (3, 4, 2, 70)])
+@pytest.mark.parametrize("tc_min_rows", [0, 2 ** 31 - 1])
+def test_tcgen05_and_split_paths_match_oracle(n, Hq, Hkv, ctx, tc_min_rows):
+    cfg = synth.GraftConfig("paths", 2, Hq, Hkv, 128, 16, 1e4, 3, ctx // 3, ctx // 3 + 40, 500, 1, 3, 3, 0,
+                            holes=((0, max(1, n // 4)), (-1, n - max(1, n // 4))) if n > 1 else ((-1, 1),))
+    wl = synth.make_workload(cfg, 13)
+    orc, lib, seg_ids = T.make_pair(cfg, wl, 13)
+    lib.set_attn_policy(tc_min_rows)
+    c_plans, o_plans = T.plans_of(wl, seg_ids)
+    orc.stitch(o_plans)
+    lib.stitch(c_plans)
+    out, ref = T.run_patch_both(orc, lib, cfg, wl.tasks[0], 14)
+    assert lib.stats()["last_attn_path"] == (2 if tc_min_rows == 0 else 1)
+    T.assert_attn_close(out, ref, f"path {'tc' if tc_min_rows == 0 else 'split'} n={n}")
+    T.compare_cache_bits(orc, lib, 0, wl.tasks[0].positions)
+    lib.close()
