@@ -182,8 +182,11 @@ fcg_status_t fcg_pool_info(fcg_library_t *lib, fcg_pool_info_t *out);
 
 /* Kernel selection for patch attention: calls whose largest task has R = n * G >= tc_min_rows query rows per
  * kv head (and head_dim 128) use the tcgen05/TMEM kernel, others the split-KV warp-MMA kernel.  Default 64
- * (north_star: tensor-core tiles only for dense patches); 0 = always tcgen05, INT32_MAX = never. */
-fcg_status_t fcg_set_attn_policy(fcg_library_t *lib, int32_t tc_min_rows);
+ * (north_star: tensor-core tiles only for dense patches); 0 = always tcgen05, INT32_MAX = never.
+ * force_splits > 0 fixes the number of KV splits per task (clamped to the task's 64-token tile count);
+ * 0 = the library's wave-filling choice.  The result does not depend on either knob beyond summation order
+ * (P11, split invariance). */
+fcg_status_t fcg_set_attn_policy(fcg_library_t *lib, int32_t tc_min_rows, int32_t force_splits);
 
 /* Launch statistics since create (kernels launched by this library; bench.py reports them). */
 typedef struct {

@@ -93,7 +93,7 @@ SYMBOLS = {
     "fcg_task_release": (_I, [_P, _I]),
     "fcg_task_read": (_I, [_P, _I, _I, _I, _I, _P, _P, _P]),
     "fcg_pool_info": (_I, [_P, C.POINTER(fcg_pool_info_t)]),
-    "fcg_set_attn_policy": (_I, [_P, _I]),
+    "fcg_set_attn_policy": (_I, [_P, _I, _I]),
     "fcg_stats": (_I, [_P, C.POINTER(fcg_stats_t)]),
     "fcg_last_error": (C.c_char_p, []),
     "fcg_version": (C.c_char_p, []),
@@ -275,8 +275,8 @@ def fcg_pool_info(handle) -> dict:
     return {f: getattr(info, f) for f, _ in fcg_pool_info_t._fields_}
 
 
-def fcg_set_attn_policy(handle, tc_min_rows: int) -> None:
-    _check(load().fcg_set_attn_policy(handle, int(tc_min_rows)))
+def fcg_set_attn_policy(handle, tc_min_rows: int, force_splits: int = 0) -> None:
+    _check(load().fcg_set_attn_policy(handle, int(tc_min_rows), int(force_splits)))
 
 
 def fcg_stats(handle) -> dict:
@@ -370,5 +370,5 @@ class FcgLibrary:
     def stats(self) -> dict:
         return fcg_stats(self.handle)
 
-    def set_attn_policy(self, tc_min_rows: int) -> None:
-        fcg_set_attn_policy(self.handle, tc_min_rows)
+    def set_attn_policy(self, tc_min_rows: int, force_splits: int = 0) -> None:
+        fcg_set_attn_policy(self.handle, tc_min_rows, force_splits)

@@ -86,6 +86,7 @@ struct fcg_library {
   fcg_stats_t stats;
   int n_segments_live = 0, n_tasks_live = 0;
   int32_t tc_min_rows = 64;                      // rows per kv head from which the tcgen05 path is used
+  int32_t force_splits = 0;                      // > 0: KV splits per task (clamped to its tile count); 0 = choose_splits
 
   uint16_t *k_pool() const { return reinterpret_cast<uint16_t *>(arena + k_pool_off); }
   uint16_t *v_pool() const { return reinterpret_cast<uint16_t *>(arena + v_pool_off); }
@@ -638,8 +639,10 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
     const int tiles = (kv_len + KV_TILE - 1) / KV_TILE;
     const int rg = (n * G + rows_per_cta - 1) / rows_per_cta;
     const int64_t base = (int64_t)rg * c.n_kv_heads * pc.n_layers * pc.n_tasks;
-    const int ns = choose_splits(base, tiles, std::min(n * G, rows_per_cta), c.head_dim, ctas_per_sm);
+    int ns = lib->force_splits > 0 ? std::min(lib->force_splits, tiles)
+                                   : choose_splits(base, tiles, std::min(n * G, rows_per_cta), c.head_dim, ctas_per_sm);
     const int tiles_per = (tiles + ns - 1) / ns;
+    ns = (tiles + tiles_per - 1) / tiles_per;      // no empty trailing split
     fcg::AttnTaskDev &d = h_tasks[t];
     d.table_off = pc.task_ids[t] * lib->pages_per_task;
     d.n = n;
@@ -857,9 +860,10 @@ fcg_status_t fcg_pool_info(fcg_library_t *lib, fcg_pool_info_t *out) {
   return FCG_OK;
 }
 
-fcg_status_t fcg_set_attn_policy(fcg_library_t *lib, int32_t tc_min_rows) {
-  if (!lib || tc_min_rows < 0) return fail(FCG_ERR_INVALID_ARG, "NULL library or negative threshold");
+fcg_status_t fcg_set_attn_policy(fcg_library_t *lib, int32_t tc_min_rows, int32_t force_splits) {
+  if (!lib || tc_min_rows < 0 || force_splits < 0) return fail(FCG_ERR_INVALID_ARG, "NULL library or negative threshold / split count");
   lib->tc_min_rows = tc_min_rows;
+  lib->force_splits = force_splits;
   return FCG_OK;
 }
 

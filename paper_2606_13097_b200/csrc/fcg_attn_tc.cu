@@ -226,6 +226,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) attn_tc_kernel(const AttnParams p
     const size_t page_stride = head_stride * p.n_kv_heads;
     const size_t layer_base = ((size_t)layer * p.n_pages) * page_stride + (size_t)g * head_stride;
     for (int j = 0; j < n_tiles + LOOKAHEAD; ++j) {
+      // Hand tile j-LOOKAHEAD over BEFORE blocking on a free stage for tile j: the stage of tile j is
+      // released by P V of tile j-KV_STAGES, which the MMA thread issues only after Q K^T of tile
+      // j-KV_STAGES+1 = j-LOOKAHEAD -- the tile signalled here.  (The other order deadlocks as soon as
+      // a CTA has more than KV_STAGES tiles.)
+      if (j >= LOOKAHEAD) {
+        cp_async_wait<LOOKAHEAD - 1>();
+        fence_proxy_async();
+        mbar_arrive(kv_full((j - LOOKAHEAD) % KV_STAGES));
+      }
       if (j < n_tiles) {
         const int st = j % KV_STAGES;
         if (j >= KV_STAGES) mbar_wait(kv_empty(st), ((j / KV_STAGES) - 1) & 1);
@@ -249,11 +258,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) attn_tc_kernel(const AttnParams p
         }
       }
       cp_async_commit();
-      if (j >= LOOKAHEAD) {
-        cp_async_wait<LOOKAHEAD>();
-        fence_proxy_async();
-        mbar_arrive(kv_full((j - LOOKAHEAD) % KV_STAGES));
-      }
     }
   } else if (warp == 8) {
     // ======================================= MMA issuer =====================================

@@ -375,3 +375,28 @@ def test_tcgen05_and_split_paths_match_oracle(n, Hq, Hkv, ctx, tc_min_rows):
     T.assert_attn_close(out, ref, f"path {'tc' if tc_min_rows == 0 else 'split'} n={n}")
     T.compare_cache_bits(orc, lib, 0, wl.tasks[0].positions)
     lib.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# P11 split invariance with the split count FORCED, so that one CTA walks many more KV tiles than the
+# shared-memory ring has stages (the auto choice gives small test grids many splits of a few tiles each
+# and never exercises ring wrap-around); also the bench's launch shape (one split over the whole cache).
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,Hq,Hkv,ctx", [(64, 2, 2, 4096), (20, 8, 2, 1500), (130, 2, 1, 2600)])
+@pytest.mark.parametrize("tc_min_rows", [0, 2 ** 31 - 1])
+@pytest.mark.parametrize("force_splits", [1, 2, 5])
+def test_forced_split_counts_long_tile_loops(n, Hq, Hkv, ctx, tc_min_rows, force_splits):
+    cfg = synth.GraftConfig("longloop", 1, Hq, Hkv, 128, 16, 1e4, 3, ctx // 3, ctx // 3 + 40, 500, 1, 3, 3, 0,
+                            holes=((0, max(1, n // 4)), (-1, n - max(1, n // 4))))
+    wl = synth.make_workload(cfg, 21)
+    orc, lib, seg_ids = T.make_pair(cfg, wl, 21)
+    lib.set_attn_policy(tc_min_rows, force_splits)
+    c_plans, o_plans = T.plans_of(wl, seg_ids)
+    orc.stitch(o_plans)
+    lib.stitch(c_plans)
+    out, ref = T.run_patch_both(orc, lib, cfg, wl.tasks[0], 22)
+    st = lib.stats()
+    assert st["last_attn_path"] == (2 if tc_min_rows == 0 else 1)
+    assert st["last_attn_splits"] == force_splits
+    T.assert_attn_close(out, ref, f"forced splits {force_splits}, path {st['last_attn_path']}, n={n}")
+    lib.close()
