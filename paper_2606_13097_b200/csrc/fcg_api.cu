@@ -1,6 +1,7 @@
 // Host side of libfcg.so: the C ABI of include/fcg.h -- segment library (S1), stitch-plan builder and
 // page allocator (S2), and the launch logic for S3-S6.  Everything here is integer bookkeeping plus
 // the fp64 evaluation of the per-entry RoPE table; all K/V/q arithmetic runs in the kernels.
+#include <cuda.h>   // CUtensorMap types only: the driver entry point is resolved at run time, libcuda is not linked
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdarg.h>
@@ -86,6 +87,8 @@ struct fcg_library {
   fcg_stats_t stats;
   int n_segments_live = 0, n_tasks_live = 0;
   int32_t tc_min_rows = 64;                      // rows per kv head from which the tcgen05 path is used
+  fcg::TmaDesc tm_k, tm_v;                       // K / V pool tensor maps for the tcgen05 path (head_dim 128)
+  bool have_tma = false;
   int32_t force_splits = 0;                      // > 0: KV splits per task (clamped to its tile count); 0 = choose_splits
 
   uint16_t *k_pool() const { return reinterpret_cast<uint16_t *>(arena + k_pool_off); }
@@ -126,6 +129,34 @@ Layout layout_of(const fcg_config_t *c) {
   l.ws_bytes = align_up(c->workspace_bytes ? c->workspace_bytes : (256ull << 20));
   l.seg_off = l.ws_off + l.ws_bytes;
   return l;
+}
+
+// TMA tensor map of one pool [L][n_pages][Hkv][P][D] bf16 as the 5-D tensor (D, P, Hkv, n_pages, L), innermost
+// first; box = (64 columns, one page, 1, 1, 1) with 128B swizzle = one 64-column half of one head's page slice,
+// which lands in shared memory exactly in the K-major / MN-major UMMA operand layout (fcg_attn_tc.cu).
+fcg_status_t make_pool_tensor_map(const fcg_config_t &c, void *pool, fcg::TmaDesc *out) {
+  typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_fn encode = nullptr;
+  if (!encode) {
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    FCG_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) return fail(FCG_ERR_CUDA, "cuTensorMapEncodeTiled is not available in this driver");
+    encode = reinterpret_cast<encode_fn>(fn);
+  }
+  static_assert(sizeof(CUtensorMap) == sizeof(fcg::TmaDesc), "CUtensorMap is 128 bytes");
+  const cuuint64_t D = c.head_dim, P = c.page_size, H = c.n_kv_heads;
+  const cuuint64_t dims[5] = {D, P, H, c.n_pages, (cuuint64_t)c.n_layers};
+  const cuuint64_t strides[4] = {D * 2, P * D * 2, H * P * D * 2, (cuuint64_t)c.n_pages * H * P * D * 2};
+  const cuuint32_t box[5] = {64, (cuuint32_t)P, 1, 1, 1};
+  const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  CUresult r = encode(reinterpret_cast<CUtensorMap *>(out), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, pool, dims, strides, box, estr,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(FCG_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+  return FCG_OK;
 }
 
 // acquire a blob slot whose previous consumer kernels have finished
@@ -223,6 +254,15 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
       return fail(FCG_ERR_CUDA, "blob slot allocation: %s", cudaGetErrorString(e));
     }
     lib->slots[i].dev = lib->arena + l.ws_off + (uint64_t)i * BLOB_BYTES;
+  }
+  if (cfg->head_dim == 128) {
+    fcg_status_t st = make_pool_tensor_map(lib->cfg, lib->k_pool(), &lib->tm_k);
+    if (st == FCG_OK) st = make_pool_tensor_map(lib->cfg, lib->v_pool(), &lib->tm_v);
+    if (st != FCG_OK) {
+      fcg_library_destroy(lib);
+      return st;
+    }
+    lib->have_tma = true;
   }
   *out = lib;
   return FCG_OK;
@@ -627,8 +667,9 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
   const int G = c.n_q_heads / c.n_kv_heads;
   int max_rows = 0;
   for (int t = 0; t < pc.n_tasks; ++t) max_rows = std::max(max_rows, pc.n_per_task[t] * G);
-  const bool use_tc = c.head_dim == 128 && max_rows >= lib->tc_min_rows;
-  const int rows_per_cta = use_tc ? 128 : (max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64));
+  const bool use_tc = lib->have_tma && max_rows >= lib->tc_min_rows;
+  const int q_tiles = max_rows > 128 ? 2 : 1;    // 128-row Q tiles per tcgen05 CTA
+  const int rows_per_cta = use_tc ? 128 * q_tiles : (max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64));
   const int max_row_groups = (max_rows + rows_per_cta - 1) / rows_per_cta;
   const int ctas_per_sm = use_tc ? 1 : fcg::attn_split_ctas_per_sm(c.head_dim);
   int max_splits = 1;
@@ -710,7 +751,7 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
   ap.n_pages = c.n_pages;
   ap.scale_log2 = (float)(1.4426950408889634 / sqrt((double)c.head_dim));
   if (use_tc) {
-    FCG_CUDA(fcg::launch_attn_tc(ap, c.head_dim, pc.stream));
+    FCG_CUDA(fcg::launch_attn_tc(ap, c.head_dim, q_tiles, &lib->tm_k, &lib->tm_v, pc.stream));
     lib->stats.attn_tc_launches++;
     lib->stats.last_attn_path = 2;
   } else {

@@ -103,7 +103,15 @@ cudaError_t launch_attn_split(const AttnParams &p, int head_dim, int rows_per_ct
 cudaError_t launch_attn_combine(const AttnParams &p, int head_dim, cudaStream_t stream);
 int attn_split_ctas_per_sm(int head_dim);
 
-// tcgen05 / TMEM path (128-row tiles); returns cudaErrorNotSupported if not built
-cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, cudaStream_t stream);
+// A TMA tensor map (CUtensorMap: 128 opaque bytes, 64-byte aligned), kept free of <cuda.h> here.
+struct alignas(64) TmaDesc {
+  unsigned char bytes[128];
+};
+
+// tcgen05 / TMEM path; q_tiles = 128-row Q tiles per CTA (1 or 2), p.max_row_groups counts groups of
+// q_tiles*128 rows.  tm_k / tm_v describe the K / V pool as a 5-D bf16 tensor (D, P, Hkv, n_pages, L)
+// with box (64, P, 1, 1, 1) and 128B swizzle (make_pool_tensor_map).
+cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, const TmaDesc *tm_k, const TmaDesc *tm_v,
+                           cudaStream_t stream);
 
 }  // namespace fcg

@@ -400,3 +400,36 @@ def test_forced_split_counts_long_tile_loops(n, Hq, Hkv, ctx, tc_min_rows, force
     assert st["last_attn_splits"] == force_splits
     T.assert_attn_close(out, ref, f"forced splits {force_splits}, path {st['last_attn_path']}, n={n}")
     lib.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# tcgen05 path details: every page size (one TMA box per page and 64-column half), two 128-row Q tiles
+# per CTA (R > 128), ragged last tiles, and a cache pool poisoned with NaN bit patterns (page slack and
+# masked positions must never reach the output: DESIGN R10)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("P", [8, 16, 32, 64])
+@pytest.mark.parametrize("n,Hq,Hkv,ctx", [(40, 4, 2, 1000), (70, 8, 2, 777), (260, 2, 2, 1500)])
+def test_tcgen05_page_sizes_two_q_tiles_and_poisoned_pool(P, n, Hq, Hkv, ctx):
+    cfg = synth.GraftConfig("tcpages", 2, Hq, Hkv, 128, P, 1e4, 3, ctx // 3, ctx // 3 + 40, 500, 1, 3, 3, 0,
+                            holes=((0, max(1, n // 4)), (-1, n - max(1, n // 4))))
+    wl = synth.make_workload(cfg, 31)
+    orc, lib, seg_ids = T.make_pair(cfg, wl, 31)
+    info = lib.pool_info()
+    pool = lib.arena[info["k_pool_offset"]:info["v_pool_offset"] + info["pool_bytes"]]
+    pool.fill_(0xFF)                                   # every bf16 in both pools is a NaN until written
+    torch.cuda.synchronize()
+    lib.set_attn_policy(0)
+    c_plans, o_plans = T.plans_of(wl, seg_ids)
+    orc.stitch(o_plans)
+    lib.stitch(c_plans)
+    out, ref = T.run_patch_both(orc, lib, cfg, wl.tasks[0], 32)
+    assert lib.stats()["last_attn_path"] == 2
+    assert torch.isfinite(out.float()).all()
+    T.assert_attn_close(out, ref, f"tc P={P} n={n} G={Hq // Hkv}")
+    # the same again with forced splits (partials + combine)
+    lib.set_attn_policy(0, 3)
+    out2 = lib.patch(0, 0, *[x.cuda().contiguous() for x in synth.patch_qkv(cfg, 0, len(wl.tasks[0].positions), 32, "cpu")],
+                     wl.tasks[0].positions)
+    torch.cuda.synchronize()
+    T.assert_attn_close(out2, ref, f"tc P={P} n={n} 3 splits")
+    lib.close()
