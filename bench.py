@@ -98,7 +98,9 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------------
 # the CUDA arm
 # --------------------------------------------------------------------------------------------------
-def build_library(cfg, wl, seed, device_index):
+def build_library(cfg, wl, seed, device_index, on_segment=None):
+    """The library exactly as the timed run uses it.  `on_segment(s, k, v)` lets the full-size parity tests
+    keep slices of the device-generated segments for the oracle."""
     from paper_2606_13097_b200 import binding
     total_pages = sum(-(-t.capacity // cfg.page_size) for t in wl.tasks)
     seg_tokens = int(wl.seg_lens.sum())
@@ -112,6 +114,8 @@ def build_library(cfg, wl, seed, device_index):
         k, v = synth.segment_kv(cfg, s, int(wl.seg_lens[s]), seed, dev)
         sid = lib.segment_register(k, v, int(wl.orig_starts[s]))
         assert sid == s
+        if on_segment is not None:
+            on_segment(s, k, v)
         del k, v
     torch.cuda.synchronize(dev)
     return lib

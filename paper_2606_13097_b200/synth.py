@@ -60,7 +60,7 @@ C3 = GraftConfig("C3-llama3-8b-gqa", 32, 32, 8, 128, 16, 5e5, 64, 256, 1024, 819
 C4 = GraftConfig("C4-batched32", 32, 32, 8, 128, 16, 1e4, 256, 64, 1024, 8192, 32, 4, 10, 0,
                  total_min=2048, total_max=6144, distinct_segments=False,
                  holes=((-1, 0),), patch_min=8, patch_max=64)
-C5 = GraftConfig("C5-long32k", 48, 64, 8, 128, 16, 1e6, 24, 1024, 1700, 32768, 1, 24, 24, 32768,
+C5 = GraftConfig("C5-long32k", 48, 64, 8, 128, 16, 1e6, 24, 1152, 1792, 32768, 1, 24, 24, 32768,
                  holes=((-1, 256),))
 CONFIGS = {"C1": C1, "C2": C2, "C3": C3, "C4": C4, "C5": C5}
 
