@@ -86,7 +86,7 @@ struct fcg_library {
   int next_slot = 0;
   fcg_stats_t stats;
   int n_segments_live = 0, n_tasks_live = 0;
-  int32_t tc_min_rows = 64;                      // rows per kv head from which the tcgen05 path is used
+  int32_t tc_min_rows = 1;                       // rows per kv head from which the tcgen05 path is used (head_dim 128)
   fcg::TmaDesc tm_k, tm_v;                       // K / V pool tensor maps for the tcgen05 path (head_dim 128)
   bool have_tma = false;
   int32_t force_splits = 0;                      // > 0: KV splits per task (clamped to its tile count); 0 = choose_splits

@@ -21,6 +21,8 @@
 //   Output: final bf16 rows (one split) or fp32 (m, l, o) partials for attn_combine_kernel.
 #include <cuda_bf16.h>
 
+#include <type_traits>
+
 #include "fcg_internal.h"
 
 namespace fcg {
@@ -63,9 +65,26 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// One elected lane of a converged warp issues the asynchronous operations (TMA, tcgen05.mma, tcgen05.commit); the
+// election is deterministic for a full mask, so every operation of a warp comes from the same thread.  All
+// operands are computed by the whole warp in uniform control flow (so they can live in uniform registers) and
+// only the issue itself is predicated.
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t"
+      "}"
+      : "=r"(pred));
+  return pred != 0;
+}
+
 // ---- TMA: one box of the 5-D pool tensor (D, P, Hkv, n_pages, L) -> shared memory ----------------
 __device__ __forceinline__ void tma_load_5d(uint32_t dst, const TmaDesc *desc, uint32_t bar, int c0, int c1, int c2, int c3,
                                             int c4) {
+  if (elect_one())
   asm volatile(
       "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(dst),
       "l"(reinterpret_cast<uint64_t>(desc)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(bar)
@@ -89,10 +108,12 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr) {
   asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(NCOLS) : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
+  if (elect_one())
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
 // D[tmem] (+)= A[smem] * B[smem]
 __device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  if (elect_one())
   asm volatile(
       "{\n\t"
       ".reg .pred p;\n\t"
@@ -127,6 +148,14 @@ constexpr uint32_t idesc_f16(int n, bool b_mn_major) {
         "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])                    \
       : "r"(taddr))
 
+#define TMEM_LD_16(taddr, r)                                                                                         \
+  asm volatile(                                                                                                      \
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "                                                                      \
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"                                              \
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),  \
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])                     \
+      : "r"(taddr))
+
 #define TMEM_ST_32(taddr, r)                                                                                         \
   asm volatile(                                                                                                      \
       "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "                                                                \
@@ -158,25 +187,29 @@ constexpr int P_BYTES = BM * BN * 2;          // [128][128 B]
 
 template <int NQ>
 struct Cfg {
-  static constexpr int KV_STAGES = NQ == 1 ? 4 : 3;
+  // separate rings: a K stage is free again as soon as Q K^T of its tile has completed, a V stage only after P V
+  static constexpr int K_STAGES = NQ == 1 ? 4 : 3;
+  static constexpr int V_STAGES = NQ == 1 ? 6 : 3;
   static constexpr int N_SOFTMAX = NQ * BM;
-  static constexpr int NTHREADS = N_SOFTMAX + 64;
-  static constexpr int LOADER_WARP = 4 * NQ, MMA_WARP = 4 * NQ + 1;
+  static constexpr int NTHREADS = N_SOFTMAX + 96;
+  static constexpr int KLOAD_WARP = 4 * NQ, VLOAD_WARP = 4 * NQ + 1, MMA_WARP = 4 * NQ + 2;
   static constexpr int TMEM_COLS = NQ * 256;
   static constexpr int OFF_Q = 0;
-  static constexpr int OFF_KV = OFF_Q + NQ * Q_TILE_B;               // stage s: K at +s*2*KV_TILE_B, V right after K
-  static constexpr int OFF_P = OFF_KV + KV_STAGES * 2 * KV_TILE_B;   // P[t][b] at +(2t+b)*P_BYTES
+  static constexpr int OFF_K = OFF_Q + NQ * Q_TILE_B;                // K stage s at +s*KV_TILE_B
+  static constexpr int OFF_V = OFF_K + K_STAGES * KV_TILE_B;         // V stage s at +s*KV_TILE_B
+  static constexpr int OFF_P = OFF_V + V_STAGES * KV_TILE_B;         // P[t][b] at +(2t+b)*P_BYTES
   static constexpr int OFF_BAR = OFF_P + NQ * 2 * P_BYTES;
-  // kv_full[ST], kv_empty[ST], s_full[NQ][2], p_full[NQ][2], pv_done[NQ][2], q_full
-  static constexpr int N_BARS = 2 * KV_STAGES + 6 * NQ + 1;
+  // k_full[SK], k_empty[SK], v_full[SV], v_empty[SV], s_full[NQ][2], p_full[NQ][2], pv_done[NQ][2], q_full
+  static constexpr int N_BARS = 2 * K_STAGES + 2 * V_STAGES + 6 * NQ + 1;
   static constexpr int SMEM_BYTES = OFF_BAR + N_BARS * 8 + 16 + 1024;   // + tmem slot + alignment slack
+  static_assert((K_STAGES + V_STAGES) * KV_TILE_B >= BM * (D + 4) * 4 + BM * 8, "merge buffer must fit in the idle rings");
 };
 
 template <int NQ>
 __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
     attn_tc_kernel(const AttnParams p, const __grid_constant__ TmaDesc tm_k, const __grid_constant__ TmaDesc tm_v) {
   using C = Cfg<NQ>;
-  constexpr int ST = C::KV_STAGES;
+  constexpr int SK = C::K_STAGES, SV = C::V_STAGES;
   extern __shared__ unsigned char smem_raw[];
   // 1024-byte alignment for the 128B-swizzle atoms
   unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -195,75 +228,105 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
   const int layer = p.layer_begin + li;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
+  // ---- row layout of this CTA (see "Row streams" in the header) ---------------------------------
+  const int Rc = min(R - row0, NQ * BM);           // valid query rows of this CTA
+  const int nq_eff = (NQ == 2 && Rc > BM) ? 2 : 1; // Q tiles that hold any valid row
+  const int dup = nq_eff == 1 ? (Rc <= 32 ? 4 : (Rc <= 64 ? 2 : 1)) : 1;
+  const int rps = BM / dup;                        // MMA rows per stream (128, 64 or 32)
+
   const int t_begin = split * tk.split_len;
   const int t_end = min(tk.kv_len, t_begin + tk.split_len);
   const int32_t *pos = p.positions + tk.tok_off;
-  const int cta_last = min(R, row0 + NQ * BM) - 1;
+  const int cta_last = row0 + Rc - 1;
   const int cta_max_lim = min(pos[cta_last / G], t_end - 1);
   const int n_tiles = cta_max_lim >= t_begin ? (cta_max_lim - t_begin) / BN + 1 : 0;
 
   const uint32_t bar0 = sbase + C::OFF_BAR;
-  auto kv_full = [&](int s) { return bar0 + 8 * s; };
-  auto kv_empty = [&](int s) { return bar0 + 8 * (ST + s); };
-  auto s_full = [&](int t, int b) { return bar0 + 8 * (2 * ST + 2 * t + b); };
-  auto p_full = [&](int t, int b) { return bar0 + 8 * (2 * ST + 2 * NQ + 2 * t + b); };
-  auto pv_done = [&](int t, int b) { return bar0 + 8 * (2 * ST + 4 * NQ + 2 * t + b); };
-  const uint32_t q_full = bar0 + 8 * (2 * ST + 6 * NQ);
+  auto k_full = [&](int s) { return bar0 + 8 * s; };
+  auto k_empty = [&](int s) { return bar0 + 8 * (SK + s); };
+  auto v_full = [&](int s) { return bar0 + 8 * (2 * SK + s); };
+  auto v_empty = [&](int s) { return bar0 + 8 * (2 * SK + SV + s); };
+  constexpr int B0 = 2 * SK + 2 * SV;
+  auto s_full = [&](int t, int b) { return bar0 + 8 * (B0 + 2 * t + b); };
+  auto p_full = [&](int t, int b) { return bar0 + 8 * (B0 + 2 * NQ + 2 * t + b); };
+  auto pv_done = [&](int t, int b) { return bar0 + 8 * (B0 + 4 * NQ + 2 * t + b); };
+  const uint32_t q_full = bar0 + 8 * (B0 + 6 * NQ);
   const uint32_t tmem_slot = bar0 + 8 * C::N_BARS;
   volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem + C::OFF_BAR + 8 * C::N_BARS);
 
+  // valid rows of Q tile t, and its softmax warps that own at least one valid row (the others never
+  // touch the tile's barriers: the P-ready barrier counts the threads of the active warps only)
+  auto tile_rows = [&](int t) { return max(0, min(Rc - t * BM, BM)); };
+  auto warp_active = [&](int t, int w) { return ((32 * w) & (rps - 1)) < tile_rows(t); };
+
   if (tid == 0) {
-    for (int s = 0; s < ST; ++s) {
-      mbar_init(kv_full(s), 1);
-      mbar_init(kv_empty(s), 1);
+    for (int s = 0; s < SK; ++s) {
+      mbar_init(k_full(s), 1);
+      mbar_init(k_empty(s), 1);
     }
-    for (int t = 0; t < NQ; ++t)
+    for (int s = 0; s < SV; ++s) {
+      mbar_init(v_full(s), 1);
+      mbar_init(v_empty(s), 1);
+    }
+    for (int t = 0; t < NQ; ++t) {
+      int act = 0;
+      for (int w = 0; w < 4; ++w) act += warp_active(t, w) ? 1 : 0;
       for (int b = 0; b < 2; ++b) {
         mbar_init(s_full(t, b), 1);
-        mbar_init(p_full(t, b), BM);
+        mbar_init(p_full(t, b), 32 * max(act, 1));
         mbar_init(pv_done(t, b), 1);
       }
+    }
     mbar_init(q_full, C::N_SOFTMAX);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == C::MMA_WARP) tmem_alloc<C::TMEM_COLS>(tmem_slot);
-  if (warp == C::LOADER_WARP && lane == 0) {
-    tma_prefetch_desc(&tm_k);
-    tma_prefetch_desc(&tm_v);
-  }
+  if (warp == C::KLOAD_WARP && lane == 0) tma_prefetch_desc(&tm_k);
+  if (warp == C::VLOAD_WARP && lane == 0) tma_prefetch_desc(&tm_v);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
-  if (warp == C::LOADER_WARP) {
-    // ======================================= loader ========================================
-    // lane i of the warp owns page i of the tile: one page-table lookup, four box copies.
+  if (warp == C::KLOAD_WARP || warp == C::VLOAD_WARP) {
+    // ======================================= loaders =======================================
+    // One warp streams K, one streams V: lanes 0..ppt-1 look up the pages of the NEXT tile (coalesced, latency
+    // hidden behind the ring wait); lane 0 then issues two box copies per page (the two 64-column halves).  All
+    // control flow is warp-uniform so that the TMA issue compiles to straight-line UTMALDG.
+    const bool is_k = warp == C::KLOAD_WARP;
+    const TmaDesc *tm = is_k ? &tm_k : &tm_v;
+    const int NS = is_k ? SK : SV;
+    const uint32_t ring = sbase + (is_k ? C::OFF_K : C::OFF_V);
+    const uint32_t full0 = is_k ? k_full(0) : v_full(0), empty0 = is_k ? k_empty(0) : v_empty(0);
     const int P = p.page_size;
-    const int ppt = BN / P;                         // pages per tile (P <= 64, power of two)
-    const int32_t *table = p.tables + tk.table_off;
+    const int pshift = __ffs(P) - 1;
+    const int ppt = BN >> pshift;                   // pages per tile (P <= 64, power of two)
+    const int32_t *table = p.tables + tk.table_off + (t_begin >> pshift);
+    const int n_pages_split = (t_end - t_begin + P - 1) >> pshift;
     auto page_of = [&](int j) -> int {
-      const int tok = t_begin + j * BN + lane * P;
-      return (j < n_tiles && lane < ppt && tok < t_end) ? __ldg(table + tok / P) : -1;
+      const int pi = j * ppt + lane;
+      return (lane < ppt && pi < n_pages_split) ? __ldg(table + pi) : -1;
     };
     int page = page_of(0);
+    int st = 0, round = 0;
     for (int j = 0; j < n_tiles; ++j) {
-      const int page_next = page_of(j + 1);         // issued before the wait: its latency hides behind it
-      const int st = j % ST;
-      if (j >= ST) mbar_wait(kv_empty(st), ((j / ST) - 1) & 1);
-      const int ts = t_begin + j * BN;
-      const int n_ok = min(ppt, (t_end - ts + P - 1) / P);
-      if (lane == 0) mbar_arrive_expect_tx(kv_full(st), (uint32_t)(n_ok * P * (D * 2 * 2)));
-      __syncwarp();
-      if (page >= 0) {
-        const uint32_t kdst = sbase + C::OFF_KV + st * (2 * KV_TILE_B) + lane * P * 128;
-        const uint32_t vdst = kdst + KV_TILE_B;
-        tma_load_5d(kdst, &tm_k, kv_full(st), 0, 0, g, page, layer);
-        tma_load_5d(kdst + BN * 128, &tm_k, kv_full(st), 64, 0, g, page, layer);
-        tma_load_5d(vdst, &tm_v, kv_full(st), 0, 0, g, page, layer);
-        tma_load_5d(vdst + BN * 128, &tm_v, kv_full(st), 64, 0, g, page, layer);
+      const int page_next = page_of(j + 1);
+      if (round > 0) mbar_wait(empty0 + 8 * st, (round - 1) & 1);
+      const int n_ok = min(ppt, n_pages_split - j * ppt);
+      const uint32_t dst = ring + st * KV_TILE_B;
+      const uint32_t bar = full0 + 8 * st;
+      if (elect_one()) mbar_arrive_expect_tx(bar, (uint32_t)(n_ok * P * (D * 2)));
+#pragma unroll 1
+      for (int i = 0; i < n_ok; ++i) {
+        const int pg = __shfl_sync(0xffffffffu, page, i);
+        tma_load_5d(dst + i * P * 128, tm, bar, 0, 0, g, pg, layer);
+        tma_load_5d(dst + i * P * 128 + BN * 128, tm, bar, 64, 0, g, pg, layer);
       }
       page = page_next;
+      if (++st == NS) {
+        st = 0;
+        ++round;
+      }
     }
   } else if (warp == C::MMA_WARP) {
     // ======================================= MMA issuer =====================================
@@ -271,15 +334,44 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
       constexpr uint32_t IDESC_S = idesc_f16(BN, false);
       constexpr uint32_t IDESC_O = idesc_f16(D, true);
       mbar_wait(q_full, 0);
+      // operand descriptors: a fixed part per operand, plus (byte offset >> 4) in the 14-bit address field
+      const uint64_t qdesc0 = smem_desc(sbase + C::OFF_Q, 16, 1024);
+      const uint64_t kdesc0 = smem_desc(sbase + C::OFF_K, 16, 1024);
+      const uint64_t pdesc0 = smem_desc(sbase + C::OFF_P, 16, 1024);
+      const uint64_t vdesc0 = smem_desc(sbase + C::OFF_V, BN * 128, 1024);   // MN-major: LBO = next 64-column half
+      int sk = 0, rk = 0;                            // K ring position of the next Q K^T
       auto issue_qk = [&](int j) {
-        const int st = j % ST;
-        mbar_wait(kv_full(st), (j / ST) & 1);
-        const uint32_t kaddr = sbase + C::OFF_KV + st * (2 * KV_TILE_B);
+        mbar_wait(k_full(sk), rk & 1);
+        const uint64_t kdesc = kdesc0 + (uint64_t)((sk * KV_TILE_B) >> 4);
+        tc_fence_after();
+#pragma unroll
+        for (int t = 0; t < NQ; ++t) {
+          if (t < nq_eff) {
+#pragma unroll
+            for (int k = 0; k < D / 16; ++k) {
+              const uint64_t a = qdesc0 + (uint64_t)((t * Q_TILE_B + (k >> 2) * (BM * 128) + (k & 3) * 32) >> 4);
+              const uint64_t b = kdesc + (uint64_t)(((k >> 2) * (BN * 128) + (k & 3) * 32) >> 4);
+              umma_ss(tmem_base + (2 * t + (j & 1)) * BN, a, b, IDESC_S, k > 0);
+            }
+            umma_commit(s_full(t, j & 1));
+          }
+        }
+        umma_commit(k_empty(sk));                    // the K stage is free once these MMAs have read it
+        if (++sk == SK) {
+          sk = 0;
+          ++rk;
+        }
+      };
+      issue_qk(0);
+      int sv = 0, rv = 0;
+      for (int j = 0; j < n_tiles; ++j) {
+        if (j + 1 < n_tiles) issue_qk(j + 1);
+        mbar_wait(v_full(sv), rv & 1);
         const int ts = t_begin + j * BN;
         if (ts + BN > t_end) {
           // ragged last tile: zero the V rows that hold no token of this split (whole warp)
           const int r0 = t_end - ts;
-          unsigned char *vt = smem + C::OFF_KV + st * (2 * KV_TILE_B) + KV_TILE_B;
+          unsigned char *vt = smem + C::OFF_V + sv * KV_TILE_B;
           for (int i = lane; i < (BN - r0) * 16; i += 32) {
             const int row = r0 + (i >> 4), c = i & 15;
             *reinterpret_cast<uint4 *>(vt + (c >> 3) * (BN * 128) + row * 128 + ((c & 7) << 4)) = make_uint4(0, 0, 0, 0);
@@ -287,70 +379,65 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
           fence_proxy_async();
           __syncwarp();
         }
-        tc_fence_after();
-        if (lane == 0) {
-#pragma unroll
-          for (int t = 0; t < NQ; ++t) {
-#pragma unroll
-            for (int k = 0; k < D / 16; ++k) {
-              const uint64_t a = smem_desc(sbase + C::OFF_Q + t * Q_TILE_B + (k >> 2) * (BM * 128) + (k & 3) * 32, 16, 1024);
-              const uint64_t b = smem_desc(kaddr + (k >> 2) * (BN * 128) + (k & 3) * 32, 16, 1024);
-              umma_ss(tmem_base + (2 * t + (j & 1)) * BN, a, b, IDESC_S, k > 0);
-            }
-            umma_commit(s_full(t, j & 1));
-          }
-        }
-        __syncwarp();
-      };
-      issue_qk(0);
-      for (int j = 0; j < n_tiles; ++j) {
-        if (j + 1 < n_tiles) issue_qk(j + 1);
-        const int st = j % ST;
-        const uint32_t vaddr = sbase + C::OFF_KV + st * (2 * KV_TILE_B) + KV_TILE_B;
+        const uint64_t vdesc = vdesc0 + (uint64_t)((sv * KV_TILE_B) >> 4);
 #pragma unroll
         for (int t = 0; t < NQ; ++t) {
-          mbar_wait(p_full(t, j & 1), (j >> 1) & 1);
-          tc_fence_after();
-          if (lane == 0) {
-            const uint32_t paddr = sbase + C::OFF_P + (2 * t + (j & 1)) * P_BYTES;
+          if (t < nq_eff) {
+            mbar_wait(p_full(t, j & 1), (j >> 1) & 1);
+            tc_fence_after();
+            const uint64_t pdesc = pdesc0 + (uint64_t)(((2 * t + (j & 1)) * P_BYTES) >> 4);
             const uint32_t tmem_o = tmem_base + NQ * 128 + t * 128;
 #pragma unroll
-            for (int k = 0; k < BN / 16; ++k) {
-              const uint64_t a = smem_desc(paddr + k * 32, 16, 1024);
-              const uint64_t b = smem_desc(vaddr + k * 2048, BN * 128, 1024);   // MN-major: LBO = next 64-column half
-              umma_ss(tmem_o, a, b, IDESC_O, (j > 0 || k > 0) ? 1u : 0u);
-            }
-            if (t == NQ - 1) umma_commit(kv_empty(st));
+            for (int k = 0; k < BN / 16; ++k)
+              umma_ss(tmem_o, pdesc + (uint64_t)((k * 32) >> 4), vdesc + (uint64_t)((k * 2048) >> 4), IDESC_O, (j > 0 || k > 0) ? 1u : 0u);
+            if (t == nq_eff - 1) umma_commit(v_empty(sv));
             umma_commit(pv_done(t, j & 1));
           }
-          __syncwarp();
+        }
+        if (++sv == SV) {
+          sv = 0;
+          ++rv;
         }
       }
     }
   } else {
     // ======================================= softmax ========================================
-    // Q tiles: rows r = row0 + row -> (token, head-in-group); rows past R are zero.  All softmax
-    // threads copy cooperatively (coalesced 16-B chunks), then hand Q to the MMA thread.
+    // Q tiles: MMA row m of tile t holds query row  row0 + t*BM + (m % rps)  -> (token, head-in-group); with
+    // dup > 1 the same query rows are replicated `dup` times (one copy per stream); rows past the valid ones
+    // are zero.  All softmax threads copy cooperatively (coalesced 16-B chunks), then hand Q to the MMA thread.
     for (int i = 0; i < 16; ++i) {
       const int ci = tid + C::N_SOFTMAX * i;
       const int row = ci >> 4, c = ci & 15;
-      const int r = row0 + row;
+      const int rt = row & (BM - 1), tq = row >> 7;
+      const int rl = rt & (rps - 1);
       uint4 val = make_uint4(0, 0, 0, 0);
-      if (r < R) {
+      if (rl < tile_rows(tq)) {
+        const int r = row0 + tq * BM + rl;
         const uint16_t *src = p.q + (((size_t)li * p.n_total + tk.tok_off + r / G) * p.n_q_heads + g * G + r % G) * D + c * 8;
         val = *reinterpret_cast<const uint4 *>(src);
       }
-      const int rt = row & (BM - 1);
-      const uint32_t dst = C::OFF_Q + (row >> 7) * Q_TILE_B + (c >> 3) * (BM * 128) + rt * 128 + (((c & 7) ^ (rt & 7)) << 4);
+      const uint32_t dst = C::OFF_Q + tq * Q_TILE_B + (c >> 3) * (BM * 128) + rt * 128 + (((c & 7) ^ (rt & 7)) << 4);
       *reinterpret_cast<uint4 *>(smem + dst) = val;
+    }
+    const int qt = warp >> 2;                  // Q tile of this warp
+    const int row = tid & (BM - 1);            // MMA row in the tile == TMEM lane
+    if (dup > 1 && qt == 0) {
+      // a stream writes only its own columns of P: the rest of the row stays zero for the whole kernel
+#pragma unroll
+      for (int b = 0; b < 2; ++b)
+#pragma unroll
+        for (int c8 = 0; c8 < 8; ++c8)
+          *reinterpret_cast<uint4 *>(smem + C::OFF_P + b * P_BYTES + row * 128 + (c8 << 4)) = make_uint4(0, 0, 0, 0);
     }
     fence_proxy_async();
     mbar_arrive(q_full);
 
-    const int qt = warp >> 2;                  // Q tile of this warp
-    const int row = tid & (BM - 1);            // row in the tile == TMEM lane
-    const int r = row0 + qt * BM + row;
-    const bool valid = r < R;
+    const int strm = row / rps;                // stream of this thread: columns [strm*NC, strm*NC + NC) of every tile
+    const int rl = row & (rps - 1);
+    const int r = row0 + qt * BM + rl;
+    const bool tile_used = qt < nq_eff;
+    const bool active = tile_used && warp_active(qt, warp & 3);
+    const bool valid = tile_used && rl < tile_rows(qt);
     const int lim = valid ? min(pos[r / G], t_end - 1) : -1;
     const uint32_t lane_addr = ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t tmem_s = tmem_base + lane_addr + (2 * qt) * BN;
@@ -358,119 +445,195 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
     const float sc = p.scale_log2;
     float m_ref = -INFINITY;                   // reference max used for exp2 (may lag the true max by < TAU)
     float l = 0.f;
-    for (int j = 0; j < n_tiles; ++j) {
-      const int ts = t_begin + j * BN;
-      const int b = j & 1;
-      mbar_wait(s_full(qt, b), (j >> 1) & 1);
-      tc_fence_after();
-      uint32_t sreg[2][32];
-      TMEM_LD_32(tmem_s + b * BN, sreg[0]);
-      TMEM_LD_32(tmem_s + b * BN + 32, sreg[1]);
-      tmem_wait_ld();
-      if (ts + BN - 1 > lim) {
-#pragma unroll
-        for (int h = 0; h < 2; ++h)
-#pragma unroll
-          for (int c = 0; c < 32; ++c)
-            if (ts + h * 32 + c > lim) sreg[h][c] = 0xff800000u;   // -inf, by selection (S may be garbage there)
-      }
-      float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-#pragma unroll
-      for (int h = 0; h < 2; ++h)
-#pragma unroll
-        for (int c = 0; c < 32; ++c) mx4[c & 3] = fmaxf(mx4[c & 3], __uint_as_float(sreg[h][c]));
-      const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
-      const float m_new = fmaxf(m_ref, mx * sc);
-      // lazy rescale: move the reference only when it is too far behind
-      float factor = 1.f;
-      const bool bump = (m_new - m_ref > RESCALE_TAU) || (m_ref == -INFINITY && m_new != -INFINITY);
-      if (bump) {
-        factor = (m_ref == -INFINITY) ? 0.f : ex2_approx(m_ref - m_new);
-        m_ref = m_new;
-      }
-      if (j > 0 && __any_sync(0xffffffffu, bump)) {
-        // O holds tiles < j only once P V of tile j-1 has completed
-        mbar_wait(pv_done(qt, (j - 1) & 1), ((j - 1) >> 1) & 1);
+
+    auto softmax_tiles = [&](auto nc_tag) {
+      constexpr int NC = decltype(nc_tag)::value;       // S columns per thread and tile
+      const int c0 = strm * NC;
+      for (int j = 0; j < n_tiles; ++j) {
+        const int ts = t_begin + j * BN + c0;           // token of this thread's first column
+        const int b = j & 1;
+        mbar_wait(s_full(qt, b), (j >> 1) & 1);
         tc_fence_after();
-#pragma unroll
-        for (int ch = 0; ch < D / 32; ++ch) {
-          uint32_t oreg[32];
-          TMEM_LD_32(tmem_o + ch * 32, oreg);
-          tmem_wait_ld();
-#pragma unroll
-          for (int c = 0; c < 32; ++c) oreg[c] = __float_as_uint(__uint_as_float(oreg[c]) * factor);
-          TMEM_ST_32(tmem_o + ch * 32, oreg);
+        uint32_t sreg[NC];
+        if constexpr (NC == 64) {
+          TMEM_LD_32(tmem_s + b * BN, sreg);
+          TMEM_LD_32(tmem_s + b * BN + 32, (sreg + 32));
+        } else if constexpr (NC == 32) {
+          TMEM_LD_32(tmem_s + b * BN + c0, sreg);
+        } else {
+          TMEM_LD_16(tmem_s + b * BN + c0, sreg);
         }
-        tmem_wait_st();
-      }
-      l *= factor;
-      const float mu = m_ref == -INFINITY ? 0.f : m_ref;
-      // the P buffer of this parity was last read by P V of tile j-2
-      if (j >= 2) mbar_wait(pv_done(qt, b), ((j - 2) >> 1) & 1);
-      unsigned char *prow = smem + C::OFF_P + (2 * qt + b) * P_BYTES + row * 128;
-      float sum4[4] = {0.f, 0.f, 0.f, 0.f};
+        tmem_wait_ld();
+        if (ts + NC - 1 > lim) {
 #pragma unroll
-      for (int c8 = 0; c8 < 8; ++c8) {
-        float e[8];
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-          e[c] = ex2_approx(fmaf(__uint_as_float(sreg[c8 >> 2][(c8 & 3) * 8 + c]), sc, -mu));
-          sum4[c & 3] += e[c];
+          for (int c = 0; c < NC; ++c)
+            if (ts + c > lim) sreg[c] = 0xff800000u;     // -inf, by selection (S may be garbage there)
         }
-        uint4 v;
-        v.x = pack_bf16(e[0], e[1]);
-        v.y = pack_bf16(e[2], e[3]);
-        v.z = pack_bf16(e[4], e[5]);
-        v.w = pack_bf16(e[6], e[7]);
-        *reinterpret_cast<uint4 *>(prow + ((c8 ^ (row & 7)) << 4)) = v;
+        float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+        for (int c = 0; c < NC; ++c) mx4[c & 3] = fmaxf(mx4[c & 3], __uint_as_float(sreg[c]));
+        const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
+        const float m_new = fmaxf(m_ref, mx * sc);
+        // lazy rescale: move the reference only when it is too far behind
+        float factor = 1.f;
+        const bool bump = (m_new - m_ref > RESCALE_TAU) || (m_ref == -INFINITY && m_new != -INFINITY);
+        if (bump) {
+          factor = (m_ref == -INFINITY) ? 0.f : ex2_approx(m_ref - m_new);
+          m_ref = m_new;
+        }
+        if (j > 0 && __any_sync(0xffffffffu, bump)) {
+          // O holds tiles < j only once P V of tile j-1 has completed
+          mbar_wait(pv_done(qt, (j - 1) & 1), ((j - 1) >> 1) & 1);
+          tc_fence_after();
+#pragma unroll
+          for (int ch = 0; ch < D / 32; ++ch) {
+            uint32_t oreg[32];
+            TMEM_LD_32(tmem_o + ch * 32, oreg);
+            tmem_wait_ld();
+#pragma unroll
+            for (int c = 0; c < 32; ++c) oreg[c] = __float_as_uint(__uint_as_float(oreg[c]) * factor);
+            TMEM_ST_32(tmem_o + ch * 32, oreg);
+          }
+          tmem_wait_st();
+        }
+        l *= factor;
+        const float mu = m_ref == -INFINITY ? 0.f : m_ref;
+        // the P buffer of this parity was last read by P V of tile j-2
+        if (j >= 2) mbar_wait(pv_done(qt, b), ((j - 2) >> 1) & 1);
+        unsigned char *prow = smem + C::OFF_P + (2 * qt + b) * P_BYTES + row * 128;
+        float sum4[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int c8 = 0; c8 < NC / 8; ++c8) {
+          float e[8];
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            e[c] = ex2_approx(fmaf(__uint_as_float(sreg[c8 * 8 + c]), sc, -mu));
+            sum4[c & 3] += e[c];
+          }
+          uint4 v;
+          v.x = pack_bf16(e[0], e[1]);
+          v.y = pack_bf16(e[2], e[3]);
+          v.z = pack_bf16(e[4], e[5]);
+          v.w = pack_bf16(e[6], e[7]);
+          *reinterpret_cast<uint4 *>(prow + (((c0 >> 3) + c8) ^ (row & 7)) * 16) = v;
+        }
+        l += (sum4[0] + sum4[1]) + (sum4[2] + sum4[3]);
+        fence_proxy_async();
+        tc_fence_before();
+        mbar_arrive(p_full(qt, b));
       }
-      l += (sum4[0] + sum4[1]) + (sum4[2] + sum4[3]);
-      fence_proxy_async();
-      tc_fence_before();
-      mbar_arrive(p_full(qt, b));
+    };
+    if (active) {
+      if (dup == 1)
+        softmax_tiles(std::integral_constant<int, 64>{});
+      else if (dup == 2)
+        softmax_tiles(std::integral_constant<int, 32>{});
+      else
+        softmax_tiles(std::integral_constant<int, 16>{});
     }
 
-    // ---- epilogue: O / l -> bf16, or partials ---------------------------------------------
-    if (n_tiles > 0) {
+    // ---- epilogue: merge the streams, then O / l -> bf16, or partials ---------------------------
+    const bool have_o = active && n_tiles > 0;
+    if (have_o) {
       mbar_wait(pv_done(qt, (n_tiles - 1) & 1), ((n_tiles - 1) >> 1) & 1);
       tc_fence_after();
     }
-    const int i_tok = valid ? r / G : 0, hh = valid ? r % G : 0;
+    constexpr int MROW = D + 4;                // fp32 row stride of the merge buffer: conflict-free 16-B accesses
+    float *mbuf = reinterpret_cast<float *>(smem + C::OFF_K);                         // [BM][MROW], over the idle K/V rings
+    float2 *mlbuf = reinterpret_cast<float2 *>(smem + C::OFF_K + BM * MROW * 4);     // [BM] (m, l)
+    if (dup > 1 && qt == 0) {
+      if (strm > 0 && active) {
+#pragma unroll
+        for (int ch = 0; ch < D / 32; ++ch) {
+          uint32_t oreg[32];
+          if (have_o) {
+            TMEM_LD_32(tmem_o + ch * 32, oreg);
+            tmem_wait_ld();
+          } else {
+#pragma unroll
+            for (int c = 0; c < 32; ++c) oreg[c] = 0u;
+          }
+#pragma unroll
+          for (int c = 0; c < 32; c += 4)
+            *reinterpret_cast<uint4 *>(mbuf + row * MROW + ch * 32 + c) = make_uint4(oreg[c], oreg[c + 1], oreg[c + 2], oreg[c + 3]);
+        }
+        mlbuf[row] = make_float2(m_ref, l);
+      }
+      asm volatile("bar.sync 1, 128;" ::: "memory");   // the four softmax warps of Q tile 0
+    }
+    float w_own = 1.f, w_oth[3] = {0.f, 0.f, 0.f};
+    float m_out = m_ref, l_out = l;
+    const bool writer = valid && strm == 0;
+    if (writer && dup > 1) {
+      float M = m_ref;
+      for (int s = 1; s < dup; ++s) M = fmaxf(M, mlbuf[row + s * rps].x);
+      const float Mu = M == -INFINITY ? 0.f : M;
+      w_own = ex2_approx(m_ref - Mu);              // exp2(-inf) = 0 for a stream that saw nothing
+      float L = w_own * l;
+      for (int s = 1; s < dup; ++s) {
+        const float2 ml = mlbuf[row + s * rps];
+        w_oth[s - 1] = ex2_approx(ml.x - Mu);
+        L += w_oth[s - 1] * ml.y;
+      }
+      m_out = M;
+      l_out = L;
+    }
+    const int i_tok = writer ? r / G : 0, hh = writer ? r % G : 0;
     const size_t out_row = ((size_t)li * p.n_total + tk.tok_off + i_tok) * p.n_q_heads + g * G + hh;
     const size_t prow_i = ((size_t)(li * p.max_splits + split) * p.n_total + tk.tok_off + i_tok) * p.n_q_heads + g * G + hh;
     const bool final_out = tk.n_splits == 1;
-    const float inv = l > 0.f ? 1.f / l : 0.f;
+    const float inv = l_out > 0.f ? 1.f / l_out : 0.f;
+    if (strm == 0 && active) {
 #pragma unroll
-    for (int ch = 0; ch < D / 32; ++ch) {
-      uint32_t oreg[32];
-      if (n_tiles > 0) {
-        TMEM_LD_32(tmem_o + ch * 32, oreg);
-        tmem_wait_ld();
-      } else {
-#pragma unroll
-        for (int c = 0; c < 32; ++c) oreg[c] = 0u;
-      }
-      if (valid) {
-        if (final_out) {
-          uint16_t *dst = p.out + out_row * D + ch * 32;
-#pragma unroll
-          for (int c = 0; c < 32; c += 8) {
-            uint4 v;
-            v.x = pack_bf16(__uint_as_float(oreg[c]) * inv, __uint_as_float(oreg[c + 1]) * inv);
-            v.y = pack_bf16(__uint_as_float(oreg[c + 2]) * inv, __uint_as_float(oreg[c + 3]) * inv);
-            v.z = pack_bf16(__uint_as_float(oreg[c + 4]) * inv, __uint_as_float(oreg[c + 5]) * inv);
-            v.w = pack_bf16(__uint_as_float(oreg[c + 6]) * inv, __uint_as_float(oreg[c + 7]) * inv);
-            *reinterpret_cast<uint4 *>(dst + c) = v;
-          }
+      for (int ch = 0; ch < D / 32; ++ch) {
+        uint32_t oreg[32];
+        if (have_o) {
+          TMEM_LD_32(tmem_o + ch * 32, oreg);
+          tmem_wait_ld();
         } else {
-          float *dst = p.part_o + prow_i * D + ch * 32;
 #pragma unroll
-          for (int c = 0; c < 32; c += 4)
-            *reinterpret_cast<uint4 *>(dst + c) = make_uint4(oreg[c], oreg[c + 1], oreg[c + 2], oreg[c + 3]);
+          for (int c = 0; c < 32; ++c) oreg[c] = 0u;
+        }
+        if (writer) {
+          float o[32];
+#pragma unroll
+          for (int c = 0; c < 32; ++c) o[c] = __uint_as_float(oreg[c]);
+          if (dup > 1) {
+#pragma unroll
+            for (int c = 0; c < 32; ++c) o[c] *= w_own;
+            for (int s = 1; s < dup; ++s) {
+              const float *src = mbuf + (row + s * rps) * MROW + ch * 32;
+              const float w = w_oth[s - 1];
+#pragma unroll
+              for (int c = 0; c < 32; c += 4) {
+                const float4 x = *reinterpret_cast<const float4 *>(src + c);
+                o[c] = fmaf(w, x.x, o[c]);
+                o[c + 1] = fmaf(w, x.y, o[c + 1]);
+                o[c + 2] = fmaf(w, x.z, o[c + 2]);
+                o[c + 3] = fmaf(w, x.w, o[c + 3]);
+              }
+            }
+          }
+          if (final_out) {
+            uint16_t *dst = p.out + out_row * D + ch * 32;
+#pragma unroll
+            for (int c = 0; c < 32; c += 8) {
+              uint4 v;
+              v.x = pack_bf16(o[c] * inv, o[c + 1] * inv);
+              v.y = pack_bf16(o[c + 2] * inv, o[c + 3] * inv);
+              v.z = pack_bf16(o[c + 4] * inv, o[c + 5] * inv);
+              v.w = pack_bf16(o[c + 6] * inv, o[c + 7] * inv);
+              *reinterpret_cast<uint4 *>(dst + c) = v;
+            }
+          } else {
+            float *dst = p.part_o + prow_i * D + ch * 32;
+#pragma unroll
+            for (int c = 0; c < 32; c += 4) *reinterpret_cast<float4 *>(dst + c) = make_float4(o[c], o[c + 1], o[c + 2], o[c + 3]);
+          }
         }
       }
+      if (writer && !final_out) *reinterpret_cast<float2 *>(p.part_ml + prow_i * 2) = make_float2(m_out, l_out);
     }
-    if (valid && !final_out) *reinterpret_cast<float2 *>(p.part_ml + prow_i * 2) = make_float2(m_ref, l);
   }
 
   tc_fence_before();
