@@ -405,19 +405,31 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
     // Q tiles: MMA row m of tile t holds query row  row0 + t*BM + (m % rps)  -> (token, head-in-group); with
     // dup > 1 the same query rows are replicated `dup` times (one copy per stream); rows past the valid ones
     // are zero.  All softmax threads copy cooperatively (coalesced 16-B chunks), then hand Q to the MMA thread.
-    for (int i = 0; i < 16; ++i) {
-      const int ci = tid + C::N_SOFTMAX * i;
-      const int row = ci >> 4, c = ci & 15;
-      const int rt = row & (BM - 1), tq = row >> 7;
-      const int rl = rt & (rps - 1);
-      uint4 val = make_uint4(0, 0, 0, 0);
-      if (rl < tile_rows(tq)) {
-        const int r = row0 + tq * BM + rl;
-        const uint16_t *src = p.q + (((size_t)li * p.n_total + tk.tok_off + r / G) * p.n_q_heads + g * G + r % G) * D + c * 8;
-        val = *reinterpret_cast<const uint4 *>(src);
+    // All 16 loads of a thread are issued before the first store: one global-memory round trip per CTA
+    // instead of sixteen (the round-1 capture had 16 % of a softmax warp's life in this prologue).
+    {
+      uint4 qv[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        const int ci = tid + C::N_SOFTMAX * i;
+        const int row = ci >> 4, c = ci & 15;
+        const int rt = row & (BM - 1), tq = row >> 7;
+        const int rl = rt & (rps - 1);
+        qv[i] = make_uint4(0, 0, 0, 0);
+        if (rl < tile_rows(tq)) {
+          const int r = row0 + tq * BM + rl;
+          const uint16_t *src = p.q + (((size_t)li * p.n_total + tk.tok_off + r / G) * p.n_q_heads + g * G + r % G) * D + c * 8;
+          qv[i] = __ldg(reinterpret_cast<const uint4 *>(src));
+        }
       }
-      const uint32_t dst = C::OFF_Q + tq * Q_TILE_B + (c >> 3) * (BM * 128) + rt * 128 + (((c & 7) ^ (rt & 7)) << 4);
-      *reinterpret_cast<uint4 *>(smem + dst) = val;
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        const int ci = tid + C::N_SOFTMAX * i;
+        const int row = ci >> 4, c = ci & 15;
+        const int rt = row & (BM - 1), tq = row >> 7;
+        const uint32_t dst = C::OFF_Q + tq * Q_TILE_B + (c >> 3) * (BM * 128) + rt * 128 + (((c & 7) ^ (rt & 7)) << 4);
+        *reinterpret_cast<uint4 *>(smem + dst) = qv[i];
+      }
     }
     const int qt = warp >> 2;                  // Q tile of this warp
     const int row = tid & (BM - 1);            // MMA row in the tile == TMEM lane
