@@ -656,7 +656,8 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
   BlobWriter bw(slot->host, BLOB_BYTES);
   const uint64_t off_pos = bw.reserve(n_total * 4), off_toff = bw.reserve(n_total * 4), off_tspl = bw.reserve(n_total * 4);
   const uint64_t off_tasks = bw.reserve((uint64_t)pc.n_tasks * sizeof(fcg::AttnTaskDev));
-  if (off_pos == UINT64_MAX || off_toff == UINT64_MAX || off_tspl == UINT64_MAX || off_tasks == UINT64_MAX)
+  const uint64_t off_tasks2 = bw.reserve((uint64_t)pc.n_tasks * sizeof(fcg::AttnTaskDev));   // tcgen05 path: tasks by Q-tile class
+  if (off_pos == UINT64_MAX || off_toff == UINT64_MAX || off_tspl == UINT64_MAX || off_tasks == UINT64_MAX || off_tasks2 == UINT64_MAX)
     return fail(FCG_ERR_OUT_OF_ARENA, "patch blob exceeds %llu bytes", (unsigned long long)BLOB_BYTES);
   auto *h_pos = reinterpret_cast<int32_t *>(slot->host + off_pos);
   auto *h_toff = reinterpret_cast<int32_t *>(slot->host + off_toff);
@@ -668,9 +669,10 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
   int max_rows = 0;
   for (int t = 0; t < pc.n_tasks; ++t) max_rows = std::max(max_rows, pc.n_per_task[t] * G);
   const bool use_tc = lib->have_tma && max_rows >= lib->tc_min_rows;
-  const int q_tiles = max_rows > 128 ? 2 : 1;    // 128-row Q tiles per tcgen05 CTA
-  const int rows_per_cta = use_tc ? 128 * q_tiles : (max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64));
-  const int max_row_groups = (max_rows + rows_per_cta - 1) / rows_per_cta;
+  // tcgen05 path: a task with <= 128 rows per kv head runs CTAs with one 128-row Q tile (deep K/V rings: the
+  // HBM-bound regime), a task with more rows CTAs with two (K/V read once per 256 rows).  A batch that mixes
+  // both is launched as two grids, one per class.
+  auto rows_per_cta_of = [&](int rows) { return use_tc ? (rows > 128 ? 256 : 128) : (max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64)); };
   const int ctas_per_sm = use_tc ? 1 : fcg::attn_split_ctas_per_sm(c.head_dim);
   int max_splits = 1;
   int64_t tok_off = 0;
@@ -678,6 +680,7 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
     const int32_t n = pc.n_per_task[t];
     const int32_t kv_len = pc.positions[tok_off + n - 1] + 1;
     const int tiles = (kv_len + KV_TILE - 1) / KV_TILE;
+    const int rows_per_cta = rows_per_cta_of(n * G);
     const int rg = (n * G + rows_per_cta - 1) / rows_per_cta;
     const int64_t base = (int64_t)rg * c.n_kv_heads * pc.n_layers * pc.n_tasks;
     int ns = lib->force_splits > 0 ? std::min(lib->force_splits, tiles)
@@ -699,6 +702,12 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
     }
     tok_off += n;
   }
+  // tcgen05 path: the same descriptors again, grouped by Q-tile class (one 128-row tile first, then two)
+  auto *h_tasks2 = reinterpret_cast<fcg::AttnTaskDev *>(slot->host + off_tasks2);
+  int n_cls[2] = {0, 0};
+  for (int cl = 0; cl < 2; ++cl)
+    for (int t = 0; t < pc.n_tasks; ++t)
+      if ((h_tasks[t].n * G > 128) == (cl == 1)) h_tasks2[n_cls[0] * cl + n_cls[cl]++] = h_tasks[t];
   // partials live at the start of the scratch area
   const uint64_t part_rows = (uint64_t)pc.n_layers * max_splits * n_total * c.n_q_heads;
   const uint64_t part_o_bytes = max_splits > 1 ? align_up(part_rows * c.head_dim * 4) : 0;
@@ -747,15 +756,25 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
   ap.page_size = c.page_size;
   ap.n_tasks = pc.n_tasks;
   ap.max_splits = max_splits;
-  ap.max_row_groups = max_row_groups;
+  ap.max_row_groups = (max_rows + rows_per_cta_of(max_rows) - 1) / rows_per_cta_of(max_rows);
   ap.n_pages = c.n_pages;
   ap.scale_log2 = (float)(1.4426950408889634 / sqrt((double)c.head_dim));
   if (use_tc) {
-    FCG_CUDA(fcg::launch_attn_tc(ap, c.head_dim, q_tiles, &lib->tm_k, &lib->tm_v, pc.stream));
-    lib->stats.attn_tc_launches++;
+    for (int q_tiles = 1; q_tiles <= 2; ++q_tiles) {
+      fcg::AttnTaskDev *cls = h_tasks2 + n_cls[0] * (q_tiles - 1);
+      if (n_cls[q_tiles - 1] == 0) continue;
+      int rgs = 1;
+      for (int t = 0; t < n_cls[q_tiles - 1]; ++t) rgs = std::max(rgs, (cls[t].n * G + 128 * q_tiles - 1) / (128 * q_tiles));
+      fcg::AttnParams apc = ap;
+      apc.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(slot->dev + off_tasks2) + n_cls[0] * (q_tiles - 1);
+      apc.n_tasks = n_cls[q_tiles - 1];
+      apc.max_row_groups = rgs;
+      FCG_CUDA(fcg::launch_attn_tc(apc, c.head_dim, q_tiles, &lib->tm_k, &lib->tm_v, pc.stream));
+      lib->stats.attn_tc_launches++;
+    }
     lib->stats.last_attn_path = 2;
   } else {
-    FCG_CUDA(fcg::launch_attn_split(ap, c.head_dim, rows_per_cta, pc.stream));
+    FCG_CUDA(fcg::launch_attn_split(ap, c.head_dim, rows_per_cta_of(max_rows), pc.stream));
     lib->stats.attn_split_launches++;
     lib->stats.last_attn_path = 1;
   }

@@ -190,26 +190,34 @@ struct Cfg {
   // separate rings: a K stage is free again as soon as Q K^T of its tile has completed, a V stage only after P V
   static constexpr int K_STAGES = NQ == 1 ? 4 : 3;
   static constexpr int V_STAGES = NQ == 1 ? 6 : 3;
-  static constexpr int N_SOFTMAX = NQ * BM;
+  // Tile-parity streams (NQ == 1 only): two softmax warpgroups, group w owns the KV tiles j = w (mod 2), its own
+  // S / P buffer and its own O accumulator, with its own running (m, l); the streams are merged by log-sum-exp in
+  // the epilogue like the row streams.  Two softmax warps per SM sub-partition hide each other's latencies.
+  static constexpr int PS = NQ == 1 ? 2 : 1;
+  static constexpr int N_SOFTMAX = 256;                 // 8 warps: (Q tile | parity stream) x 4 lane quarters
   static constexpr int NTHREADS = N_SOFTMAX + 96;
-  static constexpr int KLOAD_WARP = 4 * NQ, VLOAD_WARP = 4 * NQ + 1, MMA_WARP = 4 * NQ + 2;
-  static constexpr int TMEM_COLS = NQ * 256;
+  static constexpr int KLOAD_WARP = 8, VLOAD_WARP = 9, MMA_WARP = 10;
+  static constexpr int TMEM_COLS = 512;                 // S: 2*NQ x 64 columns, O: NQ*PS x 128 columns
+  static constexpr int TMEM_O = NQ * 128;               // first O column
+  static constexpr int Q_ITERS = NQ * BM * 16 / N_SOFTMAX;
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + NQ * Q_TILE_B;                // K stage s at +s*KV_TILE_B
   static constexpr int OFF_V = OFF_K + K_STAGES * KV_TILE_B;         // V stage s at +s*KV_TILE_B
   static constexpr int OFF_P = OFF_V + V_STAGES * KV_TILE_B;         // P[t][b] at +(2t+b)*P_BYTES
   static constexpr int OFF_BAR = OFF_P + NQ * 2 * P_BYTES;
-  // k_full[SK], k_empty[SK], v_full[SV], v_empty[SV], s_full[NQ][2], p_full[NQ][2], pv_done[NQ][2], q_full
-  static constexpr int N_BARS = 2 * K_STAGES + 2 * V_STAGES + 6 * NQ + 1;
+  // k_full[SK], k_empty[SK], v_full[SV], v_empty[SV], s_full[NQ][2], p_full[NQ][2], pv_done[NQ][2], s_free[NQ][2],
+  // q_full, all_done
+  static constexpr int N_BARS = 2 * K_STAGES + 2 * V_STAGES + 8 * NQ + 2;
   static constexpr int SMEM_BYTES = OFF_BAR + N_BARS * 8 + 16 + 1024;   // + tmem slot + alignment slack
-  static_assert((K_STAGES + V_STAGES) * KV_TILE_B >= BM * (D + 4) * 4 + BM * 8, "merge buffer must fit in the idle rings");
+  static constexpr int MROW = D + 4;                    // fp32 row stride of the merge buffer: conflict-free 16-B accesses
+  static_assert((K_STAGES + V_STAGES) * KV_TILE_B >= PS * BM * MROW * 4 + PS * BM * 8, "merge buffer must fit in the idle rings");
 };
 
 template <int NQ>
 __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
     attn_tc_kernel(const AttnParams p, const __grid_constant__ TmaDesc tm_k, const __grid_constant__ TmaDesc tm_v) {
   using C = Cfg<NQ>;
-  constexpr int SK = C::K_STAGES, SV = C::V_STAGES;
+  constexpr int SK = C::K_STAGES, SV = C::V_STAGES, PS = C::PS;
   extern __shared__ unsigned char smem_raw[];
   // 1024-byte alignment for the 128B-swizzle atoms
   unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -226,7 +234,8 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
   if (split >= tk.n_splits || row0 >= R) return;
   const int g = blockIdx.y;
   const int layer = p.layer_begin + li;
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // tells the compiler that the warp index is warp-uniform
 
   // ---- row layout of this CTA (see "Row streams" in the header) ---------------------------------
   const int Rc = min(R - row0, NQ * BM);           // valid query rows of this CTA
@@ -250,7 +259,9 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
   auto s_full = [&](int t, int b) { return bar0 + 8 * (B0 + 2 * t + b); };
   auto p_full = [&](int t, int b) { return bar0 + 8 * (B0 + 2 * NQ + 2 * t + b); };
   auto pv_done = [&](int t, int b) { return bar0 + 8 * (B0 + 4 * NQ + 2 * t + b); };
-  const uint32_t q_full = bar0 + 8 * (B0 + 6 * NQ);
+  auto s_free = [&](int t, int b) { return bar0 + 8 * (B0 + 6 * NQ + 2 * t + b); };
+  const uint32_t q_full = bar0 + 8 * (B0 + 8 * NQ);
+  const uint32_t all_done = bar0 + 8 * (B0 + 8 * NQ + 1);
   const uint32_t tmem_slot = bar0 + 8 * C::N_BARS;
   volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem + C::OFF_BAR + 8 * C::N_BARS);
 
@@ -274,10 +285,12 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
       for (int b = 0; b < 2; ++b) {
         mbar_init(s_full(t, b), 1);
         mbar_init(p_full(t, b), 32 * max(act, 1));
+        mbar_init(s_free(t, b), 32 * max(act, 1));
         mbar_init(pv_done(t, b), 1);
       }
     }
     mbar_init(q_full, C::N_SOFTMAX);
+    mbar_init(all_done, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == C::MMA_WARP) tmem_alloc<C::TMEM_COLS>(tmem_slot);
@@ -291,43 +304,50 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
   if (warp == C::KLOAD_WARP || warp == C::VLOAD_WARP) {
     // ======================================= loaders =======================================
     // One warp streams K, one streams V: lanes 0..ppt-1 look up the pages of the NEXT tile (coalesced, latency
-    // hidden behind the ring wait); lane 0 then issues two box copies per page (the two 64-column halves).  All
-    // control flow is warp-uniform so that the TMA issue compiles to straight-line UTMALDG.
-    const bool is_k = warp == C::KLOAD_WARP;
-    const TmaDesc *tm = is_k ? &tm_k : &tm_v;
-    const int NS = is_k ? SK : SV;
-    const uint32_t ring = sbase + (is_k ? C::OFF_K : C::OFF_V);
-    const uint32_t full0 = is_k ? k_full(0) : v_full(0), empty0 = is_k ? k_empty(0) : v_empty(0);
-    const int P = p.page_size;
-    const int pshift = __ffs(P) - 1;
-    const int ppt = BN >> pshift;                   // pages per tile (P <= 64, power of two)
-    const int32_t *table = p.tables + tk.table_off + (t_begin >> pshift);
-    const int n_pages_split = (t_end - t_begin + P - 1) >> pshift;
-    auto page_of = [&](int j) -> int {
-      const int pi = j * ppt + lane;
-      return (lane < ppt && pi < n_pages_split) ? __ldg(table + pi) : -1;
-    };
-    int page = page_of(0);
-    int st = 0, round = 0;
-    for (int j = 0; j < n_tiles; ++j) {
-      const int page_next = page_of(j + 1);
-      if (round > 0) mbar_wait(empty0 + 8 * st, (round - 1) & 1);
-      const int n_ok = min(ppt, n_pages_split - j * ppt);
-      const uint32_t dst = ring + st * KV_TILE_B;
-      const uint32_t bar = full0 + 8 * st;
-      if (elect_one()) mbar_arrive_expect_tx(bar, (uint32_t)(n_ok * P * (D * 2)));
+    // hidden behind the ring wait); one elected lane then issues two box copies per page (the two 64-column
+    // halves).  K and V are separate instantiations so that everything but the page id is warp-uniform at compile
+    // time (tensor map, ring and barrier addresses stay in uniform registers; UTMALDG takes uniform operands).
+    auto load_stream = [&](auto is_k_tag) {
+      constexpr bool is_k = decltype(is_k_tag)::value;
+      const TmaDesc *tm = is_k ? &tm_k : &tm_v;
+      constexpr int NS = is_k ? SK : SV;
+      const uint32_t ring = sbase + (is_k ? C::OFF_K : C::OFF_V);
+      const uint32_t full0 = is_k ? k_full(0) : v_full(0), empty0 = is_k ? k_empty(0) : v_empty(0);
+      const int P = p.page_size;
+      const int pshift = __ffs(P) - 1;
+      const int ppt = BN >> pshift;                   // pages per tile (P <= 64, power of two)
+      const int32_t *table = p.tables + tk.table_off + (t_begin >> pshift);
+      const int n_pages_split = (t_end - t_begin + P - 1) >> pshift;
+      auto page_of = [&](int j) -> int {
+        const int pi = j * ppt + lane;
+        return (lane < ppt && pi < n_pages_split) ? __ldg(table + pi) : -1;
+      };
+      int page = page_of(0);
+      int st = 0, round = 0;
+      for (int j = 0; j < n_tiles; ++j) {
+        const int page_next = page_of(j + 1);
+        if (round > 0) mbar_wait(empty0 + 8 * st, (round - 1) & 1);
+        const int n_ok = min(ppt, n_pages_split - j * ppt);
+        const uint32_t dst = ring + st * KV_TILE_B;
+        const uint32_t bar = full0 + 8 * st;
+        if (elect_one()) mbar_arrive_expect_tx(bar, (uint32_t)(n_ok * P * (D * 2)));
 #pragma unroll 1
-      for (int i = 0; i < n_ok; ++i) {
-        const int pg = __shfl_sync(0xffffffffu, page, i);
-        tma_load_5d(dst + i * P * 128, tm, bar, 0, 0, g, pg, layer);
-        tma_load_5d(dst + i * P * 128 + BN * 128, tm, bar, 64, 0, g, pg, layer);
+        for (int i = 0; i < n_ok; ++i) {
+          const int pg = __shfl_sync(0xffffffffu, page, i);
+          tma_load_5d(dst + i * P * 128, tm, bar, 0, 0, g, pg, layer);
+          tma_load_5d(dst + i * P * 128 + BN * 128, tm, bar, 64, 0, g, pg, layer);
+        }
+        page = page_next;
+        if (++st == NS) {
+          st = 0;
+          ++round;
+        }
       }
-      page = page_next;
-      if (++st == NS) {
-        st = 0;
-        ++round;
-      }
-    }
+    };
+    if (warp == C::KLOAD_WARP)
+      load_stream(std::true_type{});
+    else
+      load_stream(std::false_type{});
   } else if (warp == C::MMA_WARP) {
     // ======================================= MMA issuer =====================================
     if (n_tiles > 0) {
@@ -341,6 +361,12 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
       const uint64_t vdesc0 = smem_desc(sbase + C::OFF_V, BN * 128, 1024);   // MN-major: LBO = next 64-column half
       int sk = 0, rk = 0;                            // K ring position of the next Q K^T
       auto issue_qk = [&](int j) {
+        // S[t][j&1] was last read by the softmax of tile j-2: reuse it as soon as those threads have loaded it
+        if (j >= 2) {
+#pragma unroll
+          for (int t = 0; t < NQ; ++t)
+            if (t < nq_eff) mbar_wait(s_free(t, j & 1), ((j - 2) >> 1) & 1);
+        }
         mbar_wait(k_full(sk), rk & 1);
         const uint64_t kdesc = kdesc0 + (uint64_t)((sk * KV_TILE_B) >> 4);
         tc_fence_after();
@@ -362,10 +388,8 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
           ++rk;
         }
       };
-      issue_qk(0);
       int sv = 0, rv = 0;
-      for (int j = 0; j < n_tiles; ++j) {
-        if (j + 1 < n_tiles) issue_qk(j + 1);
+      auto issue_pv = [&](int j) {
         mbar_wait(v_full(sv), rv & 1);
         const int ts = t_begin + j * BN;
         if (ts + BN > t_end) {
@@ -386,10 +410,11 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
             mbar_wait(p_full(t, j & 1), (j >> 1) & 1);
             tc_fence_after();
             const uint64_t pdesc = pdesc0 + (uint64_t)(((2 * t + (j & 1)) * P_BYTES) >> 4);
-            const uint32_t tmem_o = tmem_base + NQ * 128 + t * 128;
+            // O accumulator of (Q tile t | parity stream j % PS); the stream's first tile overwrites it
+            const uint32_t tmem_o = tmem_base + C::TMEM_O + (PS == 2 ? (j & 1) : t) * 128;
 #pragma unroll
             for (int k = 0; k < BN / 16; ++k)
-              umma_ss(tmem_o, pdesc + (uint64_t)((k * 32) >> 4), vdesc + (uint64_t)((k * 2048) >> 4), IDESC_O, (j > 0 || k > 0) ? 1u : 0u);
+              umma_ss(tmem_o, pdesc + (uint64_t)((k * 32) >> 4), vdesc + (uint64_t)((k * 2048) >> 4), IDESC_O, (j >= PS || k > 0) ? 1u : 0u);
             if (t == nq_eff - 1) umma_commit(v_empty(sv));
             umma_commit(pv_done(t, j & 1));
           }
@@ -398,7 +423,18 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
           sv = 0;
           ++rv;
         }
+      };
+      // Issue order = expected order of the events waited for.  One stream: S(j) loaded, P(j) written, S(j+1)
+      // loaded, ...  Two parity streams run half a tile apart: S(j) loaded, P(j-1) written, S(j+1) loaded, ...
+      constexpr int LAG = PS - 1;
+      issue_qk(0);
+      if (n_tiles > 1) issue_qk(1);
+      for (int j = 0; j < n_tiles; ++j) {
+        if (j + 2 < n_tiles) issue_qk(j + 2);
+        if (j >= LAG) issue_pv(j - LAG);
       }
+      for (int j = max(0, n_tiles - LAG); j < n_tiles; ++j) issue_pv(j);
+      umma_commit(all_done);
     }
   } else {
     // ======================================= softmax ========================================
@@ -408,9 +444,9 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
     // All 16 loads of a thread are issued before the first store: one global-memory round trip per CTA
     // instead of sixteen (the round-1 capture had 16 % of a softmax warp's life in this prologue).
     {
-      uint4 qv[16];
+      uint4 qv[C::Q_ITERS];
 #pragma unroll
-      for (int i = 0; i < 16; ++i) {
+      for (int i = 0; i < C::Q_ITERS; ++i) {
         const int ci = tid + C::N_SOFTMAX * i;
         const int row = ci >> 4, c = ci & 15;
         const int rt = row & (BM - 1), tq = row >> 7;
@@ -423,7 +459,7 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
         }
       }
 #pragma unroll
-      for (int i = 0; i < 16; ++i) {
+      for (int i = 0; i < C::Q_ITERS; ++i) {
         const int ci = tid + C::N_SOFTMAX * i;
         const int row = ci >> 4, c = ci & 15;
         const int rt = row & (BM - 1), tq = row >> 7;
@@ -431,20 +467,24 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
         *reinterpret_cast<uint4 *>(smem + dst) = qv[i];
       }
     }
-    const int qt = warp >> 2;                  // Q tile of this warp
+    const int wg = warp >> 2;                  // softmax warpgroup: the Q tile (NQ == 2) or the parity stream (NQ == 1)
+    const int qt = PS == 2 ? 0 : wg;           // Q tile of this warp
+    const int par = PS == 2 ? wg : 0;          // parity stream of this warp: KV tiles j = par (mod PS)
     const int row = tid & (BM - 1);            // MMA row in the tile == TMEM lane
     if (dup > 1 && qt == 0) {
       // a stream writes only its own columns of P: the rest of the row stays zero for the whole kernel
 #pragma unroll
-      for (int b = 0; b < 2; ++b)
+      for (int b = 0; b < 2; ++b) {
+        if (PS == 2 && b != par) continue;     // with parity streams, P[b] belongs to stream b
 #pragma unroll
         for (int c8 = 0; c8 < 8; ++c8)
           *reinterpret_cast<uint4 *>(smem + C::OFF_P + b * P_BYTES + row * 128 + (c8 << 4)) = make_uint4(0, 0, 0, 0);
+      }
     }
     fence_proxy_async();
     mbar_arrive(q_full);
 
-    const int strm = row / rps;                // stream of this thread: columns [strm*NC, strm*NC + NC) of every tile
+    const int strm = row / rps;                // row stream of this thread: columns [strm*NC, strm*NC + NC) of every tile
     const int rl = row & (rps - 1);
     const int r = row0 + qt * BM + rl;
     const bool tile_used = qt < nq_eff;
@@ -453,7 +493,7 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
     const int lim = valid ? min(pos[r / G], t_end - 1) : -1;
     const uint32_t lane_addr = ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t tmem_s = tmem_base + lane_addr + (2 * qt) * BN;
-    const uint32_t tmem_o = tmem_base + lane_addr + NQ * 128 + qt * 128;
+    const uint32_t tmem_o = tmem_base + lane_addr + C::TMEM_O + wg * 128;
     const float sc = p.scale_log2;
     float m_ref = -INFINITY;                   // reference max used for exp2 (may lag the true max by < TAU)
     float l = 0.f;
@@ -461,7 +501,7 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
     auto softmax_tiles = [&](auto nc_tag) {
       constexpr int NC = decltype(nc_tag)::value;       // S columns per thread and tile
       const int c0 = strm * NC;
-      for (int j = 0; j < n_tiles; ++j) {
+      for (int j = par; j < n_tiles; j += PS) {
         const int ts = t_begin + j * BN + c0;           // token of this thread's first column
         const int b = j & 1;
         mbar_wait(s_full(qt, b), (j >> 1) & 1);
@@ -476,6 +516,8 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
           TMEM_LD_16(tmem_s + b * BN + c0, sreg);
         }
         tmem_wait_ld();
+        tc_fence_before();
+        mbar_arrive(s_free(qt, b));                     // S[b] may be overwritten by Q K^T of tile j+2
         if (ts + NC - 1 > lim) {
 #pragma unroll
           for (int c = 0; c < NC; ++c)
@@ -493,9 +535,9 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
           factor = (m_ref == -INFINITY) ? 0.f : ex2_approx(m_ref - m_new);
           m_ref = m_new;
         }
-        if (j > 0 && __any_sync(0xffffffffu, bump)) {
-          // O holds tiles < j only once P V of tile j-1 has completed
-          mbar_wait(pv_done(qt, (j - 1) & 1), ((j - 1) >> 1) & 1);
+        if (j >= PS && __any_sync(0xffffffffu, bump)) {
+          // O holds the stream's earlier tiles only once P V of its previous tile j-PS has completed
+          mbar_wait(pv_done(qt, (j - PS) & 1), ((j - PS) >> 1) & 1);
           tc_fence_after();
 #pragma unroll
           for (int ch = 0; ch < D / 32; ++ch) {
@@ -545,16 +587,22 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
     }
 
     // ---- epilogue: merge the streams, then O / l -> bf16, or partials ---------------------------
-    const bool have_o = active && n_tiles > 0;
-    if (have_o) {
-      mbar_wait(pv_done(qt, (n_tiles - 1) & 1), ((n_tiles - 1) >> 1) & 1);
+    // all_done completes when every MMA of the CTA has: the accumulators are final and the K/V rings (which the
+    // merge buffer reuses) are idle.  A stream without any tile (n_tiles <= par) contributes (m, l) = (-inf, 0).
+    const bool have_o = active && n_tiles > par;
+    if (n_tiles > 0) {
+      mbar_wait(all_done, 0);
       tc_fence_after();
     }
-    constexpr int MROW = D + 4;                // fp32 row stride of the merge buffer: conflict-free 16-B accesses
-    float *mbuf = reinterpret_cast<float *>(smem + C::OFF_K);                         // [BM][MROW], over the idle K/V rings
-    float2 *mlbuf = reinterpret_cast<float2 *>(smem + C::OFF_K + BM * MROW * 4);     // [BM] (m, l)
-    if (dup > 1 && qt == 0) {
-      if (strm > 0 && active) {
+    constexpr int MROW = C::MROW;
+    float *mbuf = reinterpret_cast<float *>(smem + C::OFF_K);                              // [PS*BM][MROW], over the idle K/V rings
+    float2 *mlbuf = reinterpret_cast<float2 *>(smem + C::OFF_K + PS * BM * MROW * 4);     // [PS*BM] (m, l)
+    const int n_streams = dup * PS;                // streams holding a copy of each query row (Q tile 0 only)
+    const bool merging = n_streams > 1 && qt == 0;
+    const bool lead = strm == 0 && par == 0;       // the stream that merges and writes the row
+    const int mrow = par * BM + row;               // this thread's row in the merge buffer
+    if (merging) {
+      if (!lead && active) {
 #pragma unroll
         for (int ch = 0; ch < D / 32; ++ch) {
           uint32_t oreg[32];
@@ -567,25 +615,30 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
           }
 #pragma unroll
           for (int c = 0; c < 32; c += 4)
-            *reinterpret_cast<uint4 *>(mbuf + row * MROW + ch * 32 + c) = make_uint4(oreg[c], oreg[c + 1], oreg[c + 2], oreg[c + 3]);
+            *reinterpret_cast<uint4 *>(mbuf + mrow * MROW + ch * 32 + c) = make_uint4(oreg[c], oreg[c + 1], oreg[c + 2], oreg[c + 3]);
         }
-        mlbuf[row] = make_float2(m_ref, l);
+        mlbuf[mrow] = make_float2(m_ref, l);
       }
-      asm volatile("bar.sync 1, 128;" ::: "memory");   // the four softmax warps of Q tile 0
+      // the softmax warps that share Q tile 0: all eight with parity streams, else the tile's four
+      if (PS == 2)
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+      else
+        asm volatile("bar.sync 1, 128;" ::: "memory");
     }
-    float w_own = 1.f, w_oth[3] = {0.f, 0.f, 0.f};
+    float w_own = 1.f, w_oth[8];
     float m_out = m_ref, l_out = l;
-    const bool writer = valid && strm == 0;
-    if (writer && dup > 1) {
+    const bool writer = valid && lead;
+    if (writer && merging) {
+      // streams other than the lead: (parity sp, row stream ss) -> merge-buffer row sp*BM + ss*rps + rl
       float M = m_ref;
-      for (int s = 1; s < dup; ++s) M = fmaxf(M, mlbuf[row + s * rps].x);
+      for (int s = 1; s < n_streams; ++s) M = fmaxf(M, mlbuf[(s / dup) * BM + (s % dup) * rps + rl].x);
       const float Mu = M == -INFINITY ? 0.f : M;
       w_own = ex2_approx(m_ref - Mu);              // exp2(-inf) = 0 for a stream that saw nothing
       float L = w_own * l;
-      for (int s = 1; s < dup; ++s) {
-        const float2 ml = mlbuf[row + s * rps];
-        w_oth[s - 1] = ex2_approx(ml.x - Mu);
-        L += w_oth[s - 1] * ml.y;
+      for (int s = 1; s < n_streams; ++s) {
+        const float2 ml = mlbuf[(s / dup) * BM + (s % dup) * rps + rl];
+        w_oth[s] = ex2_approx(ml.x - Mu);
+        L += w_oth[s] * ml.y;
       }
       m_out = M;
       l_out = L;
@@ -595,7 +648,7 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
     const size_t prow_i = ((size_t)(li * p.max_splits + split) * p.n_total + tk.tok_off + i_tok) * p.n_q_heads + g * G + hh;
     const bool final_out = tk.n_splits == 1;
     const float inv = l_out > 0.f ? 1.f / l_out : 0.f;
-    if (strm == 0 && active) {
+    if (lead && active) {
 #pragma unroll
       for (int ch = 0; ch < D / 32; ++ch) {
         uint32_t oreg[32];
@@ -610,12 +663,12 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
           float o[32];
 #pragma unroll
           for (int c = 0; c < 32; ++c) o[c] = __uint_as_float(oreg[c]);
-          if (dup > 1) {
+          if (merging) {
 #pragma unroll
             for (int c = 0; c < 32; ++c) o[c] *= w_own;
-            for (int s = 1; s < dup; ++s) {
-              const float *src = mbuf + (row + s * rps) * MROW + ch * 32;
-              const float w = w_oth[s - 1];
+            for (int s = 1; s < n_streams; ++s) {
+              const float *src = mbuf + ((s / dup) * BM + (s % dup) * rps + rl) * MROW + ch * 32;
+              const float w = w_oth[s];
 #pragma unroll
               for (int c = 0; c < 32; c += 4) {
                 const float4 x = *reinterpret_cast<const float4 *>(src + c);
