@@ -57,6 +57,31 @@ def attn_bytes(cfg, wl) -> int:
     return total
 
 
+def attn_flops(cfg, wl) -> int:
+    """Q K^T and P V over the visible cache only: per layer, q head and patch token i, 4 * D * (p_i + 1) flops."""
+    vis = sum(int((np.asarray(t.positions, np.int64) + 1).sum()) for t in wl.tasks)
+    return 4 * cfg.head_dim * cfg.n_layers * cfg.n_q_heads * vis
+
+
+def attn_rows(cfg, wl) -> int:
+    """largest R = n * G (query rows per kv head) of the batch: intensity of patch attention is R flop/B."""
+    return max(len(t.positions) for t in wl.tasks) * (cfg.n_q_heads // cfg.n_kv_heads)
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
+# (profiles/r01_final.md); None where no capture of that workload is committed.
+NCU_TRAFFIC = {"C2": {"stitch": 4.179e9, "attn": 2.184e9}}
+
+
+def tensor_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        return float(p["bf16_tflops_sustained"]), "measured (MEASURED_PEAKS.json, sustained bf16 matmul)"
+    except Exception:
+        return 1400.0, "fallback (B200_PROFILING.md, sustained)"
+
+
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -235,6 +260,20 @@ def run_cuda(args, cfg, wl, seed):
 
     sb, ab = stitch_bytes(cfg, wl), attn_bytes(cfg, wl)
     peak, peak_src = peaks()
+    # patch attention: HBM-bound while R = n*G (flop per byte) is small, tensor-bound from R ~ 250
+    af, rows = attn_flops(cfg, wl), attn_rows(cfg, wl)
+    attn_s = float(np.mean(patch_ms)) * 1e-3
+    if rows >= 250:
+        tpeak, tsrc = tensor_peak()
+        attn_roof = {"bound": "tensor", "achieved": af / attn_s / 1e12, "peak": tpeak, "unit": "TFLOP/s",
+                     "frac": af / attn_s / 1e12 / tpeak, "peak_source": tsrc, "rows_per_kv_head": rows,
+                     "hbm_GBps": ab / attn_s / 1e9}
+    else:
+        attn_roof = {"bound": "hbm", "achieved": ab / attn_s / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": ab / attn_s / 1e9 / peak, "frac_of_8TBps": ab / attn_s / 1e9 / 8000.0,
+                     "rows_per_kv_head": rows, "TFLOPs": af / attn_s / 1e12}
+    attn_roof["traffic"] = NCU_TRAFFIC.get(args.config, {}).get("attn")
+    attn_roof["note"] = "timed as scatter + attention (+ combine); scatter is ~1 % of it"
     res = {
         "metric": METRIC, "value": world * (sb + ab) / (ms_per_step * 1e-3) / 1e9, "unit": "GB/s (algorithmic, whole graft)",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
@@ -254,9 +293,9 @@ def run_cuda(args, cfg, wl, seed):
         "roofline": {"kernel": "stitch_kernel (fused gather + RoPE-shift)", "bound": "hbm",
                      "achieved": sb / (np.mean(stitch_ms) * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                      "frac": sb / (np.mean(stitch_ms) * 1e-3) / 1e9 / peak, "peak_source": peak_src,
-                     "frac_of_8TBps": sb / (np.mean(stitch_ms) * 1e-3) / 1e9 / 8000.0, "traffic": args.traffic,
-                     "patch_attention": {"bound": "hbm", "achieved": ab / (np.mean(patch_ms) * 1e-3) / 1e9,
-                                         "frac": ab / (np.mean(patch_ms) * 1e-3) / 1e9 / peak}},
+                     "frac_of_8TBps": sb / (np.mean(stitch_ms) * 1e-3) / 1e9 / 8000.0,
+                     "traffic": args.traffic if args.traffic is not None else NCU_TRAFFIC.get(args.config, {}).get("stitch"),
+                     "patch_attention": attn_roof},
         "clocks": clocks,
     }
     if e2e:

@@ -702,12 +702,20 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
     }
     tok_off += n;
   }
-  // tcgen05 path: the same descriptors again, grouped by Q-tile class (one 128-row tile first, then two)
+  // tcgen05 path: the same descriptors again, grouped by CTA class (rows per kv head <= 64 | <= 128 | more)
   auto *h_tasks2 = reinterpret_cast<fcg::AttnTaskDev *>(slot->host + off_tasks2);
-  int n_cls[2] = {0, 0};
-  for (int cl = 0; cl < 2; ++cl)
-    for (int t = 0; t < pc.n_tasks; ++t)
-      if ((h_tasks[t].n * G > 128) == (cl == 1)) h_tasks2[n_cls[0] * cl + n_cls[cl]++] = h_tasks[t];
+  auto class_of = [&](int rows) { return rows <= 64 ? 0 : (rows <= 128 ? 1 : 2); };
+  int n_cls[3] = {0, 0, 0}, cls_begin[3] = {0, 0, 0};
+  for (int t = 0; t < pc.n_tasks; ++t) n_cls[class_of(h_tasks[t].n * G)]++;
+  cls_begin[1] = n_cls[0];
+  cls_begin[2] = n_cls[0] + n_cls[1];
+  {
+    int fill[3] = {0, 0, 0};
+    for (int t = 0; t < pc.n_tasks; ++t) {
+      const int cl = class_of(h_tasks[t].n * G);
+      h_tasks2[cls_begin[cl] + fill[cl]++] = h_tasks[t];
+    }
+  }
   // partials live at the start of the scratch area
   const uint64_t part_rows = (uint64_t)pc.n_layers * max_splits * n_total * c.n_q_heads;
   const uint64_t part_o_bytes = max_splits > 1 ? align_up(part_rows * c.head_dim * 4) : 0;
@@ -760,16 +768,19 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
   ap.n_pages = c.n_pages;
   ap.scale_log2 = (float)(1.4426950408889634 / sqrt((double)c.head_dim));
   if (use_tc) {
-    for (int q_tiles = 1; q_tiles <= 2; ++q_tiles) {
-      fcg::AttnTaskDev *cls = h_tasks2 + n_cls[0] * (q_tiles - 1);
-      if (n_cls[q_tiles - 1] == 0) continue;
+    // class 0: rows replicated 2x / 4x in one softmax warpgroup (HBM-bound; the deep K/V rings matter most);
+    // class 1: two tile-parity softmax warpgroups; class 2: two Q tiles per CTA
+    for (int cl = 0; cl < 3; ++cl) {
+      if (n_cls[cl] == 0) continue;
+      const int q_tiles = cl == 2 ? 2 : 1, parity_streams = cl == 1 ? 2 : 1;
+      const fcg::AttnTaskDev *cls = h_tasks2 + cls_begin[cl];
       int rgs = 1;
-      for (int t = 0; t < n_cls[q_tiles - 1]; ++t) rgs = std::max(rgs, (cls[t].n * G + 128 * q_tiles - 1) / (128 * q_tiles));
+      for (int t = 0; t < n_cls[cl]; ++t) rgs = std::max(rgs, (cls[t].n * G + 128 * q_tiles - 1) / (128 * q_tiles));
       fcg::AttnParams apc = ap;
-      apc.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(slot->dev + off_tasks2) + n_cls[0] * (q_tiles - 1);
-      apc.n_tasks = n_cls[q_tiles - 1];
+      apc.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(slot->dev + off_tasks2) + cls_begin[cl];
+      apc.n_tasks = n_cls[cl];
       apc.max_row_groups = rgs;
-      FCG_CUDA(fcg::launch_attn_tc(apc, c.head_dim, q_tiles, &lib->tm_k, &lib->tm_v, pc.stream));
+      FCG_CUDA(fcg::launch_attn_tc(apc, c.head_dim, q_tiles, parity_streams, &lib->tm_k, &lib->tm_v, pc.stream));
       lib->stats.attn_tc_launches++;
     }
     lib->stats.last_attn_path = 2;

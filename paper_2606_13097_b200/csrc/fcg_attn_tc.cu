@@ -185,7 +185,7 @@ constexpr int Q_TILE_B = BM * D * 2;          // two 64-column halves of [128][1
 constexpr int KV_TILE_B = BN * D * 2;         // two halves of [64][128 B]
 constexpr int P_BYTES = BM * BN * 2;          // [128][128 B]
 
-template <int NQ>
+template <int NQ, int PS_>
 struct Cfg {
   // separate rings: a K stage is free again as soon as Q K^T of its tile has completed, a V stage only after P V
   static constexpr int K_STAGES = NQ == 1 ? 4 : 3;
@@ -193,10 +193,11 @@ struct Cfg {
   // Tile-parity streams (NQ == 1 only): two softmax warpgroups, group w owns the KV tiles j = w (mod 2), its own
   // S / P buffer and its own O accumulator, with its own running (m, l); the streams are merged by log-sum-exp in
   // the epilogue like the row streams.  Two softmax warps per SM sub-partition hide each other's latencies.
-  static constexpr int PS = NQ == 1 ? 2 : 1;
-  static constexpr int N_SOFTMAX = 256;                 // 8 warps: (Q tile | parity stream) x 4 lane quarters
+  static constexpr int PS = PS_;
+  static_assert(PS == 1 || (PS == 2 && NQ == 1), "parity streams need the TMEM columns of the second Q tile");
+  static constexpr int N_SOFTMAX = 128 * NQ * PS;       // (Q tile | parity stream) x 4 lane quarters x 32 rows
   static constexpr int NTHREADS = N_SOFTMAX + 96;
-  static constexpr int KLOAD_WARP = 8, VLOAD_WARP = 9, MMA_WARP = 10;
+  static constexpr int KLOAD_WARP = N_SOFTMAX / 32, VLOAD_WARP = KLOAD_WARP + 1, MMA_WARP = KLOAD_WARP + 2;
   static constexpr int TMEM_COLS = 512;                 // S: 2*NQ x 64 columns, O: NQ*PS x 128 columns
   static constexpr int TMEM_O = NQ * 128;               // first O column
   static constexpr int Q_ITERS = NQ * BM * 16 / N_SOFTMAX;
@@ -213,10 +214,10 @@ struct Cfg {
   static_assert((K_STAGES + V_STAGES) * KV_TILE_B >= PS * BM * MROW * 4 + PS * BM * 8, "merge buffer must fit in the idle rings");
 };
 
-template <int NQ>
-__global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
+template <int NQ, int PS_>
+__global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
     attn_tc_kernel(const AttnParams p, const __grid_constant__ TmaDesc tm_k, const __grid_constant__ TmaDesc tm_v) {
-  using C = Cfg<NQ>;
+  using C = Cfg<NQ, PS_>;
   constexpr int SK = C::K_STAGES, SV = C::V_STAGES, PS = C::PS;
   extern __shared__ unsigned char smem_raw[];
   // 1024-byte alignment for the 128B-swizzle atoms
@@ -623,7 +624,7 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
       if (PS == 2)
         asm volatile("bar.sync 1, 256;" ::: "memory");
       else
-        asm volatile("bar.sync 1, 128;" ::: "memory");
+        asm volatile("bar.sync 1, 128;" ::: "memory");   // NQ == 2: only the four warps of Q tile 0 get here
     }
     float w_own = 1.f, w_oth[8];
     float m_out = m_ref, l_out = l;
@@ -709,28 +710,30 @@ __global__ void __launch_bounds__(Cfg<NQ>::NTHREADS, 1)
   }
 }
 
-template <int NQ>
+template <int NQ, int PS_>
 cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv, cudaStream_t stream) {
-  using C = Cfg<NQ>;
+  using C = Cfg<NQ, PS_>;
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, PS_>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     configured = true;
   }
   dim3 grid((unsigned)(p.max_splits * p.max_row_groups), (unsigned)p.n_kv_heads, (unsigned)(p.n_layers * p.n_tasks));
-  attn_tc_kernel<NQ><<<grid, C::NTHREADS, C::SMEM_BYTES, stream>>>(p, tk, tv);
+  attn_tc_kernel<NQ, PS_><<<grid, C::NTHREADS, C::SMEM_BYTES, stream>>>(p, tk, tv);
   return cudaGetLastError();
 }
 
 }  // namespace
 
 // q_tiles = 128-row Q tiles per CTA (1 or 2); p.max_row_groups counts groups of q_tiles*128 rows.
-cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, const TmaDesc *tm_k, const TmaDesc *tm_v,
-                           cudaStream_t stream) {
+// parity_streams (q_tiles == 1 only): 2 = two softmax warpgroups on alternating KV tiles, 1 = one warpgroup.
+cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, int parity_streams, const TmaDesc *tm_k,
+                           const TmaDesc *tm_v, cudaStream_t stream) {
   if (head_dim != 128 || !tm_k || !tm_v) return cudaErrorNotSupported;
-  if (q_tiles == 1) return launch_nq<1>(p, *tm_k, *tm_v, stream);
-  if (q_tiles == 2) return launch_nq<2>(p, *tm_k, *tm_v, stream);
+  if (q_tiles == 1 && parity_streams == 2) return launch_nq<1, 2>(p, *tm_k, *tm_v, stream);
+  if (q_tiles == 1) return launch_nq<1, 1>(p, *tm_k, *tm_v, stream);
+  if (q_tiles == 2) return launch_nq<2, 1>(p, *tm_k, *tm_v, stream);
   return cudaErrorInvalidValue;
 }
 

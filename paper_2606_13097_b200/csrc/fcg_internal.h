@@ -111,7 +111,7 @@ struct alignas(64) TmaDesc {
 // tcgen05 / TMEM path; q_tiles = 128-row Q tiles per CTA (1 or 2), p.max_row_groups counts groups of
 // q_tiles*128 rows.  tm_k / tm_v describe the K / V pool as a 5-D bf16 tensor (D, P, Hkv, n_pages, L)
 // with box (64, P, 1, 1, 1) and 128B swizzle (make_pool_tensor_map).
-cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, const TmaDesc *tm_k, const TmaDesc *tm_v,
-                           cudaStream_t stream);
+cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, int parity_streams, const TmaDesc *tm_k,
+                           const TmaDesc *tm_v, cudaStream_t stream);
 
 }  // namespace fcg
