@@ -180,6 +180,26 @@ __device__ __forceinline__ float ex2_approx(float x) {
   return y;
 }
 
+// exp2 of a pair on the FMA pipe: round-to-nearest split x = n + f with the 1.5 * 2^23 constant (n lands in the low
+// mantissa bits of t), a degree-3 minimax polynomial for 2^f on [-0.5, 0.5] (relative error 7.5e-5, far below the
+// bf16 rounding of P), and n added to the exponent field.  x <= RESCALE_TAU by construction; x < -126 (masked
+// columns are -inf) is clamped, giving 2^-126 instead of 0: below anything that survives in fp32 sums.
+__device__ __forceinline__ float2 ex2_poly2(float2 x) {
+  const float MAGIC = 12582912.f;
+  x.x = fmaxf(x.x, -126.f);
+  x.y = fmaxf(x.y, -126.f);
+  const float2 t = __fadd2_rn(x, make_float2(MAGIC, MAGIC));
+  const float2 n = __fadd2_rn(t, make_float2(-MAGIC, -MAGIC));
+  const float2 f = __fadd2_rn(x, make_float2(-n.x, -n.y));
+  float2 pl = __ffma2_rn(make_float2(0.0551716685f, 0.0551716685f), f, make_float2(0.2426111251f, 0.2426111251f));
+  pl = __ffma2_rn(pl, f, make_float2(0.6932609677f, 0.6932609677f));
+  pl = __ffma2_rn(pl, f, make_float2(0.9999280572f, 0.9999280572f));
+  float2 r;
+  r.x = __int_as_float(__float_as_int(pl.x) + (__float_as_int(t.x) << 23));
+  r.y = __int_as_float(__float_as_int(pl.y) + (__float_as_int(t.y) << 23));
+  return r;
+}
+
 // ---- shared memory map -------------------------------------------------------------------------
 constexpr int Q_TILE_B = BM * D * 2;          // two 64-column halves of [128][128 B]
 constexpr int KV_TILE_B = BN * D * 2;         // two halves of [64][128 B]
@@ -556,23 +576,32 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
         // the P buffer of this parity was last read by P V of tile j-2
         if (j >= 2) mbar_wait(pv_done(qt, b), ((j - 2) >> 1) & 1);
         unsigned char *prow = smem + C::OFF_P + (2 * qt + b) * P_BYTES + row * 128;
-        float sum4[4] = {0.f, 0.f, 0.f, 0.f};
+        // packed fp32 pairs (FFMA2 / FADD2) for the scale-subtract and the row sum.  In the tensor-bound layout
+        // (64 columns per thread) one pair in four takes its exp2 from the FMA pipe instead of the MUFU, whose
+        // 16 results per clock and SM would otherwise cost as many cycles per tile as the two MMAs.
+        constexpr int EMU_EVERY = NC == 64 ? 4 : 0;        // emulate pair q when q % EMU_EVERY == EMU_EVERY - 1
+        const float2 sc2 = make_float2(sc, sc), nmu2 = make_float2(-mu, -mu);
+        float2 sum2[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
 #pragma unroll
         for (int c8 = 0; c8 < NC / 8; ++c8) {
-          float e[8];
+          float2 e[4];
 #pragma unroll
-          for (int c = 0; c < 8; ++c) {
-            e[c] = ex2_approx(fmaf(__uint_as_float(sreg[c8 * 8 + c]), sc, -mu));
-            sum4[c & 3] += e[c];
+          for (int q = 0; q < 4; ++q) {
+            const float2 x = __ffma2_rn(make_float2(__uint_as_float(sreg[c8 * 8 + 2 * q]), __uint_as_float(sreg[c8 * 8 + 2 * q + 1])), sc2, nmu2);
+            if (EMU_EVERY > 0 && ((c8 * 4 + q) % (EMU_EVERY > 0 ? EMU_EVERY : 1)) == EMU_EVERY - 1)
+              e[q] = ex2_poly2(x);
+            else
+              e[q] = make_float2(ex2_approx(x.x), ex2_approx(x.y));
+            sum2[q & 1] = __fadd2_rn(sum2[q & 1], e[q]);
           }
           uint4 v;
-          v.x = pack_bf16(e[0], e[1]);
-          v.y = pack_bf16(e[2], e[3]);
-          v.z = pack_bf16(e[4], e[5]);
-          v.w = pack_bf16(e[6], e[7]);
+          v.x = pack_bf16(e[0].x, e[0].y);
+          v.y = pack_bf16(e[1].x, e[1].y);
+          v.z = pack_bf16(e[2].x, e[2].y);
+          v.w = pack_bf16(e[3].x, e[3].y);
           *reinterpret_cast<uint4 *>(prow + (((c0 >> 3) + c8) ^ (row & 7)) * 16) = v;
         }
-        l += (sum4[0] + sum4[1]) + (sum4[2] + sum4[3]);
+        l += (sum2[0].x + sum2[0].y) + (sum2[1].x + sum2[1].y);
         fence_proxy_async();
         tc_fence_before();
         mbar_arrive(p_full(qt, b));
