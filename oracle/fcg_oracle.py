@@ -26,9 +26,14 @@ not needed at run time; DESIGN.md "Readings" lists every choice R1..R14):
   fixes it: keys are re-rotated by the integer position delta (RoPE group law),
   values are untouched (R1).  Pair layout: HF half-split (R2).
 
+NEXT rows of SURVEY.md 8(f) stated here as well: interleaved RoPE pairs
+(rope_mode 2), ``task_shift`` (re-graft of the kept suffix after a patch of
+another length, Eq. 6) and ``segment_extract`` (`update` of Alg. 1B).
+
 Pinned by tests/test_oracle_pins.py (group law, identity, synthetic one-layer
-model, brute-force attention, closed forms, torch SDPA special case ...).  No
-function here is "parity unpinned".
+model, brute-force attention, closed forms, torch SDPA special case, complex
+multiplication for both pair layouts, a hand-computed paging example for
+task_shift, extract/stitch round trips ...).  No function here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -99,13 +104,18 @@ def rope_inv_freq(head_dim: int, base: float) -> np.ndarray:
     return np.power(np.float64(base), -2.0 * j / np.float64(head_dim))
 
 
-def rope_rotate_f64(x: np.ndarray, delta, inv_freq: np.ndarray) -> np.ndarray:
+ROPE_NONE, ROPE_HALF_SPLIT, ROPE_INTERLEAVED = 0, 1, 2
+
+
+def rope_rotate_f64(x: np.ndarray, delta, inv_freq: np.ndarray, rope_mode: int = ROPE_HALF_SPLIT) -> np.ndarray:
     """Rotate x[..., D] (fp64) by the position delta; result fp64, NOT rounded.
 
-    Half-split pairs (a, b) = (x[j], x[j + D/2]) (HF convention, DESIGN R2):
+    Pair j is (a, b) = (x[j], x[j + D/2]) for half-split pairs (HF convention,
+    DESIGN R2) or (x[2j], x[2j + 1]) for interleaved pairs (GPT-J / original
+    RoFormer convention):
         phi_j  = delta * theta_j
-        out[j]       = a cos(phi_j) - b sin(phi_j)
-        out[j + D/2] = b cos(phi_j) + a sin(phi_j)
+        a' = a cos(phi_j) - b sin(phi_j)
+        b' = b cos(phi_j) + a sin(phi_j)
     ``delta`` is an integer, or an array broadcastable against x[..., :1]
     (one delta per row).
     """
@@ -114,16 +124,23 @@ def rope_rotate_f64(x: np.ndarray, delta, inv_freq: np.ndarray) -> np.ndarray:
     half = D // 2
     phi = np.asarray(delta, dtype=np.float64)[..., None] * inv_freq     # scalar delta -> [D/2]; per-row -> [..., D/2]
     c, s = np.cos(phi), np.sin(phi)
-    a, b = x[..., :half], x[..., half:]
     out = np.empty_like(x)
-    out[..., :half] = a * c - b * s
-    out[..., half:] = b * c + a * s
+    if rope_mode == ROPE_HALF_SPLIT:
+        a, b = x[..., :half], x[..., half:]
+        out[..., :half] = a * c - b * s
+        out[..., half:] = b * c + a * s
+    elif rope_mode == ROPE_INTERLEAVED:
+        a, b = x[..., 0::2], x[..., 1::2]
+        out[..., 0::2] = a * c - b * s
+        out[..., 1::2] = b * c + a * s
+    else:
+        raise OracleError(FCG_ERR_INVALID_ARG, "rope_mode must be half-split (1) or interleaved (2) to rotate")
     return out
 
 
-def rope_shift_bf16(k_bits: np.ndarray, delta, inv_freq: np.ndarray) -> np.ndarray:
+def rope_shift_bf16(k_bits: np.ndarray, delta, inv_freq: np.ndarray, rope_mode: int = ROPE_HALF_SPLIT) -> np.ndarray:
     """bf16 keys -> bf16 keys rotated by ``delta``: fp64 arithmetic, one RNE."""
-    return f64_to_bf16(rope_rotate_f64(bf16_to_f64(k_bits), delta, inv_freq))
+    return f64_to_bf16(rope_rotate_f64(bf16_to_f64(k_bits), delta, inv_freq, rope_mode))
 
 
 # ----------------------------------------------------------------------------
@@ -311,7 +328,7 @@ class OracleLibrary:
                 if self.rope_mode == 0:
                     kc[:, :, dst] = seg.k[:, :, src]                       # pure gather
                 else:
-                    kc[:, :, dst] = rope_shift_bf16(seg.k[:, :, src], delta, self.inv_freq)
+                    kc[:, :, dst] = rope_shift_bf16(seg.k[:, :, src], delta, self.inv_freq, self.rope_mode)
                 vc[:, :, dst] = seg.v[:, :, src]                           # V: bit copy
                 filled[dst] = True
             self.tasks[plan.task_id] = Task(table, cap, T, filled, kc, vc, deltas)
@@ -362,6 +379,75 @@ class OracleLibrary:
         t.filled[pos] = True
         t.n_tokens = max(t.n_tokens, int(pos[-1]) + 1)
         return out
+
+    # -- NEXT-1: length-changing patch = re-graft of the suffix ------------------
+    def task_shift(self, task_id: int, src_begin: int, n_tokens: int, dst_begin: int) -> None:
+        """Move cache positions [src_begin, src_begin+n) of a live task to [dst_begin, dst_begin+n).
+
+        Eq. (6): after the erroneous span x_err is replaced by an x_mid of another
+        length, the kept suffix sits delta = dst_begin - src_begin positions further; its keys are
+        re-rotated by delta (same rule as stitching, DESIGN R1), values are bit-copied (DESIGN R15,
+        SURVEY 8(f) NEXT-1).  Source positions become unfilled, destination positions filled (a
+        destination position that was filled is overwritten).  T never shrinks.
+
+        Paging ("copy-on-shift", so that no page is read and written in the same pass): every logical
+        page touched by the destination range gets a fresh physical page from the pool (ascending
+        logical order); slots of those pages outside the destination range keep their old contents;
+        the old physical pages go back to the pool by the rule of task_release.  delta == 0 is a no-op.
+        """
+        if task_id not in self.tasks:
+            raise OracleError(FCG_ERR_BAD_TASK, f"unknown task {task_id}")
+        t = self.tasks[task_id]
+        if n_tokens <= 0 or src_begin < 0 or dst_begin < 0 or src_begin + n_tokens > t.capacity \
+                or dst_begin + n_tokens > t.capacity:
+            raise OracleError(FCG_ERR_RANGE, "shift range outside task capacity")
+        src = slice(src_begin, src_begin + n_tokens)
+        dst = slice(dst_begin, dst_begin + n_tokens)
+        if not np.all(t.filled[src]):
+            raise OracleError(FCG_ERR_UNFILLED, "shift source holds an unfilled position")
+        delta = dst_begin - src_begin
+        if delta == 0:
+            return
+        lp0, lp1 = dst_begin // self.P, (dst_begin + n_tokens - 1) // self.P
+        new_pages = self.pool.allocate(lp1 - lp0 + 1)           # raises OUT_OF_PAGES before any change
+        k_src = t.k[:, :, src].copy()
+        v_src = t.v[:, :, src].copy()
+        if self.rope_mode == ROPE_NONE:
+            t.k[:, :, dst] = k_src
+        else:
+            t.k[:, :, dst] = rope_shift_bf16(k_src, delta, self.inv_freq, self.rope_mode)
+        t.v[:, :, dst] = v_src
+        t.filled[src] = False
+        t.filled[dst] = True
+        old_pages = t.page_table[lp0:lp1 + 1]
+        t.page_table[lp0:lp1 + 1] = new_pages
+        self.pool.release(old_pages)
+        t.n_tokens = max(t.n_tokens, dst_begin + n_tokens)
+
+    # -- NEXT-2: `update` of Alg. 1B -- cut a function out of a live cache ---------
+    def segment_extract(self, task_id: int, begin: int, n_tokens: int, new_orig_start: int) -> int:
+        """New library segment from cache positions [begin, begin+n) of a live task (PAPER.md:81, 85:
+        `update` inserts the KV state of a newly generated function into the code cache; SURVEY 8(f)
+        NEXT-2).  Keys are re-rotated by delta = new_orig_start - begin so that the stored segment is
+        encoded as if its first token sat at new_orig_start (begin -> bit copy; 0 -> canonical form);
+        values are bit-copied.  Returns the segment id (lowest free id, as segment_register).
+        """
+        if task_id not in self.tasks:
+            raise OracleError(FCG_ERR_BAD_TASK, f"unknown task {task_id}")
+        t = self.tasks[task_id]
+        if n_tokens <= 0 or begin < 0 or begin + n_tokens > t.capacity:
+            raise OracleError(FCG_ERR_RANGE, "extract range outside task capacity")
+        if new_orig_start < 0:
+            raise OracleError(FCG_ERR_INVALID_ARG, "new_orig_start must be >= 0")
+        src = slice(begin, begin + n_tokens)
+        if not np.all(t.filled[src]):
+            raise OracleError(FCG_ERR_UNFILLED, "extract range holds an unfilled position")
+        delta = new_orig_start - begin
+        if self.rope_mode == ROPE_NONE or delta == 0:
+            k = t.k[:, :, src].copy()
+        else:
+            k = rope_shift_bf16(t.k[:, :, src], delta, self.inv_freq, self.rope_mode)
+        return self.segment_register(k, t.v[:, :, src], new_orig_start)
 
     def task_release(self, task_id: int) -> None:
         if task_id not in self.tasks:

@@ -498,3 +498,175 @@ def test_p11_page_size_does_not_change_logical_results():
         assert len(lib.tasks[0].page_table) == -(-22 // P)
     for o in outs[1:]:
         assert all(np.array_equal(a, b) for a, b in zip(outs[0], o))
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT rows: interleaved pairs, suffix re-graft (task_shift), segment extraction
+# ----------------------------------------------------------------------------------------------
+def _complex_shift_bits(k_bits, delta, th, interleaved=False):
+    """independent restatement of a key shift: complex multiplication in numpy complex128, one RNE."""
+    x = O.bf16_to_f64(k_bits)
+    half = x.shape[-1] // 2
+    z = (x[..., 0::2] + 1j * x[..., 1::2]) if interleaved else (x[..., :half] + 1j * x[..., half:])
+    z = z * np.exp(1j * delta * th)
+    out = np.empty_like(x)
+    if interleaved:
+        out[..., 0::2], out[..., 1::2] = z.real, z.imag
+    else:
+        out[..., :half], out[..., half:] = z.real, z.imag
+    return O.f64_to_bf16(out)
+
+
+def _pair_err_ok(a_bits, b_bits, c):
+    """|a - b| <= c * 2^-9 * |pair| per component (half-split pairs): the error of a rounded rotation is bounded
+    relative to the norm of its rotation pair, not to the component itself (a small component next to a large one
+    moves by many of its own ulps).  Two roundings with a rotation in between: c = 1 + sqrt(2) < 3."""
+    a, b = O.bf16_to_f64(a_bits), O.bf16_to_f64(b_bits)
+    half = a.shape[-1] // 2
+    norm = np.sqrt(b[..., :half] ** 2 + b[..., half:] ** 2)
+    tol = np.concatenate([norm, norm], axis=-1) * c * 2.0 ** -9
+    return bool(np.all(np.abs(a - b) <= tol))
+
+
+def test_rope_interleaved_matches_complex_multiplication_and_permuted_half_split():
+    D = 16
+    th = O.rope_inv_freq(D, 5e5)
+    k = RNG.standard_normal((6, D))
+    perm = np.concatenate([np.arange(0, D, 2), np.arange(1, D, 2)])       # interleaved -> half-split order
+    for delta in (-1234, -1, 0, 1, 513, 32767):
+        got = O.rope_rotate_f64(k, delta, th, O.ROPE_INTERLEAVED)
+        for r in range(6):
+            for j in range(D // 2):
+                z = complex(k[r, 2 * j], k[r, 2 * j + 1]) * cmath.exp(1j * delta * th[j])
+                assert math.isclose(got[r, 2 * j], z.real, rel_tol=0, abs_tol=1e-12)
+                assert math.isclose(got[r, 2 * j + 1], z.imag, rel_tol=0, abs_tol=1e-12)
+        # the two layouts are the same rotation up to the fixed permutation of the head dimension
+        via_half = O.rope_rotate_f64(k[:, perm], delta, th, O.ROPE_HALF_SPLIT)
+        assert np.array_equal(got[:, perm], via_half)
+    # D = 2 has a single pair: both layouts coincide with the closed form (cos d, sin d) of (1, 0)
+    one = O.rope_rotate_f64(np.array([[1.0, 0.0]]), 3, np.array([1.0]), O.ROPE_INTERLEAVED)
+    assert np.allclose(one, [[math.cos(3), math.sin(3)]], rtol=0, atol=1e-15)
+    with pytest.raises(O.OracleError):
+        O.rope_rotate_f64(k, 1, th, 0)
+
+
+def test_interleaved_library_stitch():
+    lib = _small_lib(rope_mode=O.ROPE_INTERLEAVED)
+    s, k, v = _reg(lib, 9, 40)
+    lib.stitch([O.Plan(0, [O.PlanEntry(s, 1, 8, 3)])])
+    t = lib.tasks[0]
+    assert t.deltas == [3 - 40 - 1]
+    assert np.array_equal(t.k[:, :, 3:11], _complex_shift_bits(k[:, :, 1:9], -38, lib.inv_freq, interleaved=True))
+    assert np.array_equal(t.v[:, :, 3:11], v[:, :, 1:9])
+
+
+def test_task_shift_semantics_pages_and_rejection():
+    """Hand-computed paging example (P = 4, pool of 8): capacity 12 -> pages [0,1,2]; moving [4,8) to [6,10)
+    re-pages logical pages 1 and 2 onto fresh pages 3 and 4, and returns 1, 2 to the pool in that order."""
+    lib = _small_lib(n_pages=8)
+    s, k, v = _reg(lib, 8, 0)
+    lib.stitch([O.Plan(0, [O.PlanEntry(s, 0, 8, 0)], [], 12)])
+    t = lib.tasks[0]
+    assert t.page_table == [0, 1, 2] and t.n_tokens == 8
+    k_before, v_before = t.k.copy(), t.v.copy()
+    lib.task_shift(0, 4, 4, 6)
+    assert t.page_table == [0, 3, 4]
+    assert lib.pool.allocate(2) == [1, 2]
+    assert np.array_equal(t.filled, [True] * 4 + [False] * 2 + [True] * 4 + [False] * 2)
+    assert t.n_tokens == 10
+    # V is a bit copy, K is the delta rotation of the bits that were in the cache (independent complex form)
+    assert np.array_equal(t.v[:, :, 6:10], v_before[:, :, 4:8])
+    assert np.array_equal(t.k[:, :, 6:10], _complex_shift_bits(k_before[:, :, 4:8], 2, lib.inv_freq))
+    # everything outside the destination range is untouched (incl. the vacated source slots' stale bits)
+    keep = np.r_[0:6, 10:12]
+    assert np.array_equal(t.k[:, :, keep], k_before[:, :, keep]) and np.array_equal(t.v[:, :, keep], v_before[:, :, keep])
+    # rejections change nothing
+    snap = (list(t.page_table), t.filled.copy(), t.k.copy(), lib.pool.available())
+    for args, status in (((0, 4, 2, 6), O.FCG_ERR_UNFILLED),        # source [4,6) is a hole now
+                         ((0, 6, 4, 9), O.FCG_ERR_RANGE),           # 9 + 4 > capacity 12
+                         ((0, -1, 2, 0), O.FCG_ERR_RANGE),
+                         ((0, 0, 0, 2), O.FCG_ERR_RANGE),
+                         ((7, 0, 2, 2), O.FCG_ERR_BAD_TASK)):
+        with pytest.raises(O.OracleError) as e:
+            lib.task_shift(*args)
+        assert e.value.status == status
+    lib.pool.allocate(lib.pool.available())                          # drain the pool
+    with pytest.raises(O.OracleError) as e:
+        lib.task_shift(0, 0, 4, 1)
+    assert e.value.status == O.FCG_ERR_OUT_OF_PAGES
+    assert snap[0] == t.page_table and np.array_equal(snap[1], t.filled) and np.array_equal(snap[2], t.k)
+    # delta 0 is a no-op even with an empty pool
+    lib.task_shift(0, 0, 4, 0)
+    assert snap[0] == t.page_table and np.array_equal(snap[1], t.filled)
+
+
+def test_task_shift_overlapping_moves_and_round_trip():
+    lib = _small_lib()
+    s, k, v = _reg(lib, 40, 17)
+    lib.stitch([O.Plan(0, [O.PlanEntry(s, 0, 40, 5)], [O.Hole(0, 5)], 64)])
+    t = lib.tasks[0]
+    k0, v0 = t.k[:, :, 5:45].copy(), t.v[:, :, 5:45].copy()
+    lib.task_shift(0, 20, 25, 23)            # overlapping move to the right (longer x_mid): +3
+    assert np.array_equal(t.v[:, :, 23:48], v0[:, :, 15:40])
+    assert np.array_equal(t.k[:, :, 23:48], _complex_shift_bits(k0[:, :, 15:40], 3, lib.inv_freq))
+    assert not t.filled[20:23].any() and t.filled[23:48].all() and t.filled[5:20].all()
+    lib.task_shift(0, 23, 25, 20)            # and back (shorter x_mid): -3
+    assert np.array_equal(t.v[:, :, 5:45], v0)
+    assert _pair_err_ok(t.k[:, :, 5:45], k0, 3.0)             # two roundings, one per move
+    assert np.array_equal(t.k[:, :, 5:20], k0[:, :, :15])     # the untouched prefix is bit-identical
+    assert t.filled[5:45].all() and not t.filled[45:].any()
+
+
+def test_task_shift_equals_fresh_prefill_for_synthetic_model():
+    """north_star's synthetic one-layer model, for the re-grafted suffix: keys moved by task_shift equal the
+    keys a prefill at the new positions would produce, up to the stored-bf16 and output roundings."""
+    D, d_model, n = 16, 24, 12
+    lib = O.OracleLibrary(1, 1, 1, D, page_size=4, n_pages=64)
+    th = lib.inv_freq
+    Wk = RNG.standard_normal((D, d_model)) / math.sqrt(d_model)
+    x = RNG.standard_normal((n, d_model))
+    k_raw = x @ Wk.T
+
+    def prefill(start):
+        pos = start + np.arange(n)
+        z = (k_raw[:, : D // 2] + 1j * k_raw[:, D // 2:]) * np.exp(1j * pos[:, None] * th[None, :])
+        return np.concatenate([z.real, z.imag], axis=1)
+
+    sid = lib.segment_register(O.f64_to_bf16(prefill(30))[None, None], _rand_bf16((1, 1, n, D)), 30)
+    lib.stitch([O.Plan(0, [O.PlanEntry(sid, 0, n, 30)], [O.Hole(0, 30)], 64)])      # identity graft at 30
+    lib.task_shift(0, 36, 6, 41)                                                   # suffix [36,42) -> [41,47)
+    got = O.bf16_to_f64(lib.tasks[0].k[0, 0, 41:47])
+    fresh = prefill(35)[6:]                                                        # tokens 6.. at positions 41..
+    norm = np.sqrt(fresh[:, : D // 2] ** 2 + fresh[:, D // 2:] ** 2)
+    tol = np.concatenate([norm, norm], axis=1) * 2.0 * 2.0 ** -8
+    assert np.all(np.abs(got - fresh) <= tol)
+
+
+def test_segment_extract_round_trips():
+    lib = _small_lib()
+    s, k, v = _reg(lib, 30, 100)
+    lib.stitch([O.Plan(0, [O.PlanEntry(s, 0, 30, 7)], [O.Hole(0, 7)], 40)])
+    t = lib.tasks[0]
+    # (a) keep the encoding of the cache: bit copy, and stitching it back at the same place is the identity
+    e0 = lib.segment_extract(0, 12, 10, 12)
+    assert e0 == 1 and lib.segments[e0].orig_start == 12 and lib.segments[e0].n_tokens == 10
+    assert np.array_equal(lib.segments[e0].k, t.k[:, :, 12:22]) and np.array_equal(lib.segments[e0].v, t.v[:, :, 12:22])
+    lib.stitch([O.Plan(1, [O.PlanEntry(e0, 0, 10, 12)], [O.Hole(0, 12)], 24)])
+    assert lib.tasks[1].deltas == [0]
+    assert np.array_equal(lib.tasks[1].k[:, :, 12:22], t.k[:, :, 12:22])
+    # (b) canonical form: un-rotated to position 0 (independent complex form), V untouched
+    e1 = lib.segment_extract(0, 12, 10, 0)
+    assert lib.segments[e1].orig_start == 0
+    assert np.array_equal(lib.segments[e1].k, _complex_shift_bits(t.k[:, :, 12:22], -12, lib.inv_freq))
+    assert np.array_equal(lib.segments[e1].v, t.v[:, :, 12:22])
+    # grafting the canonical segment back where it came from returns the keys up to two roundings
+    lib.stitch([O.Plan(2, [O.PlanEntry(e1, 0, 10, 12)], [O.Hole(0, 12)], 24)])
+    assert lib.tasks[2].deltas == [12]
+    assert _pair_err_ok(lib.tasks[2].k[:, :, 12:22], t.k[:, :, 12:22], 3.0)
+    # rejections
+    for args, status in (((0, 0, 10, 0), O.FCG_ERR_UNFILLED), ((0, 35, 10, 0), O.FCG_ERR_RANGE),
+                         ((0, 12, 10, -1), O.FCG_ERR_INVALID_ARG), ((9, 12, 10, 0), O.FCG_ERR_BAD_TASK)):
+        n_seg = len(lib.segments)
+        with pytest.raises(O.OracleError) as e:
+            lib.segment_extract(*args)
+        assert e.value.status == status and len(lib.segments) == n_seg
