@@ -54,7 +54,7 @@ enum {
   FCG_ERR_BAD_TASK = -9      /* task id out of range, already live (stitch) or not live (patch) */
 };
 
-enum { FCG_ROPE_NONE = 0, FCG_ROPE_HALF_SPLIT = 1 };
+enum { FCG_ROPE_NONE = 0, FCG_ROPE_HALF_SPLIT = 1, FCG_ROPE_INTERLEAVED = 2 };
 
 /* Geometry and capacities, fixed at create time.
  * Arena layout (all offsets 256-byte aligned, reported by fcg_pool_info):
@@ -69,7 +69,8 @@ typedef struct {
   int32_t n_kv_heads;
   int32_t head_dim;        /* 64 or 128 */
   int32_t page_size;       /* tokens per page: 8, 16, 32 or 64 */
-  int32_t rope_mode;       /* FCG_ROPE_NONE: stitch is a pure gather; FCG_ROPE_HALF_SPLIT: pairs (j, j + head_dim/2) (R2) */
+  int32_t rope_mode;       /* FCG_ROPE_NONE: stitch is a pure gather; FCG_ROPE_HALF_SPLIT: pairs (j, j + head_dim/2) (R2);
+                              FCG_ROPE_INTERLEAVED: pairs (2j, 2j + 1) */
   double rope_base;        /* theta_j = rope_base^(-2j/head_dim) (R3); ignored if inv_freq != NULL */
   const double *inv_freq;  /* host, optional [head_dim/2] override (scaled RoPE); copied at create */
   void *arena;             /* device */
@@ -163,6 +164,28 @@ fcg_status_t fcg_task_page_table_host(fcg_library_t *lib, int32_t task_id, int32
                                       int32_t *n_pages);
 /* Returns the task's pages to the pool (pushed so that they are re-issued in ascending logical order). */
 fcg_status_t fcg_task_release(fcg_library_t *lib, int32_t task_id);
+
+/* Suffix re-graft of a length-changing patch (Eq. 6, R15):
+ * moves cache positions [src_begin, src_begin + n_tokens) of a live task to [dst_begin, dst_begin + n_tokens),
+ * all layers and kv heads: keys re-rotated by delta = dst_begin - src_begin (the stitch rule R1; bit copy for
+ * FCG_ROPE_NONE), values bit-copied.  Source positions become unfilled, destination positions filled (filled
+ * destination positions are overwritten); T never shrinks.  Both ranges must lie inside the task's capacity
+ * (RANGE) and every source position must be filled (UNFILLED).  The ranges may overlap: every logical page the
+ * destination touches is given a fresh page from the pool (ascending logical order; OUT_OF_PAGES if the pool
+ * cannot supply them), slots of those pages outside the destination keep their contents, and the replaced pages
+ * return to the pool by the rule of fcg_task_release -- so the task's page table changes.  delta == 0 is a
+ * no-op.  Asynchronous on `stream`; a failing call leaves the library unchanged. */
+fcg_status_t fcg_task_shift(fcg_library_t *lib, int32_t task_id, int32_t src_begin, int32_t n_tokens,
+                            int32_t dst_begin, void *stream);
+
+/* Segment extraction (`update` of Alg. 1B): cuts cache positions
+ * [begin, begin + n_tokens) of a live task, all layers and kv heads, into a new library segment without a host
+ * round trip.  Keys are re-rotated by delta = new_orig_start - begin, i.e. stored as if the segment's first
+ * token sat at position new_orig_start (begin: bit copy; 0: canonical form); values are bit-copied.  The range
+ * must lie inside the capacity (RANGE) and be filled (UNFILLED); new_orig_start >= 0.  The id is the lowest free
+ * one, as for fcg_segment_register; OUT_OF_ARENA as there.  Asynchronous on `stream`. */
+fcg_status_t fcg_segment_extract(fcg_library_t *lib, int32_t task_id, int32_t begin, int32_t n_tokens,
+                                 int32_t new_orig_start, void *stream, int32_t *seg_id_out);
 
 /* Gathers logical tokens [begin, begin + n) of one layer of a task's cache into contiguous device
  * buffers k_out, v_out [n_kv_heads][n][head_dim] (bit copy through the page table; for tests and for

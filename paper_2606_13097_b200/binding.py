@@ -30,6 +30,7 @@ FCG_ERR_BAD_TASK = -9
 
 FCG_ROPE_NONE = 0
 FCG_ROPE_HALF_SPLIT = 1
+FCG_ROPE_INTERLEAVED = 2
 
 
 class FcgError(RuntimeError):
@@ -91,6 +92,8 @@ SYMBOLS = {
     "fcg_task_page_table": (_I, [_P, _I, C.POINTER(_P), _PI, _PI]),
     "fcg_task_page_table_host": (_I, [_P, _I, _PI, _I, _PI]),
     "fcg_task_release": (_I, [_P, _I]),
+    "fcg_task_shift": (_I, [_P, _I, _I, _I, _I, _P]),
+    "fcg_segment_extract": (_I, [_P, _I, _I, _I, _I, _P, _PI]),
     "fcg_task_read": (_I, [_P, _I, _I, _I, _I, _P, _P, _P]),
     "fcg_pool_info": (_I, [_P, C.POINTER(fcg_pool_info_t)]),
     "fcg_set_attn_policy": (_I, [_P, _I, _I]),
@@ -264,6 +267,17 @@ def fcg_task_release(handle, task_id) -> None:
     _check(load().fcg_task_release(handle, int(task_id)))
 
 
+def fcg_task_shift(handle, task_id, src_begin, n_tokens, dst_begin, stream=None) -> None:
+    _check(load().fcg_task_shift(handle, int(task_id), int(src_begin), int(n_tokens), int(dst_begin), _stream(stream)))
+
+
+def fcg_segment_extract(handle, task_id, begin, n_tokens, new_orig_start, stream=None) -> int:
+    sid = C.c_int32(-1)
+    _check(load().fcg_segment_extract(handle, int(task_id), int(begin), int(n_tokens), int(new_orig_start),
+                                      _stream(stream), C.byref(sid)))
+    return sid.value
+
+
 def fcg_task_read(handle, task_id, layer, begin, n, k_out, v_out, stream=None) -> None:
     _check(load().fcg_task_read(handle, int(task_id), int(layer), int(begin), int(n), _ptr(k_out), _ptr(v_out),
                                 _stream(stream)))
@@ -363,6 +377,12 @@ class FcgLibrary:
 
     def task_release(self, task_id):
         fcg_task_release(self.handle, task_id)
+
+    def task_shift(self, task_id, src_begin, n_tokens, dst_begin, stream=None):
+        fcg_task_shift(self.handle, task_id, src_begin, n_tokens, dst_begin, stream)
+
+    def segment_extract(self, task_id, begin, n_tokens, new_orig_start, stream=None) -> int:
+        return fcg_segment_extract(self.handle, task_id, begin, n_tokens, new_orig_start, stream)
 
     def pool_info(self) -> dict:
         return fcg_pool_info(self.handle)

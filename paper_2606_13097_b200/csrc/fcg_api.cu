@@ -107,8 +107,8 @@ bool geometry_ok(const fcg_config_t *c) {
   if (c->n_layers <= 0 || c->n_kv_heads <= 0 || c->n_q_heads <= 0 || c->n_q_heads % c->n_kv_heads) return false;
   if (c->head_dim != 64 && c->head_dim != 128) return false;
   if (c->page_size != 8 && c->page_size != 16 && c->page_size != 32 && c->page_size != 64) return false;
-  if (c->rope_mode != FCG_ROPE_NONE && c->rope_mode != FCG_ROPE_HALF_SPLIT) return false;
-  if (c->rope_mode == FCG_ROPE_HALF_SPLIT && !c->inv_freq && !(c->rope_base > 0.0)) return false;
+  if (c->rope_mode != FCG_ROPE_NONE && c->rope_mode != FCG_ROPE_HALF_SPLIT && c->rope_mode != FCG_ROPE_INTERLEAVED) return false;
+  if (c->rope_mode != FCG_ROPE_NONE && !c->inv_freq && !(c->rope_base > 0.0)) return false;
   if (c->max_segments <= 0 || c->max_tasks <= 0 || c->max_task_tokens <= 0 || c->n_pages == 0) return false;
   return true;
 }
@@ -183,6 +183,159 @@ struct BlobWriter {
     return off;
   }
 };
+
+// lowest free segment id and first-fit arena range for an n-token segment; nothing changes until commit
+struct SegmentSlot {
+  int32_t sid = -1;
+  size_t fi = 0;
+  uint64_t off = 0, bytes = 0;
+};
+
+fcg_status_t find_segment_slot(fcg_library *lib, int32_t n_tokens, SegmentSlot &sl) {
+  const fcg_config_t &c = lib->cfg;
+  sl.sid = -1;
+  for (int32_t i = 0; i < c.max_segments; ++i)
+    if (!lib->segments[i].live) {
+      sl.sid = i;
+      break;
+    }
+  if (sl.sid < 0) return fail(FCG_ERR_OUT_OF_ARENA, "segment table full (%d)", c.max_segments);
+  sl.bytes = lib->seg_bytes_for(n_tokens);
+  sl.fi = lib->seg_free.size();
+  for (size_t i = 0; i < lib->seg_free.size(); ++i)
+    if (lib->seg_free[i].bytes >= sl.bytes) {
+      sl.fi = i;
+      break;
+    }
+  if (sl.fi == lib->seg_free.size())
+    return fail(FCG_ERR_OUT_OF_ARENA, "no free arena range of %llu bytes for a %d-token segment", (unsigned long long)sl.bytes, n_tokens);
+  sl.off = lib->seg_free[sl.fi].off;
+  return FCG_OK;
+}
+
+void commit_segment_slot(fcg_library *lib, const SegmentSlot &sl, int32_t n_tokens, int32_t orig_start) {
+  if (lib->seg_free[sl.fi].bytes == sl.bytes)
+    lib->seg_free.erase(lib->seg_free.begin() + sl.fi);
+  else {
+    lib->seg_free[sl.fi].off += sl.bytes;
+    lib->seg_free[sl.fi].bytes -= sl.bytes;
+  }
+  SegmentRec &s = lib->segments[sl.sid];
+  s.live = true;
+  s.offset = sl.off;
+  s.bytes = sl.bytes;
+  s.n_tokens = n_tokens;
+  s.orig_start = orig_start;
+  lib->n_segments_live++;
+}
+
+// Host side of one launch of the gather + RoPE-shift kernel (S3): entries, chunks, the per-delta cos/sin table
+// and the page ids that go into page tables, packed into one pinned blob and shipped with one async H2D.
+struct GatherBuilder {
+  std::vector<fcg::StitchEntryDev> entries;
+  std::vector<fcg::StitchChunkDev> chunks;
+  std::vector<float4> table;
+  std::vector<int32_t> pages;                    // page ids, copied device-to-device into page tables after the H2D
+  std::map<int32_t, int32_t> table_of_delta;
+
+  // first float4 of the table of `delta`, or -1 for a bit copy
+  int32_t table_for(const fcg_library *lib, int32_t delta) {
+    if (lib->cfg.rope_mode == FCG_ROPE_NONE || delta == 0) return -1;
+    auto it = table_of_delta.find(delta);
+    if (it != table_of_delta.end()) return it->second;
+    const int half = lib->cfg.head_dim / 2;
+    const int32_t off = (int32_t)table.size();
+    table_of_delta[delta] = off;
+    for (int j = 0; j < half; ++j) {
+      const double phi = (double)delta * lib->inv_freq[j];
+      const double cs = cos(phi), sn = sin(phi);
+      // hi part: 16 significant bits, so that (bf16 x hi) is exact in fp32; lo: the remainder
+      auto split = [](double x, float &hi, float &lo) {
+        float f = (float)x;
+        uint32_t b;
+        memcpy(&b, &f, 4);
+        b = (b + 0x80u) & 0xffffff00u;
+        memcpy(&hi, &b, 4);
+        lo = (float)(x - (double)hi);
+      };
+      float4 t;
+      split(cs, t.x, t.y);
+      split(sn, t.z, t.w);
+      table.push_back(t);
+    }
+    return off;
+  }
+
+  // row-space descriptors (fcg_internal.h)
+  void pool_side(const fcg_library *lib, uint64_t &k, uint64_t &v, int64_t &layer_stride, int32_t &head_stride) const {
+    const fcg_config_t &c = lib->cfg;
+    k = (uint64_t)(uintptr_t)lib->k_pool();
+    v = (uint64_t)(uintptr_t)lib->v_pool();
+    layer_stride = (int64_t)c.n_pages * c.n_kv_heads * c.page_size;
+    head_stride = c.page_size;
+  }
+  void segment_side(const fcg_library *lib, uint64_t off, uint64_t bytes, int32_t n, uint64_t &k, uint64_t &v,
+                    int64_t &layer_stride, int32_t &head_stride) const {
+    k = (uint64_t)(uintptr_t)(lib->arena + off);
+    v = (uint64_t)(uintptr_t)(lib->arena + off + bytes / 2);
+    layer_stride = (int64_t)lib->cfg.n_kv_heads * n;
+    head_stride = n;
+  }
+  int32_t pool_tok(const fcg_library *lib, int32_t page, int32_t slot) const {
+    return page * lib->cfg.n_kv_heads * lib->cfg.page_size + slot;
+  }
+  uint64_t blob_bytes() const {
+    return align_up(entries.size() * sizeof(fcg::StitchEntryDev), 16) + align_up(chunks.size() * sizeof(fcg::StitchChunkDev), 16) +
+           align_up(pages.size() * sizeof(int32_t), 16) + table.size() * sizeof(float4);
+  }
+};
+
+struct GatherBlob {
+  BlobSlot *slot = nullptr;
+  uint64_t off_pages = 0;
+};
+
+// pack the builder into a blob slot, ship it, launch the kernel; page ids sit at out.off_pages of the slot
+fcg_status_t enqueue_gather(fcg_library *lib, const GatherBuilder &gb, cudaStream_t stream, GatherBlob &out) {
+  const fcg_config_t &c = lib->cfg;
+  if (gb.blob_bytes() > BLOB_BYTES) return fail(FCG_ERR_OUT_OF_ARENA, "plan blob of %llu bytes exceeds %llu", (unsigned long long)gb.blob_bytes(), (unsigned long long)BLOB_BYTES);
+  if ((uint64_t)c.n_pages * c.n_kv_heads * c.page_size > 0x7fffffffull) return fail(FCG_ERR_INVALID_ARG, "pool too large for 32-bit row offsets");
+  FCG_CUDA(cudaSetDevice(c.device));
+  BlobSlot *slot = nullptr;
+  fcg_status_t st = acquire_slot(lib, &slot);
+  if (st != FCG_OK) return st;
+  BlobWriter bw(slot->host, BLOB_BYTES);
+  const uint64_t off_entries = bw.reserve(gb.entries.size() * sizeof(fcg::StitchEntryDev));
+  const uint64_t off_chunks = bw.reserve(gb.chunks.size() * sizeof(fcg::StitchChunkDev));
+  const uint64_t off_pages = bw.reserve(gb.pages.size() * sizeof(int32_t));
+  const uint64_t off_table = bw.reserve(gb.table.size() * sizeof(float4));
+  if (!gb.entries.empty()) memcpy(slot->host + off_entries, gb.entries.data(), gb.entries.size() * sizeof(fcg::StitchEntryDev));
+  if (!gb.chunks.empty()) memcpy(slot->host + off_chunks, gb.chunks.data(), gb.chunks.size() * sizeof(fcg::StitchChunkDev));
+  if (!gb.pages.empty()) memcpy(slot->host + off_pages, gb.pages.data(), gb.pages.size() * sizeof(int32_t));
+  if (!gb.table.empty()) memcpy(slot->host + off_table, gb.table.data(), gb.table.size() * sizeof(float4));
+  if (bw.used > 0) FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, bw.used, cudaMemcpyHostToDevice, stream));
+  fcg::StitchParams sp;
+  sp.entries = reinterpret_cast<const fcg::StitchEntryDev *>(slot->dev + off_entries);
+  sp.chunks = reinterpret_cast<const fcg::StitchChunkDev *>(slot->dev + off_chunks);
+  sp.table = reinterpret_cast<const float4 *>(slot->dev + off_table);
+  sp.n_chunks = (int32_t)gb.chunks.size();
+  sp.n_layers = c.n_layers;
+  sp.n_kv_heads = c.n_kv_heads;
+  sp.interleaved = c.rope_mode == FCG_ROPE_INTERLEAVED ? 1 : 0;
+  if (!gb.chunks.empty()) {
+    FCG_CUDA(fcg::launch_stitch(sp, c.head_dim, stream));
+    lib->stats.stitch_launches++;
+  }
+  out.slot = slot;
+  out.off_pages = off_pages;
+  return FCG_OK;
+}
+
+fcg_status_t finish_gather(GatherBlob &gbl, cudaStream_t stream) {
+  FCG_CUDA(cudaEventRecord(gbl.slot->ev, stream));
+  gbl.slot->in_flight = true;
+  return FCG_OK;
+}
 
 }  // namespace
 
@@ -295,23 +448,11 @@ fcg_status_t fcg_segment_register(fcg_library_t *lib, const void *k, const void 
     }
   }
   if (((uintptr_t)k % 16) || ((uintptr_t)v % 16)) return fail(FCG_ERR_INVALID_ARG, "k and v must be 16-byte aligned");
-  int32_t sid = -1;
-  for (int32_t i = 0; i < c.max_segments; ++i)
-    if (!lib->segments[i].live) {
-      sid = i;
-      break;
-    }
-  if (sid < 0) return fail(FCG_ERR_OUT_OF_ARENA, "segment table full (%d)", c.max_segments);
-  const uint64_t bytes = lib->seg_bytes_for(n_tokens);
-  size_t fi = lib->seg_free.size();
-  for (size_t i = 0; i < lib->seg_free.size(); ++i)
-    if (lib->seg_free[i].bytes >= bytes) {
-      fi = i;
-      break;
-    }
-  if (fi == lib->seg_free.size())
-    return fail(FCG_ERR_OUT_OF_ARENA, "no free arena range of %llu bytes for a %d-token segment", (unsigned long long)bytes, n_tokens);
-  const uint64_t off = lib->seg_free[fi].off;
+  SegmentSlot sl;
+  fcg_status_t sst = find_segment_slot(lib, n_tokens, sl);
+  if (sst != FCG_OK) return sst;
+  const int32_t sid = sl.sid;
+  const uint64_t off = sl.off, bytes = sl.bytes;
 
   fcg::RegisterParams rp;
   rp.k_src = static_cast<const uint16_t *>(k);
@@ -329,20 +470,7 @@ fcg_status_t fcg_segment_register(fcg_library_t *lib, const void *k, const void 
   FCG_CUDA(fcg::launch_register_copy(rp, static_cast<cudaStream_t>(stream)));
   lib->stats.register_launches++;
 
-  // commit
-  if (lib->seg_free[fi].bytes == bytes)
-    lib->seg_free.erase(lib->seg_free.begin() + fi);
-  else {
-    lib->seg_free[fi].off += bytes;
-    lib->seg_free[fi].bytes -= bytes;
-  }
-  SegmentRec &s = lib->segments[sid];
-  s.live = true;
-  s.offset = off;
-  s.bytes = bytes;
-  s.n_tokens = n_tokens;
-  s.orig_start = orig_start;
-  lib->n_segments_live++;
+  commit_segment_slot(lib, sl, n_tokens, orig_start);
   *seg_id_out = sid;
   return FCG_OK;
 }
@@ -433,128 +561,57 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
   if (need_pages > (int64_t)lib->page_stack.size())
     return fail(FCG_ERR_OUT_OF_PAGES, "need %lld pages, %zu free", (long long)need_pages, lib->page_stack.size());
 
-  // ---- build the plan blob (host) --------------------------------------------------------------
-  FCG_CUDA(cudaSetDevice(c.device));
-  BlobSlot *slot = nullptr;
-  fcg_status_t st = acquire_slot(lib, &slot);
-  if (st != FCG_OK) return st;
-  const int P = c.page_size, half = c.head_dim / 2;
-  int64_t n_entries_total = 0, n_chunks_total = 0, n_table_pages = 0;
-  for (int i = 0; i < n_plans; ++i) {
-    n_entries_total += plans[i].n_entries;
-    n_table_pages += checked[i].n_pages;
-    for (int e = 0; e < plans[i].n_entries; ++e) {
-      const fcg_plan_entry_t &pe = plans[i].entries[e];
-      n_chunks_total += (pe.dst_offset + pe.n_tokens - 1) / P - pe.dst_offset / P + 1;
-    }
-  }
-  BlobWriter bw(slot->host, BLOB_BYTES);
-  const uint64_t off_entries = bw.reserve(n_entries_total * sizeof(fcg::StitchEntryDev));
-  const uint64_t off_chunks = bw.reserve(n_chunks_total * sizeof(fcg::StitchChunkDev));
-  const uint64_t off_pages = bw.reserve(n_table_pages * sizeof(int32_t));
-  const uint64_t off_table = bw.reserve(0);
-  if (off_entries == UINT64_MAX || off_chunks == UINT64_MAX || off_pages == UINT64_MAX || off_table == UINT64_MAX)
-    return fail(FCG_ERR_OUT_OF_ARENA, "stitch plan blob exceeds %llu bytes", (unsigned long long)BLOB_BYTES);
-  auto *entries = reinterpret_cast<fcg::StitchEntryDev *>(slot->host + off_entries);
-  auto *chunks = reinterpret_cast<fcg::StitchChunkDev *>(slot->host + off_chunks);
-  auto *pages = reinterpret_cast<int32_t *>(slot->host + off_pages);
-  auto *table = reinterpret_cast<float4 *>(slot->host + off_table);
-  const uint64_t table_cap = (BLOB_BYTES - off_table) / sizeof(float4);
-
+  // ---- build the launch (host) ----------------------------------------------------------------
+  const int P = c.page_size;
+  GatherBuilder gb;
   // page ids are taken from a COPY of the stack; committed only when everything has been enqueued
   std::vector<int32_t> stack = lib->page_stack;
-  std::map<int32_t, int32_t> table_of_delta;
-  uint64_t table_used = 0;
-  int64_t ei = 0, ci = 0, pi = 0;
   std::vector<int64_t> plan_page_base(n_plans);
   for (int i = 0; i < n_plans; ++i) {
-    plan_page_base[i] = pi;
+    plan_page_base[i] = (int64_t)gb.pages.size();
     for (int k = 0; k < checked[i].n_pages; ++k) {
-      pages[pi++] = stack.back();
+      gb.pages.push_back(stack.back());
       stack.pop_back();
     }
-    const int32_t *ptab = pages + plan_page_base[i];
-    for (int e = 0; e < plans[i].n_entries; ++e, ++ei) {
+    for (int e = 0; e < plans[i].n_entries; ++e) {
       const fcg_plan_entry_t &pe = plans[i].entries[e];
       const SegmentRec &s = lib->segments[pe.seg_id];
-      const int32_t delta = checked[i].deltas[e];
-      fcg::StitchEntryDev &de = entries[ei];
-      de.k_src = (uint64_t)(uintptr_t)(lib->arena + s.offset);
-      de.v_src = (uint64_t)(uintptr_t)(lib->arena + s.offset + s.bytes / 2);
-      de.seg_n = s.n_tokens;
-      de.pad0 = de.pad1 = 0;
-      if (c.rope_mode == FCG_ROPE_NONE || delta == 0) {
-        de.table_off = -1;
-      } else {
-        auto it = table_of_delta.find(delta);
-        if (it != table_of_delta.end()) {
-          de.table_off = it->second;
-        } else {
-          if (table_used + half > table_cap)
-            return fail(FCG_ERR_OUT_OF_ARENA, "stitch plan blob exceeds %llu bytes (rope tables)", (unsigned long long)BLOB_BYTES);
-          de.table_off = (int32_t)table_used;
-          table_of_delta[delta] = de.table_off;
-          for (int j = 0; j < half; ++j) {
-            const double phi = (double)delta * lib->inv_freq[j];
-            const double cs = cos(phi), sn = sin(phi);
-            // hi part: 16 significant bits, so that (bf16 x hi) is exact in fp32; lo: the remainder
-            auto split = [](double x, float &hi, float &lo) {
-              float f = (float)x;
-              uint32_t b;
-              memcpy(&b, &f, 4);
-              b = (b + 0x80u) & 0xffffff00u;
-              memcpy(&hi, &b, 4);
-              lo = (float)(x - (double)hi);
-            };
-            float4 t;
-            split(cs, t.x, t.y);
-            split(sn, t.z, t.w);
-            table[table_used + j] = t;
-          }
-          table_used += half;
-        }
-      }
+      fcg::StitchEntryDev de;
+      gb.segment_side(lib, s.offset, s.bytes, s.n_tokens, de.k_src, de.v_src, de.src_layer_stride, de.src_head_stride);
+      gb.pool_side(lib, de.k_dst, de.v_dst, de.dst_layer_stride, de.dst_head_stride);
+      de.table_off = gb.table_for(lib, checked[i].deltas[e]);
+      de.pad0 = 0;
+      const int32_t ei = (int32_t)gb.entries.size();
+      gb.entries.push_back(de);
       // chunks: one per destination page touched
       int32_t done = 0;
       while (done < pe.n_tokens) {
         const int32_t dst = pe.dst_offset + done;
         const int32_t slot0 = dst % P;
         const int32_t n = std::min(P - slot0, pe.n_tokens - done);
-        fcg::StitchChunkDev &dc = chunks[ci++];
-        dc.entry = (int32_t)ei;
-        dc.page = ptab[dst / P];
+        fcg::StitchChunkDev dc;
+        dc.entry = ei;
+        dc.dst_tok = gb.pool_tok(lib, gb.pages[plan_page_base[i] + dst / P], slot0);
         dc.src_tok = pe.src_begin + done;
-        dc.slot_ntok = slot0 | (n << 16);
+        dc.ntok = n;
+        gb.chunks.push_back(dc);
         done += n;
       }
     }
   }
-  const uint64_t blob_used = off_table + table_used * sizeof(float4);
 
-  // ---- enqueue: blob, page tables, kernel -----------------------------------------------------
-  FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, blob_used, cudaMemcpyHostToDevice, stream));
+  // ---- enqueue: blob, kernel, page tables -----------------------------------------------------
+  GatherBlob gbl;
+  fcg_status_t st = enqueue_gather(lib, gb, stream, gbl);
+  if (st != FCG_OK) return st;
   for (int i = 0; i < n_plans; ++i) {
     int32_t *dst = lib->tables() + (int64_t)plans[i].task_id * lib->pages_per_task;
-    FCG_CUDA(cudaMemcpyAsync(dst, slot->dev + off_pages + plan_page_base[i] * sizeof(int32_t),
+    FCG_CUDA(cudaMemcpyAsync(dst, gbl.slot->dev + gbl.off_pages + plan_page_base[i] * sizeof(int32_t),
                              (size_t)checked[i].n_pages * sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
   }
-  fcg::StitchParams sp;
-  sp.entries = reinterpret_cast<const fcg::StitchEntryDev *>(slot->dev + off_entries);
-  sp.chunks = reinterpret_cast<const fcg::StitchChunkDev *>(slot->dev + off_chunks);
-  sp.table = reinterpret_cast<const float4 *>(slot->dev + off_table);
-  sp.k_pool = lib->k_pool();
-  sp.v_pool = lib->v_pool();
-  sp.n_chunks = (int32_t)n_chunks_total;
-  sp.n_layers = c.n_layers;
-  sp.n_kv_heads = c.n_kv_heads;
-  sp.page_size = P;
-  sp.n_pages = c.n_pages;
-  if (n_chunks_total > 0) {
-    FCG_CUDA(fcg::launch_stitch(sp, c.head_dim, stream));
-    lib->stats.stitch_launches++;
-  }
-  FCG_CUDA(cudaEventRecord(slot->ev, stream));
-  slot->in_flight = true;
+  st = finish_gather(gbl, stream);
+  if (st != FCG_OK) return st;
+  const int32_t *pages = gb.pages.data();
 
   // ---- commit ------------------------------------------------------------------------------------
   lib->page_stack.swap(stack);
@@ -883,6 +940,126 @@ fcg_status_t fcg_task_release(fcg_library_t *lib, int32_t task_id) {
   for (auto it = t.pages.rbegin(); it != t.pages.rend(); ++it) lib->page_stack.push_back(*it);
   t = TaskRec();
   lib->n_tasks_live--;
+  return FCG_OK;
+}
+
+// ------------------------------------------------------------- NEXT-1: suffix re-graft (Eq. 6)
+fcg_status_t fcg_task_shift(fcg_library_t *lib, int32_t task_id, int32_t src_begin, int32_t n_tokens, int32_t dst_begin,
+                            void *stream_) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  const fcg_config_t &c = lib->cfg;
+  if (task_id < 0 || task_id >= c.max_tasks || !lib->tasks[task_id].live) return fail(FCG_ERR_BAD_TASK, "unknown task %d", task_id);
+  TaskRec &t = lib->tasks[task_id];
+  if (n_tokens <= 0 || src_begin < 0 || dst_begin < 0 || (int64_t)src_begin + n_tokens > t.capacity ||
+      (int64_t)dst_begin + n_tokens > t.capacity)
+    return fail(FCG_ERR_RANGE, "shift range outside the capacity %d of task %d", t.capacity, task_id);
+  for (int32_t x = src_begin; x < src_begin + n_tokens; ++x)
+    if (!t.filled[x]) return fail(FCG_ERR_UNFILLED, "task %d: shift source position %d was never filled", task_id, x);
+  const int32_t delta = dst_begin - src_begin;
+  if (delta == 0) return FCG_OK;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  const int P = c.page_size;
+  const int32_t dst_end = dst_begin + n_tokens;
+  const int32_t lp0 = dst_begin / P, lp1 = (dst_end - 1) / P, n_new = lp1 - lp0 + 1;
+  if ((size_t)n_new > lib->page_stack.size())
+    return fail(FCG_ERR_OUT_OF_PAGES, "need %d pages, %zu free", n_new, lib->page_stack.size());
+
+  // copy-on-shift: destination pages are fresh, so no page is read and written by the same launch
+  GatherBuilder gb;
+  std::vector<int32_t> stack = lib->page_stack;
+  for (int32_t k = 0; k < n_new; ++k) {
+    gb.pages.push_back(stack.back());
+    stack.pop_back();
+  }
+  fcg::StitchEntryDev de;
+  gb.pool_side(lib, de.k_src, de.v_src, de.src_layer_stride, de.src_head_stride);
+  gb.pool_side(lib, de.k_dst, de.v_dst, de.dst_layer_stride, de.dst_head_stride);
+  de.pad0 = 0;
+  de.table_off = gb.table_for(lib, delta);
+  gb.entries.push_back(de);          // entry 0: the moved range, rotated by delta
+  de.table_off = -1;
+  gb.entries.push_back(de);          // entry 1: the other slots of the re-paged pages, bit copy
+  auto add_chunk = [&](int32_t entry, int32_t dst_pos, int32_t src_pos, int32_t n) {
+    fcg::StitchChunkDev dc;
+    dc.entry = entry;
+    dc.dst_tok = gb.pool_tok(lib, gb.pages[dst_pos / P - lp0], dst_pos % P);
+    dc.src_tok = gb.pool_tok(lib, t.pages[src_pos / P], src_pos % P);
+    dc.ntok = n;
+    gb.chunks.push_back(dc);
+  };
+  for (int32_t done = 0; done < n_tokens;) {          // runs contiguous in one source page and one destination page
+    const int32_t d = dst_begin + done, sp = src_begin + done;
+    const int32_t n = std::min(std::min(P - d % P, P - sp % P), n_tokens - done);
+    add_chunk(0, d, sp, n);
+    done += n;
+  }
+  if (dst_begin > lp0 * P) add_chunk(1, lp0 * P, lp0 * P, dst_begin - lp0 * P);
+  const int32_t page_end = std::min((lp1 + 1) * P, t.capacity);
+  if (dst_end < page_end) add_chunk(1, dst_end, dst_end, page_end - dst_end);
+
+  GatherBlob gbl;
+  fcg_status_t st = enqueue_gather(lib, gb, stream, gbl);
+  if (st != FCG_OK) return st;
+  FCG_CUDA(cudaMemcpyAsync(lib->tables() + (int64_t)task_id * lib->pages_per_task + lp0, gbl.slot->dev + gbl.off_pages,
+                           (size_t)n_new * sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
+  st = finish_gather(gbl, stream);
+  if (st != FCG_OK) return st;
+
+  // ---- commit: new pages in, replaced pages back to the pool (re-issued in ascending logical order) ----
+  lib->page_stack.swap(stack);
+  for (int32_t lp = lp1; lp >= lp0; --lp) lib->page_stack.push_back(t.pages[lp]);
+  for (int32_t lp = lp0; lp <= lp1; ++lp) t.pages[lp] = gb.pages[lp - lp0];
+  std::fill(t.filled.begin() + src_begin, t.filled.begin() + src_begin + n_tokens, (uint8_t)0);
+  std::fill(t.filled.begin() + dst_begin, t.filled.begin() + dst_end, (uint8_t)1);
+  t.filled_prefix = 0;
+  while (t.filled_prefix < t.capacity && t.filled[t.filled_prefix]) t.filled_prefix++;
+  t.n_tokens = std::max(t.n_tokens, dst_end);
+  return FCG_OK;
+}
+
+// ------------------------------------------------------- NEXT-2: segment extraction (Alg. 1B update)
+fcg_status_t fcg_segment_extract(fcg_library_t *lib, int32_t task_id, int32_t begin, int32_t n_tokens, int32_t new_orig_start,
+                                 void *stream_, int32_t *seg_id_out) {
+  if (!lib || !seg_id_out) return fail(FCG_ERR_INVALID_ARG, "NULL argument");
+  const fcg_config_t &c = lib->cfg;
+  if (task_id < 0 || task_id >= c.max_tasks || !lib->tasks[task_id].live) return fail(FCG_ERR_BAD_TASK, "unknown task %d", task_id);
+  const TaskRec &t = lib->tasks[task_id];
+  if (n_tokens <= 0 || begin < 0 || (int64_t)begin + n_tokens > t.capacity)
+    return fail(FCG_ERR_RANGE, "extract range outside the capacity %d of task %d", t.capacity, task_id);
+  if (new_orig_start < 0) return fail(FCG_ERR_INVALID_ARG, "new_orig_start must be >= 0");
+  for (int32_t x = begin; x < begin + n_tokens; ++x)
+    if (!t.filled[x]) return fail(FCG_ERR_UNFILLED, "task %d: extract position %d was never filled", task_id, x);
+  SegmentSlot sl;
+  fcg_status_t st = find_segment_slot(lib, n_tokens, sl);
+  if (st != FCG_OK) return st;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  const int P = c.page_size;
+
+  GatherBuilder gb;
+  fcg::StitchEntryDev de;
+  gb.pool_side(lib, de.k_src, de.v_src, de.src_layer_stride, de.src_head_stride);
+  gb.segment_side(lib, sl.off, sl.bytes, n_tokens, de.k_dst, de.v_dst, de.dst_layer_stride, de.dst_head_stride);
+  de.table_off = gb.table_for(lib, new_orig_start - begin);
+  de.pad0 = 0;
+  gb.entries.push_back(de);
+  for (int32_t done = 0; done < n_tokens;) {          // one chunk per source page
+    const int32_t sp = begin + done;
+    const int32_t n = std::min(P - sp % P, n_tokens - done);
+    fcg::StitchChunkDev dc;
+    dc.entry = 0;
+    dc.dst_tok = done;
+    dc.src_tok = gb.pool_tok(lib, t.pages[sp / P], sp % P);
+    dc.ntok = n;
+    gb.chunks.push_back(dc);
+    done += n;
+  }
+  GatherBlob gbl;
+  st = enqueue_gather(lib, gb, stream, gbl);
+  if (st != FCG_OK) return st;
+  st = finish_gather(gbl, stream);
+  if (st != FCG_OK) return st;
+  commit_segment_slot(lib, sl, n_tokens, new_orig_start);
+  *seg_id_out = sl.sid;
   return FCG_OK;
 }
 

@@ -8,32 +8,38 @@
 namespace fcg {
 
 // ---------------------------------------------------------------------------------------------
-// S3: fused gather + RoPE-shift.  One work item ("chunk") = the tokens of one plan entry that land
-// in one destination page; the kernel grid is (chunk, layer) and warps stride over kv heads.
+// S3: fused gather + RoPE-shift.  One kernel moves token rows between any two of {library segment,
+// paged cache}: stitch (segment -> cache), suffix re-graft (cache -> cache, fcg_task_shift) and segment
+// extraction (cache -> segment).  An entry fixes source, destination and the rotation; a chunk is a run
+// of consecutive token rows of one entry that is contiguous on both sides (at most one page).
+// Row address of (layer, kv head g, token t) = base + (layer * layer_stride + g * head_stride + tok + t) * D * 2:
+//   segment [L][Hkv][n][D]:          layer_stride = Hkv * n,           head_stride = n, tok = index in the segment
+//   pool    [L][n_pages][Hkv][P][D]: layer_stride = n_pages * Hkv * P, head_stride = P, tok = page * Hkv * P + slot
 // ---------------------------------------------------------------------------------------------
-struct StitchEntryDev {  // 32 B
-  uint64_t k_src;        // device address of the segment's K  [L][Hkv][seg_n][D]
-  uint64_t v_src;        // device address of the segment's V
-  int32_t seg_n;         // tokens in the segment (= head stride in tokens)
-  int32_t table_off;     // first float4 of this entry's rope table; -1 -> bit copy (delta 0 / rope off)
-  int32_t pad0, pad1;
+struct StitchEntryDev {  // 64 B
+  uint64_t k_src, v_src;         // device addresses of the source K / V
+  uint64_t k_dst, v_dst;         // device addresses of the destination K / V
+  int64_t src_layer_stride;      // in token rows
+  int64_t dst_layer_stride;
+  int32_t src_head_stride;
+  int32_t dst_head_stride;
+  int32_t table_off;             // first float4 of this entry's rope table; -1 -> bit copy (delta 0 / rope off)
+  int32_t pad0;
 };
 
 struct StitchChunkDev {  // 16 B
   int32_t entry;         // index into the entry array
-  int32_t page;          // physical destination page
-  int32_t src_tok;       // token index inside the segment of the chunk's first token
-  int32_t slot_ntok;     // first slot in the page | (number of tokens << 16)
+  int32_t dst_tok;       // destination row offset of the chunk's first token (see above)
+  int32_t src_tok;       // source row offset of the chunk's first token
+  int32_t ntok;          // tokens in the chunk
 };
 
 struct StitchParams {
   const StitchEntryDev *entries;
   const StitchChunkDev *chunks;
   const float4 *table;   // per (entry, j): {c_hi, c_lo, s_hi, s_lo}; c_hi/s_hi have <= 16 significant bits
-  uint16_t *k_pool;
-  uint16_t *v_pool;
-  int32_t n_chunks, n_layers, n_kv_heads, page_size;
-  uint32_t n_pages;
+  int32_t n_chunks, n_layers, n_kv_heads;
+  int32_t interleaved;   // 0: pairs (j, j + D/2) (half-split); 1: pairs (2j, 2j + 1)
 };
 
 cudaError_t launch_stitch(const StitchParams &p, int head_dim, cudaStream_t stream);

@@ -1,4 +1,6 @@
-// S3: fused gather + RoPE-shift (cache-stitching, Eq. 4).
+// S3: fused gather + RoPE-shift (cache-stitching, Eq. 4).  The same
+// kernel serves the suffix re-graft of a length-changing patch (Eq. 6, cache -> cache) and segment extraction
+// (Alg. 1B `update`, cache -> segment): source and destination are strided row spaces (fcg_internal.h).
 //
 // HBM-bound streaming kernel: every K/V byte of a stitched segment is read once and written once.
 // Work item = (chunk, layer): the tokens of one plan entry that land in one destination page, for
@@ -65,6 +67,13 @@ __device__ __forceinline__ void rot_word(uint32_t wa, uint32_t wb, const float4 
   ob = pack_bf16(y0, y1);
 }
 
+// interleaved pairs: one 32-bit word holds the pair (2j, 2j + 1)
+__device__ __forceinline__ uint32_t rot_word_il(uint32_t w, const float4 &t) {
+  float x, y;
+  rot_pair(bf16_lo(w), bf16_hi(w), t, x, y);
+  return pack_bf16(x, y);
+}
+
 template <int D>
 __global__ void __launch_bounds__(128, 4) stitch_kernel(const StitchParams p) {
   constexpr int LPT = D / 16;      // lanes per token: one 16-byte column of each half per lane
@@ -79,24 +88,30 @@ __global__ void __launch_bounds__(128, 4) stitch_kernel(const StitchParams p) {
   const int warp = threadIdx.x >> 5;
   const int col = lane % LPT;
   const int tl = lane / LPT;
-  const int slot0 = ch.slot_ntok & 0xffff;
-  const int ntok = ch.slot_ntok >> 16;
+  const int ntok = ch.ntok;
   const bool rotate = en.table_off >= 0;
+  const bool il = p.interleaved != 0;
 
+  // the lane's two 16-byte vectors of a key row: elements [col*8, col*8+8) and [D/2 + col*8, D/2 + col*8 + 8).
+  // half-split: pair i of the lane = (lo[i], hi[i]) with frequency col*8 + i;
+  // interleaved: pairs (lo[2i], lo[2i+1]) with frequency col*4 + i and (hi[2i], hi[2i+1]) with D/4 + col*4 + i.
   float4 tab[8];
   if (rotate) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) tab[i] = __ldg(p.table + en.table_off + col * 8 + i);
+    for (int i = 0; i < 8; ++i) {
+      const int j = il ? ((i >> 2) * (D / 4) + col * 4 + (i & 3)) : (col * 8 + i);
+      tab[i] = __ldg(p.table + en.table_off + j);
+    }
   }
 
   const int Hkv = p.n_kv_heads;
   for (int g = warp; g < Hkv; g += 4) {
-    const size_t src_row = ((size_t)layer * Hkv + g) * (size_t)en.seg_n + (size_t)ch.src_tok;
-    const size_t dst_row = (((size_t)layer * p.n_pages + (size_t)ch.page) * Hkv + g) * (size_t)p.page_size + slot0;
+    const size_t src_row = (size_t)layer * (size_t)en.src_layer_stride + (size_t)g * (size_t)en.src_head_stride + (size_t)ch.src_tok;
+    const size_t dst_row = (size_t)layer * (size_t)en.dst_layer_stride + (size_t)g * (size_t)en.dst_head_stride + (size_t)ch.dst_tok;
     const char *ksrc = reinterpret_cast<const char *>(en.k_src) + src_row * ROW_BYTES + col * 16;
     const char *vsrc = reinterpret_cast<const char *>(en.v_src) + src_row * ROW_BYTES + col * 16;
-    char *kdst = reinterpret_cast<char *>(p.k_pool) + dst_row * ROW_BYTES + col * 16;
-    char *vdst = reinterpret_cast<char *>(p.v_pool) + dst_row * ROW_BYTES + col * 16;
+    char *kdst = reinterpret_cast<char *>(en.k_dst) + dst_row * ROW_BYTES + col * 16;
+    char *vdst = reinterpret_cast<char *>(en.v_dst) + dst_row * ROW_BYTES + col * 16;
 
     for (int t0 = 0; t0 < ntok; t0 += TPS * STEPS) {
       uint4 klo[STEPS], khi[STEPS], vlo[STEPS], vhi[STEPS];
@@ -118,10 +133,21 @@ __global__ void __launch_bounds__(128, 4) stitch_kernel(const StitchParams p) {
           const size_t off = (size_t)t * ROW_BYTES;
           uint4 olo = klo[s], ohi = khi[s];
           if (rotate) {
-            rot_word(klo[s].x, khi[s].x, tab[0], tab[1], olo.x, ohi.x);
-            rot_word(klo[s].y, khi[s].y, tab[2], tab[3], olo.y, ohi.y);
-            rot_word(klo[s].z, khi[s].z, tab[4], tab[5], olo.z, ohi.z);
-            rot_word(klo[s].w, khi[s].w, tab[6], tab[7], olo.w, ohi.w);
+            if (!il) {
+              rot_word(klo[s].x, khi[s].x, tab[0], tab[1], olo.x, ohi.x);
+              rot_word(klo[s].y, khi[s].y, tab[2], tab[3], olo.y, ohi.y);
+              rot_word(klo[s].z, khi[s].z, tab[4], tab[5], olo.z, ohi.z);
+              rot_word(klo[s].w, khi[s].w, tab[6], tab[7], olo.w, ohi.w);
+            } else {
+              olo.x = rot_word_il(klo[s].x, tab[0]);
+              olo.y = rot_word_il(klo[s].y, tab[1]);
+              olo.z = rot_word_il(klo[s].z, tab[2]);
+              olo.w = rot_word_il(klo[s].w, tab[3]);
+              ohi.x = rot_word_il(khi[s].x, tab[4]);
+              ohi.y = rot_word_il(khi[s].y, tab[5]);
+              ohi.z = rot_word_il(khi[s].z, tab[6]);
+              ohi.w = rot_word_il(khi[s].w, tab[7]);
+            }
           }
           stg_16(kdst + off, olo);
           stg_16(kdst + off + D, ohi);
