@@ -82,6 +82,54 @@ def tensor_peak():
         return 1400.0, "fallback (B200_PROFILING.md, sustained)"
 
 
+EXTRACT_TOKENS = 1024
+
+
+def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
+    """SURVEY.md 8(f) NEXT rows, timed on task 0 of the stitched workload after the main measurement (CUDA events,
+    2 warm-ups): suffix re-graft by -16 / +16 tokens (fcg_task_shift), extraction of EXTRACT_TOKENS tokens into the
+    library (fcg_segment_extract), and one decode step (fcg_patch, n = 1, R = G) over the whole cache."""
+    t = wl.tasks[0]
+    cap = t.capacity
+    mid = (cap // 2) & ~15
+    n_shift = cap - mid - 16
+    n_ext = min(EXTRACT_TOKENS, mid)
+    q, k, v = synth.patch_qkv(cfg, t.task_id, 1, seed + 100, dev)
+    out = torch.empty_like(q)
+    pos = np.asarray([cap - 1], np.int32)
+
+    def shift_pair():
+        lib.task_shift(t.task_id, mid + 16, n_shift, mid)
+        lib.task_shift(t.task_id, mid, n_shift, mid + 16)
+
+    def extract():
+        lib.segment_release(lib.segment_extract(t.task_id, 0, n_ext, 0))
+
+    def decode():
+        lib.patch(t.task_id, 0, q, k, v, pos, out)
+
+    res = {}
+    per_tok = cfg.kv_bytes_per_token
+    for name, fn, nbytes in (("decode_step", decode, cfg.n_layers * cap * cfg.n_kv_heads * cfg.head_dim * 4),
+                             ("segment_extract", extract, n_ext * per_tok * 2),
+                             ("task_shift", shift_pair, 2 * n_shift * per_tok * 2)):
+        for _ in range(2):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        a.record()
+        for _ in range(iters):
+            fn()
+        b.record()
+        torch.cuda.synchronize(dev)
+        ms = a.elapsed_time(b) / iters
+        res[name] = {"ms": ms, "GBps": nbytes / (ms * 1e-3) / 1e9, "bytes": int(nbytes)}
+    res["task_shift"]["note"] = f"two moves of {n_shift} tokens (-16, +16) per iteration"
+    res["segment_extract"]["note"] = f"{n_ext} tokens un-rotated to orig_start 0"
+    res["decode_step"]["note"] = f"n = 1 at position {cap - 1}, R = {cfg.n_q_heads // cfg.n_kv_heads} rows per kv head"
+    return res
+
+
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -128,10 +176,13 @@ def build_library(cfg, wl, seed, device_index, on_segment=None):
     keep slices of the device-generated segments for the oracle."""
     from paper_2606_13097_b200 import binding
     total_pages = sum(-(-t.capacity // cfg.page_size) for t in wl.tasks)
-    seg_tokens = int(wl.seg_lens.sum())
+    # + EXTRACT_TOKENS of arena and + half a task of pages: room for the NEXT-row measurements (segment extraction,
+    # copy-on-shift); neither changes what the graft step itself touches
+    seg_tokens = int(wl.seg_lens.sum()) + EXTRACT_TOKENS
+    total_pages += max(-(-t.capacity // cfg.page_size) for t in wl.tasks) // 2 + 8
     lib = binding.FcgLibrary(n_layers=cfg.n_layers, n_q_heads=cfg.n_q_heads, n_kv_heads=cfg.n_kv_heads,
                              head_dim=cfg.head_dim, page_size=cfg.page_size, rope_base=cfg.rope_base,
-                             max_segments=cfg.n_segments, max_tasks=max(cfg.n_tasks, 1),
+                             max_segments=cfg.n_segments + 1, max_tasks=max(cfg.n_tasks, 1),
                              max_task_tokens=max(t.capacity for t in wl.tasks), n_pages=total_pages + 16,
                              workspace_bytes=1 << 30, segment_tokens=seg_tokens, device=device_index)
     dev = torch.device("cuda", device_index)
@@ -301,6 +352,11 @@ def run_cuda(args, cfg, wl, seed):
     if e2e:
         res["e2e"] = {"value": world * (sb + ab) / (e2e[0] * 1e-3) / 1e9, "unit": "GB/s (algorithmic, whole graft)",
                       "ms_per_step": e2e[0], "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2]}
+    if rank == 0 and not args.no_next:
+        try:
+            res["next_rows"] = time_next_rows(lib, cfg, wl, seed, dev)
+        except Exception as e:       # never lose the main line to an extra
+            res["next_rows"] = {"error": repr(e)}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         res["cpu_baseline"] = cpu_baseline(cfg, wl, seed, lib_segments=lambda s: synth.segment_kv(cfg, s, int(wl.seg_lens[s]), seed, dev))
     lib.close()
@@ -412,6 +468,7 @@ def main():
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next", action="store_true", help="skip the NEXT-row timings (shift, extract, decode)")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per stitch launch, if known (profiles/)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
