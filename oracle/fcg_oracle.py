@@ -180,6 +180,7 @@ class Segment:
     v: np.ndarray
     n_tokens: int
     orig_start: int          # position at which token 0's key was RoPE-encoded
+    resident: bool = True    # False: offloaded to the host tier (Eq. 3); the bits are the same wherever they live
 
 
 @dataclass
@@ -255,6 +256,28 @@ class OracleLibrary:
         if seg_id not in self.segments:
             raise OracleError(FCG_ERR_BAD_SEGMENT, f"unknown segment {seg_id}")
         del self.segments[seg_id]
+
+    # -- NEXT-3: two-tier residency (Eq. 3, Table 19) ----------------
+    def segment_offload(self, seg_id: int) -> None:
+        """Low-scored entries "are offloaded to DRAM".  Which entries is the caller's policy (the
+        locality score of Eq. 3 is not on the path); the library only moves the bits.  Values do not change:
+        stitching from an offloaded segment gives the same cache.  Idempotent."""
+        if seg_id not in self.segments:
+            raise OracleError(FCG_ERR_BAD_SEGMENT, f"unknown segment {seg_id}")
+        self.segments[seg_id].resident = False
+
+    def segment_prefetch(self, seg_id: int) -> None:
+        """CPU -> GPU reload "only when a required function cache is not resident".  Idempotent."""
+        if seg_id not in self.segments:
+            raise OracleError(FCG_ERR_BAD_SEGMENT, f"unknown segment {seg_id}")
+        self.segments[seg_id].resident = True
+
+    def segment_info(self, seg_id: int):
+        """(n_tokens, orig_start, resident)"""
+        if seg_id not in self.segments:
+            raise OracleError(FCG_ERR_BAD_SEGMENT, f"unknown segment {seg_id}")
+        sg = self.segments[seg_id]
+        return sg.n_tokens, sg.orig_start, sg.resident
 
     # -- S2 ------------------------------------------------------------------
     def validate_plan(self, plan: Plan):

@@ -670,3 +670,28 @@ def test_segment_extract_round_trips():
         with pytest.raises(O.OracleError) as e:
             lib.segment_extract(*args)
         assert e.value.status == status and len(lib.segments) == n_seg
+
+
+def test_segment_residency_state_machine():
+    """NEXT-3: residency is bookkeeping only -- the same plan over resident and offloaded segments gives the same
+    cache bits; offload / prefetch are idempotent; ids of offloaded segments stay taken until released."""
+    lib = _small_lib()
+    s0, k0, v0 = _reg(lib, 12, 5)
+    s1, k1, v1 = _reg(lib, 9, 0)
+    plan = lambda tid: O.Plan(tid, [O.PlanEntry(s0, 1, 10, 0), O.PlanEntry(s1, 0, 9, 10)])
+    lib.stitch([plan(0)])
+    assert lib.segment_info(s0) == (12, 5, True)
+    lib.segment_offload(s0), lib.segment_offload(s0)
+    assert lib.segment_info(s0) == (12, 5, False) and lib.segment_info(s1)[2] is True
+    lib.stitch([plan(1)])
+    assert np.array_equal(lib.tasks[0].k, lib.tasks[1].k) and np.array_equal(lib.tasks[0].v, lib.tasks[1].v)
+    assert _reg(lib, 3, 0)[0] == 2                       # the offloaded segment still owns id 0
+    lib.segment_prefetch(s0), lib.segment_prefetch(s0)
+    assert lib.segment_info(s0) == (12, 5, True)
+    lib.segment_offload(s1)
+    lib.segment_release(s1)
+    assert _reg(lib, 3, 0)[0] == s1
+    for fn in (lib.segment_offload, lib.segment_prefetch, lib.segment_info):
+        with pytest.raises(O.OracleError) as e:
+            fn(77)
+        assert e.value.status == O.FCG_ERR_BAD_SEGMENT
