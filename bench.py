@@ -124,6 +124,41 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
         torch.cuda.synchronize(dev)
         ms = a.elapsed_time(b) / iters
         res[name] = {"ms": ms, "GBps": nbytes / (ms * 1e-3) / 1e9, "bytes": int(nbytes)}
+    # NEXT-3 two-tier residency: one library segment to the pinned host tier and back (copy engine), and a stitch
+    # that reads it in place from the host tier (zero-copy over the host link)
+    seg = int(t.entries[0][0])
+    n_seg = int(wl.seg_lens[seg])
+    seg_bytes = n_seg * per_tok
+    try:
+        lib.task_release(t.task_id)
+        plan = [{"task_id": t.task_id, "entries": [(seg, 0, n_seg, 0)], "holes": [], "capacity_tokens": n_seg}]
+
+        def timed(fn, before=None, n=3):
+            ms = []
+            for _ in range(n + 1):
+                if before:
+                    before()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize(dev)
+                a.record()
+                fn()
+                b.record()
+                torch.cuda.synchronize(dev)
+                ms.append(a.elapsed_time(b))
+            return float(np.mean(ms[1:]))
+
+        off_ms = timed(lambda: lib.segment_offload(seg), before=lambda: lib.segment_prefetch(seg))
+        pre_ms = timed(lambda: lib.segment_prefetch(seg), before=lambda: lib.segment_offload(seg))
+        lib.segment_offload(seg)
+        host_ms = timed(lambda: lib.stitch(plan), before=lambda: lib.pool_info()["n_tasks_live"] and lib.task_release(t.task_id))
+        lib.task_release(t.task_id)
+        lib.segment_prefetch(seg)
+        res["segment_offload"] = {"ms": off_ms, "GBps": seg_bytes / (off_ms * 1e-3) / 1e9, "bytes": int(seg_bytes)}
+        res["segment_prefetch"] = {"ms": pre_ms, "GBps": seg_bytes / (pre_ms * 1e-3) / 1e9, "bytes": int(seg_bytes)}
+        res["stitch_from_host_tier"] = {"ms": host_ms, "GBps": seg_bytes / (host_ms * 1e-3) / 1e9, "bytes": int(seg_bytes),
+                                        "note": f"{n_seg}-token segment read in place from pinned host memory (bytes = one-way)"}
+    except Exception as e:
+        res["two_tier"] = {"error": repr(e)}
     res["task_shift"]["note"] = f"two moves of {n_shift} tokens (-16, +16) per iteration"
     res["segment_extract"]["note"] = f"{n_ext} tokens un-rotated to orig_start 0"
     res["decode_step"]["note"] = f"n = 1 at position {cap - 1}, R = {cfg.n_q_heads // cfg.n_kv_heads} rows per kv head"
@@ -184,7 +219,8 @@ def build_library(cfg, wl, seed, device_index, on_segment=None):
                              head_dim=cfg.head_dim, page_size=cfg.page_size, rope_base=cfg.rope_base,
                              max_segments=cfg.n_segments + 1, max_tasks=max(cfg.n_tasks, 1),
                              max_task_tokens=max(t.capacity for t in wl.tasks), n_pages=total_pages + 16,
-                             workspace_bytes=1 << 30, segment_tokens=seg_tokens, device=device_index)
+                             workspace_bytes=1 << 30, segment_tokens=seg_tokens, device=device_index,
+                             host_tier_tokens=int(wl.seg_lens[wl.tasks[0].entries[0][0]]) + 16)
     dev = torch.device("cuda", device_index)
     for s in range(cfg.n_segments):
         k, v = synth.segment_kv(cfg, s, int(wl.seg_lens[s]), seed, dev)

@@ -81,6 +81,9 @@ typedef struct {
   uint32_t n_pages;        /* pages in the pool, shared by all live tasks */
   uint64_t workspace_bytes;/* 0 -> 256 MiB */
   int32_t device;          /* CUDA device ordinal the arena lives on */
+  void *host_arena;        /* optional second tier (Eq. 3): PINNED host memory (cudaHostAlloc / cudaHostRegister, e.g. a
+                              torch pin_memory tensor), 256-byte aligned, caller-owned; NULL -> no host tier */
+  uint64_t host_arena_bytes;
 } fcg_config_t;
 
 /* Bytes of arena needed for a configuration that must hold `segment_tokens` library tokens in total
@@ -165,6 +168,20 @@ fcg_status_t fcg_task_page_table_host(fcg_library_t *lib, int32_t task_id, int32
 /* Returns the task's pages to the pool (pushed so that they are re-issued in ascending logical order). */
 fcg_status_t fcg_task_release(fcg_library_t *lib, int32_t task_id);
 
+/* Two-tier residency (Eq. 3; transfer cost in Table 19).
+ * Which entries to move is the caller's policy (the locality score is not on the path); the library moves bits.
+ * fcg_segment_offload: device -> host tier (one async copy on `stream`), the arena range is returned to the
+ *   segment allocator.  fcg_segment_prefetch: host tier -> device (first-fit arena range, one async copy), the host
+ *   range is returned.  Both are no-ops when the segment already is where it is asked to be.  INVALID_ARG without a
+ *   host tier, BAD_SEGMENT, OUT_OF_ARENA when the receiving tier has no free range (state unchanged).
+ * A plan may name an offloaded segment: fcg_stitch then reads it straight from the pinned host range (zero-copy
+ *   over the host link), with the same result.  fcg_segment_release frees whichever tier holds the segment.
+ * fcg_segment_info: any of the three outputs may be NULL; resident = 1 (device) or 0 (host tier). */
+fcg_status_t fcg_segment_offload(fcg_library_t *lib, int32_t seg_id, void *stream);
+fcg_status_t fcg_segment_prefetch(fcg_library_t *lib, int32_t seg_id, void *stream);
+fcg_status_t fcg_segment_info(fcg_library_t *lib, int32_t seg_id, int32_t *n_tokens, int32_t *orig_start,
+                              int32_t *resident);
+
 /* Suffix re-graft of a length-changing patch (Eq. 6, R15):
  * moves cache positions [src_begin, src_begin + n_tokens) of a live task to [dst_begin, dst_begin + n_tokens),
  * all layers and kv heads: keys re-rotated by delta = dst_begin - src_begin (the stitch rule R1; bit copy for
@@ -217,6 +234,7 @@ typedef struct {
       attn_tc_launches, read_launches;
   int32_t last_attn_path;   /* 0 none, 1 split-KV warp-MMA, 2 tcgen05 */
   int32_t last_attn_splits;
+  uint64_t offload_copies, prefetch_copies;   /* tier moves (copy engine, not kernels) */
 } fcg_stats_t;
 fcg_status_t fcg_stats(fcg_library_t *lib, fcg_stats_t *out);
 

@@ -45,7 +45,8 @@ class fcg_config_t(C.Structure):
                 ("rope_base", C.c_double), ("inv_freq", C.POINTER(C.c_double)),
                 ("arena", C.c_void_p), ("arena_bytes", C.c_uint64),
                 ("max_segments", C.c_int32), ("max_tasks", C.c_int32), ("max_task_tokens", C.c_int32),
-                ("n_pages", C.c_uint32), ("workspace_bytes", C.c_uint64), ("device", C.c_int32)]
+                ("n_pages", C.c_uint32), ("workspace_bytes", C.c_uint64), ("device", C.c_int32),
+                ("host_arena", C.c_void_p), ("host_arena_bytes", C.c_uint64)]
 
 
 class fcg_plan_entry_t(C.Structure):
@@ -72,7 +73,8 @@ class fcg_stats_t(C.Structure):
     _fields_ = [("stitch_launches", C.c_uint64), ("register_launches", C.c_uint64), ("scatter_launches", C.c_uint64),
                 ("attn_split_launches", C.c_uint64), ("attn_combine_launches", C.c_uint64),
                 ("attn_tc_launches", C.c_uint64), ("read_launches", C.c_uint64),
-                ("last_attn_path", C.c_int32), ("last_attn_splits", C.c_int32)]
+                ("last_attn_path", C.c_int32), ("last_attn_splits", C.c_int32),
+                ("offload_copies", C.c_uint64), ("prefetch_copies", C.c_uint64)]
 
 
 # every symbol include/fcg.h declares: name -> (restype, argtypes)
@@ -85,6 +87,9 @@ SYMBOLS = {
     "fcg_library_destroy": (_I, [_P]),
     "fcg_segment_register": (_I, [_P, _P, _P, _I, _I, C.POINTER(C.c_int64), _P, _PI]),
     "fcg_segment_release": (_I, [_P, _I]),
+    "fcg_segment_offload": (_I, [_P, _I, _P]),
+    "fcg_segment_prefetch": (_I, [_P, _I, _P]),
+    "fcg_segment_info": (_I, [_P, _I, _PI, _PI, _PI]),
     "fcg_stitch": (_I, [_P, C.POINTER(fcg_plan_t), _I, _P]),
     "fcg_patch": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
     "fcg_patch_host": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
@@ -162,8 +167,9 @@ def fcg_last_error() -> str:
 
 def make_config(*, n_layers, n_q_heads, n_kv_heads, head_dim, page_size=16, rope_mode=FCG_ROPE_HALF_SPLIT,
                 rope_base=1e4, inv_freq=None, arena=0, arena_bytes=0, max_segments=64, max_tasks=8,
-                max_task_tokens=8192, n_pages=1024, workspace_bytes=0, device=0):
+                max_task_tokens=8192, n_pages=1024, workspace_bytes=0, device=0, host_arena=None, host_arena_bytes=0):
     cfg = fcg_config_t()
+    cfg.host_arena, cfg.host_arena_bytes = _ptr(host_arena), int(host_arena_bytes)
     cfg.n_layers, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim = n_layers, n_q_heads, n_kv_heads, head_dim
     cfg.page_size, cfg.rope_mode, cfg.rope_base = page_size, rope_mode, float(rope_base)
     keep = None
@@ -267,6 +273,20 @@ def fcg_task_release(handle, task_id) -> None:
     _check(load().fcg_task_release(handle, int(task_id)))
 
 
+def fcg_segment_offload(handle, seg_id, stream=None) -> None:
+    _check(load().fcg_segment_offload(handle, int(seg_id), _stream(stream)))
+
+
+def fcg_segment_prefetch(handle, seg_id, stream=None) -> None:
+    _check(load().fcg_segment_prefetch(handle, int(seg_id), _stream(stream)))
+
+
+def fcg_segment_info(handle, seg_id):
+    n, o, r = C.c_int32(), C.c_int32(), C.c_int32()
+    _check(load().fcg_segment_info(handle, int(seg_id), C.byref(n), C.byref(o), C.byref(r)))
+    return n.value, o.value, bool(r.value)
+
+
 def fcg_task_shift(handle, task_id, src_begin, n_tokens, dst_begin, stream=None) -> None:
     _check(load().fcg_task_shift(handle, int(task_id), int(src_begin), int(n_tokens), int(dst_begin), _stream(stream)))
 
@@ -307,14 +327,22 @@ class FcgLibrary:
 
     def __init__(self, *, n_layers, n_q_heads, n_kv_heads, head_dim, page_size=16, rope_mode=FCG_ROPE_HALF_SPLIT,
                  rope_base=1e4, inv_freq=None, max_segments=64, max_tasks=8, max_task_tokens=8192, n_pages=1024,
-                 workspace_bytes=0, segment_tokens=0, device=0):
+                 workspace_bytes=0, segment_tokens=0, device=0, host_tier_tokens=0):
         self.n_layers, self.n_q_heads, self.n_kv_heads, self.head_dim = n_layers, n_q_heads, n_kv_heads, head_dim
         self.page_size = page_size
         self.device = torch.device("cuda", device)
+        # second tier (Eq. 3): a pinned host tensor for `host_tier_tokens` tokens of offloaded segments
+        self.host_arena = None
+        if host_tier_tokens > 0:
+            nbytes = host_tier_tokens * n_layers * n_kv_heads * head_dim * 4 + 512 * (max_segments + 1)
+            self.host_arena = torch.empty(nbytes + 256, dtype=torch.uint8).pin_memory()
+        hptr = 0 if self.host_arena is None else (self.host_arena.data_ptr() + 255) // 256 * 256
         cfg = make_config(n_layers=n_layers, n_q_heads=n_q_heads, n_kv_heads=n_kv_heads, head_dim=head_dim,
                           page_size=page_size, rope_mode=rope_mode, rope_base=rope_base, inv_freq=inv_freq,
                           max_segments=max_segments, max_tasks=max_tasks, max_task_tokens=max_task_tokens,
-                          n_pages=n_pages, workspace_bytes=workspace_bytes, device=device)
+                          n_pages=n_pages, workspace_bytes=workspace_bytes, device=device,
+                          host_arena=hptr or None,
+                          host_arena_bytes=0 if self.host_arena is None else self.host_arena.numel() - 256)
         need = fcg_arena_bytes_required(cfg, segment_tokens)
         if need == 0:
             raise FcgError(FCG_ERR_INVALID_ARG, "bad configuration")
@@ -327,6 +355,7 @@ class FcgLibrary:
             fcg_library_destroy(self.handle)
             self.handle = None
             self.arena = None
+            self.host_arena = None
 
     def __del__(self):
         try:
@@ -341,6 +370,15 @@ class FcgLibrary:
 
     def segment_release(self, seg_id):
         fcg_segment_release(self.handle, seg_id)
+
+    def segment_offload(self, seg_id, stream=None):
+        fcg_segment_offload(self.handle, seg_id, stream)
+
+    def segment_prefetch(self, seg_id, stream=None):
+        fcg_segment_prefetch(self.handle, seg_id, stream)
+
+    def segment_info(self, seg_id):
+        return fcg_segment_info(self.handle, seg_id)
 
     def stitch(self, plans, stream=None):
         fcg_stitch(self.handle, plans, stream)

@@ -46,7 +46,8 @@ uint64_t align_up(uint64_t x, uint64_t a = ALIGN) { return (x + a - 1) / a * a; 
 
 struct SegmentRec {
   bool live = false;
-  uint64_t offset = 0, bytes = 0;   // in the arena; K then V
+  uint64_t offset = 0, bytes = 0;   // in the arena (resident) or in the host tier (offloaded); K then V
+  bool resident = true;
   int32_t n_tokens = 0, orig_start = 0;
 };
 
@@ -81,6 +82,9 @@ struct fcg_library {
   std::vector<int32_t> page_stack;               // LIFO: back() is handed out next
   std::vector<SegmentRec> segments;
   std::vector<FreeRange> seg_free;               // sorted by offset
+  unsigned char *host_arena = nullptr;           // second tier: pinned host memory (Eq. 3), NULL if none
+  unsigned char *host_dev = nullptr;             // the same memory as the device sees it (zero-copy stitch)
+  std::vector<FreeRange> host_free;              // offsets relative to host_arena, sorted
   std::vector<TaskRec> tasks;
   BlobSlot slots[BLOB_SLOTS];
   int next_slot = 0;
@@ -184,6 +188,35 @@ struct BlobWriter {
   }
 };
 
+// first-fit over a sorted free list; returns the index of the range or free_list.size()
+size_t range_find(const std::vector<FreeRange> &fl, uint64_t bytes) {
+  for (size_t i = 0; i < fl.size(); ++i)
+    if (fl[i].bytes >= bytes) return i;
+  return fl.size();
+}
+void range_take(std::vector<FreeRange> &fl, size_t i, uint64_t bytes) {
+  if (fl[i].bytes == bytes)
+    fl.erase(fl.begin() + i);
+  else {
+    fl[i].off += bytes;
+    fl[i].bytes -= bytes;
+  }
+}
+// insert and coalesce with the neighbours
+void range_give(std::vector<FreeRange> &fl, uint64_t off, uint64_t bytes) {
+  FreeRange fr{off, bytes};
+  auto it = std::lower_bound(fl.begin(), fl.end(), fr, [](const FreeRange &a, const FreeRange &b) { return a.off < b.off; });
+  it = fl.insert(it, fr);
+  if (it + 1 != fl.end() && it->off + it->bytes == (it + 1)->off) {
+    it->bytes += (it + 1)->bytes;
+    fl.erase(it + 1);
+  }
+  if (it != fl.begin() && (it - 1)->off + (it - 1)->bytes == it->off) {
+    (it - 1)->bytes += it->bytes;
+    fl.erase(it);
+  }
+}
+
 // lowest free segment id and first-fit arena range for an n-token segment; nothing changes until commit
 struct SegmentSlot {
   int32_t sid = -1;
@@ -201,12 +234,7 @@ fcg_status_t find_segment_slot(fcg_library *lib, int32_t n_tokens, SegmentSlot &
     }
   if (sl.sid < 0) return fail(FCG_ERR_OUT_OF_ARENA, "segment table full (%d)", c.max_segments);
   sl.bytes = lib->seg_bytes_for(n_tokens);
-  sl.fi = lib->seg_free.size();
-  for (size_t i = 0; i < lib->seg_free.size(); ++i)
-    if (lib->seg_free[i].bytes >= sl.bytes) {
-      sl.fi = i;
-      break;
-    }
+  sl.fi = range_find(lib->seg_free, sl.bytes);
   if (sl.fi == lib->seg_free.size())
     return fail(FCG_ERR_OUT_OF_ARENA, "no free arena range of %llu bytes for a %d-token segment", (unsigned long long)sl.bytes, n_tokens);
   sl.off = lib->seg_free[sl.fi].off;
@@ -214,18 +242,14 @@ fcg_status_t find_segment_slot(fcg_library *lib, int32_t n_tokens, SegmentSlot &
 }
 
 void commit_segment_slot(fcg_library *lib, const SegmentSlot &sl, int32_t n_tokens, int32_t orig_start) {
-  if (lib->seg_free[sl.fi].bytes == sl.bytes)
-    lib->seg_free.erase(lib->seg_free.begin() + sl.fi);
-  else {
-    lib->seg_free[sl.fi].off += sl.bytes;
-    lib->seg_free[sl.fi].bytes -= sl.bytes;
-  }
+  range_take(lib->seg_free, sl.fi, sl.bytes);
   SegmentRec &s = lib->segments[sl.sid];
   s.live = true;
   s.offset = sl.off;
   s.bytes = sl.bytes;
   s.n_tokens = n_tokens;
   s.orig_start = orig_start;
+  s.resident = true;
   lib->n_segments_live++;
 }
 
@@ -274,10 +298,10 @@ struct GatherBuilder {
     layer_stride = (int64_t)c.n_pages * c.n_kv_heads * c.page_size;
     head_stride = c.page_size;
   }
-  void segment_side(const fcg_library *lib, uint64_t off, uint64_t bytes, int32_t n, uint64_t &k, uint64_t &v,
-                    int64_t &layer_stride, int32_t &head_stride) const {
-    k = (uint64_t)(uintptr_t)(lib->arena + off);
-    v = (uint64_t)(uintptr_t)(lib->arena + off + bytes / 2);
+  void segment_side(const fcg_library *lib, const unsigned char *tier_base, uint64_t off, uint64_t bytes, int32_t n,
+                    uint64_t &k, uint64_t &v, int64_t &layer_stride, int32_t &head_stride) const {
+    k = (uint64_t)(uintptr_t)(tier_base + off);
+    v = (uint64_t)(uintptr_t)(tier_base + off + bytes / 2);
     layer_stride = (int64_t)lib->cfg.n_kv_heads * n;
     head_stride = n;
   }
@@ -408,6 +432,18 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
     }
     lib->slots[i].dev = lib->arena + l.ws_off + (uint64_t)i * BLOB_BYTES;
   }
+  if (cfg->host_arena && cfg->host_arena_bytes) {
+    cudaPointerAttributes attr;
+    cudaError_t e = cudaPointerGetAttributes(&attr, cfg->host_arena);
+    if (e != cudaSuccess || attr.type != cudaMemoryTypeHost || !attr.devicePointer || ((uintptr_t)cfg->host_arena % ALIGN)) {
+      cudaGetLastError();
+      fcg_library_destroy(lib);
+      return fail(FCG_ERR_INVALID_ARG, "host_arena must be pinned (cudaHostAlloc / cudaHostRegister) and 256-byte aligned");
+    }
+    lib->host_arena = static_cast<unsigned char *>(cfg->host_arena);
+    lib->host_dev = static_cast<unsigned char *>(attr.devicePointer);
+    lib->host_free.push_back({0, cfg->host_arena_bytes / ALIGN * ALIGN});
+  }
   if (cfg->head_dim == 128) {
     fcg_status_t st = make_pool_tensor_map(lib->cfg, lib->k_pool(), &lib->tm_k);
     if (st == FCG_OK) st = make_pool_tensor_map(lib->cfg, lib->v_pool(), &lib->tm_v);
@@ -475,25 +511,70 @@ fcg_status_t fcg_segment_register(fcg_library_t *lib, const void *k, const void 
   return FCG_OK;
 }
 
+// ------------------------------------------------------------------ NEXT-3: two-tier residency
+fcg_status_t fcg_segment_offload(fcg_library_t *lib, int32_t seg_id, void *stream) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  if (seg_id < 0 || seg_id >= lib->cfg.max_segments || !lib->segments[seg_id].live)
+    return fail(FCG_ERR_BAD_SEGMENT, "unknown segment %d", seg_id);
+  if (!lib->host_arena) return fail(FCG_ERR_INVALID_ARG, "the library was created without a host tier (host_arena)");
+  SegmentRec &s = lib->segments[seg_id];
+  if (!s.resident) return FCG_OK;
+  const size_t fi = range_find(lib->host_free, s.bytes);
+  if (fi == lib->host_free.size())
+    return fail(FCG_ERR_OUT_OF_ARENA, "no free host-tier range of %llu bytes for segment %d", (unsigned long long)s.bytes, seg_id);
+  const uint64_t hoff = lib->host_free[fi].off;
+  FCG_CUDA(cudaSetDevice(lib->cfg.device));
+  FCG_CUDA(cudaMemcpyAsync(lib->host_arena + hoff, lib->arena + s.offset, s.bytes, cudaMemcpyDeviceToHost,
+                           static_cast<cudaStream_t>(stream)));
+  range_take(lib->host_free, fi, s.bytes);
+  range_give(lib->seg_free, s.offset, s.bytes);
+  s.offset = hoff;
+  s.resident = false;
+  lib->stats.offload_copies++;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_segment_prefetch(fcg_library_t *lib, int32_t seg_id, void *stream) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  if (seg_id < 0 || seg_id >= lib->cfg.max_segments || !lib->segments[seg_id].live)
+    return fail(FCG_ERR_BAD_SEGMENT, "unknown segment %d", seg_id);
+  if (!lib->host_arena) return fail(FCG_ERR_INVALID_ARG, "the library was created without a host tier (host_arena)");
+  SegmentRec &s = lib->segments[seg_id];
+  if (s.resident) return FCG_OK;
+  const size_t fi = range_find(lib->seg_free, s.bytes);
+  if (fi == lib->seg_free.size())
+    return fail(FCG_ERR_OUT_OF_ARENA, "no free arena range of %llu bytes for segment %d", (unsigned long long)s.bytes, seg_id);
+  const uint64_t off = lib->seg_free[fi].off;
+  FCG_CUDA(cudaSetDevice(lib->cfg.device));
+  FCG_CUDA(cudaMemcpyAsync(lib->arena + off, lib->host_arena + s.offset, s.bytes, cudaMemcpyHostToDevice,
+                           static_cast<cudaStream_t>(stream)));
+  range_take(lib->seg_free, fi, s.bytes);
+  range_give(lib->host_free, s.offset, s.bytes);
+  s.offset = off;
+  s.resident = true;
+  lib->stats.prefetch_copies++;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_segment_info(fcg_library_t *lib, int32_t seg_id, int32_t *n_tokens, int32_t *orig_start, int32_t *resident) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  if (seg_id < 0 || seg_id >= lib->cfg.max_segments || !lib->segments[seg_id].live)
+    return fail(FCG_ERR_BAD_SEGMENT, "unknown segment %d", seg_id);
+  const SegmentRec &s = lib->segments[seg_id];
+  if (n_tokens) *n_tokens = s.n_tokens;
+  if (orig_start) *orig_start = s.orig_start;
+  if (resident) *resident = s.resident ? 1 : 0;
+  return FCG_OK;
+}
+
 fcg_status_t fcg_segment_release(fcg_library_t *lib, int32_t seg_id) {
   if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
   if (seg_id < 0 || seg_id >= lib->cfg.max_segments || !lib->segments[seg_id].live)
     return fail(FCG_ERR_BAD_SEGMENT, "unknown segment %d", seg_id);
   SegmentRec &s = lib->segments[seg_id];
-  FreeRange fr{s.offset, s.bytes};
-  auto it = std::lower_bound(lib->seg_free.begin(), lib->seg_free.end(), fr,
-                             [](const FreeRange &a, const FreeRange &b) { return a.off < b.off; });
-  it = lib->seg_free.insert(it, fr);
-  // coalesce with the next, then with the previous
-  if (it + 1 != lib->seg_free.end() && it->off + it->bytes == (it + 1)->off) {
-    it->bytes += (it + 1)->bytes;
-    lib->seg_free.erase(it + 1);
-  }
-  if (it != lib->seg_free.begin() && (it - 1)->off + (it - 1)->bytes == it->off) {
-    (it - 1)->bytes += it->bytes;
-    lib->seg_free.erase(it);
-  }
+  range_give(s.resident ? lib->seg_free : lib->host_free, s.offset, s.bytes);
   s.live = false;
+  s.resident = true;
   lib->n_segments_live--;
   return FCG_OK;
 }
@@ -577,7 +658,9 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
       const fcg_plan_entry_t &pe = plans[i].entries[e];
       const SegmentRec &s = lib->segments[pe.seg_id];
       fcg::StitchEntryDev de;
-      gb.segment_side(lib, s.offset, s.bytes, s.n_tokens, de.k_src, de.v_src, de.src_layer_stride, de.src_head_stride);
+      // an offloaded segment is read in place from the pinned host tier
+      gb.segment_side(lib, s.resident ? lib->arena : lib->host_dev, s.offset, s.bytes, s.n_tokens, de.k_src, de.v_src,
+                      de.src_layer_stride, de.src_head_stride);
       gb.pool_side(lib, de.k_dst, de.v_dst, de.dst_layer_stride, de.dst_head_stride);
       de.table_off = gb.table_for(lib, checked[i].deltas[e]);
       de.pad0 = 0;
@@ -1038,7 +1121,7 @@ fcg_status_t fcg_segment_extract(fcg_library_t *lib, int32_t task_id, int32_t be
   GatherBuilder gb;
   fcg::StitchEntryDev de;
   gb.pool_side(lib, de.k_src, de.v_src, de.src_layer_stride, de.src_head_stride);
-  gb.segment_side(lib, sl.off, sl.bytes, n_tokens, de.k_dst, de.v_dst, de.dst_layer_stride, de.dst_head_stride);
+  gb.segment_side(lib, lib->arena, sl.off, sl.bytes, n_tokens, de.k_dst, de.v_dst, de.dst_layer_stride, de.dst_head_stride);
   de.table_off = gb.table_for(lib, new_orig_start - begin);
   de.pad0 = 0;
   gb.entries.push_back(de);

@@ -49,7 +49,7 @@ def plans_of(wl: synth.Workload, seg_ids):
 
 
 def make_pair(cfg: synth.GraftConfig, wl: synth.Workload, seed: int, *, n_pages=None, max_tasks=None,
-              workspace_bytes=0, only_segments=None, rope_mode=1, inv_freq=None):
+              workspace_bytes=0, only_segments=None, rope_mode=1, inv_freq=None, host_tier_tokens=0):
     """Create oracle + CUDA library holding the same segment bits.  Returns (orc, lib, seg_ids)."""
     from paper_2606_13097_b200.binding import FcgLibrary
     used = sorted({s for t in wl.tasks for (s, _, _, _) in t.entries}) if only_segments is None else only_segments
@@ -61,7 +61,7 @@ def make_pair(cfg: synth.GraftConfig, wl: synth.Workload, seed: int, *, n_pages=
                      page_size=cfg.page_size, rope_mode=rope_mode, rope_base=cfg.rope_base, inv_freq=inv_freq,
                      max_segments=max(len(used), 1), max_tasks=max_tasks or max(len(wl.tasks), 1),
                      max_task_tokens=cap_tokens, n_pages=n_pages, workspace_bytes=workspace_bytes,
-                     segment_tokens=seg_tokens)
+                     segment_tokens=seg_tokens, host_tier_tokens=host_tier_tokens)
     orc = O.OracleLibrary(cfg.n_layers, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, page_size=cfg.page_size,
                           rope_mode=rope_mode, rope_base=cfg.rope_base, inv_freq=inv_freq,
                           max_segments=max(len(used), 1), max_tasks=max_tasks or max(len(wl.tasks), 1), n_pages=n_pages,

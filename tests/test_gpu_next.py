@@ -197,3 +197,63 @@ def test_decode_steps_append_one_token_at_a_time(Hq, Hkv):
         T.assert_attn_close(out, ref, f"decode step {step}")
     _compare_task(orc, lib, 0, "after 4 decode steps")
     lib.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-3: two-tier residency -- offload to the pinned host tier, stitch from it in place, prefetch back
+# ------------------------------------------------------------------------------------------------
+def test_two_tier_residency_stitch_from_host_and_prefetch():
+    B = _binding()
+    cfg = synth.GraftConfig("tier", 2, 4, 2, 128, 16, 1e4, 5, 40, 160, 3000, 1, 4, 4, 0)
+    wl = synth.make_workload(cfg, 1)
+    total_pages = sum(-(-t.capacity // cfg.page_size) for t in wl.tasks)
+    orc, lib, seg_ids = T.make_pair(cfg, wl, 1, n_pages=4 * total_pages, max_tasks=4, only_segments=list(range(5)),
+                                    host_tier_tokens=int(wl.seg_lens.sum()))
+    free0 = lib.pool_info()["segments_bytes_free"]
+    used = [s for (s, _, _, _) in wl.tasks[0].entries]
+    # offload two of the four segments of the plan: the stitch reads them over the host link, same result
+    for s in used[:2]:
+        lib.segment_offload(s), orc.segment_offload(s)
+        lib.segment_offload(s)                                   # idempotent
+        assert lib.segment_info(s) == orc.segment_info(s) == (int(wl.seg_lens[s]), int(wl.orig_starts[s]), False)
+    assert lib.pool_info()["segments_bytes_free"] > free0
+    c_plans, o_plans = T.plans_of(wl, seg_ids)
+    orc.stitch(o_plans)
+    lib.stitch(c_plans)
+    T.compare_stitched(orc, lib, wl)
+    # bring one back, release the other while offloaded; the arena accounting returns
+    lib.segment_prefetch(used[0]), orc.segment_prefetch(used[0])
+    assert lib.segment_info(used[0])[2] is True
+    c_plans[0]["task_id"] = o_plans[0].task_id = 1
+    orc.stitch(o_plans)
+    lib.stitch(c_plans)
+    wl.tasks[0].task_id = 1
+    T.compare_stitched(orc, lib, wl)
+    lib.segment_prefetch(used[1])
+    assert lib.pool_info()["segments_bytes_free"] == free0
+    lib.segment_offload(used[1])
+    lib.segment_release(used[1]), orc.segment_release(used[1])
+    k, v = synth.segment_kv(cfg, used[1], int(wl.seg_lens[used[1]]), 1, "cpu")
+    assert lib.segment_register(k.cuda(), v.cuda(), 0) == orc.segment_register(synth.to_bits(k), synth.to_bits(v), 0) == used[1]
+    # extraction from a cache stitched out of host-tier segments, then offload of the extracted segment
+    spare = next(s for s in range(5) if s not in used)           # frees a table slot and an arena range
+    lib.segment_release(spare), orc.segment_release(spare)
+    sid = lib.segment_extract(1, 3, 20, 0)
+    assert sid == orc.segment_extract(1, 3, 20, 0) == spare
+    lib.segment_offload(sid), orc.segment_offload(sid)
+    plan_c = {"task_id": 2, "entries": [(sid, 0, 20, 9)], "holes": [(0, 9)], "capacity_tokens": 29}
+    orc.stitch([O.Plan(2, [O.PlanEntry(sid, 0, 20, 9)], [O.Hole(0, 9)], 29)])
+    lib.stitch([plan_c])
+    _compare_task(orc, lib, 2, "graft of an extracted, offloaded segment")
+    st = lib.stats()
+    assert st["offload_copies"] == 4 and st["prefetch_copies"] == 2
+    with pytest.raises(B.FcgError) as e:
+        lib.segment_offload(99)
+    assert e.value.status == B.FCG_ERR_BAD_SEGMENT
+    lib.close()
+    # without a host tier the calls are refused
+    orc, lib, seg_ids = T.make_pair(cfg, wl, 1, only_segments=[0])
+    with pytest.raises(B.FcgError) as e:
+        lib.segment_offload(0)
+    assert e.value.status == B.FCG_ERR_INVALID_ARG
+    lib.close()
