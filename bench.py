@@ -165,6 +165,58 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
     return res
 
 
+def time_prefill_compare(lib, cfg, wl, seed, dev, layers_per_call=4):
+    """BASELINE.json configs[4]: "compare graft time to causal attention prefill over the same 32k tokens".
+    Prefill attention = the same fcg_patch kernel with every position of a fresh task as a patch token (an empty cache
+    plus one patch is causal self-attention, DESIGN.md pin P12); timed for `layers_per_call` layers and scaled to all
+    layers (every layer does identical work).  The projections / MLP a real prefill also pays are NOT included, so
+    the ratio understates what grafting saves.  torch SDPA on the same shapes is quoted as library context."""
+    t = wl.tasks[0]
+    T_ = t.capacity
+    try:
+        lib.task_release(t.task_id)          # live unless the NEXT-row timings already released it
+    except Exception:
+        pass
+    lib.stitch([{"task_id": t.task_id, "entries": [], "holes": [(0, T_)], "capacity_tokens": T_}])
+    sub = synth.scaled(cfg, n_layers=layers_per_call)
+    q, k, v = synth.patch_qkv(sub, t.task_id, T_, seed + 7, dev)
+    out = torch.empty_like(q)
+    pos = np.arange(T_, dtype=np.int32)
+    ms = []
+    for _ in range(3):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        a.record()
+        lib.patch(t.task_id, 0, q, k, v, pos, out)
+        b.record()
+        torch.cuda.synchronize(dev)
+        ms.append(a.elapsed_time(b))
+    own_ms = float(np.min(ms[1:])) * cfg.n_layers / layers_per_call
+    flops = 4 * cfg.head_dim * cfg.n_q_heads * cfg.n_layers * (T_ * (T_ + 1) // 2)
+    res = {"tokens": T_, "own_kernel_ms_all_layers": own_ms, "own_kernel_TFLOPs": flops / (own_ms * 1e-3) / 1e12,
+           "timed_layers": layers_per_call, "flops_all_layers": int(flops)}
+    try:
+        import torch.nn.functional as F
+        qs = q[0].permute(1, 0, 2).unsqueeze(0).contiguous()          # [1][Hq][T][D]
+        ks = k[0].permute(1, 0, 2).unsqueeze(0).contiguous()
+        vs = v[0].permute(1, 0, 2).unsqueeze(0).contiguous()
+        sm = []
+        for _ in range(3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(dev)
+            a.record()
+            F.scaled_dot_product_attention(qs, ks, vs, is_causal=True, enable_gqa=True)
+            b.record()
+            torch.cuda.synchronize(dev)
+            sm.append(a.elapsed_time(b))
+        res["torch_sdpa_ms_all_layers"] = float(np.min(sm[1:])) * cfg.n_layers
+    except Exception as e:
+        res["torch_sdpa_ms_all_layers"] = None
+        res["torch_sdpa_error"] = repr(e)
+    lib.task_release(t.task_id)
+    return res
+
+
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -393,6 +445,13 @@ def run_cuda(args, cfg, wl, seed):
             res["next_rows"] = time_next_rows(lib, cfg, wl, seed, dev)
         except Exception as e:       # never lose the main line to an extra
             res["next_rows"] = {"error": repr(e)}
+    if rank == 0 and args.prefill_compare:
+        try:
+            res["prefill_compare"] = time_prefill_compare(lib, cfg, wl, seed, dev)
+            res["prefill_compare"]["graft_ms"] = ms_per_step
+            res["prefill_compare"]["prefill_attention_over_graft"] = res["prefill_compare"]["own_kernel_ms_all_layers"] / ms_per_step
+        except Exception as e:
+            res["prefill_compare"] = {"error": repr(e)}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         res["cpu_baseline"] = cpu_baseline(cfg, wl, seed, lib_segments=lambda s: synth.segment_kv(cfg, s, int(wl.seg_lens[s]), seed, dev))
     lib.close()
@@ -504,6 +563,8 @@ def main():
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--prefill-compare", action="store_true",
+                    help="also time causal prefill attention over the task's whole length (C5's comparison)")
     ap.add_argument("--no-next", action="store_true", help="skip the NEXT-row timings (shift, extract, decode)")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per stitch launch, if known (profiles/)")
     args = ap.parse_args()

@@ -124,6 +124,19 @@ __device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t a_desc, uint64
       : "memory");
 }
 
+// D[tmem] (+)= A[tmem] * B[smem]: A (M x 16 bf16) sits in TMEM, row == lane, two K elements per 32-bit column
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  if (elect_one())
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+      "}" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+
 // shared-memory matrix descriptor, 128B swizzle, version 1 (sm_100).  Offsets in bytes.
 __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo, uint32_t sbo) {
   const uint32_t lo = ((addr >> 4) & 0x3FFFu) | (((lbo >> 4) & 0x3FFFu) << 16);
@@ -167,6 +180,19 @@ constexpr uint32_t idesc_f16(int n, bool b_mn_major) {
       "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])                                                                 \
       : "memory")
 
+#define TMEM_ST_16(taddr, r)                                                                                         \
+  asm volatile(                                                                                                      \
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "                                                                \
+      "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),                                       \
+      "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),  \
+      "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])                                         \
+      : "memory")
+
+#define TMEM_ST_8(taddr, r)                                                                                          \
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "r"(r[0]),     \
+               "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])                            \
+               : "memory")
+
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
@@ -203,13 +229,17 @@ __device__ __forceinline__ float2 ex2_poly2(float2 x) {
 // ---- shared memory map -------------------------------------------------------------------------
 constexpr int Q_TILE_B = BM * D * 2;          // two 64-column halves of [128][128 B]
 constexpr int KV_TILE_B = BN * D * 2;         // two halves of [64][128 B]
-constexpr int P_BYTES = BM * BN * 2;          // [128][128 B]
 
 template <int NQ, int PS_>
 struct Cfg {
   // separate rings: a K stage is free again as soon as Q K^T of its tile has completed, a V stage only after P V
-  static constexpr int K_STAGES = NQ == 1 ? 4 : 3;
-  static constexpr int V_STAGES = NQ == 1 ? 6 : 3;
+  // P (the A operand of P V) lives in TMEM: the softmax threads write it with tcgen05.st and the MMA reads it from
+  // there, so it never crosses shared memory (whose bandwidth -- Q, K, P, V operand reads plus the TMA and P writes,
+  // 224 KB per 64-token step with two Q tiles -- was the limiter of the tensor-bound class).  One Q tile: own
+  // columns; two Q tiles: P overwrites the first half of its S tile in place (S is then freed by P V, not by s_free).
+  static constexpr bool P_ALIAS = NQ == 2;
+  static constexpr int K_STAGES = NQ == 1 ? 6 : 5;
+  static constexpr int V_STAGES = NQ == 1 ? 6 : 5;
   // Tile-parity streams (NQ == 1 only): two softmax warpgroups, group w owns the KV tiles j = w (mod 2), its own
   // S / P buffer and its own O accumulator, with its own running (m, l); the streams are merged by log-sum-exp in
   // the epilogue like the row streams.  Two softmax warps per SM sub-partition hide each other's latencies.
@@ -224,8 +254,8 @@ struct Cfg {
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + NQ * Q_TILE_B;                // K stage s at +s*KV_TILE_B
   static constexpr int OFF_V = OFF_K + K_STAGES * KV_TILE_B;         // V stage s at +s*KV_TILE_B
-  static constexpr int OFF_P = OFF_V + V_STAGES * KV_TILE_B;         // P[t][b] at +(2t+b)*P_BYTES
-  static constexpr int OFF_BAR = OFF_P + NQ * 2 * P_BYTES;
+  static constexpr int OFF_BAR = OFF_V + V_STAGES * KV_TILE_B;
+  static constexpr int TMEM_P = 384;                    // one Q tile: P[b] at TMEM_P + b*32 (S 0..127, O 128..383)
   // k_full[SK], k_empty[SK], v_full[SV], v_empty[SV], s_full[NQ][2], p_full[NQ][2], pv_done[NQ][2], s_free[NQ][2],
   // q_full, all_done
   static constexpr int N_BARS = 2 * K_STAGES + 2 * V_STAGES + 8 * NQ + 2;
@@ -261,7 +291,9 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
   // ---- row layout of this CTA (see "Row streams" in the header) ---------------------------------
   const int Rc = min(R - row0, NQ * BM);           // valid query rows of this CTA
   const int nq_eff = (NQ == 2 && Rc > BM) ? 2 : 1; // Q tiles that hold any valid row
-  const int dup = nq_eff == 1 ? (Rc <= 32 ? 4 : (Rc <= 64 ? 2 : 1)) : 1;
+  // row streams only with one Q tile per CTA: with two, P overwrites its S tile in TMEM, which leaves no zeroed columns
+  // for the slices a stream does not own (a trailing row group of <= 64 rows simply runs with idle lanes)
+  const int dup = NQ == 1 ? (Rc <= 32 ? 4 : (Rc <= 64 ? 2 : 1)) : 1;
   const int rps = BM / dup;                        // MMA rows per stream (128, 64 or 32)
 
   const int t_begin = split * tk.split_len;
@@ -378,15 +410,15 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
       // operand descriptors: a fixed part per operand, plus (byte offset >> 4) in the 14-bit address field
       const uint64_t qdesc0 = smem_desc(sbase + C::OFF_Q, 16, 1024);
       const uint64_t kdesc0 = smem_desc(sbase + C::OFF_K, 16, 1024);
-      const uint64_t pdesc0 = smem_desc(sbase + C::OFF_P, 16, 1024);
       const uint64_t vdesc0 = smem_desc(sbase + C::OFF_V, BN * 128, 1024);   // MN-major: LBO = next 64-column half
       int sk = 0, rk = 0;                            // K ring position of the next Q K^T
       auto issue_qk = [&](int j) {
-        // S[t][j&1] was last read by the softmax of tile j-2: reuse it as soon as those threads have loaded it
+        // S[t][j&1] was last read by the softmax of tile j-2: reuse it as soon as those threads have loaded it -- or,
+        // where P sits inside the S tile, once P V of tile j-2 has consumed it
         if (j >= 2) {
 #pragma unroll
           for (int t = 0; t < NQ; ++t)
-            if (t < nq_eff) mbar_wait(s_free(t, j & 1), ((j - 2) >> 1) & 1);
+            if (t < nq_eff) mbar_wait(C::P_ALIAS ? pv_done(t, j & 1) : s_free(t, j & 1), ((j - 2) >> 1) & 1);
         }
         mbar_wait(k_full(sk), rk & 1);
         const uint64_t kdesc = kdesc0 + (uint64_t)((sk * KV_TILE_B) >> 4);
@@ -430,12 +462,12 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
           if (t < nq_eff) {
             mbar_wait(p_full(t, j & 1), (j >> 1) & 1);
             tc_fence_after();
-            const uint64_t pdesc = pdesc0 + (uint64_t)(((2 * t + (j & 1)) * P_BYTES) >> 4);
+            const uint32_t tmem_p = tmem_base + (C::P_ALIAS ? (2 * t + (j & 1)) * BN : C::TMEM_P + (j & 1) * 32);
             // O accumulator of (Q tile t | parity stream j % PS); the stream's first tile overwrites it
             const uint32_t tmem_o = tmem_base + C::TMEM_O + (PS == 2 ? (j & 1) : t) * 128;
 #pragma unroll
             for (int k = 0; k < BN / 16; ++k)
-              umma_ss(tmem_o, pdesc + (uint64_t)((k * 32) >> 4), vdesc + (uint64_t)((k * 2048) >> 4), IDESC_O, (j >= PS || k > 0) ? 1u : 0u);
+              umma_ts(tmem_o, tmem_p + k * 8, vdesc + (uint64_t)((k * 2048) >> 4), IDESC_O, (j >= PS || k > 0) ? 1u : 0u);
             if (t == nq_eff - 1) umma_commit(v_empty(sv));
             umma_commit(pv_done(t, j & 1));
           }
@@ -451,8 +483,14 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
       issue_qk(0);
       if (n_tiles > 1) issue_qk(1);
       for (int j = 0; j < n_tiles; ++j) {
-        if (j + 2 < n_tiles) issue_qk(j + 2);
-        if (j >= LAG) issue_pv(j - LAG);
+        if (C::P_ALIAS) {
+          // P sits inside S[j&1]: Q K^T of tile j+2 may only overwrite it after P V of tile j
+          issue_pv(j);
+          if (j + 2 < n_tiles) issue_qk(j + 2);
+        } else {
+          if (j + 2 < n_tiles) issue_qk(j + 2);
+          if (j >= LAG) issue_pv(j - LAG);
+        }
       }
       for (int j = max(0, n_tiles - LAG); j < n_tiles; ++j) issue_pv(j);
       umma_commit(all_done);
@@ -492,15 +530,16 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
     const int qt = PS == 2 ? 0 : wg;           // Q tile of this warp
     const int par = PS == 2 ? wg : 0;          // parity stream of this warp: KV tiles j = par (mod PS)
     const int row = tid & (BM - 1);            // MMA row in the tile == TMEM lane
-    if (dup > 1 && qt == 0) {
+    const uint32_t lane_addr = ((uint32_t)((warp & 3) * 32) << 16);
+    if (!C::P_ALIAS && dup > 1) {
       // a stream writes only its own columns of P: the rest of the row stays zero for the whole kernel
+      uint32_t zero[32];
 #pragma unroll
-      for (int b = 0; b < 2; ++b) {
-        if (PS == 2 && b != par) continue;     // with parity streams, P[b] belongs to stream b
-#pragma unroll
-        for (int c8 = 0; c8 < 8; ++c8)
-          *reinterpret_cast<uint4 *>(smem + C::OFF_P + b * P_BYTES + row * 128 + (c8 << 4)) = make_uint4(0, 0, 0, 0);
-      }
+      for (int c = 0; c < 32; ++c) zero[c] = 0u;
+      TMEM_ST_32(tmem_base + lane_addr + C::TMEM_P + par * 32, zero);
+      if (PS == 1) TMEM_ST_32(tmem_base + lane_addr + C::TMEM_P + 32, zero);
+      tmem_wait_st();
+      tc_fence_before();
     }
     fence_proxy_async();
     mbar_arrive(q_full);
@@ -512,7 +551,6 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
     const bool active = tile_used && warp_active(qt, warp & 3);
     const bool valid = tile_used && rl < tile_rows(qt);
     const int lim = valid ? min(pos[r / G], t_end - 1) : -1;
-    const uint32_t lane_addr = ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t tmem_s = tmem_base + lane_addr + (2 * qt) * BN;
     const uint32_t tmem_o = tmem_base + lane_addr + C::TMEM_O + wg * 128;
     const float sc = p.scale_log2;
@@ -573,9 +611,10 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
         }
         l *= factor;
         const float mu = m_ref == -INFINITY ? 0.f : m_ref;
-        // the P buffer of this parity was last read by P V of tile j-2
-        if (j >= 2) mbar_wait(pv_done(qt, b), ((j - 2) >> 1) & 1);
-        unsigned char *prow = smem + C::OFF_P + (2 * qt + b) * P_BYTES + row * 128;
+        // the P buffer of this parity was last read by P V of tile j-2 (implied when P sits inside S: Q K^T of this
+        // tile was only issued after that P V)
+        if (!C::P_ALIAS && j >= 2) mbar_wait(pv_done(qt, b), ((j - 2) >> 1) & 1);
+        uint32_t preg[NC / 2];
         // packed fp32 pairs (FFMA2 / FADD2) for the scale-subtract and the row sum.  In the tensor-bound layout
         // (64 columns per thread) one pair in four takes its exp2 from the FMA pipe instead of the MUFU, whose
         // 16 results per clock and SM would otherwise cost as many cycles per tile as the two MMAs.
@@ -594,15 +633,20 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
               e[q] = make_float2(ex2_approx(x.x), ex2_approx(x.y));
             sum2[q & 1] = __fadd2_rn(sum2[q & 1], e[q]);
           }
-          uint4 v;
-          v.x = pack_bf16(e[0].x, e[0].y);
-          v.y = pack_bf16(e[1].x, e[1].y);
-          v.z = pack_bf16(e[2].x, e[2].y);
-          v.w = pack_bf16(e[3].x, e[3].y);
-          *reinterpret_cast<uint4 *>(prow + (((c0 >> 3) + c8) ^ (row & 7)) * 16) = v;
+#pragma unroll
+          for (int q = 0; q < 4; ++q) preg[c8 * 4 + q] = pack_bf16(e[q].x, e[q].y);
         }
         l += (sum2[0].x + sum2[0].y) + (sum2[1].x + sum2[1].y);
-        fence_proxy_async();
+        // P row -> TMEM (row == lane, two bf16 per column): this stream's slice of the 32 packed columns
+        const uint32_t tmem_p = tmem_base + lane_addr + (C::P_ALIAS ? (2 * qt + b) * BN : C::TMEM_P + b * 32) + (c0 >> 1);
+        if constexpr (NC == 64) {
+          TMEM_ST_32(tmem_p, preg);
+        } else if constexpr (NC == 32) {
+          TMEM_ST_16(tmem_p, preg);
+        } else {
+          TMEM_ST_8(tmem_p, preg);
+        }
+        tmem_wait_st();
         tc_fence_before();
         mbar_arrive(p_full(qt, b));
       }
