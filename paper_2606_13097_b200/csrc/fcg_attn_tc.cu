@@ -352,7 +352,9 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot_ptr;
+  // shuffle broadcast: the value is warp-uniform, and saying so keeps every TMEM address of the MMA warp in uniform
+  // registers (the MMA warp was issue-bound: ~255 SASS instructions per KV tile, a third of them R2UR / UMOV)
+  const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot_ptr, 0);
 
   if (warp == C::KLOAD_WARP || warp == C::VLOAD_WARP) {
     // ======================================= loaders =======================================
@@ -415,10 +417,10 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
       auto issue_qk = [&](int j) {
         // S[t][j&1] was last read by the softmax of tile j-2: reuse it as soon as those threads have loaded it -- or,
         // where P sits inside the S tile, once P V of tile j-2 has consumed it
-        if (j >= 2) {
+        if (!C::P_ALIAS && j >= 2) {
 #pragma unroll
           for (int t = 0; t < NQ; ++t)
-            if (t < nq_eff) mbar_wait(C::P_ALIAS ? pv_done(t, j & 1) : s_free(t, j & 1), ((j - 2) >> 1) & 1);
+            if (t < nq_eff) mbar_wait(s_free(t, j & 1), ((j - 2) >> 1) & 1);
         }
         mbar_wait(k_full(sk), rk & 1);
         const uint64_t kdesc = kdesc0 + (uint64_t)((sk * KV_TILE_B) >> 4);
@@ -426,6 +428,12 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
 #pragma unroll
         for (int t = 0; t < NQ; ++t) {
           if (t < nq_eff) {
+            // P inside S: wait for P V of tile j-2 of THIS Q tile only, right before overwriting its S -- the other Q
+            // tile's MMAs keep the tensor pipe busy meanwhile (no drain between P V and Q K^T)
+            if (C::P_ALIAS && j >= 2) {
+              mbar_wait(pv_done(t, j & 1), ((j - 2) >> 1) & 1);
+              tc_fence_after();
+            }
 #pragma unroll
             for (int k = 0; k < D / 16; ++k) {
               const uint64_t a = qdesc0 + (uint64_t)((t * Q_TILE_B + (k >> 2) * (BM * 128) + (k & 3) * 32) >> 4);
