@@ -1,20 +1,23 @@
 // S6: tensor-core patch attention on tcgen05 / TMEM (cache-patching, Eq. 6, PAPER.md:118-123, 718;
-// DESIGN.md "Kernel S6").  Same result as the split-KV warp-MMA kernel, for R = n*G >= 64 query rows
-// per kv head, where the two contractions Q K^T and P V are dense enough for the 5th-gen tensor cores.
+// DESIGN.md "Kernel S6").  Default attention path for head_dim 128: short patches and decode steps (HBM-bound)
+// as well as long patches (tensor-bound).
 //
-//   CTA   = (KV split x row group of NQ*128 rows, kv head, layer x task); NQ*128 + 64 threads, 1 CTA / SM
-//   warps [0, 4*NQ)  softmax: thread == query row == TMEM lane of its 128-row Q tile.  S tile read with
-//                    tcgen05.ld, online softmax in the exp2 domain with a lazy (threshold 2^8) O rescale,
-//                    P written as bf16 into a 128B-swizzled K-major shared tile (the A operand of P V)
-//   warp  4*NQ       loader: one TMA box copy (cp.async.bulk.tensor.5d, 128B swizzle) per (page, K|V,
-//                    64-column half) through the page table into a ring of 64-token K/V tiles; the
-//                    transaction-count mbarrier of the stage completes when the bytes have landed, so
-//                    loading is decoupled from the MMA / softmax chain
-//   warp  4*NQ+1     MMA issuer: one thread issues tcgen05.mma (M=128, kind::f16, fp32 accumulate):
-//                    S[t][j&1] = Q_t K_j^T (N=64, K=128, both K-major) and O_t += P_t,j V_j (N=128, K=64,
-//                    V as an MN-major B operand), accumulators in TMEM.  Q K^T of tile j+1 is issued
-//                    before P V of tile j, so the softmax of tile j overlaps tensor work.
-//   TMEM  = S[t][b] at columns (2t+b)*64, O_t at NQ*128 + t*128   (256 columns for NQ=1, 512 for NQ=2)
+//   CTA   = (KV split x row group of NQ*128 rows, kv head, layer x task), 1 CTA / SM, template <NQ, PS>:
+//             <1,1>  one 128-row Q tile; R <= 64 rows are held 2x / 4x ("row streams": stream s owns the columns
+//                    [s*NC, (s+1)*NC) of every KV tile with its own (m, l, O)), merged by log-sum-exp at the end
+//             <1,2>  one Q tile, two softmax warpgroups on alternating KV tiles ("tile-parity streams")
+//             <2,1>  two Q tiles, one softmax warpgroup each (K/V read once per 256 rows)
+//   softmax warps    thread == query row == TMEM lane.  S tile read with tcgen05.ld, online softmax in the exp2
+//                    domain with a lazy (threshold 2^8) O rescale, packed fp32 pairs, part of the exp2 on the FMA
+//                    pipe; P goes back to TMEM as packed bf16 (tcgen05.st) -- with two Q tiles in place, over the
+//                    first half of its S tile
+//   K / V loader     one warp each: a TMA box copy (cp.async.bulk.tensor.5d, 128B swizzle) per (page, 64-column
+//                    half) through the page table into a ring of 64-token tiles; transaction-count mbarriers
+//   MMA warp         tcgen05.mma, M = 128, kind::f16, fp32 accumulate, issued from uniform registers:
+//                    S[t][j&1] = Q_t K_j^T (N = 64, K = 128, operands in shared memory, K-major) and
+//                    O += P_j V_j (N = 128, K = 64, A = P from TMEM, B = V MN-major from shared memory)
+//   TMEM  (512 columns)  NQ = 1: S[b] at b*64, O[stream] at 128 + stream*128, P[b] at 384 + b*32
+//                        NQ = 2: S[t][b] at (2t+b)*64 (P inside it), O_t at 256 + t*128
 //   Tail  : tokens >= the end of the split inside the last tile are never valid data (page slack or
 //           stale shared memory).  Their S columns are masked by selection; their V rows are zeroed
 //           in shared memory by the MMA warp before P V, so no 0 x NaN can reach O.
