@@ -117,3 +117,69 @@ def test_c4_full_size_sampled_slices():
 
 def test_c5_full_size_sampled_slices():
     run_fullsize("C5", 1, 2, 1)
+
+
+def test_c2_full_size_next_rows():
+    """The NEXT rows at C2's full size, in the order bench.time_next_rows issues them (decode step at the last
+    position, segment extraction of 1024 tokens, suffix re-graft by -16), against the oracle on sampled
+    (layer, kv head) slices; the extracted segment is read back by grafting it alone at delta 0."""
+    name, seed = "C2", 1
+    cfg = synth.CONFIGS[name]
+    wl = synth.make_workload(cfg, seed)
+    G = cfg.n_q_heads // cfg.n_kv_heads
+    dev = torch.device("cuda", 0)
+    picks = sample_slices(cfg, 2, seed)
+    t = wl.tasks[0]
+    used = sorted({s for (s, _, _, _) in t.entries})
+    kept = {pk: {} for pk in picks}
+
+    def keep(s, k, v):
+        if s in used:
+            for (l, g) in picks:
+                kept[(l, g)][s] = (synth.to_bits(k[l:l + 1, g:g + 1]), synth.to_bits(v[l:l + 1, g:g + 1]))
+
+    lib = bench.build_library(cfg, wl, seed, 0, on_segment=keep)
+    try:
+        cap = t.capacity
+        mid = (cap // 2) & ~15
+        n_shift, n_ext = cap - mid - 16, bench.EXTRACT_TOKENS
+        q, k, v = synth.patch_qkv(cfg, t.task_id, len(t.positions), seed, dev)
+        q1, k1, v1 = synth.patch_qkv(cfg, t.task_id, 1, seed + 100, dev)
+        last = np.asarray([cap - 1], np.int32)
+        lib.stitch(bench.plans_for(wl))
+        lib.patch(t.task_id, 0, q, k, v, t.positions)
+        out1 = lib.patch(t.task_id, 0, q1, k1, v1, last)
+        sid_g = lib.segment_extract(t.task_id, 0, n_ext, 0)
+        lib.task_shift(t.task_id, mid + 16, n_shift, mid)
+        torch.cuda.synchronize()
+        table_g = lib.task_page_table_host(t.task_id)
+        shifted = {pk: [synth.to_bits(x[pk[1]]) for x in lib.task_read(t.task_id, pk[0], 0, cap)] for pk in picks}
+        lib.task_release(t.task_id)
+        lib.stitch([{"task_id": t.task_id, "entries": [(sid_g, 0, n_ext, 0)], "holes": [], "capacity_tokens": n_ext}])
+        for (l, g) in picks:
+            orc = O.OracleLibrary(1, G, 1, cfg.head_dim, page_size=cfg.page_size, rope_base=cfg.rope_base,
+                                  n_pages=lib.pool_info()["n_pages"], max_segments=cfg.n_segments + 1)
+            # same segment ids as the library: register all, keeping the used ones' bits (others: 1-token dummies)
+            for s in range(cfg.n_segments):
+                if s in used:
+                    orc.segment_register(kept[(l, g)][s][0], kept[(l, g)][s][1], int(wl.orig_starts[s]))
+                else:
+                    orc.segment_register(np.zeros((1, 1, 1, cfg.head_dim), np.uint16), np.zeros((1, 1, 1, cfg.head_dim), np.uint16), 0)
+            orc.stitch([O.Plan(t.task_id, [O.PlanEntry(*e) for e in t.entries], [O.Hole(*h) for h in t.holes], cap)])
+            sl = lambda x, heads: synth.to_bits(x[l:l + 1, :, heads])
+            orc.patch(t.task_id, 0, sl(q, slice(g * G, (g + 1) * G)), sl(k, slice(g, g + 1)), sl(v, slice(g, g + 1)), t.positions)
+            ref1 = orc.patch(t.task_id, 0, sl(q1, slice(g * G, (g + 1) * G)), sl(k1, slice(g, g + 1)), sl(v1, slice(g, g + 1)), last)
+            assert_attn_close(out1[l:l + 1, :, g * G:(g + 1) * G], ref1, f"decode step layer {l} kv head {g}")
+            sid_o = orc.segment_extract(t.task_id, 0, n_ext, 0)
+            assert sid_o == sid_g
+            orc.task_shift(t.task_id, mid + 16, n_shift, mid)
+            ot = orc.tasks[t.task_id]
+            assert np.array_equal(table_g, np.asarray(ot.page_table, np.int32)), "page table after copy-on-shift"
+            f = ot.filled
+            assert np.array_equal(shifted[(l, g)][1][f], ot.v[0][0][f]), "V after shift not bit-exact"
+            assert_k_within_1ulp(shifted[(l, g)][0][f], ot.k[0][0][f], f"K after shift, layer {l} head {g}")
+            kx, vx = lib.task_read(t.task_id, l, 0, n_ext)
+            assert np.array_equal(synth.to_bits(vx[g]), orc.segments[sid_o].v[0][0]), "extracted V not bit-exact"
+            assert_k_within_1ulp(synth.to_bits(kx[g]), orc.segments[sid_o].k[0][0], f"extracted K, layer {l} head {g}")
+    finally:
+        lib.close()
