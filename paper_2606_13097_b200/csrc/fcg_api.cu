@@ -724,7 +724,10 @@ namespace {
 int choose_splits(int64_t base_ctas, int tiles, int rows, int head_dim, int ctas_per_sm) {
   if (tiles <= 1) return 1;
   const double slots = (double)N_SMS * ctas_per_sm;
-  double best_cost = 1e30;
+  // everything in bytes streamed by one SM (an SM's share of HBM is ~44 GB/s: 10 us ~ 440 KB)
+  const double kFixedPerCta = 6000.0;            // launch + prologue + epilogue of a CTA
+  const double kCombineLaunch = 400000.0;        // the extra combine kernel: launch gap + its own ramp
+  double best_cost = 1e30, cost_1 = 1e30;
   int best = 1;
   const int max_s = std::min(tiles, 64);
   for (int s = 1; s <= max_s; ++s) {
@@ -733,17 +736,20 @@ int choose_splits(int64_t base_ctas, int tiles, int rows, int head_dim, int ctas
     if (s_eff != s) continue;
     const double ctas = (double)base_ctas * s;
     const double waves = ceil(ctas / slots);
-    // time ~ waves * (tiles per CTA) in units of one tile of streaming, plus partial traffic
+    // time ~ waves * (one CTA's K/V stream + its fp32 partial rows), plus what the combine kernel reads and writes
     const double kv_bytes = (double)tiles_per * KV_TILE * head_dim * 4.0;
-    const double part_bytes = s > 1 ? 2.0 * rows * (head_dim + 2) * 4.0 : 0.0;
-    const double per_cta = kv_bytes + part_bytes + 6000.0 /* fixed per-CTA latency in byte-equivalents */;
-    const double cost = waves * per_cta;
+    const double part_bytes = s > 1 ? (double)rows * (head_dim + 2) * 4.0 : 0.0;
+    const double combine = s > 1 ? kCombineLaunch + ctas * part_bytes / N_SMS : 0.0;
+    const double cost = waves * (kv_bytes + part_bytes + kFixedPerCta) + combine;
+    if (s == 1) cost_1 = cost;
     if (cost < best_cost * 0.999) {
       best_cost = cost;
       best = s;
     }
   }
-  return best;
+  // a split must pay for itself with margin: partials are fp32 and the measured cost of splitting when the grid
+  // already fills the GPU is 20-25 % (C3: 0.41 ms unsplit, 0.50 ms with two splits)
+  return best_cost < 0.85 * cost_1 ? best : 1;
 }
 
 struct PatchCall {
