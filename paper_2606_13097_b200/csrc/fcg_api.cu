@@ -87,6 +87,11 @@ struct fcg_library {
   std::vector<FreeRange> host_free;              // offsets relative to host_arena, sorted
   std::vector<TaskRec> tasks;
   BlobSlot slots[BLOB_SLOTS];
+  // fcg_patch_host: the host->device copies run on the library's own stream, ordered after the last patch call
+  // (the staging area belongs to patch calls only), so they overlap a stitch enqueued just before on the caller's stream
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t last_patch_ev = nullptr, h2d_ev = nullptr;
+  bool have_last_patch = false;
   int next_slot = 0;
   fcg_stats_t stats;
   int n_segments_live = 0, n_tasks_live = 0;
@@ -432,6 +437,15 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
     }
     lib->slots[i].dev = lib->arena + l.ws_off + (uint64_t)i * BLOB_BYTES;
   }
+  {
+    cudaError_t e = cudaStreamCreateWithFlags(&lib->copy_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->last_patch_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->h2d_ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+      fcg_library_destroy(lib);
+      return fail(FCG_ERR_CUDA, "copy stream / events: %s", cudaGetErrorString(e));
+    }
+  }
   if (cfg->host_arena && cfg->host_arena_bytes) {
     cudaPointerAttributes attr;
     cudaError_t e = cudaPointerGetAttributes(&attr, cfg->host_arena);
@@ -465,6 +479,9 @@ fcg_status_t fcg_library_destroy(fcg_library_t *lib) {
     if (lib->slots[i].host) cudaFreeHost(lib->slots[i].host);
     if (lib->slots[i].ev) cudaEventDestroy(lib->slots[i].ev);
   }
+  if (lib->copy_stream) cudaStreamDestroy(lib->copy_stream);
+  if (lib->last_patch_ev) cudaEventDestroy(lib->last_patch_ev);
+  if (lib->h2d_ev) cudaEventDestroy(lib->h2d_ev);
   delete lib;
   return FCG_OK;
 }
@@ -942,6 +959,8 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
   }
   FCG_CUDA(cudaEventRecord(slot->ev, pc.stream));
   slot->in_flight = true;
+  FCG_CUDA(cudaEventRecord(lib->last_patch_ev, pc.stream));
+  lib->have_last_patch = true;
 
   // ---- commit fill state ---------------------------------------------------------------------
   tok_off = 0;
@@ -987,9 +1006,14 @@ fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_b
   unsigned char *base = lib->arena + lib->scratch_off + lib->scratch_bytes - need;
   unsigned char *dq = base, *dk = dq + align_up(q_bytes), *dv = dk + align_up(kv_bytes), *dout = dv + align_up(kv_bytes);
   FCG_CUDA(cudaSetDevice(c.device));
-  FCG_CUDA(cudaMemcpyAsync(dq, q, q_bytes, cudaMemcpyHostToDevice, stream));
-  FCG_CUDA(cudaMemcpyAsync(dk, k, kv_bytes, cudaMemcpyHostToDevice, stream));
-  FCG_CUDA(cudaMemcpyAsync(dv, v, kv_bytes, cudaMemcpyHostToDevice, stream));
+  // copies on the library's stream: after the last user of the staging / partial area, but NOT after a stitch the
+  // caller has just enqueued on `stream` (stitch never touches the scratch area)
+  if (lib->have_last_patch) FCG_CUDA(cudaStreamWaitEvent(lib->copy_stream, lib->last_patch_ev, 0));
+  FCG_CUDA(cudaMemcpyAsync(dq, q, q_bytes, cudaMemcpyHostToDevice, lib->copy_stream));
+  FCG_CUDA(cudaMemcpyAsync(dk, k, kv_bytes, cudaMemcpyHostToDevice, lib->copy_stream));
+  FCG_CUDA(cudaMemcpyAsync(dv, v, kv_bytes, cudaMemcpyHostToDevice, lib->copy_stream));
+  FCG_CUDA(cudaEventRecord(lib->h2d_ev, lib->copy_stream));
+  FCG_CUDA(cudaStreamWaitEvent(stream, lib->h2d_ev, 0));
   // partials must not collide with the staging area: temporarily shrink the scratch
   const uint64_t saved = lib->scratch_bytes;
   lib->scratch_bytes = saved - need;
@@ -998,6 +1022,7 @@ fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_b
   lib->scratch_bytes = saved;
   if (st != FCG_OK) return st;
   FCG_CUDA(cudaMemcpyAsync(out, dout, q_bytes, cudaMemcpyDeviceToHost, stream));
+  FCG_CUDA(cudaEventRecord(lib->last_patch_ev, stream));   // the staged output is in use until this copy is done
   return FCG_OK;
 }
 
