@@ -70,7 +70,7 @@ def attn_rows(cfg, wl) -> int:
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r01_final.md); None where no capture of that workload is committed.
-NCU_TRAFFIC = {"C2": {"stitch": 4.179e9, "attn": 2.183e9}, "C5": {"attn": 7.013e9}}
+NCU_TRAFFIC = {"C2": {"stitch": 4.178e9, "attn": 2.183e9}, "C5": {"attn": 7.011e9}}
 
 
 def tensor_peak():
