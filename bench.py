@@ -442,7 +442,9 @@ def run_cuda(args, cfg, wl, seed):
                    "l2": "inputs larger than L2 (each step streams >= 1 GiB; no flush needed)" if sb > 4 * 126e6
                    else "working set fits L2: latency only, no roofline claim",
                    "stitch_ms": float(np.mean(stitch_ms)), "stitch_ms_min": float(np.min(stitch_ms)),
+                   "stitch_ms_median": float(np.median(stitch_ms)),
                    "patch_ms": float(np.mean(patch_ms)), "patch_ms_min": float(np.min(patch_ms)),
+                   "patch_ms_median": float(np.median(patch_ms)),
                    "stitch_GBps": sb / (np.mean(stitch_ms) * 1e-3) / 1e9, "patch_attn_GBps": ab / (np.mean(patch_ms) * 1e-3) / 1e9,
                    "stitch_bytes": sb, "attn_bytes": ab, "attn_path": s1["last_attn_path"], "attn_splits": s1["last_attn_splits"],
                    "parallelism": f"task-replica x{world}"},
