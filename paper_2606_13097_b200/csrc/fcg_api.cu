@@ -933,7 +933,8 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
   if (use_tc) {
     // class 0: rows replicated 2x / 4x in one softmax warpgroup (HBM-bound; the deep K/V rings matter most);
     // class 1: two tile-parity softmax warpgroups; class 2: two Q tiles per CTA
-    for (int cl = 0; cl < 3; ++cl) {
+    // launched longest-CTA class first, so that the tail of the batch is made of the short CTAs
+    for (int cl = 2; cl >= 0; --cl) {
       if (n_cls[cl] == 0) continue;
       const int q_tiles = cl == 2 ? 2 : 1, parity_streams = cl == 1 ? 2 : 1;
       const fcg::AttnTaskDev *cls = h_tasks2 + cls_begin[cl];

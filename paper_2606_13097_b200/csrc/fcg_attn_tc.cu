@@ -8,8 +8,8 @@
 //             <1,2>  one Q tile, two softmax warpgroups on alternating KV tiles ("tile-parity streams")
 //             <2,1>  two Q tiles, one softmax warpgroup each (K/V read once per 256 rows)
 //   softmax warps    thread == query row == TMEM lane.  S tile read with tcgen05.ld, online softmax in the exp2
-//                    domain with a lazy (threshold 2^8) O rescale, packed fp32 pairs, part of the exp2 on the FMA
-//                    pipe; P goes back to TMEM as packed bf16 (tcgen05.st) -- with two Q tiles in place, over the
+//                    domain with a lazy (threshold 2^8) O rescale, packed fp32 pairs;
+//                    P goes back to TMEM as packed bf16 (tcgen05.st) -- with two Q tiles in place, over the
 //                    first half of its S tile
 //   K / V loader     one warp each: a TMA box copy (cp.async.bulk.tensor.5d, 128B swizzle) per (page, 64-column
 //                    half) through the page table into a ring of 64-token tiles; transaction-count mbarriers
@@ -207,26 +207,6 @@ __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
-}
-
-// exp2 of a pair on the FMA pipe: round-to-nearest split x = n + f with the 1.5 * 2^23 constant (n lands in the low
-// mantissa bits of t), a degree-3 minimax polynomial for 2^f on [-0.5, 0.5] (relative error 7.5e-5, far below the
-// bf16 rounding of P), and n added to the exponent field.  x <= RESCALE_TAU by construction; x < -126 (masked
-// columns are -inf) is clamped, giving 2^-126 instead of 0: below anything that survives in fp32 sums.
-__device__ __forceinline__ float2 ex2_poly2(float2 x) {
-  const float MAGIC = 12582912.f;
-  x.x = fmaxf(x.x, -126.f);
-  x.y = fmaxf(x.y, -126.f);
-  const float2 t = __fadd2_rn(x, make_float2(MAGIC, MAGIC));
-  const float2 n = __fadd2_rn(t, make_float2(-MAGIC, -MAGIC));
-  const float2 f = __fadd2_rn(x, make_float2(-n.x, -n.y));
-  float2 pl = __ffma2_rn(make_float2(0.0551716685f, 0.0551716685f), f, make_float2(0.2426111251f, 0.2426111251f));
-  pl = __ffma2_rn(pl, f, make_float2(0.6932609677f, 0.6932609677f));
-  pl = __ffma2_rn(pl, f, make_float2(0.9999280572f, 0.9999280572f));
-  float2 r;
-  r.x = __int_as_float(__float_as_int(pl.x) + (__float_as_int(t.x) << 23));
-  r.y = __int_as_float(__float_as_int(pl.y) + (__float_as_int(t.y) << 23));
-  return r;
 }
 
 // ---- shared memory map -------------------------------------------------------------------------
@@ -626,10 +606,8 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
         // tile was only issued after that P V)
         if (!C::P_ALIAS && j >= 2) mbar_wait(pv_done(qt, b), ((j - 2) >> 1) & 1);
         uint32_t preg[NC / 2];
-        // packed fp32 pairs (FFMA2 / FADD2) for the scale-subtract and the row sum.  In the tensor-bound layout
-        // (64 columns per thread) one pair in four takes its exp2 from the FMA pipe instead of the MUFU, whose
-        // 16 results per clock and SM would otherwise cost as many cycles per tile as the two MMAs.
-        constexpr int EMU_EVERY = NC == 64 ? 4 : 0;        // emulate pair q when q % EMU_EVERY == EMU_EVERY - 1
+        // packed fp32 pairs (FFMA2 / FADD2) for the scale-subtract and the row sum; every exp2 on the MUFU (moving a
+        // share of them to a polynomial on the FMA pipe cost more issue slots than the MUFU time it saved)
         const float2 sc2 = make_float2(sc, sc), nmu2 = make_float2(-mu, -mu);
         float2 sum2[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
 #pragma unroll
@@ -638,10 +616,7 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
             const float2 x = __ffma2_rn(make_float2(__uint_as_float(sreg[c8 * 8 + 2 * q]), __uint_as_float(sreg[c8 * 8 + 2 * q + 1])), sc2, nmu2);
-            if (EMU_EVERY > 0 && ((c8 * 4 + q) % (EMU_EVERY > 0 ? EMU_EVERY : 1)) == EMU_EVERY - 1)
-              e[q] = ex2_poly2(x);
-            else
-              e[q] = make_float2(ex2_approx(x.x), ex2_approx(x.y));
+            e[q] = make_float2(ex2_approx(x.x), ex2_approx(x.y));
             sum2[q & 1] = __fadd2_rn(sum2[q & 1], e[q]);
           }
 #pragma unroll
