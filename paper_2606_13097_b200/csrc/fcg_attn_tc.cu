@@ -566,8 +566,10 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
           TMEM_LD_16(tmem_s + b * BN + c0, sreg);
         }
         tmem_wait_ld();
-        tc_fence_before();
-        mbar_arrive(s_free(qt, b));                     // S[b] may be overwritten by Q K^T of tile j+2
+        if (!C::P_ALIAS) {
+          tc_fence_before();
+          mbar_arrive(s_free(qt, b));                   // S[b] may be overwritten by Q K^T of tile j+2
+        }
         if (ts + NC - 1 > lim) {
 #pragma unroll
           for (int c = 0; c < NC; ++c)

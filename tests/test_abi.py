@@ -83,3 +83,15 @@ def test_product_does_not_import_the_oracle():
     for f in ("fcg_oracle.py",):
         src = open(os.path.join(ROOT, "oracle", f)).read()
         assert "import paper_2606_13097_b200" not in src and "from paper_2606_13097_b200" not in src
+
+
+def test_header_is_plain_c():
+    """include/fcg.h compiles as C99 on its own (no C++, no CUDA, no torch types in the boundary)."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc")
+    r = subprocess.run([gcc, "-std=c99", "-Wall", "-Werror", "-fsyntax-only", "-x", "c", os.path.join(ROOT, "include", "fcg.h")],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
