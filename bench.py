@@ -581,6 +581,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C2", choices=sorted(synth.CONFIGS))
     ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--page-size", type=int, default=0, choices=[0, 8, 16, 32, 64],
+                    help="override the config's page size (secondary measurement; default: the config's 16)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--prefill-compare", action="store_true",
@@ -590,6 +592,8 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     cfg = synth.CONFIGS[args.config]
+    if args.page_size:
+        cfg = synth.scaled(cfg, page_size=args.page_size)
     wl = synth.make_workload(cfg, args.seed)
     if args.impl == "reference":
         res = run_reference(args, cfg, wl, args.seed)
