@@ -89,8 +89,9 @@ struct fcg_library {
   BlobSlot slots[BLOB_SLOTS];
   // fcg_patch_host: the host->device copies run on the library's own stream, ordered after the last patch call
   // (the staging area belongs to patch calls only), so they overlap a stitch enqueued just before on the caller's stream
-  cudaStream_t copy_stream = nullptr;
-  cudaEvent_t last_patch_ev = nullptr, h2d_ev = nullptr;
+  cudaStream_t copy_stream = nullptr, d2h_stream = nullptr;
+  static constexpr int HOST_GROUPS = 4;          // layer groups of a host call: copy in / attend / copy out pipelined
+  cudaEvent_t last_patch_ev = nullptr, h2d_ev[HOST_GROUPS] = {}, attn_ev[HOST_GROUPS] = {}, d2h_ev = nullptr;
   bool have_last_patch = false;
   int next_slot = 0;
   fcg_stats_t stats;
@@ -439,8 +440,13 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
   }
   {
     cudaError_t e = cudaStreamCreateWithFlags(&lib->copy_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&lib->d2h_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->last_patch_ev, cudaEventDisableTiming);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->h2d_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->d2h_ev, cudaEventDisableTiming);
+    for (int g = 0; g < fcg_library::HOST_GROUPS && e == cudaSuccess; ++g) {
+      e = cudaEventCreateWithFlags(&lib->h2d_ev[g], cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->attn_ev[g], cudaEventDisableTiming);
+    }
     if (e != cudaSuccess) {
       fcg_library_destroy(lib);
       return fail(FCG_ERR_CUDA, "copy stream / events: %s", cudaGetErrorString(e));
@@ -480,8 +486,13 @@ fcg_status_t fcg_library_destroy(fcg_library_t *lib) {
     if (lib->slots[i].ev) cudaEventDestroy(lib->slots[i].ev);
   }
   if (lib->copy_stream) cudaStreamDestroy(lib->copy_stream);
+  if (lib->d2h_stream) cudaStreamDestroy(lib->d2h_stream);
   if (lib->last_patch_ev) cudaEventDestroy(lib->last_patch_ev);
-  if (lib->h2d_ev) cudaEventDestroy(lib->h2d_ev);
+  if (lib->d2h_ev) cudaEventDestroy(lib->d2h_ev);
+  for (int g = 0; g < fcg_library::HOST_GROUPS; ++g) {
+    if (lib->h2d_ev[g]) cudaEventDestroy(lib->h2d_ev[g]);
+    if (lib->attn_ev[g]) cudaEventDestroy(lib->attn_ev[g]);
+  }
   delete lib;
   return FCG_OK;
 }
@@ -1007,23 +1018,53 @@ fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_b
   unsigned char *base = lib->arena + lib->scratch_off + lib->scratch_bytes - need;
   unsigned char *dq = base, *dk = dq + align_up(q_bytes), *dv = dk + align_up(kv_bytes), *dout = dv + align_up(kv_bytes);
   FCG_CUDA(cudaSetDevice(c.device));
-  // copies on the library's stream: after the last user of the staging / partial area, but NOT after a stitch the
-  // caller has just enqueued on `stream` (stitch never touches the scratch area)
+  // Copies in on the library's copy stream: after the last user of the staging / partial area, but NOT after a
+  // stitch the caller has just enqueued on `stream` (stitch never touches the scratch area).  Large calls are cut
+  // into layer groups: group g attends while group g+1 is still arriving and group g-1 is leaving (second copy
+  // stream), all joined back into `stream` at the end.
+  const int groups = (q_bytes >= (8ull << 20) && n_layers >= fcg_library::HOST_GROUPS) ? fcg_library::HOST_GROUPS : 1;
+  const uint64_t q_layer = q_bytes / n_layers, kv_layer = kv_bytes / n_layers;
+  auto group_begin = [&](int g) { return (int)((int64_t)n_layers * g / groups); };
   if (lib->have_last_patch) FCG_CUDA(cudaStreamWaitEvent(lib->copy_stream, lib->last_patch_ev, 0));
-  FCG_CUDA(cudaMemcpyAsync(dq, q, q_bytes, cudaMemcpyHostToDevice, lib->copy_stream));
-  FCG_CUDA(cudaMemcpyAsync(dk, k, kv_bytes, cudaMemcpyHostToDevice, lib->copy_stream));
-  FCG_CUDA(cudaMemcpyAsync(dv, v, kv_bytes, cudaMemcpyHostToDevice, lib->copy_stream));
-  FCG_CUDA(cudaEventRecord(lib->h2d_ev, lib->copy_stream));
-  FCG_CUDA(cudaStreamWaitEvent(stream, lib->h2d_ev, 0));
+  for (int g = 0; g < groups; ++g) {
+    const int lb = group_begin(g), nl = group_begin(g + 1) - lb;
+    FCG_CUDA(cudaMemcpyAsync(dq + lb * q_layer, (const char *)q + lb * q_layer, nl * q_layer, cudaMemcpyHostToDevice, lib->copy_stream));
+    FCG_CUDA(cudaMemcpyAsync(dk + lb * kv_layer, (const char *)k + lb * kv_layer, nl * kv_layer, cudaMemcpyHostToDevice, lib->copy_stream));
+    FCG_CUDA(cudaMemcpyAsync(dv + lb * kv_layer, (const char *)v + lb * kv_layer, nl * kv_layer, cudaMemcpyHostToDevice, lib->copy_stream));
+    FCG_CUDA(cudaEventRecord(lib->h2d_ev[g], lib->copy_stream));
+  }
   // partials must not collide with the staging area: temporarily shrink the scratch
   const uint64_t saved = lib->scratch_bytes;
   lib->scratch_bytes = saved - need;
-  PatchCall pc{&task_id, &n, 1, layer_begin, n_layers, dq, dk, dv, positions, dout, stream};
-  fcg_status_t st = patch_common(lib, pc);
+  fcg_status_t st = FCG_OK;
+  for (int g = 0; g < groups && st == FCG_OK; ++g) {
+    const int lb = group_begin(g), nl = group_begin(g + 1) - lb;
+    cudaError_t e = cudaStreamWaitEvent(stream, lib->h2d_ev[g], 0);
+    if (e != cudaSuccess) {
+      st = fail(FCG_ERR_CUDA, "cudaStreamWaitEvent: %s", cudaGetErrorString(e));
+      break;
+    }
+    PatchCall pc{&task_id, &n, 1, layer_begin + lb, nl, dq + lb * q_layer, dk + lb * kv_layer, dv + lb * kv_layer, positions,
+                 dout + lb * q_layer, stream};
+    st = patch_common(lib, pc);
+    if (st != FCG_OK) break;
+    if (groups > 1) {
+      e = cudaEventRecord(lib->attn_ev[g], stream);
+      if (e == cudaSuccess) e = cudaStreamWaitEvent(lib->d2h_stream, lib->attn_ev[g], 0);
+      if (e == cudaSuccess)
+        e = cudaMemcpyAsync((char *)out + lb * q_layer, dout + lb * q_layer, nl * q_layer, cudaMemcpyDeviceToHost, lib->d2h_stream);
+      if (e != cudaSuccess) st = fail(FCG_ERR_CUDA, "copy out: %s", cudaGetErrorString(e));
+    }
+  }
   lib->scratch_bytes = saved;
   if (st != FCG_OK) return st;
-  FCG_CUDA(cudaMemcpyAsync(out, dout, q_bytes, cudaMemcpyDeviceToHost, stream));
-  FCG_CUDA(cudaEventRecord(lib->last_patch_ev, stream));   // the staged output is in use until this copy is done
+  if (groups > 1) {
+    FCG_CUDA(cudaEventRecord(lib->d2h_ev, lib->d2h_stream));
+    FCG_CUDA(cudaStreamWaitEvent(stream, lib->d2h_ev, 0));
+  } else {
+    FCG_CUDA(cudaMemcpyAsync(out, dout, q_bytes, cudaMemcpyDeviceToHost, stream));
+  }
+  FCG_CUDA(cudaEventRecord(lib->last_patch_ev, stream));   // the staged output is in use until these copies are done
   return FCG_OK;
 }
 
