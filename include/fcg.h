@@ -1,7 +1,7 @@
 /* fcg.h -- C ABI of the B200-native FCGRAFT KV-cache grafting library (libfcg.so).
  *
  * What the calls compute is defined by the paper (PAPER.md = the text of arxiv/paper_2606_13097)
- * and, where the paper is silent, by the readings R1..R16 in DESIGN.md:
+ * and, where the paper is silent, by the readings R1..R23 in DESIGN.md:
  *
  *   segment library   the KV half of the two-tier code cache H = (I, C), Eq. (2), PAPER.md:66-79:
  *                     per function a cached K/V state that can be re-injected "without being tied
