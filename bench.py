@@ -477,6 +477,7 @@ def run_cuda(args, cfg, wl, seed):
     lib.close()
     if world > 1:
         import torch.distributed as dist
+        dist.barrier()                      # rank 0 may still have been timing its extras
         dist.destroy_process_group()
     return res if rank == 0 else None
 
