@@ -373,6 +373,22 @@ class OracleLibrary:
         if not np.all(f[: pos[-1] + 1]):
             raise OracleError(FCG_ERR_UNFILLED, "a patch query would attend over an unfilled position")
 
+    def patch_rope(self, task_id: int, layer_begin: int, q_bits, k_bits, v_bits, positions) -> np.ndarray:
+        """patch() for callers that hold the projections BEFORE position encoding (DESIGN R13
+        variant): token i's query and key are first rotated to its absolute position p_i by the library's RoPE
+        (theta_j and pair layout of the configuration), each rounded once to bf16 -- what a model's own RoPE would
+        have handed to patch() -- then scattered / attended exactly as in patch().  rope_mode NONE: identical to patch().
+        """
+        pos = np.asarray(positions, dtype=np.int64)
+        q_bits = np.asarray(q_bits, np.uint16)
+        k_bits = np.asarray(k_bits, np.uint16)
+        if self.rope_mode != ROPE_NONE and pos.ndim == 1 and q_bits.ndim == 4 and k_bits.ndim == 4 \
+                and q_bits.shape[1] == pos.size and k_bits.shape[1] == pos.size:
+            per_row = pos[None, :, None]                                   # one delta per (layer, token, head) row
+            q_bits = rope_shift_bf16(q_bits, np.broadcast_to(per_row, q_bits.shape[:3]), self.inv_freq, self.rope_mode)
+            k_bits = rope_shift_bf16(k_bits, np.broadcast_to(per_row, k_bits.shape[:3]), self.inv_freq, self.rope_mode)
+        return self.patch(task_id, layer_begin, q_bits, k_bits, v_bits, positions)
+
     def patch(self, task_id: int, layer_begin: int, q_bits, k_bits, v_bits, positions) -> np.ndarray:
         """Scatter then causal patch attention (Eq. 6).
 

@@ -695,3 +695,47 @@ def test_segment_residency_state_machine():
         with pytest.raises(O.OracleError) as e:
             fn(77)
         assert e.value.status == O.FCG_ERR_BAD_SEGMENT
+
+
+def test_patch_rope_is_rotation_to_absolute_positions_then_patch():
+    """patch_rope == rotate q_i, k_i to p_i (independent complex form, one rounding) then patch; and what it computes
+    depends on relative positions only (P7 through the whole call): the same tokens patched at positions c.. instead
+    of 0.. give the same output once the mass of the c zero-key / zero-value filler tokens is accounted for."""
+    lib = _small_lib()
+    L, Hq, Hkv, D = lib.L, lib.Hq, lib.Hkv, lib.D
+    n = 9
+    q, k, v = _rand_bf16((L, n, Hq, D)), _rand_bf16((L, n, Hkv, D)), _rand_bf16((L, n, Hkv, D))
+    pos = np.arange(n)
+    lib.stitch([O.Plan(0, [], [O.Hole(0, n)], n)])
+    out = lib.patch_rope(0, 0, q, k, v, pos)
+    manual_q = np.stack([_complex_shift_bits(q[:, i], int(p), lib.inv_freq) for i, p in enumerate(pos)], axis=1)
+    manual_k = np.stack([_complex_shift_bits(k[:, i], int(p), lib.inv_freq) for i, p in enumerate(pos)], axis=1)
+    assert np.array_equal(np.transpose(lib.tasks[0].k[:, :, pos], (0, 2, 1, 3)), manual_k)
+    lib2 = _small_lib()
+    lib2.stitch([O.Plan(0, [], [O.Hole(0, n)], n)])
+    assert np.array_equal(lib2.patch(0, 0, manual_q, manual_k, v, pos), out)
+    # shifted by c = 40 behind filler tokens with zero keys (score 0) and zero values
+    lib3 = _small_lib()
+    c = 40
+    lib3.stitch([O.Plan(0, [], [O.Hole(0, c + n)], c + n)])
+    zeros = lambda h: np.zeros((L, c, h, D), np.uint16)
+    lib3.patch(0, 0, zeros(Hq), zeros(Hkv), zeros(Hkv), np.arange(c))
+    out_shift = lib3.patch_rope(0, 0, q, k, v, np.arange(c, c + n))
+    qf, kf = O.bf16_to_f64(q), O.bf16_to_f64(k)
+    for li in range(L):
+        for i in range(n):
+            for h in range(Hq):
+                g = h // lib.G
+                s_rel = np.array([np.dot(O.rope_rotate_f64(qf[li, i, h], i, lib.inv_freq), O.rope_rotate_f64(kf[li, x, g], x, lib.inv_freq))
+                                  for x in range(i + 1)]) / math.sqrt(D)
+                m = max(s_rel.max(), 0.0)
+                w = np.exp(s_rel - m)
+                ref = (w @ O.bf16_to_f64(v[li, : i + 1, g])) / (w.sum() + c * math.exp(-m))
+                assert np.allclose(out_shift[li, i, h], ref, rtol=0, atol=0.06), (li, i, h)
+    # rope_mode NONE: patch_rope is patch
+    lib0 = _small_lib(rope_mode=0)
+    lib0.stitch([O.Plan(0, [], [O.Hole(0, n)], n)])
+    a = lib0.patch_rope(0, 0, q, k, v, np.arange(n))
+    lib0.task_release(0)
+    lib0.stitch([O.Plan(0, [], [O.Hole(0, n)], n)])
+    assert np.array_equal(a, lib0.patch(0, 0, q, k, v, np.arange(n)))
