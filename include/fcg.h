@@ -143,6 +143,15 @@ fcg_status_t fcg_patch(fcg_library_t *lib, int32_t task_id, int32_t layer_begin,
                        const void *q, const void *k, const void *v, const int32_t *positions, int32_t n,
                        void *out, void *stream);
 
+/* fcg_patch for callers that hold q and k BEFORE position encoding (R13 variant): token
+ * i's q and k rows are first rotated to the absolute position positions[i] with the library's RoPE (theta_j and pair
+ * layout of the configuration; each rounded once to bf16, within 1 ulp of the fp64 value), then scattered and attended
+ * exactly as in fcg_patch.  FCG_ROPE_NONE: identical to fcg_patch.  The rotated copies live in the workspace
+ * (OUT_OF_ARENA if they, or the n x head_dim/2 cos/sin table, do not fit). */
+fcg_status_t fcg_patch_rope(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers,
+                            const void *q, const void *k, const void *v, const int32_t *positions, int32_t n,
+                            void *out, void *stream);
+
 /* Same as fcg_patch with q, k, v, out in HOST memory (pinned for true asynchrony): the call enqueues the
  * host->device copies, the kernels and the device->host copy of `out`; out is valid (and q, k, v may be reused)
  * once `stream` has been synchronised.  The host->device copies run on a stream of the library's own, ordered
@@ -239,6 +248,7 @@ typedef struct {
   int32_t last_attn_path;   /* 0 none, 1 split-KV warp-MMA, 2 tcgen05 */
   int32_t last_attn_splits;
   uint64_t offload_copies, prefetch_copies;   /* tier moves (copy engine, not kernels) */
+  uint64_t rope_qk_launches;
 } fcg_stats_t;
 fcg_status_t fcg_stats(fcg_library_t *lib, fcg_stats_t *out);
 

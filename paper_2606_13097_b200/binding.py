@@ -74,7 +74,7 @@ class fcg_stats_t(C.Structure):
                 ("attn_split_launches", C.c_uint64), ("attn_combine_launches", C.c_uint64),
                 ("attn_tc_launches", C.c_uint64), ("read_launches", C.c_uint64),
                 ("last_attn_path", C.c_int32), ("last_attn_splits", C.c_int32),
-                ("offload_copies", C.c_uint64), ("prefetch_copies", C.c_uint64)]
+                ("offload_copies", C.c_uint64), ("prefetch_copies", C.c_uint64), ("rope_qk_launches", C.c_uint64)]
 
 
 # every symbol include/fcg.h declares: name -> (restype, argtypes)
@@ -93,6 +93,7 @@ SYMBOLS = {
     "fcg_stitch": (_I, [_P, C.POINTER(fcg_plan_t), _I, _P]),
     "fcg_patch": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
     "fcg_patch_host": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
+    "fcg_patch_rope": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
     "fcg_patch_batch": (_I, [_P, _PI, _PI, _I, _I, _I, _P, _P, _P, _PI, _P, _P]),
     "fcg_task_page_table": (_I, [_P, _I, C.POINTER(_P), _PI, _PI]),
     "fcg_task_page_table_host": (_I, [_P, _I, _PI, _I, _PI]),
@@ -239,6 +240,12 @@ def fcg_patch(handle, task_id, layer_begin, n_layers, q, k, v, positions, out, s
     pos = _i32(positions)
     _check(load().fcg_patch(handle, int(task_id), int(layer_begin), int(n_layers), _ptr(q), _ptr(k), _ptr(v),
                             pos.ctypes.data_as(_PI), int(pos.size), _ptr(out), _stream(stream)))
+
+
+def fcg_patch_rope(handle, task_id, layer_begin, n_layers, q, k, v, positions, out, stream=None) -> None:
+    pos = np.ascontiguousarray(positions, dtype=np.int32)
+    _check(load().fcg_patch_rope(handle, int(task_id), int(layer_begin), int(n_layers), _ptr(q), _ptr(k), _ptr(v),
+                                 pos.ctypes.data_as(_PI), int(pos.size), _ptr(out), _stream(stream)))
 
 
 def fcg_patch_host(handle, task_id, layer_begin, n_layers, q, k, v, positions, out, stream=None) -> None:
@@ -388,6 +395,13 @@ class FcgLibrary:
         if out is None:
             out = torch.empty_like(q)
         fcg_patch(self.handle, task_id, layer_begin, q.shape[0], q, k, v, positions, out, stream)
+        return out
+
+    def patch_rope(self, task_id, layer_begin, q, k, v, positions, out=None, stream=None) -> torch.Tensor:
+        assert q.is_cuda and q.is_contiguous() and k.is_contiguous() and v.is_contiguous()
+        if out is None:
+            out = torch.empty_like(q)
+        fcg_patch_rope(self.handle, task_id, layer_begin, q.shape[0], q, k, v, positions, out, stream)
         return out
 
     def patch_host(self, task_id, layer_begin, q, k, v, positions, out, stream=None) -> torch.Tensor:

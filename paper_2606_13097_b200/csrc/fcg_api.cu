@@ -1004,6 +1004,90 @@ fcg_status_t fcg_patch_batch(fcg_library_t *lib, const int32_t *task_ids, const 
   return patch_common(lib, pc);
 }
 
+// NEXT-4 (R13 variant): q and k arrive before position encoding; rotate them to positions[i], then patch
+fcg_status_t fcg_patch_rope(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers, const void *q,
+                            const void *k, const void *v, const int32_t *positions, int32_t n, void *out, void *stream_) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  const fcg_config_t &c = lib->cfg;
+  if (c.rope_mode == FCG_ROPE_NONE) return fcg_patch(lib, task_id, layer_begin, n_layers, q, k, v, positions, n, out, stream_);
+  if (!q || !k || !v || !out || !positions || n <= 0 || n_layers <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty argument");
+  for (int i = 0; i < n; ++i)
+    if (positions[i] < 0 || (i > 0 && positions[i] <= positions[i - 1]))
+      return fail(FCG_ERR_INVALID_ARG, "positions must be non-negative and strictly increasing");
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  const int half = c.head_dim / 2;
+  const uint64_t q_bytes = (uint64_t)n_layers * n * c.n_q_heads * c.head_dim * 2;
+  const uint64_t kv_bytes = (uint64_t)n_layers * n * c.n_kv_heads * c.head_dim * 2;
+  const uint64_t tab_bytes = (uint64_t)n * half * sizeof(float4);
+  const uint64_t need = align_up(q_bytes) + align_up(kv_bytes);
+  if (tab_bytes > BLOB_BYTES) return fail(FCG_ERR_OUT_OF_ARENA, "rope table of %d tokens exceeds the %llu-byte plan blob", n, (unsigned long long)BLOB_BYTES);
+  if (need > lib->scratch_bytes / 2) return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for %llu bytes of rotated q / k", (unsigned long long)need);
+  // rotated copies at the END of the scratch area (where fcg_patch_host stages too); split partials grow from its start
+  unsigned char *dq = lib->arena + lib->scratch_off + lib->scratch_bytes - need, *dk = dq + align_up(q_bytes);
+
+  FCG_CUDA(cudaSetDevice(c.device));
+  BlobSlot *slot = nullptr;
+  fcg_status_t st = acquire_slot(lib, &slot);
+  if (st != FCG_OK) return st;
+  // cos / sin of p_i * theta_j in fp64: exact evaluation at the start of every run of consecutive positions (and every
+  // 32 tokens), angle addition by theta_j in between (error ~1e-16 per step), then the hi / lo split of the stitch table
+  float4 *tab = reinterpret_cast<float4 *>(slot->host);
+  std::vector<double> cs(half), sn(half), c1(half), s1(half);
+  for (int j = 0; j < half; ++j) {
+    c1[j] = cos(lib->inv_freq[j]);
+    s1[j] = sin(lib->inv_freq[j]);
+  }
+  auto split = [](double x, float &hi, float &lo) {
+    float f = (float)x;
+    uint32_t b;
+    memcpy(&b, &f, 4);
+    b = (b + 0x80u) & 0xffffff00u;
+    memcpy(&hi, &b, 4);
+    lo = (float)(x - (double)hi);
+  };
+  for (int i = 0, run = 0; i < n; ++i) {
+    const bool anchor = i == 0 || positions[i] != positions[i - 1] + 1 || run >= 32;
+    for (int j = 0; j < half; ++j) {
+      if (anchor) {
+        const double phi = (double)positions[i] * lib->inv_freq[j];
+        cs[j] = cos(phi);
+        sn[j] = sin(phi);
+      } else {
+        const double cn = cs[j] * c1[j] - sn[j] * s1[j], snn = sn[j] * c1[j] + cs[j] * s1[j];
+        cs[j] = cn;
+        sn[j] = snn;
+      }
+      float4 t;
+      split(cs[j], t.x, t.y);
+      split(sn[j], t.z, t.w);
+      tab[(size_t)i * half + j] = t;
+    }
+    run = anchor ? 0 : run + 1;
+  }
+  FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, tab_bytes, cudaMemcpyHostToDevice, stream));
+  fcg::RopeQkParams rp;
+  rp.q = static_cast<const uint16_t *>(q);
+  rp.k = static_cast<const uint16_t *>(k);
+  rp.q_out = reinterpret_cast<uint16_t *>(dq);
+  rp.k_out = reinterpret_cast<uint16_t *>(dk);
+  rp.table = reinterpret_cast<const float4 *>(slot->dev);
+  rp.n_layers = n_layers;
+  rp.n_total = n;
+  rp.n_q_heads = c.n_q_heads;
+  rp.n_kv_heads = c.n_kv_heads;
+  rp.interleaved = c.rope_mode == FCG_ROPE_INTERLEAVED ? 1 : 0;
+  FCG_CUDA(fcg::launch_rope_qk(rp, c.head_dim, stream));
+  lib->stats.rope_qk_launches++;
+  FCG_CUDA(cudaEventRecord(slot->ev, stream));
+  slot->in_flight = true;
+  const uint64_t saved = lib->scratch_bytes;
+  lib->scratch_bytes = saved - need;
+  PatchCall pc{&task_id, &n, 1, layer_begin, n_layers, dq, dk, v, positions, out, stream};
+  st = patch_common(lib, pc);
+  lib->scratch_bytes = saved;
+  return st;
+}
+
 fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers, const void *q,
                             const void *k, const void *v, const int32_t *positions, int32_t n, void *out, void *stream_) {
   if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");

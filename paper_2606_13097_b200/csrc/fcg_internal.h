@@ -44,6 +44,16 @@ struct StitchParams {
 
 cudaError_t launch_stitch(const StitchParams &p, int head_dim, cudaStream_t stream);
 
+// fcg_patch_rope: rotate the patch's q and k rows (given before position encoding) to their absolute positions.
+// table: per (token i, j): {c_hi, c_lo, s_hi, s_lo} of p_i * theta_j, same split as the stitch table.
+struct RopeQkParams {
+  const uint16_t *q, *k;     // [n_layers][n_total][Hq | Hkv][D]
+  uint16_t *q_out, *k_out;   // same shapes
+  const float4 *table;       // [n_total][D/2]
+  int32_t n_layers, n_total, n_q_heads, n_kv_heads, interleaved;
+};
+cudaError_t launch_rope_qk(const RopeQkParams &p, int head_dim, cudaStream_t stream);
+
 // ---------------------------------------------------------------------------------------------
 // S1 (register copy), S4 (scatter), task read
 // ---------------------------------------------------------------------------------------------

@@ -159,7 +159,62 @@ __global__ void __launch_bounds__(128, 4) stitch_kernel(const StitchParams p) {
   }
 }
 
+// q / k rows of the patch tokens -> rotated to their absolute positions (fcg_patch_rope).  One CTA per (token, layer);
+// a thread owns the two 16-byte vectors [col*8, +8) and [D/2 + col*8, +8) of one head row, as in stitch_kernel.
+template <int D>
+__global__ void __launch_bounds__(128) rope_qk_kernel(const RopeQkParams p) {
+  constexpr int LPT = D / 16;
+  const int tok = blockIdx.x, layer = blockIdx.y;
+  const int rows = p.n_q_heads + p.n_kv_heads;
+  const bool il = p.interleaved != 0;
+  for (int w = threadIdx.x; w < rows * LPT; w += blockDim.x) {
+    const int r = w / LPT, col = w % LPT;
+    const bool is_q = r < p.n_q_heads;
+    const size_t row = is_q ? ((size_t)layer * p.n_total + tok) * p.n_q_heads + r
+                            : ((size_t)layer * p.n_total + tok) * p.n_kv_heads + (r - p.n_q_heads);
+    const char *src = reinterpret_cast<const char *>(is_q ? p.q : p.k) + row * (D * 2) + col * 16;
+    char *dst = reinterpret_cast<char *>(is_q ? p.q_out : p.k_out) + row * (D * 2) + col * 16;
+    const uint4 lo = *reinterpret_cast<const uint4 *>(src), hi = *reinterpret_cast<const uint4 *>(src + D);
+    float4 tab[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int j = il ? ((i >> 2) * (D / 4) + col * 4 + (i & 3)) : (col * 8 + i);
+      tab[i] = __ldg(p.table + (size_t)tok * (D / 2) + j);
+    }
+    uint4 olo, ohi;
+    if (!il) {
+      rot_word(lo.x, hi.x, tab[0], tab[1], olo.x, ohi.x);
+      rot_word(lo.y, hi.y, tab[2], tab[3], olo.y, ohi.y);
+      rot_word(lo.z, hi.z, tab[4], tab[5], olo.z, ohi.z);
+      rot_word(lo.w, hi.w, tab[6], tab[7], olo.w, ohi.w);
+    } else {
+      olo.x = rot_word_il(lo.x, tab[0]);
+      olo.y = rot_word_il(lo.y, tab[1]);
+      olo.z = rot_word_il(lo.z, tab[2]);
+      olo.w = rot_word_il(lo.w, tab[3]);
+      ohi.x = rot_word_il(hi.x, tab[4]);
+      ohi.y = rot_word_il(hi.y, tab[5]);
+      ohi.z = rot_word_il(hi.z, tab[6]);
+      ohi.w = rot_word_il(hi.w, tab[7]);
+    }
+    *reinterpret_cast<uint4 *>(dst) = olo;
+    *reinterpret_cast<uint4 *>(dst + D) = ohi;
+  }
+}
+
 }  // namespace
+
+cudaError_t launch_rope_qk(const RopeQkParams &p, int head_dim, cudaStream_t stream) {
+  if (p.n_total <= 0 || p.n_layers <= 0) return cudaSuccess;
+  dim3 grid((unsigned)p.n_total, (unsigned)p.n_layers, 1);
+  if (head_dim == 128)
+    rope_qk_kernel<128><<<grid, 128, 0, stream>>>(p);
+  else if (head_dim == 64)
+    rope_qk_kernel<64><<<grid, 128, 0, stream>>>(p);
+  else
+    return cudaErrorInvalidValue;
+  return cudaGetLastError();
+}
 
 cudaError_t launch_stitch(const StitchParams &p, int head_dim, cudaStream_t stream) {
   if (p.n_chunks <= 0) return cudaSuccess;

@@ -257,3 +257,43 @@ def test_two_tier_residency_stitch_from_host_and_prefetch():
         lib.segment_offload(0)
     assert e.value.status == B.FCG_ERR_INVALID_ARG
     lib.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4: fcg_patch_rope -- q / k given before position encoding
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("rope_mode,D", [(1, 128), (2, 128), (1, 64), (0, 128)])
+def test_patch_rope_matches_oracle(rope_mode, D):
+    cfg = synth.GraftConfig("prope", 2, 8, 2, D, 16, 5e5, 3, 100, 300, 30000, 1, 3, 3, 0, holes=((0, 45), (-1, 50)))
+    wl, orc, lib, seg_ids = _pair(cfg, seed=4, rope_mode=rope_mode)
+    task = wl.tasks[0]
+    c_plans, o_plans = T.plans_of(wl, seg_ids)
+    orc.stitch(o_plans)
+    lib.stitch(c_plans)
+    # first the mid hole (45 consecutive positions: one exact anchor + a re-anchor after 32), then the end hole in two
+    # calls with a gap pattern (non-consecutive positions are not allowed to leave holes: use consecutive chunks)
+    holes = sorted(task.holes)
+    chunks = [np.arange(holes[0][0], holes[0][0] + holes[0][1]), np.arange(holes[1][0], holes[1][0] + 7),
+              np.arange(holes[1][0] + 7, holes[1][0] + holes[1][1])]
+    for ci, pos in enumerate(chunks):
+        pos = pos.astype(np.int32)
+        q, k, v = synth.patch_qkv(cfg, 0, len(pos), 40 + ci, "cpu")
+        ref = orc.patch_rope(0, 0, synth.to_bits(q), synth.to_bits(k), synth.to_bits(v), pos)
+        out = lib.patch_rope(0, 0, q.cuda(), k.cuda(), v.cuda(), pos)
+        torch.cuda.synchronize()
+        T.assert_attn_close(out, ref, f"patch_rope chunk {ci}")
+        ot = orc.tasks[0]
+        for layer in range(cfg.n_layers):
+            kg, vg = lib.task_read(0, layer, 0, ot.capacity)
+            kb, vb = synth.to_bits(kg), synth.to_bits(vg)
+            assert np.array_equal(vb[:, pos], ot.v[layer][:, pos]), "V scatter not bit-exact"
+            if rope_mode == 0:
+                assert np.array_equal(kb[:, pos], ot.k[layer][:, pos])
+            else:
+                T.assert_k_within_1ulp(kb[:, pos], ot.k[layer][:, pos], f"rotated patch K, chunk {ci} layer {layer}")
+    assert lib.stats()["rope_qk_launches"] == (0 if rope_mode == 0 else len(chunks))
+    B = _binding()
+    with pytest.raises(B.FcgError) as e:
+        lib.patch_rope(0, 0, q.cuda(), k.cuda(), v.cuda(), pos[::-1].copy())
+    assert e.value.status == B.FCG_ERR_INVALID_ARG
+    lib.close()
