@@ -252,6 +252,25 @@ typedef struct {
 } fcg_stats_t;
 fcg_status_t fcg_stats(fcg_library_t *lib, fcg_stats_t *out);
 
+/* Locality score of the cache management scheme (Eq. 3, 8, 9, 10): host-only bookkeeping, no
+ * CUDA, independent of any library handle.  Ids are the caller's function ids (normally segment ids).
+ *   l(f_k) = (1 - l_curr) (alpha l_freq + beta sum_j l_asso(f_j | f_k) + gamma l_sema) + l_curr
+ *   l_freq = count(f_k) / max_j count(f_j);  l_asso(f_j | f_k) = cooccur(f_k, f_j) / count(f_k);  l_sema = PPL / max PPL.
+ * Readings (R24): fcg_scorer_record takes ONE task's execution trace, the functions in invocation order;
+ * count = invocations over all recorded traces; cooccur(f_k, f_j) = times f_j was the next invocation after f_k (j != k),
+ * so the sum over j lies in [0, 1]; l_curr = 1 for the functions of the most recent trace; PPL comes from the caller
+ * (0 where never set).  fcg_scorer_rank sorts `ids` by ascending score (ties: ascending id): the front of the list is
+ * what to hand to fcg_segment_offload first.  fcg_scorer_forget drops a released function from the statistics. */
+typedef struct fcg_scorer fcg_scorer_t;
+fcg_status_t fcg_scorer_create(fcg_scorer_t **out);
+fcg_status_t fcg_scorer_destroy(fcg_scorer_t *s);
+fcg_status_t fcg_scorer_record(fcg_scorer_t *s, const int32_t *ids, int32_t n);
+fcg_status_t fcg_scorer_set_ppl(fcg_scorer_t *s, int32_t id, double ppl);
+fcg_status_t fcg_scorer_forget(fcg_scorer_t *s, int32_t id);
+fcg_status_t fcg_scorer_score(fcg_scorer_t *s, int32_t id, double alpha, double beta, double gamma, double *score);
+fcg_status_t fcg_scorer_rank(fcg_scorer_t *s, const int32_t *ids, int32_t n, double alpha, double beta, double gamma,
+                             int32_t *ids_out, double *scores_out);
+
 /* Message for the last non-OK status returned on this thread (never NULL). */
 const char *fcg_last_error(void);
 /* "x.y.z sm_100a" */

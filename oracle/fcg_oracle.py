@@ -28,7 +28,8 @@ not needed at run time; DESIGN.md "Readings" lists every choice R1..R14):
 
 NEXT rows of SURVEY.md 8(f) stated here as well: interleaved RoPE pairs
 (rope_mode 2), ``task_shift`` (re-graft of the kept suffix after a patch of
-another length, Eq. 6) and ``segment_extract`` (`update` of Alg. 1B).
+another length, Eq. 6), ``segment_extract`` (`update` of Alg. 1B),
+residency flags (Eq. 3), ``patch_rope`` and the locality score of Eq. 3 / 8-10 (``LocalityScore``).
 
 Pinned by tests/test_oracle_pins.py (group law, identity, synthetic one-layer
 model, brute-force attention, closed forms, torch SDPA special case, complex
@@ -520,3 +521,63 @@ def patch_attention(k_cache, v_cache, q_bits, positions, group: int) -> np.ndarr
             w = np.exp(s - s.max())
             out[i, h] = (w @ vf[g, :vis]) / w.sum()
     return out
+
+
+# ----------------------------------------------------------------------------
+# 6. locality score of the cache management scheme   (Eq. 3, 8, 9, 10)
+# ----------------------------------------------------------------------------
+class LocalityScore:
+    """Bookkeeping behind Eq. (3): which function entries to keep on the GPU and which to offload.
+
+        l(f_k)            = (1 - l_curr) * (alpha * l_freq + beta * sum_j l_asso(f_j | f_k) + gamma * l_sema) + l_curr
+        l_freq(f_k)       = count(f_k) / max_j count(f_j)                                   (Eq. 8)
+        l_asso(f_j | f_k) = cooccur(f_k, f_j) / count(f_k)                                  (Eq. 9)
+        l_sema(f_k)       = PPL(f_k) / max_i PPL(f_i)                                       (Eq. 10)
+
+    Readings (R24): a trace is the sequence of functions one task invoked, in order; count = number of
+    invocations over all recorded traces; cooccur(f_k, f_j) = number of times f_j is the NEXT invocation after f_k
+    inside a trace ("invoked following f_k"), j != k -- so the sum over j is a conditional likelihood in [0, 1] as
+    the paper requires of every component; l_curr = 1 for the functions of the most recently recorded trace; PPL is
+    supplied by the caller (it needs the CodeLLM), 0 where unknown.
+    """
+
+    def __init__(self):
+        self.count = {}
+        self.follow = {}        # (k, j) -> times j directly followed k
+        self.ppl = {}
+        self.last = set()
+
+    def record(self, trace) -> None:
+        trace = [int(x) for x in trace]
+        for f in trace:
+            self.count[f] = self.count.get(f, 0) + 1
+        for a, b in zip(trace, trace[1:]):
+            if a != b:
+                self.follow[(a, b)] = self.follow.get((a, b), 0) + 1
+        self.last = set(trace)
+
+    def set_ppl(self, f: int, ppl: float) -> None:
+        self.ppl[int(f)] = float(ppl)
+
+    def forget(self, f: int) -> None:
+        f = int(f)
+        self.count.pop(f, None)
+        self.ppl.pop(f, None)
+        self.last.discard(f)
+        self.follow = {kj: c for kj, c in self.follow.items() if f not in kj}
+
+    def score(self, f: int, alpha: float, beta: float, gamma: float) -> float:
+        f = int(f)
+        if f in self.last:
+            return 1.0
+        cnt = self.count.get(f, 0)
+        max_cnt = max(self.count.values(), default=0)
+        freq = cnt / max_cnt if max_cnt else 0.0
+        asso = sum(c for (k, j), c in self.follow.items() if k == f) / cnt if cnt else 0.0
+        max_ppl = max(self.ppl.values(), default=0.0)
+        sema = self.ppl.get(f, 0.0) / max_ppl if max_ppl > 0 else 0.0
+        return alpha * freq + beta * asso + gamma * sema
+
+    def rank(self, ids, alpha: float, beta: float, gamma: float):
+        """ids sorted by ascending score (offload candidates first); ties by ascending id."""
+        return sorted((int(f) for f in ids), key=lambda f: (self.score(f, alpha, beta, gamma), f))

@@ -104,6 +104,13 @@ SYMBOLS = {
     "fcg_pool_info": (_I, [_P, C.POINTER(fcg_pool_info_t)]),
     "fcg_set_attn_policy": (_I, [_P, _I, _I]),
     "fcg_stats": (_I, [_P, C.POINTER(fcg_stats_t)]),
+    "fcg_scorer_create": (_I, [C.POINTER(_P)]),
+    "fcg_scorer_destroy": (_I, [_P]),
+    "fcg_scorer_record": (_I, [_P, _PI, _I]),
+    "fcg_scorer_set_ppl": (_I, [_P, _I, C.c_double]),
+    "fcg_scorer_forget": (_I, [_P, _I]),
+    "fcg_scorer_score": (_I, [_P, _I, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double)]),
+    "fcg_scorer_rank": (_I, [_P, _PI, _I, C.c_double, C.c_double, C.c_double, _PI, C.POINTER(C.c_double)]),
     "fcg_last_error": (C.c_char_p, []),
     "fcg_version": (C.c_char_p, []),
 }
@@ -324,6 +331,49 @@ def fcg_stats(handle) -> dict:
     st = fcg_stats_t()
     _check(load().fcg_stats(handle, C.byref(st)))
     return {f: getattr(st, f) for f, _ in fcg_stats_t._fields_}
+
+
+class FcgScorer:
+    """Locality score bookkeeping (Eq. 3, 8-10): host only, works without a GPU."""
+
+    def __init__(self):
+        h = _P()
+        _check(load().fcg_scorer_create(C.byref(h)))
+        self.handle = h.value
+
+    def close(self):
+        if getattr(self, "handle", None):
+            load().fcg_scorer_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def record(self, trace) -> None:
+        ids = np.ascontiguousarray(trace, dtype=np.int32)
+        _check(load().fcg_scorer_record(self.handle, ids.ctypes.data_as(_PI), int(ids.size)))
+
+    def set_ppl(self, fid, ppl) -> None:
+        _check(load().fcg_scorer_set_ppl(self.handle, int(fid), float(ppl)))
+
+    def forget(self, fid) -> None:
+        _check(load().fcg_scorer_forget(self.handle, int(fid)))
+
+    def score(self, fid, alpha, beta, gamma) -> float:
+        out = C.c_double()
+        _check(load().fcg_scorer_score(self.handle, int(fid), float(alpha), float(beta), float(gamma), C.byref(out)))
+        return out.value
+
+    def rank(self, ids, alpha, beta, gamma):
+        ids = np.ascontiguousarray(ids, dtype=np.int32)
+        out = np.empty_like(ids)
+        sc = np.empty(ids.size, np.float64)
+        _check(load().fcg_scorer_rank(self.handle, ids.ctypes.data_as(_PI), int(ids.size), float(alpha), float(beta),
+                                      float(gamma), out.ctypes.data_as(_PI), sc.ctypes.data_as(C.POINTER(C.c_double))))
+        return out.tolist(), sc.tolist()
 
 
 # ------------------------------------------------------------------------------------------------
