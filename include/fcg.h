@@ -178,6 +178,13 @@ fcg_status_t fcg_task_page_table(fcg_library_t *lib, int32_t task_id, const int3
 /* Host copy of the same table (no device access): writes min(n_pages, cap) entries to `out`. */
 fcg_status_t fcg_task_page_table_host(fcg_library_t *lib, int32_t task_id, int32_t *out, int32_t cap,
                                       int32_t *n_pages);
+/* Boundary-recompute plan (the related work of PAPER.md:47, 588): the positions worth
+ * recomputing after a stitch -- the first `width` tokens of every stitched entry that does not start at position 0,
+ * ascending and without duplicates.  Host only.  Writes min(count, cap) positions to `out` (may be NULL with cap 0)
+ * and the count to *n_out; the caller recomputes those tokens with the model and hands them to fcg_patch (re-patching
+ * a filled position overwrites it, R14).  Describes the stitch; later fcg_task_shift moves are not tracked. */
+fcg_status_t fcg_task_boundary_positions(fcg_library_t *lib, int32_t task_id, int32_t width, int32_t *out, int32_t cap,
+                                         int32_t *n_out);
 /* Returns the task's pages to the pool (pushed so that they are re-issued in ascending logical order). */
 fcg_status_t fcg_task_release(fcg_library_t *lib, int32_t task_id);
 

@@ -215,6 +215,7 @@ class Task:
     k: np.ndarray             # logical cache [L][Hkv][capacity][D] uint16
     v: np.ndarray
     deltas: list              # per entry, for inspection
+    spans: list = field(default_factory=list)   # (dst_offset, n_tokens) of every stitched entry, in plan order
 
 
 class OracleLibrary:
@@ -355,7 +356,8 @@ class OracleLibrary:
                     kc[:, :, dst] = rope_shift_bf16(seg.k[:, :, src], delta, self.inv_freq, self.rope_mode)
                 vc[:, :, dst] = seg.v[:, :, src]                           # V: bit copy
                 filled[dst] = True
-            self.tasks[plan.task_id] = Task(table, cap, T, filled, kc, vc, deltas)
+            self.tasks[plan.task_id] = Task(table, cap, T, filled, kc, vc, deltas,
+                                            [(e.dst_offset, e.n_tokens) for e in plan.entries])
 
     # -- S4 + S5/S6 ----------------------------------------------------------
     def check_patch(self, task_id: int, positions) -> None:
@@ -488,6 +490,22 @@ class OracleLibrary:
         else:
             k = rope_shift_bf16(t.k[:, :, src], delta, self.inv_freq, self.rope_mode)
         return self.segment_register(k, t.v[:, :, src], new_orig_start)
+
+    def task_boundary_positions(self, task_id: int, width: int) -> list:
+        """Positions worth recomputing after a stitch (the boundary-recompute idea of the
+        related work the paper positions itself against): the first `width` tokens of every
+        stitched entry that does not start at position 0 -- the tokens whose keys / values were computed without
+        seeing what now precedes them.  Ascending, without duplicates; the caller recomputes them with the model and
+        hands them to patch().  Entries moved later by task_shift are not tracked (the list describes the stitch)."""
+        if task_id not in self.tasks:
+            raise OracleError(FCG_ERR_BAD_TASK, f"unknown task {task_id}")
+        if width <= 0:
+            raise OracleError(FCG_ERR_INVALID_ARG, "width must be > 0")
+        out = set()
+        for (dst, n) in self.tasks[task_id].spans:
+            if dst > 0:
+                out.update(range(dst, dst + min(width, n)))
+        return sorted(out)
 
     def task_release(self, task_id: int) -> None:
         if task_id not in self.tasks:

@@ -98,6 +98,7 @@ SYMBOLS = {
     "fcg_task_page_table": (_I, [_P, _I, C.POINTER(_P), _PI, _PI]),
     "fcg_task_page_table_host": (_I, [_P, _I, _PI, _I, _PI]),
     "fcg_task_release": (_I, [_P, _I]),
+    "fcg_task_boundary_positions": (_I, [_P, _I, _I, _PI, _I, _PI]),
     "fcg_task_shift": (_I, [_P, _I, _I, _I, _I, _P]),
     "fcg_segment_extract": (_I, [_P, _I, _I, _I, _I, _P, _PI]),
     "fcg_task_read": (_I, [_P, _I, _I, _I, _I, _P, _P, _P]),
@@ -280,6 +281,14 @@ def fcg_task_page_table_host(handle, task_id) -> np.ndarray:
     _check(load().fcg_task_page_table_host(handle, int(task_id), None, 0, C.byref(n)))
     out = np.empty(n.value, np.int32)
     _check(load().fcg_task_page_table_host(handle, int(task_id), out.ctypes.data_as(_PI), n.value, C.byref(n)))
+    return out
+
+
+def fcg_task_boundary_positions(handle, task_id, width) -> np.ndarray:
+    n = C.c_int32()
+    _check(load().fcg_task_boundary_positions(handle, int(task_id), int(width), None, 0, C.byref(n)))
+    out = np.empty(n.value, np.int32)
+    _check(load().fcg_task_boundary_positions(handle, int(task_id), int(width), out.ctypes.data_as(_PI), n.value, C.byref(n)))
     return out
 
 
@@ -479,6 +488,9 @@ class FcgLibrary:
 
     def task_release(self, task_id):
         fcg_task_release(self.handle, task_id)
+
+    def task_boundary_positions(self, task_id, width) -> np.ndarray:
+        return fcg_task_boundary_positions(self.handle, task_id, width)
 
     def task_shift(self, task_id, src_begin, n_tokens, dst_begin, stream=None):
         fcg_task_shift(self.handle, task_id, src_begin, n_tokens, dst_begin, stream)

@@ -57,6 +57,7 @@ struct TaskRec {
   int32_t capacity = 0, n_tokens = 0;
   std::vector<uint8_t> filled;
   int32_t filled_prefix = 0;        // every x < filled_prefix is filled
+  std::vector<std::pair<int32_t, int32_t>> spans;   // (dst_offset, n_tokens) of the stitched entries, plan order
 };
 
 struct BlobSlot {
@@ -733,9 +734,11 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
     t.n_tokens = checked[i].T;
     t.pages.assign(pages + plan_page_base[i], pages + plan_page_base[i] + checked[i].n_pages);
     t.filled.assign(t.capacity, 0);
+    t.spans.clear();
     for (int e = 0; e < plans[i].n_entries; ++e) {
       const fcg_plan_entry_t &pe = plans[i].entries[e];
       std::fill(t.filled.begin() + pe.dst_offset, t.filled.begin() + pe.dst_offset + pe.n_tokens, (uint8_t)1);
+      t.spans.push_back({pe.dst_offset, pe.n_tokens});
     }
     t.filled_prefix = 0;
     while (t.filled_prefix < t.capacity && t.filled[t.filled_prefix]) t.filled_prefix++;
@@ -1170,6 +1173,22 @@ fcg_status_t fcg_task_page_table_host(fcg_library_t *lib, int32_t task_id, int32
   const TaskRec &t = lib->tasks[task_id];
   if (n_pages) *n_pages = (int32_t)t.pages.size();
   if (out && cap > 0) memcpy(out, t.pages.data(), sizeof(int32_t) * std::min<size_t>(cap, t.pages.size()));
+  return FCG_OK;
+}
+
+fcg_status_t fcg_task_boundary_positions(fcg_library_t *lib, int32_t task_id, int32_t width, int32_t *out, int32_t cap,
+                                         int32_t *n_out) {
+  if (!lib || !n_out) return fail(FCG_ERR_INVALID_ARG, "NULL argument");
+  if (task_id < 0 || task_id >= lib->cfg.max_tasks || !lib->tasks[task_id].live) return fail(FCG_ERR_BAD_TASK, "unknown task %d", task_id);
+  if (width <= 0) return fail(FCG_ERR_INVALID_ARG, "width must be > 0");
+  std::vector<int32_t> pos;
+  for (auto &sp : lib->tasks[task_id].spans)
+    if (sp.first > 0)
+      for (int32_t x = sp.first; x < sp.first + std::min(width, sp.second); ++x) pos.push_back(x);
+  std::sort(pos.begin(), pos.end());
+  pos.erase(std::unique(pos.begin(), pos.end()), pos.end());
+  *n_out = (int32_t)pos.size();
+  if (out && cap > 0) memcpy(out, pos.data(), sizeof(int32_t) * std::min<size_t>(cap, pos.size()));
   return FCG_OK;
 }
 

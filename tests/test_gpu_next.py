@@ -297,3 +297,25 @@ def test_patch_rope_matches_oracle(rope_mode, D):
         lib.patch_rope(0, 0, q.cuda(), k.cuda(), v.cuda(), pos[::-1].copy())
     assert e.value.status == B.FCG_ERR_INVALID_ARG
     lib.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4: boundary-recompute plan -- positions from the library, re-patched over the stitched cache
+# ------------------------------------------------------------------------------------------------
+def test_boundary_positions_and_repatch():
+    cfg = synth.GraftConfig("bound", 2, 4, 2, 128, 16, 1e4, 5, 40, 120, 3000, 1, 4, 4, 0)
+    wl, orc, lib, seg_ids = _pair(cfg, seed=6)
+    task = wl.tasks[0]
+    c_plans, o_plans = T.plans_of(wl, seg_ids)
+    orc.stitch(o_plans)
+    lib.stitch(c_plans)
+    for width in (1, 4, 1000):
+        assert lib.task_boundary_positions(0, width).tolist() == orc.task_boundary_positions(0, width)
+    pos = lib.task_boundary_positions(0, 4)
+    assert len(pos) == 4 * (len(task.entries) - 1)
+    # the caller's recomputed tokens overwrite the stitched ones; every query sees its whole prefix
+    out, ref = T.run_patch_both(orc, lib, cfg, task, 9, positions=pos)
+    T.assert_attn_close(out, ref, "re-patch of the boundary tokens")
+    T.compare_cache_bits(orc, lib, 0, pos)
+    _compare_task(orc, lib, 0, "after the boundary re-patch")
+    lib.close()

@@ -739,3 +739,19 @@ def test_patch_rope_is_rotation_to_absolute_positions_then_patch():
     lib0.task_release(0)
     lib0.stitch([O.Plan(0, [], [O.Hole(0, n)], n)])
     assert np.array_equal(a, lib0.patch(0, 0, q, k, v, np.arange(n)))
+
+
+def test_boundary_positions_by_hand():
+    """entries at 0 (n 10), 14 (n 7), 21 (n 2) and a hole [10, 14): width 3 -> the first 3 tokens of the entries that
+    do not start at 0, the short one contributing only its 2."""
+    lib = _small_lib()
+    s0, _, _ = _reg(lib, 10, 0)
+    s1, _, _ = _reg(lib, 7, 50)
+    lib.stitch([O.Plan(0, [O.PlanEntry(s0, 0, 10, 0), O.PlanEntry(s1, 0, 7, 14), O.PlanEntry(s0, 3, 2, 21)], [O.Hole(10, 4)], 30)])
+    assert lib.task_boundary_positions(0, 3) == [14, 15, 16, 21, 22]
+    assert lib.task_boundary_positions(0, 1) == [14, 21]
+    assert lib.task_boundary_positions(0, 100) == list(range(14, 23))
+    with pytest.raises(O.OracleError):
+        lib.task_boundary_positions(0, 0)
+    with pytest.raises(O.OracleError):
+        lib.task_boundary_positions(5, 2)
