@@ -108,9 +108,15 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
     def decode():
         lib.patch(t.task_id, 0, q, k, v, pos, out)
 
+    kr, vr = synth.segment_kv(cfg, 0, n_ext, seed + 200, dev)      # S1: a caller's K/V copied into the library
+
+    def register():
+        lib.segment_release(lib.segment_register(kr, vr, 0))
+
     res = {}
     per_tok = cfg.kv_bytes_per_token
     for name, fn, nbytes in (("decode_step", decode, cfg.n_layers * cap * cfg.n_kv_heads * cfg.head_dim * 4),
+                             ("segment_register", register, n_ext * per_tok * 2),
                              ("segment_extract", extract, n_ext * per_tok * 2),
                              ("task_shift", shift_pair, 2 * n_shift * per_tok * 2)):
         for _ in range(2):
@@ -161,6 +167,7 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
         res["two_tier"] = {"error": repr(e)}
     res["task_shift"]["note"] = f"two moves of {n_shift} tokens (-16, +16) per iteration"
     res["segment_extract"]["note"] = f"{n_ext} tokens un-rotated to orig_start 0"
+    res["segment_register"]["note"] = f"S1: {n_ext} tokens copied into the library (read + write)"
     res["decode_step"]["note"] = f"n = 1 at position {cap - 1}, R = {cfg.n_q_heads // cfg.n_kv_heads} rows per kv head"
     return res
 
