@@ -11,6 +11,15 @@ for _p in (ROOT, os.path.join(ROOT, "tests")):
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
+    # libfcg.so is a build artefact (git-ignored): on a fresh checkout build it once (nvcc cross-compiles without a GPU);
+    # if that is impossible the tests that need it fail with the binding's own "build it first" message
+    lib = os.path.join(ROOT, "paper_2606_13097_b200", "libfcg.so")
+    if not os.path.exists(lib):
+        try:
+            from paper_2606_13097_b200.build import build
+            build()
+        except Exception as e:                      # pragma: no cover
+            print(f"conftest: could not build libfcg.so: {e}", file=sys.stderr)
 
 
 def pytest_collection_modifyitems(config, items):
