@@ -433,3 +433,38 @@ def test_tcgen05_page_sizes_two_q_tiles_and_poisoned_pool(P, n, Hq, Hkv, ctx):
     torch.cuda.synchronize()
     T.assert_attn_close(out2, ref, f"tc P={P} n={n} 3 splits")
     lib.close()
+
+
+@pytest.mark.parametrize("tc_min_rows", [0, 2 ** 31 - 1])
+def test_growing_scores_force_the_rescale_path(tc_min_rows):
+    """Scores that grow steadily along the cache (keys scaled by position, queries aligned with them) push the running
+    row max up by far more than the lazy-rescale threshold (2^8) many times over: the O-rescale branch of every CTA
+    class (prefill-like 2 Q tiles, tile-parity streams, row streams / decode) and of the split-KV kernel must run."""
+    B = _binding()
+    L, Hq, Hkv, D, T_ = 1, 4, 2, 128, 700
+    cfg = synth.GraftConfig("grow", L, Hq, Hkv, D, 16, 1e4, 1, 8, 8, 0, 1, 1, 1, 0)
+    wl = synth.make_workload(cfg, 1)
+    wl.tasks[0].entries, wl.tasks[0].holes, wl.tasks[0].capacity = [], [(0, T_)], T_
+    orc, lib, _ = T.make_pair(cfg, wl, 1, only_segments=[0], n_pages=T_ // 16 + 4)
+    lib.set_attn_policy(tc_min_rows, 0)
+    orc.stitch([O.Plan(0, [], [O.Hole(0, T_)], T_)])
+    lib.stitch([{"task_id": 0, "entries": [], "holes": [(0, T_)], "capacity_tokens": T_}])
+    g = torch.Generator().manual_seed(3)
+    u = torch.rand(D, generator=g) + 0.5                                   # all-positive direction
+    u = u / u.norm()
+    ramp = torch.linspace(0.05, 1.0, T_)                                   # key length grows with the position
+    k = (u[None, None, None, :] * ramp[None, :, None, None] * 30.0).expand(L, T_, Hkv, D).to(torch.bfloat16).contiguous()
+    q = (u[None, None, None, :] * 25.0).expand(L, T_, Hq, D).to(torch.bfloat16).contiguous()   # s_x up to 25*30/sqrt(128) = 66
+    v = torch.randn(L, T_, Hkv, D, generator=g).to(torch.bfloat16)
+    pos = np.arange(T_, dtype=np.int32)
+    ref = orc.patch(0, 0, synth.to_bits(q), synth.to_bits(k), synth.to_bits(v), pos)
+    out = lib.patch(0, 0, q.cuda(), k.cuda(), v.cuda(), pos)
+    torch.cuda.synchronize()
+    T.assert_attn_close(out, ref, "prefill-like, growing scores")
+    for n in (1, 20, 100):                                                 # re-patch the tail: the other CTA classes
+        sl = slice(T_ - n, T_)
+        ref = orc.patch(0, 0, synth.to_bits(q[:, sl]), synth.to_bits(k[:, sl]), synth.to_bits(v[:, sl]), pos[sl])
+        out = lib.patch(0, 0, q[:, sl].contiguous().cuda(), k[:, sl].contiguous().cuda(), v[:, sl].contiguous().cuda(), pos[sl])
+        torch.cuda.synchronize()
+        T.assert_attn_close(out, ref, f"growing scores, last {n} tokens")
+    lib.close()
