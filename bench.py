@@ -294,7 +294,7 @@ def build_library(cfg, wl, seed, device_index, on_segment=None):
                              head_dim=cfg.head_dim, page_size=cfg.page_size, rope_base=cfg.rope_base,
                              max_segments=cfg.n_segments + 1, max_tasks=max(cfg.n_tasks, 1),
                              max_task_tokens=max(t.capacity for t in wl.tasks), n_pages=total_pages + 16,
-                             workspace_bytes=1 << 30, segment_tokens=seg_tokens, device=device_index,
+                             workspace_bytes=2 << 30, segment_tokens=seg_tokens, device=device_index,
                              host_tier_tokens=int(wl.seg_lens[wl.tasks[0].entries[0][0]]) + 16)
     dev = torch.device("cuda", device_index)
     for s in range(cfg.n_segments):
@@ -392,14 +392,18 @@ def run_cuda(args, cfg, wl, seed):
     # ---- e2e: same step through the C ABI with HOST buffers (H2D of q/k/v, D2H of out inside) ----
     single = len(ids) == 1
     e2e = None
-    if single:
+    if True:
         qh, kh, vh = [x.cpu().contiguous().pin_memory() for x in (q, k, v)]
         oh = torch.empty_like(qh).pin_memory()
 
         def step_host():
-            lib.task_release(ids[0])
+            for tid in ids:
+                lib.task_release(tid)
             lib.stitch(plans)
-            lib.patch_host(ids[0], 0, qh, kh, vh, pos, oh)
+            if single:
+                lib.patch_host(ids[0], 0, qh, kh, vh, pos, oh)
+            else:
+                lib.patch_batch_host(ids, npt, 0, qh, kh, vh, pos, oh)
             torch.cuda.synchronize(dev)          # the caller reads `out` on the host every step
 
         for _ in range(min(args.warmup, 3)):

@@ -170,6 +170,11 @@ fcg_status_t fcg_patch_batch(fcg_library_t *lib, const int32_t *task_ids, const 
                              int32_t n_tasks, int32_t layer_begin, int32_t n_layers, const void *q,
                              const void *k, const void *v, const int32_t *positions, void *out, void *stream);
 
+/* fcg_patch_batch with q, k, v, out in HOST memory: staging, copy streams and layer-group pipelining as fcg_patch_host. */
+fcg_status_t fcg_patch_batch_host(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task,
+                                  int32_t n_tasks, int32_t layer_begin, int32_t n_layers, const void *q,
+                                  const void *k, const void *v, const int32_t *positions, void *out, void *stream);
+
 /* Device pointer to the task's page table (int32[n_pages], logical page -> physical page id), its page
  * count and current token count T (max end of stitched/declared/patched ranges).  Token x lives at
  * (table[x / page_size], x % page_size). */

@@ -95,6 +95,7 @@ SYMBOLS = {
     "fcg_patch_host": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
     "fcg_patch_rope": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
     "fcg_patch_batch": (_I, [_P, _PI, _PI, _I, _I, _I, _P, _P, _P, _PI, _P, _P]),
+    "fcg_patch_batch_host": (_I, [_P, _PI, _PI, _I, _I, _I, _P, _P, _P, _PI, _P, _P]),
     "fcg_task_page_table": (_I, [_P, _I, C.POINTER(_P), _PI, _PI]),
     "fcg_task_page_table_host": (_I, [_P, _I, _PI, _I, _PI]),
     "fcg_task_release": (_I, [_P, _I]),
@@ -267,6 +268,13 @@ def fcg_patch_batch(handle, task_ids, n_per_task, layer_begin, n_layers, q, k, v
     _check(load().fcg_patch_batch(handle, ids.ctypes.data_as(_PI), npt.ctypes.data_as(_PI), int(ids.size),
                                   int(layer_begin), int(n_layers), _ptr(q), _ptr(k), _ptr(v),
                                   pos.ctypes.data_as(_PI), _ptr(out), _stream(stream)))
+
+
+def fcg_patch_batch_host(handle, task_ids, n_per_task, layer_begin, n_layers, q, k, v, positions, out, stream=None) -> None:
+    ids, npt, pos = _i32(task_ids), _i32(n_per_task), _i32(positions)
+    _check(load().fcg_patch_batch_host(handle, ids.ctypes.data_as(_PI), npt.ctypes.data_as(_PI), int(ids.size),
+                                       int(layer_begin), int(n_layers), _ptr(q), _ptr(k), _ptr(v),
+                                       pos.ctypes.data_as(_PI), _ptr(out), _stream(stream)))
 
 
 def fcg_task_page_table(handle, task_id):
@@ -472,6 +480,11 @@ class FcgLibrary:
         if out is None:
             out = torch.empty_like(q)
         fcg_patch_batch(self.handle, task_ids, n_per_task, layer_begin, q.shape[0], q, k, v, positions, out, stream)
+        return out
+
+    def patch_batch_host(self, task_ids, n_per_task, layer_begin, q, k, v, positions, out, stream=None) -> torch.Tensor:
+        assert not q.is_cuda and q.is_contiguous() and k.is_contiguous() and v.is_contiguous() and out.is_contiguous()
+        fcg_patch_batch_host(self.handle, task_ids, n_per_task, layer_begin, q.shape[0], q, k, v, positions, out, stream)
         return out
 
     def task_page_table(self, task_id):

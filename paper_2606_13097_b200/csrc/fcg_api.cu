@@ -1091,9 +1091,13 @@ fcg_status_t fcg_patch_rope(fcg_library_t *lib, int32_t task_id, int32_t layer_b
   return st;
 }
 
-fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers, const void *q,
-                            const void *k, const void *v, const int32_t *positions, int32_t n, void *out, void *stream_) {
-  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+}  // extern "C"
+
+namespace {
+// host-buffer patch of one task or of a batch: n = total patch tokens over the tasks
+fcg_status_t patch_host_common(fcg_library *lib, const int32_t *task_ids, const int32_t *n_per_task, int32_t n_tasks,
+                               int32_t layer_begin, int32_t n_layers, const void *q, const void *k, const void *v,
+                               const int32_t *positions, int32_t n, void *out, void *stream_) {
   if (!q || !k || !v || !out || n <= 0 || n_layers <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty argument");
   const fcg_config_t &c = lib->cfg;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
@@ -1131,8 +1135,8 @@ fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_b
       st = fail(FCG_ERR_CUDA, "cudaStreamWaitEvent: %s", cudaGetErrorString(e));
       break;
     }
-    PatchCall pc{&task_id, &n, 1, layer_begin + lb, nl, dq + lb * q_layer, dk + lb * kv_layer, dv + lb * kv_layer, positions,
-                 dout + lb * q_layer, stream};
+    PatchCall pc{task_ids, n_per_task, n_tasks, layer_begin + lb, nl, dq + lb * q_layer, dk + lb * kv_layer, dv + lb * kv_layer,
+                 positions, dout + lb * q_layer, stream};
     st = patch_common(lib, pc);
     if (st != FCG_OK) break;
     if (groups > 1) {
@@ -1153,6 +1157,29 @@ fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_b
   }
   FCG_CUDA(cudaEventRecord(lib->last_patch_ev, stream));   // the staged output is in use until these copies are done
   return FCG_OK;
+}
+}  // namespace
+
+extern "C" {
+
+fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers, const void *q,
+                            const void *k, const void *v, const int32_t *positions, int32_t n, void *out, void *stream) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  return patch_host_common(lib, &task_id, &n, 1, layer_begin, n_layers, q, k, v, positions, n, out, stream);
+}
+
+fcg_status_t fcg_patch_batch_host(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task, int32_t n_tasks,
+                                  int32_t layer_begin, int32_t n_layers, const void *q, const void *k, const void *v,
+                                  const int32_t *positions, void *out, void *stream) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  if (!task_ids || !n_per_task || n_tasks <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty task list");
+  int64_t n = 0;
+  for (int32_t t = 0; t < n_tasks; ++t) {
+    if (n_per_task[t] <= 0) return fail(FCG_ERR_INVALID_ARG, "task %d: n must be > 0", task_ids[t]);
+    n += n_per_task[t];
+  }
+  if (n > (1 << 20)) return fail(FCG_ERR_INVALID_ARG, "too many patch tokens in one call");
+  return patch_host_common(lib, task_ids, n_per_task, n_tasks, layer_begin, n_layers, q, k, v, positions, (int32_t)n, out, stream);
 }
 
 // ------------------------------------------------------------------------------- task utilities
