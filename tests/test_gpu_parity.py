@@ -242,6 +242,13 @@ def test_patch_host_and_batch_variants_match_device_call():
     od = lib.patch(0, 0, qs[0].cuda(), ks[0].cuda(), vs[0].cuda(), t0.positions)
     torch.cuda.synchronize()
     assert torch.equal(oh, od.cpu())
+    # batched host-buffer call == batched device call
+    qh, kh, vh = [x.cpu().contiguous().pin_memory() for x in (q, k, v)]
+    oh = torch.empty_like(qh).pin_memory()
+    lib.patch_batch_host([t.task_id for t in wl.tasks], [len(t.positions) for t in wl.tasks], 0, qh, kh, vh,
+                         np.concatenate([t.positions for t in wl.tasks]), oh)
+    torch.cuda.synchronize()
+    assert torch.equal(oh, out.cpu())
     lib.close()
 
 
