@@ -70,7 +70,8 @@ def attn_rows(cfg, wl) -> int:
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r01_final.md); None where no capture of that workload is committed.
-NCU_TRAFFIC = {"C2": {"stitch": 4.178e9, "attn": 2.183e9}, "C5": {"attn": 7.011e9}}
+NCU_TRAFFIC = {"C2": {"stitch": 4.178e9, "attn": 2.183e9}, "C3": {"stitch": 2.061e9, "attn": 1.137e9},
+               "C4": {"stitch": 30.15e9, "attn": 16.14e9}, "C5": {"attn": 6.993e9}}
 
 
 def tensor_peak():
