@@ -115,6 +115,33 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
         lib.segment_release(lib.segment_register(kr, vr, 0))
 
     res = {}
+    # the call pattern of a model that patches layer by layer: L calls of one layer each (task 0's own patch tokens)
+    try:
+        qp, kp, vp = synth.patch_qkv(cfg, t.task_id, len(t.positions), seed, dev)
+        op = torch.empty_like(qp)
+        views = [(qp[l:l + 1], kp[l:l + 1], vp[l:l + 1], op[l:l + 1]) for l in range(cfg.n_layers)]
+
+        def per_layer():
+            for l, (a_, b_, c_, d_) in enumerate(views):
+                lib.patch(t.task_id, l, a_, b_, c_, t.positions, d_)
+
+        for _ in range(2):
+            per_layer()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        a.record()
+        for _ in range(iters):
+            per_layer()
+        b.record()
+        t1 = time.perf_counter()
+        torch.cuda.synchronize(dev)
+        res["patch_one_call_per_layer"] = {"ms": a.elapsed_time(b) / iters, "host_enqueue_ms": (t1 - t0) * 1e3 / iters,
+                                           "calls": cfg.n_layers, "splits": lib.stats()["last_attn_splits"],
+                                           "note": "same patch as the timed step, issued as one fcg_patch per layer"}
+        del qp, kp, vp, op, views
+    except Exception as e:
+        res["patch_one_call_per_layer"] = {"error": repr(e)}
     per_tok = cfg.kv_bytes_per_token
     for name, fn, nbytes in (("decode_step", decode, cfg.n_layers * cap * cfg.n_kv_heads * cfg.head_dim * 4),
                              ("segment_register", register, n_ext * per_tok * 2),
