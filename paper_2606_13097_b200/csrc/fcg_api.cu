@@ -65,6 +65,7 @@ struct BlobSlot {
   unsigned char *dev = nullptr;     // inside the workspace
   cudaEvent_t ev = nullptr;
   bool in_flight = false;
+  uint64_t gen = 0;                 // bumped at every acquisition (validates the cached patch blob)
 };
 
 struct FreeRange {
@@ -94,6 +95,11 @@ struct fcg_library {
   static constexpr int HOST_GROUPS = 4;          // layer groups of a host call: copy in / attend / copy out pipelined
   cudaEvent_t last_patch_ev = nullptr, h2d_ev[HOST_GROUPS] = {}, attn_ev[HOST_GROUPS] = {}, d2h_ev = nullptr;
   bool have_last_patch = false;
+  // the plan blob of the last patch call: a call that produces the same bytes (the same patch issued for the next layer)
+  // reuses the copy that is already on the device instead of uploading it again
+  std::vector<unsigned char> patch_blob_copy;
+  int patch_blob_slot = -1;
+  uint64_t patch_blob_gen = 0;
   int next_slot = 0;
   fcg_stats_t stats;
   int n_segments_live = 0, n_tasks_live = 0;
@@ -178,6 +184,7 @@ fcg_status_t acquire_slot(fcg_library *lib, BlobSlot **out) {
     FCG_CUDA(cudaEventSynchronize(s.ev));
     s.in_flight = false;
   }
+  s.gen++;
   *out = &s;
   return FCG_OK;
 }
@@ -901,7 +908,21 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
     return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for %d-way split partials (%llu bytes)", max_splits,
                 (unsigned long long)(part_o_bytes + part_ml_bytes));
 
-  FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, bw.used, cudaMemcpyHostToDevice, pc.stream));
+  {
+    const int cached = lib->patch_blob_slot;
+    if (cached >= 0 && lib->slots[cached].gen == lib->patch_blob_gen && lib->patch_blob_copy.size() == bw.used &&
+        memcmp(lib->patch_blob_copy.data(), slot->host, bw.used) == 0) {
+      // same bytes as the previous patch call and its device copy is intact: hand the fresh slot back, use that one
+      lib->next_slot = (lib->next_slot + BLOB_SLOTS - 1) % BLOB_SLOTS;
+      slot->gen--;
+      slot = &lib->slots[cached];
+    } else {
+      FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, bw.used, cudaMemcpyHostToDevice, pc.stream));
+      lib->patch_blob_copy.assign(slot->host, slot->host + bw.used);
+      lib->patch_blob_slot = (int)(slot - lib->slots);
+      lib->patch_blob_gen = slot->gen;
+    }
+  }
 
   fcg::ScatterParams sp;
   sp.k_new = static_cast<const uint16_t *>(pc.k);
