@@ -340,6 +340,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) attn_split_kernel(const AttnParam
 // one warp per (layer, token, q head) row: log-sum-exp merge of the splits
 template <int D>
 __global__ void __launch_bounds__(256) attn_combine_kernel(const AttnParams p) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");   // pre-launched behind the attention kernel (no-op otherwise)
   constexpr int CPL = D / 32;
   const size_t n_rows = (size_t)p.n_layers * p.n_total * p.n_q_heads;
   const size_t rowi = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -411,13 +412,18 @@ cudaError_t launch_attn_split(const AttnParams &p, int head_dim, int rows_per_ct
 cudaError_t launch_attn_combine(const AttnParams &p, int head_dim, cudaStream_t stream) {
   const size_t n_rows = (size_t)p.n_layers * p.n_total * p.n_q_heads;
   const unsigned blocks = (unsigned)((n_rows + 7) / 8);
-  if (head_dim == 128)
-    attn_combine_kernel<128><<<blocks, 256, 0, stream>>>(p);
-  else if (head_dim == 64)
-    attn_combine_kernel<64><<<blocks, 256, 0, stream>>>(p);
-  else
-    return cudaErrorInvalidValue;
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(blocks, 1, 1);
+  cfg.blockDim = dim3(256, 1, 1);
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  if (head_dim == 128) return cudaLaunchKernelEx(&cfg, attn_combine_kernel<128>, p);
+  if (head_dim == 64) return cudaLaunchKernelEx(&cfg, attn_combine_kernel<64>, p);
+  return cudaErrorInvalidValue;
 }
 
 }  // namespace fcg

@@ -338,6 +338,11 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
   // shuffle broadcast: the value is warp-uniform, and saying so keeps every TMEM address of the MMA warp in uniform
   // registers (the MMA warp was issue-bound: ~255 SASS instructions per KV tile, a third of them R2UR / UMOV)
   const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot_ptr, 0);
+  // programmatic dependent launch: everything above (barrier init, TMEM allocation, tensor-map prefetch) may overlap the
+  // scatter kernel that precedes this launch; the cache rows it writes are only read below.  A no-op when the
+  // launch does not carry the attribute.  The combine kernel that may follow is allowed to pre-launch right away.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   if (warp == C::KLOAD_WARP || warp == C::VLOAD_WARP) {
     // ======================================= loaders =======================================
@@ -780,9 +785,17 @@ cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv,
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  dim3 grid((unsigned)(p.max_splits * p.max_row_groups), (unsigned)p.n_kv_heads, (unsigned)(p.n_layers * p.n_tasks));
-  attn_tc_kernel<NQ, PS_><<<grid, C::NTHREADS, C::SMEM_BYTES, stream>>>(p, tk, tv);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(p.max_splits * p.max_row_groups), (unsigned)p.n_kv_heads, (unsigned)(p.n_layers * p.n_tasks));
+  cfg.blockDim = dim3(C::NTHREADS, 1, 1);
+  cfg.dynamicSmemBytes = C::SMEM_BYTES;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, attn_tc_kernel<NQ, PS_>, p, tk, tv);
 }
 
 }  // namespace

@@ -29,6 +29,8 @@ __global__ void __launch_bounds__(256) register_copy_kernel(const RegisterParams
 }
 
 __global__ void __launch_bounds__(256) scatter_kernel(const ScatterParams p) {
+  // the attention kernel that follows may start its prologue now (it waits for this grid before reading the cache)
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const int vpr = p.head_dim >> 3;
   const size_t total = (size_t)p.n_layers * p.n_total * p.n_kv_heads * vpr;
   for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
