@@ -12,7 +12,7 @@ at the very end of each step that stores bf16.  K/V/q are carried around as
 equality of those arrays.
 
 What the paper fixes and what it leaves open (``PAPER.md`` = /root/reference/PAPER.md,
-not needed at run time; DESIGN.md "Readings" lists every choice R1..R14):
+not needed at run time; DESIGN.md "Readings" lists every choice R1..R26):
 
 * segment library  = the KV half of the two-tier code cache H=(I,C), Eq. (2),
   PAPER.md:66-79: per function a K/V state that can be re-injected "without
@@ -29,12 +29,15 @@ not needed at run time; DESIGN.md "Readings" lists every choice R1..R14):
 NEXT rows of SURVEY.md 8(f) stated here as well: interleaved RoPE pairs
 (rope_mode 2), ``task_shift`` (re-graft of the kept suffix after a patch of
 another length, Eq. 6), ``segment_extract`` (`update` of Alg. 1B),
-residency flags (Eq. 3), ``patch_rope`` and the locality score of Eq. 3 / 8-10 (``LocalityScore``).
+residency flags (Eq. 3), ``patch_rope``, the locality score of Eq. 3 / 8-10 (``LocalityScore``), fp8 (e4m3)
+segment storage (``segment_register_fp8``, R26) and appends beyond the reserved capacity (``check_patch``, R25).
 
 Pinned by tests/test_oracle_pins.py (group law, identity, synthetic one-layer
 model, brute-force attention, closed forms, torch SDPA special case, complex
 multiplication for both pair layouts, a hand-computed paging example for
-task_shift, extract/stitch round trips ...).  No function here is "parity unpinned".
+task_shift, extract/stitch round trips ...) and tests/test_oracle_pins_r2.py (hand-computed
+page tables of a growing task; all 256 e4m3 codes against torch's float8 type, nearest-code
+brute force, a hand-worked quantised row).  No function here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -145,6 +148,71 @@ def rope_shift_bf16(k_bits: np.ndarray, delta, inv_freq: np.ndarray, rope_mode: 
 
 
 # ----------------------------------------------------------------------------
+# 2b. fp8 (e4m3) segment storage                     (DESIGN R26)
+# ----------------------------------------------------------------------------
+# OCP 8-bit float E4M3 ("e4m3fn"): 1 sign, 4 exponent bits (bias 7), 3 mantissa bits; no infinities; the only NaN
+# is S.1111.111; largest finite value 1.75 * 2^8 = 448; subnormals m/8 * 2^-6.  A stored row (the D elements of one
+# (layer, kv head, token)) shares one power-of-two scale 2^e (an E8M0 exponent, as in the OCP MX formats), so that
+# de-quantisation code * 2^e is exact and the shifted key is still ONE rounding away from the exact rotation.
+E4M3_MAX = 448.0
+FMT_BF16, FMT_FP8_E4M3 = 0, 1
+
+
+def e4m3_to_f64(codes) -> np.ndarray:
+    """e4m3 codes (uint8) -> float64, exact."""
+    c = np.ascontiguousarray(codes, dtype=np.uint8).astype(np.int64)
+    sign = np.where(c & 0x80, -1.0, 1.0)
+    e, m = (c >> 3) & 0xF, (c & 7).astype(np.float64)
+    val = np.where(e == 0, np.ldexp(m / 8.0, -6), np.ldexp(1.0 + m / 8.0, e - 7))
+    return np.where((e == 15) & (m == 7), np.nan, sign * val)
+
+
+def f64_to_e4m3(x) -> np.ndarray:
+    """float64 -> e4m3 code, round-to-nearest-even on the e4m3 grid, finite overflow saturates to +-448
+    ("satfinite"); NaN and +-inf have no e4m3 value and become the NaN code 0x7F."""
+    x = np.asarray(x, dtype=np.float64)
+    a = np.abs(x)
+    finite = np.isfinite(x)
+    a = np.where(finite, a, 0.0)
+    _, ex = np.frexp(a)                                   # a = m * 2^ex, m in [0.5, 1)
+    E = np.maximum(ex - 1, -6)                            # exponent of the binade; subnormals share 2^-6's quantum
+    q = np.ldexp(1.0, E - 3)                              # grid spacing: 3 mantissa bits
+    r = np.minimum(np.rint(a / q) * q, E4M3_MAX)          # a / q is exact; rint = half to even; then saturate
+    _, rex = np.frexp(r)
+    rE = rex - 1
+    normal = r >= 2.0 ** -6
+    e_bits = np.where(normal, rE + 7, 0).astype(np.int64)
+    m_bits = np.where(normal, np.rint((np.ldexp(r, -rE) - 1.0) * 8.0), np.rint(np.ldexp(r, 9))).astype(np.int64)
+    code = (e_bits << 3) | m_bits
+    code = np.where(np.signbit(x), code | 0x80, code)
+    return np.where(finite, code, 0x7F).astype(np.uint8)
+
+
+def fp8_row_exponent(x) -> np.ndarray:
+    """Per-row scale exponent e for rows x[..., D] (fp64): the smallest integer with amax <= 448 * 2^e, clamped to
+    the E8M0 range [-127, 127]; amax is taken over the finite elements; an all-zero row gets e = 0.  Integer
+    arithmetic on the binary exponent (448 = 0.875 * 2^9), no logarithm."""
+    x = np.asarray(x, dtype=np.float64)
+    amax = np.max(np.where(np.isfinite(x), np.abs(x), 0.0), axis=-1)
+    m, ex = np.frexp(amax)
+    e = np.where(m <= 0.875, ex - 9, ex - 8)
+    e = np.where(amax == 0.0, 0, e)
+    return np.clip(e, -127, 127).astype(np.int32)
+
+
+def fp8_quantize_rows(bits):
+    """bf16 rows [..., D] -> (e4m3 codes uint8 [..., D], scale exponents int32 [...]): code = e4m3(x * 2^-e)."""
+    x = bf16_to_f64(bits)
+    e = fp8_row_exponent(x)
+    return f64_to_e4m3(np.ldexp(x, -e[..., None])), e
+
+
+def fp8_dequantize_rows(codes, exps) -> np.ndarray:
+    """(codes [..., D], exponents [...]) -> float64 [..., D] = value(code) * 2^e, exact."""
+    return np.ldexp(e4m3_to_f64(codes), np.asarray(exps, dtype=np.int32)[..., None])
+
+
+# ----------------------------------------------------------------------------
 # 3. page pool                                         (SURVEY §8(c).3, DESIGN R9)
 # ----------------------------------------------------------------------------
 class PagePool:
@@ -182,6 +250,9 @@ class Segment:
     n_tokens: int
     orig_start: int          # position at which token 0's key was RoPE-encoded
     resident: bool = True    # False: offloaded to the host tier (Eq. 3); the bits are the same wherever they live
+    fmt: int = 0             # FMT_BF16: k, v hold bf16 bits; FMT_FP8_E4M3: k, v hold e4m3 codes (uint8) and
+    k_exp: np.ndarray = None  # k_exp, v_exp [L][Hkv][n] the per-row power-of-two scale exponents (R26)
+    v_exp: np.ndarray = None
 
 
 @dataclass
@@ -252,6 +323,16 @@ class OracleLibrary:
         if sid >= self.max_segments:
             raise OracleError(FCG_ERR_OUT_OF_ARENA, "segment table full")
         self.segments[sid] = Segment(k, v, k.shape[2], int(orig_start))
+        return sid
+
+    def segment_register_fp8(self, k_bits, v_bits, orig_start: int) -> int:
+        """S1 with fp8 storage (DESIGN R26): the bf16 K/V handed in are quantised row by row to
+        e4m3 codes with a power-of-two row scale; the library keeps codes + exponents (half the bytes of bf16)."""
+        sid = self.segment_register(k_bits, v_bits, orig_start)      # shape checks and id rule as for bf16
+        sg = self.segments[sid]
+        sg.k, sg.k_exp = fp8_quantize_rows(sg.k)
+        sg.v, sg.v_exp = fp8_quantize_rows(sg.v)
+        sg.fmt = FMT_FP8_E4M3
         return sid
 
     def segment_release(self, seg_id: int) -> None:
@@ -350,6 +431,16 @@ class OracleLibrary:
                 seg = self.segments[e.seg_id]
                 src = slice(e.src_begin, e.src_begin + e.n_tokens)
                 dst = slice(e.dst_offset, e.dst_offset + e.n_tokens)
+                if seg.fmt == FMT_FP8_E4M3:
+                    # R26: de-quantise (exact), rotate in fp64, ONE rounding to bf16; V: de-quantise, round to bf16
+                    # (exact whenever code * 2^e is a bf16 value, i.e. everywhere but the deepest subnormals)
+                    kf = fp8_dequantize_rows(seg.k[:, :, src], seg.k_exp[:, :, src])
+                    if self.rope_mode != 0:
+                        kf = rope_rotate_f64(kf, delta, self.inv_freq, self.rope_mode)
+                    kc[:, :, dst] = f64_to_bf16(kf)
+                    vc[:, :, dst] = f64_to_bf16(fp8_dequantize_rows(seg.v[:, :, src], seg.v_exp[:, :, src]))
+                    filled[dst] = True
+                    continue
                 if self.rope_mode == 0:
                     kc[:, :, dst] = seg.k[:, :, src]                       # pure gather
                 else:
@@ -360,7 +451,15 @@ class OracleLibrary:
                                             [(e.dst_offset, e.n_tokens) for e in plan.entries])
 
     # -- S4 + S5/S6 ----------------------------------------------------------
-    def check_patch(self, task_id: int, positions) -> None:
+    def check_patch(self, task_id: int, positions) -> int:
+        """Validates a patch; changes no state.  Returns the number of pages the patch has to add.
+
+        SURVEY 8(c).5 / DESIGN R25: positions beyond the task's current capacity APPEND -- the task grows to
+        capacity' = positions[-1] + 1 (never beyond max_task_tokens: RANGE) and takes the logical pages
+        ceil(capacity / P) .. ceil(capacity' / P) - 1 from the pool on demand (OUT_OF_PAGES if it cannot supply
+        them).  Positions between the old and the new capacity are unfilled until somebody writes them, so the
+        rule "every x <= positions[-1] is filled by earlier work or by this call" (R6) covers growth as well.
+        """
         if task_id not in self.tasks:
             raise OracleError(FCG_ERR_BAD_TASK, f"unknown task {task_id}")
         t = self.tasks[task_id]
@@ -369,12 +468,30 @@ class OracleLibrary:
             raise OracleError(FCG_ERR_INVALID_ARG, "positions must be a non-empty 1-d array")
         if np.any(np.diff(pos) <= 0):
             raise OracleError(FCG_ERR_INVALID_ARG, "positions must be strictly increasing")
-        if pos[0] < 0 or pos[-1] >= t.capacity:
-            raise OracleError(FCG_ERR_RANGE, "position outside task capacity")
-        f = t.filled.copy()
+        if pos[0] < 0 or pos[-1] >= self.max_task_tokens:
+            raise OracleError(FCG_ERR_RANGE, "position outside [0, max_task_tokens)")
+        cap = max(t.capacity, int(pos[-1]) + 1)
+        f = np.zeros(cap, bool)
+        f[: t.capacity] = t.filled
         f[pos] = True
         if not np.all(f[: pos[-1] + 1]):
             raise OracleError(FCG_ERR_UNFILLED, "a patch query would attend over an unfilled position")
+        need = -(-cap // self.P) - len(t.page_table)
+        if need > self.pool.available():
+            raise OracleError(FCG_ERR_OUT_OF_PAGES, f"need {need} pages to grow, {self.pool.available()} free")
+        return max(need, 0)
+
+    def _grow(self, task_id: int, capacity: int, n_new_pages: int) -> None:
+        """Append pages (ascending logical order, from the LIFO pool) and extend the logical cache (R25)."""
+        t = self.tasks[task_id]
+        t.page_table.extend(self.pool.allocate(n_new_pages))
+        if capacity > t.capacity:
+            extra = capacity - t.capacity
+            pad = np.zeros((self.L, self.Hkv, extra, self.D), np.uint16)
+            t.k = np.concatenate([t.k, pad], axis=2)
+            t.v = np.concatenate([t.v, pad.copy()], axis=2)
+            t.filled = np.concatenate([t.filled, np.zeros(extra, bool)])
+            t.capacity = capacity
 
     def patch_rope(self, task_id: int, layer_begin: int, q_bits, k_bits, v_bits, positions) -> np.ndarray:
         """patch() for callers that hold the projections BEFORE position encoding (DESIGN R13
@@ -399,9 +516,9 @@ class OracleLibrary:
         already position-encoded by the caller, DESIGN R13).  Returns the
         attention output as float64 [nl][n][Hq][D], NOT rounded.
         Query i at position p_i sees cache positions x <= p_i (DESIGN R12).
+        Positions at or beyond the current capacity append: the task grows page by page (check_patch, R25).
         """
-        self.check_patch(task_id, positions)
-        t = self.tasks[task_id]
+        n_new_pages = self.check_patch(task_id, positions)
         pos = np.asarray(positions, dtype=np.int64)
         q_bits = np.asarray(q_bits, np.uint16)
         k_bits = np.asarray(k_bits, np.uint16)
@@ -411,6 +528,8 @@ class OracleLibrary:
                 or q_bits.shape != (nl, n, self.Hq, self.D) or k_bits.shape != (nl, n, self.Hkv, self.D) \
                 or v_bits.shape != k_bits.shape:
             raise OracleError(FCG_ERR_INVALID_ARG, "patch tensor shapes / layer range")
+        self._grow(task_id, max(self.tasks[task_id].capacity, int(pos[-1]) + 1), n_new_pages)   # R25: append on demand
+        t = self.tasks[task_id]
         out = np.empty((nl, n, self.Hq, self.D), np.float64)
         for li in range(nl):
             layer = layer_begin + li
@@ -436,13 +555,15 @@ class OracleLibrary:
         page touched by the destination range gets a fresh physical page from the pool (ascending
         logical order); slots of those pages outside the destination range keep their old contents;
         the old physical pages go back to the pool by the rule of task_release.  delta == 0 is a no-op.
+        The source must lie inside the capacity; the destination may reach beyond it (up to max_task_tokens): the
+        task then grows as for an appending patch (R25).
         """
         if task_id not in self.tasks:
             raise OracleError(FCG_ERR_BAD_TASK, f"unknown task {task_id}")
         t = self.tasks[task_id]
         if n_tokens <= 0 or src_begin < 0 or dst_begin < 0 or src_begin + n_tokens > t.capacity \
-                or dst_begin + n_tokens > t.capacity:
-            raise OracleError(FCG_ERR_RANGE, "shift range outside task capacity")
+                or dst_begin + n_tokens > self.max_task_tokens:
+            raise OracleError(FCG_ERR_RANGE, "shift source outside the capacity / destination outside max_task_tokens")
         src = slice(src_begin, src_begin + n_tokens)
         dst = slice(dst_begin, dst_begin + n_tokens)
         if not np.all(t.filled[src]):
@@ -450,10 +571,16 @@ class OracleLibrary:
         delta = dst_begin - src_begin
         if delta == 0:
             return
+        # R25: a destination beyond the capacity appends.  Every logical page that receives a new physical page --
+        # the gap pages between the end of the table and the destination, then the destination's pages -- is served
+        # in ascending logical order; destination pages that already existed give their old page back.
+        n_old = len(t.page_table)
         lp0, lp1 = dst_begin // self.P, (dst_begin + n_tokens - 1) // self.P
-        new_pages = self.pool.allocate(lp1 - lp0 + 1)           # raises OUT_OF_PAGES before any change
+        first_new = min(lp0, n_old)
+        new_pages = self.pool.allocate(lp1 - first_new + 1)     # raises OUT_OF_PAGES before any change
         k_src = t.k[:, :, src].copy()
         v_src = t.v[:, :, src].copy()
+        self._grow(task_id, max(t.capacity, dst_begin + n_tokens), 0)
         if self.rope_mode == ROPE_NONE:
             t.k[:, :, dst] = k_src
         else:
@@ -461,8 +588,8 @@ class OracleLibrary:
         t.v[:, :, dst] = v_src
         t.filled[src] = False
         t.filled[dst] = True
-        old_pages = t.page_table[lp0:lp1 + 1]
-        t.page_table[lp0:lp1 + 1] = new_pages
+        old_pages = t.page_table[lp0:lp1 + 1]                   # destination pages that existed before
+        t.page_table[first_new:lp1 + 1] = new_pages
         self.pool.release(old_pages)
         t.n_tokens = max(t.n_tokens, dst_begin + n_tokens)
 

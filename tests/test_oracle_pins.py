@@ -450,8 +450,10 @@ def test_patch_scatter_fill_rules_and_sequencing():
     with pytest.raises(O.OracleError) as e:
         lib.patch(0, 0, q, k, v, [20, 21, 22])
     assert e.value.status == O.FCG_ERR_UNFILLED and np.array_equal(before, lib.tasks[0].k)
+    # positions beyond the capacity (23) append (R25, pinned in test_oracle_pins_r2.py) -- here the hole at 20
+    # is still unfilled, so the call fails as UNFILLED; RANGE is left for negative positions
     for bad, status in (([9, 8, 10], O.FCG_ERR_INVALID_ARG), ([8, 8, 9], O.FCG_ERR_INVALID_ARG),
-                        ([21, 22, 23], O.FCG_ERR_RANGE), ([-1, 0, 1], O.FCG_ERR_RANGE)):
+                        ([21, 22, 23], O.FCG_ERR_UNFILLED), ([-1, 0, 1], O.FCG_ERR_RANGE)):
         with pytest.raises(O.OracleError) as e:
             lib.patch(0, 0, q, k, v, bad)
         assert e.value.status == status
@@ -562,8 +564,9 @@ def test_interleaved_library_stitch():
 
 def test_task_shift_semantics_pages_and_rejection():
     """Hand-computed paging example (P = 4, pool of 8): capacity 12 -> pages [0,1,2]; moving [4,8) to [6,10)
-    re-pages logical pages 1 and 2 onto fresh pages 3 and 4, and returns 1, 2 to the pool in that order."""
-    lib = _small_lib(n_pages=8)
+    re-pages logical pages 1 and 2 onto fresh pages 3 and 4, and returns 1, 2 to the pool in that order.
+    (max_task_tokens = 12 here: a destination beyond the capacity would otherwise append, R25.)"""
+    lib = _small_lib(n_pages=8, max_task_tokens=12)
     s, k, v = _reg(lib, 8, 0)
     lib.stitch([O.Plan(0, [O.PlanEntry(s, 0, 8, 0)], [], 12)])
     t = lib.tasks[0]
@@ -583,7 +586,7 @@ def test_task_shift_semantics_pages_and_rejection():
     # rejections change nothing
     snap = (list(t.page_table), t.filled.copy(), t.k.copy(), lib.pool.available())
     for args, status in (((0, 4, 2, 6), O.FCG_ERR_UNFILLED),        # source [4,6) is a hole now
-                         ((0, 6, 4, 9), O.FCG_ERR_RANGE),           # 9 + 4 > capacity 12
+                         ((0, 6, 4, 9), O.FCG_ERR_RANGE),           # 9 + 4 > max_task_tokens 12
                          ((0, -1, 2, 0), O.FCG_ERR_RANGE),
                          ((0, 0, 0, 2), O.FCG_ERR_RANGE),
                          ((7, 0, 2, 2), O.FCG_ERR_BAD_TASK)):
