@@ -1,17 +1,28 @@
 """bench.py -- one "step" = one pass of the whole grafting hot path (S2 plan -> S3 fused gather +
 RoPE-shift -> S4 scatter -> S5/S6 patch attention, all layers) over one synthetic batch.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|C1..C5] [--impl reference] [--shard ...]
 
-Prints ONE JSON line (rank 0).  metric = BASELINE.json's: graft latency (ms_per_step) and achieved
-algorithmic HBM GB/s (value) against the roofline on a B200.  Multi-GPU: the path shards by task
-(independent grafting tasks, no collective): every rank grafts its own copy of the workload
-("scaling": "weak").  --impl reference times the CPU oracle (the only reference this paper has).
+Prints ONE JSON line (rank 0).  metric = BASELINE.json's: graft latency (ms_per_step) and achieved algorithmic HBM
+GB/s (value) against the roofline on a B200.  With the default `--config all` the headline (value, ms_per_step,
+roofline, e2e, config.workload) is C4 -- BASELINE.json configs[3], the largest configuration that exercises both
+north_star kernels -- timed for EXACTLY K steps, and the key `configs` carries C2, C3, C4, C5 (and C1 as latency only)
+with per-config stitch / patch times, algorithmic bytes and flops, roofline fractions, ncu traffic (read from
+profiles/*.csv), end-to-end time, clock samples of that config's own timed region and layout seeds 1, 2, 3; C5 also
+carries the graft-vs-prefill comparison BASELINE.json asks for.
+
+Multi-GPU (`--gpus N` spawns N ranks through torch.distributed.run unless it already runs under it): the path shards
+by task and by kv head with no data-path collective (paper_2606_13097_b200/shard.py).  Default at N > 1: the batched
+configuration with 32 x N tasks, balanced over the ranks longest-first ("scaling": "weak"); `--shard task|head` split
+the fixed single-GPU workload instead ("strong"); `--shard replica` runs N identical copies.
+--impl reference times the CPU oracle (the only reference this paper has) on a bounded sample of the headline workload.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
+import math
 import os
 import subprocess
 import sys
@@ -25,71 +36,479 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2606_13097_b200 import synth  # noqa: E402
+from paper_2606_13097_b200 import shard, synth  # noqa: E402
 
 METRIC = "graft latency ms + HBM GB/s (stitch+RoPE shift, patch attn) vs roofline, 1 B200"
+UNIT = "GB/s (algorithmic, whole graft)"
 FALLBACK_HBM_GBS = 6650.0          # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+FALLBACK_BF16_SUSTAINED = 1400.0
+HEADLINE = "C4"
+ALL_CONFIGS = ("C4", "C2", "C3", "C5")
+EXTRACT_TOKENS = 1024
+
+
+def _peaks_file():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f)
+    except Exception:
+        return None
 
 
 def peaks():
-    try:
-        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-            p = json.load(f)
+    p = _peaks_file()
+    if p and "hbm_gbs" in p:
         return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json, torch copy_ read+write)"
-    except Exception:
-        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def tensor_peak():
+    p = _peaks_file()
+    if p and "bf16_tflops_sustained" in p:
+        return float(p["bf16_tflops_sustained"]), "measured (MEASURED_PEAKS.json, sustained bf16 matmul)"
+    return FALLBACK_BF16_SUSTAINED, "fallback (B200_PROFILING.md, sustained)"
 
 
 # --------------------------------------------------------------------------------------------------
 # algorithmic bytes
 # --------------------------------------------------------------------------------------------------
-def stitch_bytes(cfg, wl) -> int:
+def stitch_bytes(cfg, wl, tasks=None) -> int:
     """every stitched K/V byte is read once and written once: T_stitched * L * Hkv * D * 2 B * 2 (K,V) * 2 (r+w)."""
-    return wl.stitched_tokens * cfg.kv_bytes_per_token * 2
+    tasks = wl.tasks if tasks is None else tasks
+    return int(sum(n for t in tasks for (_, _, n, _) in t.entries)) * cfg.kv_bytes_per_token * 2
 
 
-def attn_bytes(cfg, wl) -> int:
+def attn_bytes(cfg, wl, tasks=None) -> int:
     """visible K+V read once per kv head: sum over tasks of L * kv_len * Hkv * D * 4 B (q/out/partials < 1 %)."""
-    total = 0
-    for t in wl.tasks:
-        kv_len = int(t.positions[-1]) + 1
-        total += cfg.n_layers * kv_len * cfg.n_kv_heads * cfg.head_dim * 4
-    return total
+    tasks = wl.tasks if tasks is None else tasks
+    return int(sum(cfg.n_layers * (int(t.positions[-1]) + 1) * cfg.n_kv_heads * cfg.head_dim * 4 for t in tasks))
 
 
-def attn_flops(cfg, wl) -> int:
+def attn_flops(cfg, wl, tasks=None) -> int:
     """Q K^T and P V over the visible cache only: per layer, q head and patch token i, 4 * D * (p_i + 1) flops."""
-    vis = sum(int((np.asarray(t.positions, np.int64) + 1).sum()) for t in wl.tasks)
+    tasks = wl.tasks if tasks is None else tasks
+    vis = sum(int((np.asarray(t.positions, np.int64) + 1).sum()) for t in tasks)
     return 4 * cfg.head_dim * cfg.n_layers * cfg.n_q_heads * vis
 
 
-def attn_rows(cfg, wl) -> int:
+def attn_rows(cfg, wl, tasks=None) -> int:
     """largest R = n * G (query rows per kv head) of the batch: intensity of patch attention is R flop/B."""
-    return max(len(t.positions) for t in wl.tasks) * (cfg.n_q_heads // cfg.n_kv_heads)
+    tasks = wl.tasks if tasks is None else tasks
+    return max(len(t.positions) for t in tasks) * (cfg.n_q_heads // cfg.n_kv_heads)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
-# (profiles/r01_final.md); None where no capture of that workload is committed.
-NCU_TRAFFIC = {"C2": {"stitch": 4.178e9, "attn": 2.183e9}, "C3": {"stitch": 2.061e9, "attn": 1.137e9},
-               "C4": {"stitch": 30.15e9, "attn": 16.14e9}, "C5": {"attn": 6.993e9}}
-
-
-def tensor_peak():
+def ncu_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed `ncu --set full` summaries:
+    the newest profiles/r*_traffic.csv (columns: config, kernel, dram_bytes_per_launch, capture).  {} if none."""
+    pdir = os.path.join(ROOT, "profiles")
     try:
-        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-            p = json.load(f)
-        return float(p["bf16_tflops_sustained"]), "measured (MEASURED_PEAKS.json, sustained bf16 matmul)"
+        files = sorted(f for f in os.listdir(pdir) if f.endswith("_traffic.csv"))
+    except OSError:
+        return {}, None
+    if not files:
+        return {}, None
+    out = {}
+    with open(os.path.join(pdir, files[-1])) as f:
+        for row in csv.DictReader(f):
+            try:
+                out.setdefault(row["config"], {})[row["kernel"]] = float(row["dram_bytes_per_launch"])
+            except (KeyError, ValueError):
+                continue
+    return out, "profiles/" + files[-1]
+
+
+# --------------------------------------------------------------------------------------------------
+# clocks during the timed regions
+# --------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """SM clock, power and clock-event (throttle) reasons of one GPU, sampled for the whole run by a background thread
+    and cut into windows afterwards, so that every timed region reports the samples that fall INSIDE it.
+    Source: NVML (what nvidia-smi reads) polled every ~4 ms; if pynvml cannot be used, `nvidia-smi -lms 20` with the
+    query of B200_PROFILING.md."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, cuda_index: int):
+        self.index, self.rows, self.proc, self.thread = cuda_index, [], None, None
+        self.source, self.sm_max, self._stop = None, None, False
+
+    def start(self):
+        try:
+            import pynvml as N
+            N.nvmlInit()
+            h = None
+            try:
+                uuid = str(torch.cuda.get_device_properties(self.index).uuid)
+                h = N.nvmlDeviceGetHandleByUUID(("GPU-" + uuid) if not uuid.startswith("GPU-") else uuid)
+            except Exception:
+                vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+                idx = int(vis.split(",")[self.index]) if vis and all(x.strip().isdigit() for x in vis.split(",")) else self.index
+                h = N.nvmlDeviceGetHandleByIndex(idx)
+            self.sm_max = float(N.nvmlDeviceGetMaxClockInfo(h, N.NVML_CLOCK_SM))
+            masks = (("hw_slowdown", N.nvmlClocksEventReasonHwSlowdown), ("hw_thermal_slowdown", N.nvmlClocksEventReasonHwThermalSlowdown),
+                     ("sw_thermal_slowdown", N.nvmlClocksEventReasonSwThermalSlowdown), ("sw_power_cap", N.nvmlClocksEventReasonSwPowerCap),
+                     ("hw_power_brake_slowdown", N.nvmlClocksEventReasonHwPowerBrakeSlowdown))
+
+            def loop():
+                while not self._stop:
+                    try:
+                        sm = float(N.nvmlDeviceGetClockInfo(h, N.NVML_CLOCK_SM))
+                        bits = int(N.nvmlDeviceGetCurrentClocksEventReasons(h))
+                        pw = N.nvmlDeviceGetPowerUsage(h) / 1000.0
+                        self.rows.append((time.time(), sm, [n for n, m in masks if bits & m], pw))
+                    except Exception:
+                        pass
+                    time.sleep(0.004)
+
+            N.nvmlDeviceGetClockInfo(h, N.NVML_CLOCK_SM)          # fail here, not in the thread
+            self.source = "nvml (pynvml), ~4 ms period"
+            self.thread = threading.Thread(target=loop, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            pass
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "20", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.source = "nvidia-smi -lms 20"
+            threading.Thread(target=self._read_smi, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read_smi(self):
+        for line in self.proc.stdout:
+            r = [x.strip() for x in line.split(",")]
+            try:
+                reasons = [n for n, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9])
+                           if v.lower().startswith("active")]
+                self.sm_max = float(r[2])
+                self.rows.append((time.time(), float(r[1]), reasons, float(r[3])))
+            except Exception:
+                continue
+
+    def window(self, t0: float, t1: float) -> dict:
+        if self.source is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no clock source (pynvml and nvidia-smi unavailable)"], "samples": 0}
+        inside = [r for r in list(self.rows) if t0 <= r[0] <= t1]
+        where = "timed region"
+        if len(inside) < 3:
+            inside = [r for r in list(self.rows) if t0 - 0.1 <= r[0] <= t1 + 0.1]
+            where = "timed region +- 0.1 s (fewer than 3 samples fell inside)"
+        sm = [r[1] for r in inside]
+        reasons = sorted({x for r in inside for x in r[2]})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_min_mhz": float(np.min(sm)) if sm else None,
+                "sm_max_mhz": self.sm_max, "power_w_max": float(max(r[3] for r in inside)) if inside else None,
+                "reasons": reasons, "samples": len(sm), "window": where, "source": self.source}
+
+    def stop(self):
+        self._stop = True
+        if self.proc is not None:
+            self.proc.terminate()
+
+
+# --------------------------------------------------------------------------------------------------
+# the CUDA arm: library, inputs, one timed region
+# --------------------------------------------------------------------------------------------------
+def build_library(cfg, wl, seed, device_index, on_segment=None, kv_heads=None, tasks=None, extra=True):
+    """The library exactly as the timed run uses it.  `on_segment(s, k, v)` lets the full-size parity tests keep
+    slices of the device-generated segments for the oracle.  `kv_heads = (begin, end)`: head-parallel shard -- `cfg`
+    is then the sharded configuration and every segment is cut to those kv heads after generation (same bits as the
+    unsharded run).  `tasks`: the tasks this rank grafts (task-parallel shard); default all."""
+    from paper_2606_13097_b200 import binding
+    tasks = wl.tasks if tasks is None else tasks
+    total_pages = sum(-(-t.capacity // cfg.page_size) for t in tasks)
+    seg_tokens = int(wl.seg_lens.sum())
+    if extra:
+        # + EXTRACT_TOKENS of arena and + half a task of pages: room for the NEXT-row measurements (segment extraction,
+        # copy-on-shift); neither changes what the graft step itself touches
+        seg_tokens += EXTRACT_TOKENS
+        total_pages += max(-(-t.capacity // cfg.page_size) for t in tasks) // 2 + 8
+    full = wl.cfg
+    lib = binding.FcgLibrary(n_layers=cfg.n_layers, n_q_heads=cfg.n_q_heads, n_kv_heads=cfg.n_kv_heads,
+                             head_dim=cfg.head_dim, page_size=cfg.page_size, rope_base=cfg.rope_base,
+                             max_segments=full.n_segments + 1, max_tasks=max(max(t.task_id for t in tasks) + 1, 1),
+                             max_task_tokens=max(t.capacity for t in tasks), n_pages=total_pages + 16,
+                             workspace_bytes=2 << 30, segment_tokens=seg_tokens, device=device_index,
+                             host_tier_tokens=(int(wl.seg_lens[tasks[0].entries[0][0]]) + 16) if extra else 0)
+    dev = torch.device("cuda", device_index)
+    gen_cfg = synth.scaled(full, page_size=cfg.page_size)
+    for s in range(full.n_segments):
+        k, v = synth.segment_kv(gen_cfg, s, int(wl.seg_lens[s]), seed, dev)
+        if kv_heads is not None:
+            k, v = k[:, kv_heads[0]:kv_heads[1]].contiguous(), v[:, kv_heads[0]:kv_heads[1]].contiguous()
+        sid = lib.segment_register(k, v, int(wl.orig_starts[s]))
+        assert sid == s
+        if on_segment is not None:
+            on_segment(s, k, v)
+        del k, v
+    torch.cuda.synchronize(dev)
+    return lib
+
+
+def plans_for(wl, tasks=None):
+    tasks = wl.tasks if tasks is None else tasks
+    return [{"task_id": t.task_id, "entries": t.entries, "holes": t.holes, "capacity_tokens": t.capacity} for t in tasks]
+
+
+def patch_inputs(full_cfg, tasks, seed, dev, q_heads=None, kv_heads=None):
+    """q, k, v of every task's patch, concatenated along the token axis (the layout fcg_patch_batch takes); head-parallel
+    shards cut the same tensors to their heads."""
+    qs = [synth.patch_qkv(full_cfg, t.task_id, len(t.positions), seed, dev) for t in tasks]
+    q = torch.cat([x[0] for x in qs], dim=1)
+    k = torch.cat([x[1] for x in qs], dim=1)
+    v = torch.cat([x[2] for x in qs], dim=1)
+    if q_heads is not None:
+        q, k, v = q[:, :, q_heads[0]:q_heads[1]], k[:, :, kv_heads[0]:kv_heads[1]], v[:, :, kv_heads[0]:kv_heads[1]]
+    return q.contiguous(), k.contiguous(), v.contiguous()
+
+
+class Dist:
+    """rank / world and the two collectives the bench needs (barrier, max over ranks); a no-op at world 1."""
+
+    def __init__(self, args):
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.local = 0 if args.devices == "same" else int(os.environ.get("LOCAL_RANK", "0"))
+        self.backend = None
+        if self.world > 1:
+            import torch.distributed as dist
+            self.backend = "gloo" if args.devices == "same" else "nccl"
+            if self.backend == "nccl":
+                dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+            else:
+                dist.init_process_group("gloo")
+        torch.cuda.set_device(self.local)
+        self.dev = torch.device("cuda", self.local)
+
+    def barrier(self):
+        torch.cuda.synchronize(self.dev)
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize(self.dev)
+
+    def max(self, x: float) -> float:
+        if self.world == 1:
+            return float(x)
+        return shard.max_over_ranks(x, device=self.dev if self.backend == "nccl" else "cpu")
+
+    def sum(self, x: float) -> float:
+        if self.world == 1:
+            return float(x)
+        import torch.distributed as dist
+        t = torch.tensor([float(x)], dtype=torch.float64, device=self.dev if self.backend == "nccl" else "cpu")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    def close(self):
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+            dist.destroy_process_group()
+
+
+def time_region(lib, plans, ids, npt, pos, q, k, v, out, steps, warmup, D: Dist):
+    """W warm-up steps, barrier + synchronize, EXACTLY `steps` timed steps bracketed by CUDA events on the launching
+    stream (torch's current stream, which the binding passes to the library), barrier + synchronize."""
+    live = [False]
+
+    def step(ev=None):
+        if live[0]:
+            for tid in ids:
+                lib.task_release(tid)
+        if ev:
+            ev[0].record()
+        lib.stitch(plans)
+        live[0] = True
+        if ev:
+            ev[1].record()
+        if len(ids) == 1:
+            lib.patch(ids[0], 0, q, k, v, pos, out)
+        else:
+            lib.patch_batch(ids, npt, 0, q, k, v, pos, out)
+        if ev:
+            ev[2].record()
+
+    for _ in range(warmup):
+        step()
+    D.barrier()
+    s0 = lib.stats()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    w0 = time.time()
+    t_begin.record()
+    for i in range(steps):
+        step(evs[i])
+    t_end.record()
+    D.barrier()
+    w1 = time.time()
+    s1 = lib.stats()
+    total_ms = D.max(t_begin.elapsed_time(t_end))
+    return {"ms_per_step": total_ms / steps, "steps": steps,
+            "stitch_ms": [e[0].elapsed_time(e[1]) for e in evs], "patch_ms": [e[1].elapsed_time(e[2]) for e in evs],
+            "launches": int(sum(s1[f] - s0[f] for f in s1 if f.endswith("_launches"))), "wall": (w0, w1), "stats": s1}
+
+
+def time_e2e(lib, plans, ids, npt, pos, q, k, v, out, steps, warmup, D: Dist):
+    """the same step through the C ABI with HOST buffers: H2D of q/k/v and D2H of out inside the timed region, the host
+    reads `out` every step (synchronize).  Returns (ms per step, h2d bytes, d2h bytes)."""
+    qh, kh, vh = [x.cpu().contiguous().pin_memory() for x in (q, k, v)]
+    oh = torch.empty_like(qh).pin_memory()
+    single = len(ids) == 1
+
+    def step_host():
+        for tid in ids:
+            lib.task_release(tid)
+        lib.stitch(plans)
+        if single:
+            lib.patch_host(ids[0], 0, qh, kh, vh, pos, oh)
+        else:
+            lib.patch_batch_host(ids, npt, 0, qh, kh, vh, pos, oh)
+        torch.cuda.synchronize(D.dev)          # the caller reads `out` on the host every step
+
+    for _ in range(min(warmup, 3)):
+        step_host()
+    D.barrier()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(steps):
+        step_host()
+    b.record()
+    D.barrier()
+    ms = D.max(a.elapsed_time(b) / steps)
+    assert torch.equal(oh, out.cpu()), "host-buffer call and device call disagree"
+    return ms, int(qh.numel() + kh.numel() + vh.numel()) * 2, int(oh.numel()) * 2
+
+
+def rooflines(cfg, wl, tasks, timing, traffic, name):
+    """stitch (HBM) and patch-attention (HBM below R ~ 250 rows per kv head, bf16 tensor peak above) rooflines of one
+    timed region, from the mean CUDA-event durations of its steps."""
+    sb, ab = stitch_bytes(cfg, wl, tasks), attn_bytes(cfg, wl, tasks)
+    af, rows = attn_flops(cfg, wl, tasks), attn_rows(cfg, wl, tasks)
+    peak, peak_src = peaks()
+    st_s, at_s = float(np.mean(timing["stitch_ms"])) * 1e-3, float(np.mean(timing["patch_ms"])) * 1e-3
+    tr = traffic.get(name, {})
+    stitch = {"kernel": "stitch_kernel (fused gather + RoPE-shift)", "bound": "hbm", "achieved": sb / st_s / 1e9, "peak": peak,
+              "unit": "GB/s", "frac": sb / st_s / 1e9 / peak, "peak_source": peak_src, "frac_of_8TBps": sb / st_s / 1e9 / 8000.0,
+              "traffic": tr.get("stitch")}
+    if rows >= 250:
+        tpeak, tsrc = tensor_peak()
+        attn = {"kernel": "attn_tc_kernel (tcgen05 / TMEM)", "bound": "tensor", "achieved": af / at_s / 1e12, "peak": tpeak, "unit": "TFLOP/s",
+                "frac": af / at_s / 1e12 / tpeak, "peak_source": tsrc, "rows_per_kv_head": rows, "hbm_GBps": ab / at_s / 1e9,
+                "hbm_frac": ab / at_s / 1e9 / peak}
+    else:
+        attn = {"kernel": "attn_tc_kernel (tcgen05 / TMEM)" if timing["stats"]["last_attn_path"] == 2 else "attn_split_kernel (mma.sync split-KV)",
+                "bound": "hbm", "achieved": ab / at_s / 1e9, "peak": peak, "unit": "GB/s", "frac": ab / at_s / 1e9 / peak,
+                "frac_of_8TBps": ab / at_s / 1e9 / 8000.0, "rows_per_kv_head": rows, "TFLOPs": af / at_s / 1e12}
+    attn["traffic"] = tr.get("attn")
+    attn["note"] = "timed as scatter + attention (+ combine); scatter is ~1 % of it"
+    return stitch, attn, sb, ab, af
+
+
+def describe(cfg, name, wl, tasks, seed):
+    return (f"{cfg.name} ({name}): L={cfg.n_layers} Hq={cfg.n_q_heads} Hkv={cfg.n_kv_heads} D={cfg.head_dim} page={cfg.page_size} "
+            f"base={cfg.rope_base:g}; library {wl.cfg.n_segments} segments ({int(wl.seg_lens.sum())} tokens); {len(tasks)} task(s), "
+            f"{int(sum(n for t in tasks for (_, _, n, _) in t.entries))} stitched + {int(sum(len(t.positions) for t in tasks))} patch tokens; "
+            f"layout seed {seed}")
+
+
+def measure_config(args, name, seed, D: Dist, sampler, traffic, steps, *, full, shard_mode="none"):
+    """One configuration on this rank's shard: build the library, time `steps` graft steps; `full` adds the end-to-end
+    leg and (rank 0) the NEXT rows.  Returns the per-config record (rank 0 decides what to print)."""
+    cfg_full = synth.CONFIGS[name]
+    if args.page_size:
+        cfg_full = synth.scaled(cfg_full, page_size=args.page_size)
+    kv_heads = q_heads = None
+    cfg = cfg_full
+    scaling = "weak"
+    if shard_mode == "weak" and D.world > 1:
+        # 32 x N independent tasks over one shared library, balanced over the ranks longest-first
+        wl = synth.make_workload(synth.scaled(cfg_full, n_tasks=cfg_full.n_tasks * D.world), seed)
+        mine, _ = shard.rank_workload(wl, D.rank, D.world, cfg.kv_bytes_per_token)
+        tasks = [wl.tasks[i] for i in mine]
+    elif shard_mode == "task" and D.world > 1:
+        wl = synth.make_workload(cfg_full, seed)
+        mine, _ = shard.rank_workload(wl, D.rank, D.world, cfg.kv_bytes_per_token)
+        tasks = [wl.tasks[i] for i in mine]
+        scaling = "strong"
+    elif shard_mode == "head" and D.world > 1:
+        wl = synth.make_workload(cfg_full, seed)
+        tasks = wl.tasks
+        cfg = shard.head_sharded_config(cfg_full, D.rank, D.world)
+        kv_heads = shard.kv_head_range(cfg_full.n_kv_heads, D.rank, D.world)
+        q_heads = shard.q_head_range(cfg_full.n_q_heads, cfg_full.n_kv_heads, D.rank, D.world)
+        scaling = "strong"
+    else:
+        wl = synth.make_workload(cfg_full, seed)
+        tasks = wl.tasks
+    if not tasks:
+        raise RuntimeError(f"rank {D.rank} has no task of {name} (world {D.world} > tasks)")
+    lib = build_library(cfg, wl, seed, D.local, kv_heads=kv_heads, tasks=tasks, extra=full)
+    try:
+        plans = plans_for(wl, tasks)
+        ids = [t.task_id for t in tasks]
+        npt = [len(t.positions) for t in tasks]
+        pos = np.concatenate([t.positions for t in tasks]).astype(np.int32)
+        q, k, v = patch_inputs(synth.scaled(cfg_full, page_size=cfg.page_size), tasks, seed, D.dev, q_heads, kv_heads)
+        out = torch.empty_like(q)
+        timing = time_region(lib, plans, ids, npt, pos, q, k, v, out, steps, args.warmup, D)
+        stitch_roof, attn_roof, sb, ab, af = rooflines(cfg, wl, tasks, timing, traffic, name)
+        # whole-job units: every rank's bytes (summed) over the max-over-ranks time
+        job_bytes = D.sum(sb + ab)
+        ms = timing["ms_per_step"]
+        rec = {
+            "workload": describe(cfg, name, wl, tasks, seed) + (f"; rank 0 of {D.world}, shard = {shard_mode}" if D.world > 1 else ""),
+            "ms_per_step": ms, "steps": steps, "value_GBps": job_bytes / (ms * 1e-3) / 1e9,
+            "stitch_ms": float(np.mean(timing["stitch_ms"])), "stitch_ms_min": float(np.min(timing["stitch_ms"])),
+            "stitch_ms_median": float(np.median(timing["stitch_ms"])),
+            "patch_ms": float(np.mean(timing["patch_ms"])), "patch_ms_min": float(np.min(timing["patch_ms"])),
+            "patch_ms_median": float(np.median(timing["patch_ms"])),
+            "stitch_bytes": sb, "attn_bytes": ab, "attn_flops": af,
+            "attn_path": timing["stats"]["last_attn_path"], "attn_splits": timing["stats"]["last_attn_splits"],
+            "gpu_launches": timing["launches"], "scaling": scaling,
+            "l2": "inputs larger than L2 (each step streams >= 1 GiB; no flush needed)" if sb > 4 * 126e6
+            else "working set fits L2: latency only, no roofline claim",
+            "roofline": dict(stitch_roof, patch_attention=attn_roof),
+            "clocks": sampler.window(*timing["wall"]) if sampler else None,
+            "_job_bytes": job_bytes,
+        }
+        if sb <= 4 * 126e6:
+            rec["roofline"] = None
+        if full:
+            e_ms, h2d, d2h = time_e2e(lib, plans, ids, npt, pos, q, k, v, out, max(3, min(steps, 10)), args.warmup, D)
+            rec["e2e"] = {"value": job_bytes / (e_ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": e_ms,
+                          "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+            if D.rank == 0 and not args.no_next and shard_mode in ("none", "replica"):
+                try:
+                    rec["next_rows"] = time_next_rows(lib, cfg, wl, seed, D.dev)
+                except Exception as e:       # never lose the main line to an extra
+                    rec["next_rows"] = {"error": repr(e)}
+            if D.rank == 0 and name == "C5" and not args.no_prefill_compare and shard_mode in ("none", "replica"):
+                try:
+                    pc = time_prefill_compare(lib, cfg, wl, seed, D.dev)
+                    pc["graft_ms"] = ms
+                    pc["prefill_attention_over_graft"] = pc["own_kernel_ms_all_layers"] / ms
+                    rec["prefill_compare"] = pc
+                except Exception as e:
+                    rec["prefill_compare"] = {"error": repr(e)}
+        if D.world > 1 and shard_mode in ("head", "task", "weak") and out.numel() * 2 * D.world <= (1 << 30) and D.backend == "nccl":
+            # results are exchanged only here, outside every timed region (shard.py); head shards concatenate along the
+            # head axis, task shards are put back in task order
+            if shard_mode == "head":
+                whole = shard.gather_head_outputs(out)
+                rec["gathered_out_shape"] = list(whole.shape)
+                del whole
+        return rec, lib, (cfg, wl, tasks)
     except Exception:
-        return 1400.0, "fallback (B200_PROFILING.md, sustained)"
-
-
-EXTRACT_TOKENS = 1024
+        lib.close()
+        raise
 
 
 def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
     """SURVEY.md 8(f) NEXT rows, timed on task 0 of the stitched workload after the main measurement (CUDA events,
     2 warm-ups): suffix re-graft by -16 / +16 tokens (fcg_task_shift), extraction of EXTRACT_TOKENS tokens into the
-    library (fcg_segment_extract), and one decode step (fcg_patch, n = 1, R = G) over the whole cache."""
+    library (fcg_segment_extract), one decode step (fcg_patch, n = 1, R = G) over the whole cache, the one-call-per-layer
+    pattern (plain calls, a patch plan, and the plan captured into one CUDA graph) and the two-tier moves."""
     t = wl.tasks[0]
     cap = t.capacity
     mid = (cap // 2) & ~15
@@ -114,6 +533,20 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
     def register():
         lib.segment_release(lib.segment_register(kr, vr, 0))
 
+    def timed_loop(fn, n=iters, warm=2):
+        for _ in range(warm):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        t1 = time.perf_counter()
+        torch.cuda.synchronize(dev)
+        return a.elapsed_time(b) / n, (t1 - t0) * 1e3 / n
+
     res = {}
     # the call pattern of a model that patches layer by layer: L calls of one layer each (task 0's own patch tokens)
     try:
@@ -125,38 +558,37 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
             for l, (a_, b_, c_, d_) in enumerate(views):
                 lib.patch(t.task_id, l, a_, b_, c_, t.positions, d_)
 
-        for _ in range(2):
-            per_layer()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize(dev)
-        t0 = time.perf_counter()
-        a.record()
-        for _ in range(iters):
-            per_layer()
-        b.record()
-        t1 = time.perf_counter()
-        torch.cuda.synchronize(dev)
-        res["patch_one_call_per_layer"] = {"ms": a.elapsed_time(b) / iters, "host_enqueue_ms": (t1 - t0) * 1e3 / iters,
-                                           "calls": cfg.n_layers, "splits": lib.stats()["last_attn_splits"],
+        ms, host = timed_loop(per_layer)
+        res["patch_one_call_per_layer"] = {"ms": ms, "host_enqueue_ms": host, "calls": cfg.n_layers, "splits": lib.stats()["last_attn_splits"],
                                            "note": "same patch as the timed step, issued as one fcg_patch per layer"}
+        plan = lib.patch_plan_create([t.task_id], [len(t.positions)], t.positions, 1)
+
+        def per_layer_planned():
+            for l, (a_, b_, c_, d_) in enumerate(views):
+                lib.patch_planned(plan, l, a_, b_, c_, d_)
+
+        ms, host = timed_loop(per_layer_planned)
+        res["patch_one_call_per_layer_planned"] = {"ms": ms, "host_enqueue_ms": host, "calls": cfg.n_layers,
+                                                   "note": "fcg_patch_plan_create once, then one fcg_patch_planned per layer (launches only)"}
+        side = torch.cuda.Stream(device=dev)
+        side.wait_stream(torch.cuda.current_stream(dev))
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            per_layer_planned()
+        ms, host = timed_loop(g.replay)
+        res["patch_one_call_per_layer_graph"] = {"ms": ms, "host_enqueue_ms": host, "calls": 1,
+                                                 "note": f"the {cfg.n_layers} planned per-layer calls captured into one CUDA graph, one replay per step"}
+        del g
+        lib.patch_plan_destroy(plan)
         del qp, kp, vp, op, views
     except Exception as e:
-        res["patch_one_call_per_layer"] = {"error": repr(e)}
+        res["patch_one_call_per_layer_error"] = repr(e)
     per_tok = cfg.kv_bytes_per_token
     for name, fn, nbytes in (("decode_step", decode, cfg.n_layers * cap * cfg.n_kv_heads * cfg.head_dim * 4),
                              ("segment_register", register, n_ext * per_tok * 2),
                              ("segment_extract", extract, n_ext * per_tok * 2),
                              ("task_shift", shift_pair, 2 * n_shift * per_tok * 2)):
-        for _ in range(2):
-            fn()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize(dev)
-        a.record()
-        for _ in range(iters):
-            fn()
-        b.record()
-        torch.cuda.synchronize(dev)
-        ms = a.elapsed_time(b) / iters
+        ms, _ = timed_loop(fn)
         res[name] = {"ms": ms, "GBps": nbytes / (ms * 1e-3) / 1e9, "bytes": int(nbytes)}
     # NEXT-3 two-tier residency: one library segment to the pinned host tier and back (copy engine), and a stitch
     # that reads it in place from the host tier (zero-copy over the host link)
@@ -245,6 +677,7 @@ def time_prefill_compare(lib, cfg, wl, seed, dev, layers_per_call=4):
             torch.cuda.synchronize(dev)
             sm.append(a.elapsed_time(b))
         res["torch_sdpa_ms_all_layers"] = float(np.min(sm[1:])) * cfg.n_layers
+        res["torch_sdpa_note"] = "library kernel, context only"
     except Exception as e:
         res["torch_sdpa_ms_all_layers"] = None
         res["torch_sdpa_error"] = repr(e)
@@ -252,273 +685,134 @@ def time_prefill_compare(lib, cfg, wl, seed, dev, layers_per_call=4):
     return res
 
 
-class ClockSampler:
-    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe).  nvidia-smi is started
-    before the warm-up (it needs ~0.1 s to come up) and samples every 20 ms; rows are time-stamped on arrival and
-    only those inside [mark_begin, mark_end] count.  If the region was too short to catch one, the rows nearest to
-    it (within 0.3 s, i.e. warm-up steps of the same workload) are used and `window` says so."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
-
-    def __init__(self, index: int):
-        self.index, self.rows, self.proc = index, [], None
-        self.t0 = self.t1 = None
-
-    def start(self):
-        try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "20", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
-            threading.Thread(target=self._read, daemon=True).start()
-        except Exception:
-            self.proc = None
-
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
-
-    def mark_begin(self):
-        self.t0 = time.time()
-
-    def mark_end(self):
-        self.t1 = time.time()
-
-    def stop(self) -> dict:
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.05)
-        self.proc.terminate()
-        t0, t1 = self.t0 or 0.0, self.t1 or time.time()
-        inside = [r for (ts, r) in self.rows if t0 <= ts <= t1 + 0.02]
-        window = "timed region"
-        if not inside:
-            inside = [r for (ts, r) in self.rows if t0 - 0.3 <= ts <= t1 + 0.3]
-            window = "nearest samples within 0.3 s of the timed region (region shorter than the sampling period)"
-        sm, smax, reasons = [], [], set()
-        for r in inside:
-            try:
-                sm.append(float(r[1])), smax.append(float(r[2]))
-            except Exception:
-                continue
-            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
-                if val.lower().startswith("active"):
-                    reasons.add(name)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
-                "reasons": sorted(reasons), "samples": len(sm), "window": window}
+def c1_latency(args, D, seed):
+    """C1 (0.65 MiB, fits L2): launch-bound, latency only, no roofline claim."""
+    cfg = synth.CONFIGS["C1"]
+    wl = synth.make_workload(cfg, seed)
+    lib = build_library(cfg, wl, seed, D.local, extra=False)
+    try:
+        t = wl.tasks[0]
+        q, k, v = patch_inputs(cfg, wl.tasks, seed, D.dev)
+        out = torch.empty_like(q)
+        timing = time_region(lib, plans_for(wl), [t.task_id], [len(t.positions)], t.positions.astype(np.int32), q, k, v, out, 200, 5,
+                             Dist.__new__(Dist)._solo(D))
+        return {"workload": describe(cfg, "C1", wl, wl.tasks, seed), "ms_per_step": timing["ms_per_step"], "steps": 200,
+                "stitch_ms_median": float(np.median(timing["stitch_ms"])), "patch_ms_median": float(np.median(timing["patch_ms"])),
+                "attn_path": timing["stats"]["last_attn_path"], "note": "working set fits L2 and the step is launch-bound: latency only"}
+    finally:
+        lib.close()
 
 
-# --------------------------------------------------------------------------------------------------
-# the CUDA arm
-# --------------------------------------------------------------------------------------------------
-def build_library(cfg, wl, seed, device_index, on_segment=None):
-    """The library exactly as the timed run uses it.  `on_segment(s, k, v)` lets the full-size parity tests
-    keep slices of the device-generated segments for the oracle."""
-    from paper_2606_13097_b200 import binding
-    total_pages = sum(-(-t.capacity // cfg.page_size) for t in wl.tasks)
-    # + EXTRACT_TOKENS of arena and + half a task of pages: room for the NEXT-row measurements (segment extraction,
-    # copy-on-shift); neither changes what the graft step itself touches
-    seg_tokens = int(wl.seg_lens.sum()) + EXTRACT_TOKENS
-    total_pages += max(-(-t.capacity // cfg.page_size) for t in wl.tasks) // 2 + 8
-    lib = binding.FcgLibrary(n_layers=cfg.n_layers, n_q_heads=cfg.n_q_heads, n_kv_heads=cfg.n_kv_heads,
-                             head_dim=cfg.head_dim, page_size=cfg.page_size, rope_base=cfg.rope_base,
-                             max_segments=cfg.n_segments + 1, max_tasks=max(cfg.n_tasks, 1),
-                             max_task_tokens=max(t.capacity for t in wl.tasks), n_pages=total_pages + 16,
-                             workspace_bytes=2 << 30, segment_tokens=seg_tokens, device=device_index,
-                             host_tier_tokens=int(wl.seg_lens[wl.tasks[0].entries[0][0]]) + 16)
-    dev = torch.device("cuda", device_index)
-    for s in range(cfg.n_segments):
-        k, v = synth.segment_kv(cfg, s, int(wl.seg_lens[s]), seed, dev)
-        sid = lib.segment_register(k, v, int(wl.orig_starts[s]))
-        assert sid == s
-        if on_segment is not None:
-            on_segment(s, k, v)
-        del k, v
-    torch.cuda.synchronize(dev)
-    return lib
+def _solo(self, D):
+    """a world-1 view of this rank (local measurements that the other ranks do not take part in)"""
+    self.rank, self.world, self.local, self.backend, self.dev = 0, 1, D.local, None, D.dev
+    return self
 
 
-def plans_for(wl):
-    return [{"task_id": t.task_id, "entries": t.entries, "holes": t.holes, "capacity_tokens": t.capacity} for t in wl.tasks]
+Dist._solo = _solo
 
 
-def run_cuda(args, cfg, wl, seed):
-    from paper_2606_13097_b200 import binding
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    lib = build_library(cfg, wl, seed, local)
-    plans = plans_for(wl)
-    ids = [t.task_id for t in wl.tasks]
-    npt = [len(t.positions) for t in wl.tasks]
-    pos = np.concatenate([t.positions for t in wl.tasks]).astype(np.int32)
-    n_total = int(pos.size)
-    qs = [synth.patch_qkv(cfg, t.task_id, len(t.positions), seed, dev) for t in wl.tasks]
-    q = torch.cat([x[0] for x in qs], dim=1).contiguous()
-    k = torch.cat([x[1] for x in qs], dim=1).contiguous()
-    v = torch.cat([x[2] for x in qs], dim=1).contiguous()
-    out = torch.empty_like(q)
-    del qs
-    live = [False]
-
-    def step_device(ev=None):
-        if live[0]:
-            for tid in ids:
-                lib.task_release(tid)
-        if ev:
-            ev[0].record()
-        lib.stitch(plans)
-        live[0] = True
-        if ev:
-            ev[1].record()
-        if len(ids) == 1:
-            lib.patch(ids[0], 0, q, k, v, pos, out)
-        else:
-            lib.patch_batch(ids, npt, 0, q, k, v, pos, out)
-        if ev:
-            ev[2].record()
-
-    def barrier():
-        torch.cuda.synchronize(dev)
-        if world > 1:
-            import torch.distributed as dist
-            dist.barrier()
-        torch.cuda.synchronize(dev)
-
-    sampler = ClockSampler(local)
-    if rank == 0:
+def run_cuda(args):
+    D = Dist(args)
+    sampler = ClockSampler(D.local) if D.rank == 0 else None
+    if sampler:
         sampler.start()
-    for _ in range(args.warmup):
-        step_device()
-    barrier()
-    s0 = lib.stats()
-    sampler.mark_begin()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
-    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t_begin.record()
-    for i in range(args.steps):
-        step_device(evs[i])
-    t_end.record()
-    barrier()
-    sampler.mark_end()
-    clocks = sampler.stop() if rank == 0 else None
-    s1 = lib.stats()
-    total_ms = t_begin.elapsed_time(t_end)
-    stitch_ms = [e[0].elapsed_time(e[1]) for e in evs]
-    patch_ms = [e[1].elapsed_time(e[2]) for e in evs]
-    if world > 1:
-        import torch.distributed as dist
-        tt = torch.tensor([total_ms], device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
-    ms_per_step = total_ms / args.steps
-    launches = sum(s1[f] - s0[f] for f in s1 if f.endswith("_launches"))
-
-    # ---- e2e: same step through the C ABI with HOST buffers (H2D of q/k/v, D2H of out inside) ----
-    single = len(ids) == 1
-    e2e = None
-    if True:
-        qh, kh, vh = [x.cpu().contiguous().pin_memory() for x in (q, k, v)]
-        oh = torch.empty_like(qh).pin_memory()
-
-        def step_host():
-            for tid in ids:
-                lib.task_release(tid)
-            lib.stitch(plans)
-            if single:
-                lib.patch_host(ids[0], 0, qh, kh, vh, pos, oh)
-            else:
-                lib.patch_batch_host(ids, npt, 0, qh, kh, vh, pos, oh)
-            torch.cuda.synchronize(dev)          # the caller reads `out` on the host every step
-
-        for _ in range(min(args.warmup, 3)):
-            step_host()
-        barrier()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        for _ in range(args.steps):
-            step_host()
-        b.record()
-        barrier()
-        e2e_ms = a.elapsed_time(b) / args.steps
-        if world > 1:
-            import torch.distributed as dist
-            tt = torch.tensor([e2e_ms], device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e2e_ms = float(tt.item())
-        h2d = int(qh.numel() + kh.numel() + vh.numel()) * 2
-        d2h = int(oh.numel()) * 2
-        e2e = (e2e_ms, h2d, d2h)
-        assert torch.equal(oh, out.cpu()), "host-buffer call and device call disagree"
-
-    sb, ab = stitch_bytes(cfg, wl), attn_bytes(cfg, wl)
-    peak, peak_src = peaks()
-    # patch attention: HBM-bound while R = n*G (flop per byte) is small, tensor-bound from R ~ 250 (SURVEY.md 8(d))
-    af, rows = attn_flops(cfg, wl), attn_rows(cfg, wl)
-    attn_s = float(np.mean(patch_ms)) * 1e-3
-    if rows >= 250:
-        tpeak, tsrc = tensor_peak()
-        attn_roof = {"bound": "tensor", "achieved": af / attn_s / 1e12, "peak": tpeak, "unit": "TFLOP/s",
-                     "frac": af / attn_s / 1e12 / tpeak, "peak_source": tsrc, "rows_per_kv_head": rows,
-                     "hbm_GBps": ab / attn_s / 1e9}
+    traffic, traffic_src = ncu_traffic()
+    single = args.config != "all"
+    head_name = args.config if single else HEADLINE
+    if D.world > 1:
+        mode = args.shard if args.shard != "auto" else ("weak" if synth.CONFIGS[head_name].n_tasks > 1 else "head")
     else:
-        attn_roof = {"bound": "hbm", "achieved": ab / attn_s / 1e9, "peak": peak, "unit": "GB/s",
-                     "frac": ab / attn_s / 1e9 / peak, "frac_of_8TBps": ab / attn_s / 1e9 / 8000.0,
-                     "rows_per_kv_head": rows, "TFLOPs": af / attn_s / 1e12}
-    attn_roof["traffic"] = NCU_TRAFFIC.get(args.config, {}).get("attn")
-    attn_roof["note"] = "timed as scatter + attention (+ combine); scatter is ~1 % of it"
+        mode = "none"
+    if mode == "head" and synth.CONFIGS[head_name].n_kv_heads % D.world:
+        mode = "replica"
+    seeds = [int(s) for s in args.seeds.split(",") if s]
+    configs = {}
+    # ---- headline: EXACTLY K steps ----------------------------------------------------------------
+    rec, lib, (cfg, wl, tasks) = measure_config(args, head_name, args.seed, D, sampler, traffic, args.steps, full=True, shard_mode=mode)
     res = {
-        "metric": METRIC, "value": world * (sb + ab) / (ms_per_step * 1e-3) / 1e9, "unit": "GB/s (algorithmic, whole graft)",
-        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": f"{cfg.name} ({args.config}): L={cfg.n_layers} Hq={cfg.n_q_heads} Hkv={cfg.n_kv_heads} "
-                               f"D={cfg.head_dim} page={cfg.page_size} base={cfg.rope_base:g}; library {cfg.n_segments} segments "
-                               f"({int(wl.seg_lens.sum())} tokens); {len(wl.tasks)} task(s), {wl.stitched_tokens} stitched + "
-                               f"{wl.patch_tokens} patch tokens; layout seed {seed}",
-                   "l2": "inputs larger than L2 (each step streams >= 1 GiB; no flush needed)" if sb > 4 * 126e6
-                   else "working set fits L2: latency only, no roofline claim",
-                   "stitch_ms": float(np.mean(stitch_ms)), "stitch_ms_min": float(np.min(stitch_ms)),
-                   "stitch_ms_median": float(np.median(stitch_ms)),
-                   "patch_ms": float(np.mean(patch_ms)), "patch_ms_min": float(np.min(patch_ms)),
-                   "patch_ms_median": float(np.median(patch_ms)),
-                   "stitch_GBps": sb / (np.mean(stitch_ms) * 1e-3) / 1e9, "patch_attn_GBps": ab / (np.mean(patch_ms) * 1e-3) / 1e9,
-                   "stitch_bytes": sb, "attn_bytes": ab, "attn_path": s1["last_attn_path"], "attn_splits": s1["last_attn_splits"],
-                   "parallelism": f"task-replica x{world}"},
-        "gpu_launches": int(launches),
-        "roofline": {"kernel": "stitch_kernel (fused gather + RoPE-shift)", "bound": "hbm",
-                     "achieved": sb / (np.mean(stitch_ms) * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                     "frac": sb / (np.mean(stitch_ms) * 1e-3) / 1e9 / peak, "peak_source": peak_src,
-                     "frac_of_8TBps": sb / (np.mean(stitch_ms) * 1e-3) / 1e9 / 8000.0,
-                     "traffic": args.traffic if args.traffic is not None else NCU_TRAFFIC.get(args.config, {}).get("stitch"),
-                     "patch_attention": attn_roof},
-        "clocks": clocks,
+        "metric": METRIC, "value": rec["value_GBps"], "unit": UNIT, "n_gpus": D.world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": rec["ms_per_step"], "higher_is_better": True, "scaling": rec["scaling"], "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": rec["workload"], "l2": rec["l2"], "stitch_ms": rec["stitch_ms"], "stitch_ms_min": rec["stitch_ms_min"],
+                   "stitch_ms_median": rec["stitch_ms_median"], "patch_ms": rec["patch_ms"], "patch_ms_min": rec["patch_ms_min"],
+                   "patch_ms_median": rec["patch_ms_median"], "stitch_bytes": rec["stitch_bytes"], "attn_bytes": rec["attn_bytes"],
+                   "attn_flops": rec["attn_flops"], "attn_path": rec["attn_path"], "attn_splits": rec["attn_splits"],
+                   "parallelism": {"none": "1 GPU", "replica": f"task-replica x{D.world}", "weak": f"task-parallel, {len(wl.tasks)} tasks LPT-balanced over {D.world} ranks",
+                                   "task": f"task-parallel (strong), {D.world} ranks", "head": f"kv-head-parallel (strong), {D.world} ranks"}[mode],
+                   "traffic_source": traffic_src},
+        "gpu_launches": rec["gpu_launches"],
+        "roofline": rec["roofline"],
+        "clocks": rec["clocks"],
+        "e2e": rec.get("e2e"),
     }
-    if e2e:
-        res["e2e"] = {"value": world * (sb + ab) / (e2e[0] * 1e-3) / 1e9, "unit": "GB/s (algorithmic, whole graft)",
-                      "ms_per_step": e2e[0], "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2]}
-    if rank == 0 and not args.no_next:
-        try:
-            res["next_rows"] = time_next_rows(lib, cfg, wl, seed, dev)
-        except Exception as e:       # never lose the main line to an extra
-            res["next_rows"] = {"error": repr(e)}
-    if rank == 0 and args.prefill_compare:
-        try:
-            res["prefill_compare"] = time_prefill_compare(lib, cfg, wl, seed, dev)
-            res["prefill_compare"]["graft_ms"] = ms_per_step
-            res["prefill_compare"]["prefill_attention_over_graft"] = res["prefill_compare"]["own_kernel_ms_all_layers"] / ms_per_step
-        except Exception as e:
-            res["prefill_compare"] = {"error": repr(e)}
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        res["cpu_baseline"] = cpu_baseline(cfg, wl, seed, lib_segments=lambda s: synth.segment_kv(cfg, s, int(wl.seg_lens[s]), seed, dev))
+    if "next_rows" in rec:
+        res["next_rows"] = rec["next_rows"]
+    if "prefill_compare" in rec:
+        res["prefill_compare"] = rec["prefill_compare"]
+    if D.rank == 0 and D.world == 1 and not args.no_cpu_baseline:
+        gen_cfg = synth.scaled(wl.cfg, page_size=cfg.page_size)
+        res["cpu_baseline"] = cpu_baseline(cfg, wl, args.seed, lib_segments=lambda s: synth.segment_kv(gen_cfg, s, int(wl.seg_lens[s]), args.seed, D.dev))
     lib.close()
-    if world > 1:
-        import torch.distributed as dist
-        dist.barrier()                      # rank 0 may still have been timing its extras
-        dist.destroy_process_group()
-    return res if rank == 0 else None
+    del lib
+    torch.cuda.empty_cache()
+    configs[head_name] = {k: v for k, v in rec.items() if not k.startswith("_") and k not in ("next_rows",)}
+    configs[head_name]["seeds"] = {str(args.seed): {"ms_per_step": rec["ms_per_step"], "stitch_ms": rec["stitch_ms"], "patch_ms": rec["patch_ms"]}}
+
+    def region_steps(name):
+        # sub-configurations: at least 20 steps and a region of >= ~0.12 s, so that the clock samples fall inside it
+        est = {"C2": 1.0, "C3": 0.75, "C4": 8.0, "C5": 13.5}.get(name, 5.0)
+        return int(max(20, args.steps, math.ceil(120.0 / est)))
+
+    def other_seeds(name, mode_):
+        out = {}
+        for s in seeds:
+            if s == args.seed:
+                continue
+            try:
+                r, l, _ = measure_config(args, name, s, D, sampler, traffic, region_steps(name), full=False, shard_mode=mode_)
+                l.close()
+                del l
+                torch.cuda.empty_cache()
+                out[str(s)] = {"ms_per_step": r["ms_per_step"], "stitch_ms": r["stitch_ms"], "patch_ms": r["patch_ms"],
+                               "stitch_frac": r["roofline"]["frac"] if r["roofline"] else None,
+                               "patch_frac": r["roofline"]["patch_attention"]["frac"] if r["roofline"] else None}
+            except Exception as e:
+                out[str(s)] = {"error": repr(e)}
+        return out
+
+    if not args.no_seeds:
+        configs[head_name]["seeds"].update(other_seeds(head_name, mode))
+    # ---- the other configurations -------------------------------------------------------------------
+    if not single:
+        for name in ALL_CONFIGS:
+            if name == head_name:
+                continue
+            c = synth.CONFIGS[name]
+            m = "none" if D.world == 1 else ("head" if c.n_kv_heads % D.world == 0 else "replica")
+            try:
+                r, l, _ = measure_config(args, name, args.seed, D, sampler, traffic, region_steps(name), full=True, shard_mode=m)
+                l.close()
+                del l
+                torch.cuda.empty_cache()
+                if "prefill_compare" in r:
+                    res["prefill_compare"] = r["prefill_compare"]
+                configs[name] = {k: v for k, v in r.items() if not k.startswith("_")}
+                configs[name]["seeds"] = {str(args.seed): {"ms_per_step": r["ms_per_step"], "stitch_ms": r["stitch_ms"], "patch_ms": r["patch_ms"]}}
+                if not args.no_seeds:
+                    configs[name]["seeds"].update(other_seeds(name, m))
+            except Exception as e:
+                configs[name] = {"error": repr(e)}
+        if D.rank == 0:
+            try:
+                configs["C1"] = c1_latency(args, D, args.seed)
+            except Exception as e:
+                configs["C1"] = {"error": repr(e)}
+    res["configs"] = configs
+    if sampler:
+        sampler.stop()
+    D.close()
+    return res if D.rank == 0 else None
 
 
 # --------------------------------------------------------------------------------------------------
@@ -577,16 +871,20 @@ def sample_shape(cfg, wl, seed, lib_segments, budget_s):
 def cpu_baseline(cfg, wl, seed, lib_segments, budget_s=15.0):
     layers, heads = sample_shape(cfg, wl, seed, lib_segments, budget_s)
     secs, nbytes, desc = oracle_sample(cfg, wl, seed, lib_segments, layers, heads)
-    return {"value": nbytes / secs / 1e9, "unit": "GB/s (algorithmic, whole graft)", "cores": blas_threads(),
+    return {"value": nbytes / secs / 1e9, "unit": UNIT, "cores": blas_threads(),
             "host_cpus": os.cpu_count(), "kind": "oracle", "seconds": secs,
             "sample": desc + "; numpy fp64 (elementwise single-threaded, BLAS matvec multi-threaded)"}
 
 
-def run_reference(args, cfg, wl, seed):
+def run_reference(args):
     """--impl reference: the oracle IS the reference for this paper.  Rank 0 only.  Each of the K steps is the
-    same bounded sample, sized so that warmup + K steps take about two minutes."""
+    same bounded sample of the headline workload, sized so that warmup + K steps take about two minutes."""
     if int(os.environ.get("RANK", "0")) != 0:
         return None
+    name = args.config if args.config != "all" else HEADLINE
+    cfg = synth.CONFIGS[name]
+    wl = synth.make_workload(cfg, args.seed)
+    seed = args.seed
     cache = {}
 
     def segs(s):
@@ -603,15 +901,26 @@ def run_reference(args, cfg, wl, seed):
             times.append(secs)
     ms = float(np.mean(times)) * 1e3
     val = nbytes / (ms * 1e-3) / 1e9
-    unit = "GB/s (algorithmic, whole graft)"
-    cb = {"value": val, "unit": unit, "cores": blas_threads(), "host_cpus": os.cpu_count(),
+    cb = {"value": val, "unit": UNIT, "cores": blas_threads(), "host_cpus": os.cpu_count(),
           "kind": "oracle", "sample": "each step = " + desc}
-    return {"impl": "reference", "metric": METRIC, "value": val, "unit": unit,
+    return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT,
             "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{cfg.name} ({args.config}); CPU oracle, each step = {layers} layer(s) x {heads} kv head(s) of task 0"},
-            "cpu_baseline": cb, "e2e": {"value": val, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "config": {"workload": f"{cfg.name} ({name}); CPU oracle, each step = {layers} layer(s) x {heads} kv head(s) of task 0"},
+            "cpu_baseline": cb, "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
+
+
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` outside torchrun: start N ranks (one per GPU) through torch.distributed.run and pass
+    the child's output through.  Rank 0 prints the JSON line."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -619,26 +928,31 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C2", choices=sorted(synth.CONFIGS))
-    ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--config", default="all", choices=["all"] + sorted(synth.CONFIGS),
+                    help="all (default): headline C4 plus C2, C3, C5 and C1 in the `configs` key; or one configuration only")
+    ap.add_argument("--seed", type=int, default=1, help="layout seed of the headline numbers")
+    ap.add_argument("--seeds", default="1,2,3", help="layout seeds reported per configuration (the paper's seeds)")
+    ap.add_argument("--no-seeds", action="store_true", help="skip the other layout seeds")
     ap.add_argument("--page-size", type=int, default=0, choices=[0, 8, 16, 32, 64],
                     help="override the config's page size (secondary measurement; default: the config's 16)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--shard", default="auto", choices=["auto", "weak", "task", "head", "replica"],
+                    help="multi-GPU: weak = 32 x N tasks LPT-balanced (default for the batched config), task / head = split the "
+                         "single-GPU workload by task / kv head (strong scaling), replica = N identical copies")
+    ap.add_argument("--devices", default="own", choices=["own", "same"],
+                    help="own: rank r uses cuda:LOCAL_RANK over NCCL; same: every rank uses cuda:0 with gloo for the control plane "
+                         "(exercises the multi-rank code on a 1-GPU box; the ranks' kernels never wait on one another)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--prefill-compare", action="store_true",
-                    help="also time causal prefill attention over the task's whole length (C5's comparison)")
-    ap.add_argument("--no-next", action="store_true", help="skip the NEXT-row timings (shift, extract, decode)")
-    ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per stitch launch, if known (profiles/)")
+    ap.add_argument("--no-prefill-compare", action="store_true", help="skip C5's graft-vs-prefill comparison")
+    ap.add_argument("--no-next", action="store_true", help="skip the NEXT-row timings (shift, extract, decode, plans)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
-    cfg = synth.CONFIGS[args.config]
-    if args.page_size:
-        cfg = synth.scaled(cfg, page_size=args.page_size)
-    wl = synth.make_workload(cfg, args.seed)
     if args.impl == "reference":
-        res = run_reference(args, cfg, wl, args.seed)
+        res = run_reference(args)
     else:
-        res = run_cuda(args, cfg, wl, args.seed)
+        if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+            sys.exit(spawn_ranks(args))
+        res = run_cuda(args)
     if res is not None:
         print(json.dumps(res))
 

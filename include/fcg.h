@@ -1,7 +1,7 @@
 /* fcg.h -- C ABI of the B200-native FCGRAFT KV-cache grafting library (libfcg.so).
  *
  * What the calls compute is defined by the paper (PAPER.md = the text of arxiv/paper_2606_13097)
- * and, where the paper is silent, by the readings R1..R23 in DESIGN.md:
+ * and, where the paper is silent, by the readings R1..R29 in DESIGN.md:
  *
  *   segment library   the KV half of the two-tier code cache H = (I, C), Eq. (2), PAPER.md:66-79:
  *                     per function a cached K/V state that can be re-injected "without being tied
@@ -16,13 +16,20 @@
  *
  * Conventions
  *   - Plain C, no exceptions cross the boundary.  Every call returns an fcg_status_t; on a non-OK
- *     status fcg_last_error() holds a message and the library state is unchanged (host-side
- *     validation happens before any allocation or launch: allocate-then-commit).
+ *     status fcg_last_error() (thread-local, R28) holds a message and the library state is unchanged:
+ *     every host-side check of a call happens before any allocation, copy or launch
+ *     (allocate-then-commit).  FCG_ERR_CUDA is the exception: a CUDA runtime failure in the middle of a
+ *     call may leave work enqueued.
  *   - "device" pointers are CUDA device pointers valid on the library's device; "host" pointers are
- *     ordinary host memory read only during the call (unless stated otherwise).
+ *     ordinary host memory read only during the call (unless stated otherwise).  Every call makes the
+ *     library's device current for its own duration and puts the caller's current device back.
  *   - All device work is enqueued on the given `stream` (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream).  Calls return after enqueueing.  Calls on one library must come from
- *     one thread at a time, and work on one task must be issued on one stream (or externally ordered).
+ *     one thread at a time.  Streams (R29): the scratch area, the plan blobs and recycled pages are
+ *     library-wide, so a call issued on another stream than the previous call on this library first
+ *     waits (one event) for that call's device work; consecutive calls on one stream pay nothing.
+ *     The exception is fcg_segment_release, which enqueues nothing (see there), and calls made while
+ *     the stream is being captured into a CUDA graph (only fcg_patch_planned may be: see there).
  *   - bf16 everywhere for K, V, q, out (2 bytes/element, the bit layout of __nv_bfloat16).
  *   - The library owns everything inside `arena` (page pool, page tables, segments, workspace); the
  *     caller owns the arena allocation itself and all q/k/v/out buffers.
@@ -67,7 +74,7 @@ typedef struct {
   int32_t n_layers;
   int32_t n_q_heads;       /* multiple of n_kv_heads */
   int32_t n_kv_heads;
-  int32_t head_dim;        /* 64 or 128 */
+  int32_t head_dim;        /* 64 or 128 (R27) */
   int32_t page_size;       /* tokens per page: 8, 16, 32 or 64 */
   int32_t rope_mode;       /* FCG_ROPE_NONE: stitch is a pure gather; FCG_ROPE_HALF_SPLIT: pairs (j, j + head_dim/2) (R2);
                               FCG_ROPE_INTERLEAVED: pairs (2j, 2j + 1) */
@@ -77,7 +84,8 @@ typedef struct {
   uint64_t arena_bytes;
   int32_t max_segments;
   int32_t max_tasks;
-  int32_t max_task_tokens; /* largest capacity a single task may have */
+  int32_t max_task_tokens; /* largest length a single task may reach (sizes the per-task page table); a task may grow up
+                              to it by appending patches (R25) */
   uint32_t n_pages;        /* pages in the pool, shared by all live tasks */
   uint64_t workspace_bytes;/* 0 -> 256 MiB */
   int32_t device;          /* CUDA device ordinal the arena lives on */
@@ -115,7 +123,8 @@ typedef struct {
   int32_t n_entries;
   const fcg_hole_t *holes;          /* host; may be NULL if n_holes == 0 */
   int32_t n_holes;
-  int32_t capacity_tokens;          /* 0 -> max end of entries/holes; pages are reserved for the capacity */
+  int32_t capacity_tokens;          /* 0 -> max end of entries/holes; pages are reserved for the capacity.  A reservation,
+                                       not a limit: later patches may append beyond it (R25) */
 } fcg_plan_t;
 
 /* S2 + S3 (Eq. 4).  For every plan: validates it (R5-R7: 0 <= src_begin, n > 0, src_begin + n <= n_seg,
@@ -133,12 +142,18 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
 /* S4 + S5/S6 (Eq. 6).  q [n_layers][n][n_q_heads][head_dim], k, v [n_layers][n][n_kv_heads][head_dim],
  * out [n_layers][n][n_q_heads][head_dim]: device bf16, contiguous, for cache layers
  * [layer_begin, layer_begin + n_layers).  k (and q) are already position-encoded by the caller (R13).
- * positions: host int32[n], strictly increasing, < capacity.  For each layer the n fresh K/V rows are
+ * positions: host int32[n], strictly increasing, in [0, max_task_tokens).  Positions at or beyond the task's
+ * capacity APPEND (R25): the task grows to positions[n-1] + 1 and takes the missing pages from the
+ * pool at the time of the call (ascending logical order, tasks of a batch in array order; OUT_OF_PAGES leaves
+ * everything unchanged) -- so a caller can decode the x_mid of Eq. 6 token by token without knowing its length.
+ * For each layer the n fresh K/V rows are
  * written to the slots of `positions` (bit copy), then for each patch token i and q-head h
  *     out[i][h] = softmax_{x <= positions[i]}(q[i][h] . K[x][h / G] / sqrt(head_dim)) V[x][h / G],   G = n_q_heads / n_kv_heads
  * with fp32 softmax/accumulation, bf16 result.  Every x <= positions[n-1] must be filled (stitched, or
- * patched by this or an earlier call), else UNFILLED.  Rows per KV head R = n * G selects the kernel:
- * split-KV warp-MMA path, or tcgen05/TMEM tiles for large R. */
+ * patched by this or an earlier call), else UNFILLED (a gap between the old end and an appended position is a hole,
+ * not an append).  The kernel is chosen by fcg_set_attn_policy (default: tcgen05 / TMEM tiles whenever the geometry
+ * has them, the split-KV warp-MMA kernel otherwise).  Not capturable into a CUDA graph (the call uploads a plan blob
+ * from pinned host memory): see fcg_patch_plan_create. */
 fcg_status_t fcg_patch(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers,
                        const void *q, const void *k, const void *v, const int32_t *positions, int32_t n,
                        void *out, void *stream);
@@ -175,6 +190,24 @@ fcg_status_t fcg_patch_batch_host(fcg_library_t *lib, const int32_t *task_ids, c
                                   int32_t n_tasks, int32_t layer_begin, int32_t n_layers, const void *q,
                                   const void *k, const void *v, const int32_t *positions, void *out, void *stream);
 
+/* Patch plans: the per-layer call pattern of a real model without per-call host work, and CUDA-graph capture.
+ * fcg_patch_plan_create does everything of fcg_patch_batch that does not depend on the tensors -- validation (R6),
+ * growth (R25), split selection for calls of `layers_per_call` layers, the upload of positions / descriptors into a
+ * device range of the plan's own (taken from the segment arena; OUT_OF_ARENA), and the COMMIT of the fill state:
+ * the positions count as filled from here on, the caller runs the plan for every layer before relying on them.
+ * fcg_patch_planned then only launches scatter -> attention (-> combine) for layers [layer_begin, layer_begin +
+ * n_layers) with q, k, v, out as in fcg_patch_batch; it may be called any number of times, with any tensors, and
+ * may be captured into a CUDA graph (it makes no copies and touches no host state besides launch statistics; while
+ * the stream is capturing, the stream-ordering rule above is skipped and the caller orders the graph against other
+ * work on the library).  BAD_TASK if a task of the plan was released or re-stitched since.  Destroy returns the
+ * device range; the caller guarantees no enqueued work still reads it. */
+typedef struct fcg_patch_plan fcg_patch_plan_t;
+fcg_status_t fcg_patch_plan_create(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task, int32_t n_tasks,
+                                   const int32_t *positions, int32_t layers_per_call, void *stream, fcg_patch_plan_t **out);
+fcg_status_t fcg_patch_planned(fcg_library_t *lib, fcg_patch_plan_t *plan, int32_t layer_begin, int32_t n_layers,
+                               const void *q, const void *k, const void *v, void *out, void *stream);
+fcg_status_t fcg_patch_plan_destroy(fcg_library_t *lib, fcg_patch_plan_t *plan);
+
 /* Device pointer to the task's page table (int32[n_pages], logical page -> physical page id), its page
  * count and current token count T (max end of stitched/declared/patched ranges).  Token x lives at
  * (table[x / page_size], x % page_size). */
@@ -190,7 +223,9 @@ fcg_status_t fcg_task_page_table_host(fcg_library_t *lib, int32_t task_id, int32
  * a filled position overwrites it, R14).  Describes the stitch; later fcg_task_shift moves are not tracked. */
 fcg_status_t fcg_task_boundary_positions(fcg_library_t *lib, int32_t task_id, int32_t width, int32_t *out, int32_t cap,
                                          int32_t *n_out);
-/* Returns the task's pages to the pool (pushed so that they are re-issued in ascending logical order). */
+/* Returns the task's pages to the pool (pushed so that they are re-issued in ascending logical order).  Enqueues
+ * nothing: work still in flight on the task is protected by the stream rule above (the next call that could reuse
+ * the pages on another stream waits for it). */
 fcg_status_t fcg_task_release(fcg_library_t *lib, int32_t task_id);
 
 /* Two-tier residency (Eq. 3; transfer cost in Table 19).
@@ -211,8 +246,9 @@ fcg_status_t fcg_segment_info(fcg_library_t *lib, int32_t seg_id, int32_t *n_tok
  * moves cache positions [src_begin, src_begin + n_tokens) of a live task to [dst_begin, dst_begin + n_tokens),
  * all layers and kv heads: keys re-rotated by delta = dst_begin - src_begin (the stitch rule R1; bit copy for
  * FCG_ROPE_NONE), values bit-copied.  Source positions become unfilled, destination positions filled (filled
- * destination positions are overwritten); T never shrinks.  Both ranges must lie inside the task's capacity
- * (RANGE) and every source position must be filled (UNFILLED).  The ranges may overlap: every logical page the
+ * destination positions are overwritten); T never shrinks.  The source must lie inside the task's capacity and the
+ * destination inside [0, max_task_tokens) (RANGE); a destination beyond the capacity grows the task like an appending
+ * patch (R25: gap pages, then destination pages, ascending).  Every source position must be filled (UNFILLED).  The ranges may overlap: every logical page the
  * destination touches is given a fresh page from the pool (ascending logical order; OUT_OF_PAGES if the pool
  * cannot supply them), slots of those pages outside the destination keep their contents, and the replaced pages
  * return to the pool by the rule of fcg_task_release -- so the task's page table changes.  delta == 0 is a
@@ -246,8 +282,9 @@ typedef struct {
 fcg_status_t fcg_pool_info(fcg_library_t *lib, fcg_pool_info_t *out);
 
 /* Kernel selection for patch attention: calls whose largest task has R = n * G >= tc_min_rows query rows per
- * kv head (and head_dim 128) use the tcgen05/TMEM kernel, others the split-KV warp-MMA kernel.  Default 64
- * (north_star: tensor-core tiles only for dense patches); 0 = always tcgen05, INT32_MAX = never.
+ * kv head use the tcgen05/TMEM kernel, others the split-KV warp-MMA kernel.  Default 1: tcgen05 for every R
+ * (measured faster than the split-KV kernel down to a decode step, DESIGN.md section 6 -- north_star expected the
+ * opposite for short patches); INT32_MAX = never.
  * force_splits > 0 fixes the number of KV splits per task (clamped to the task's 64-token tile count);
  * 0 = the library's wave-filling choice.  The result does not depend on either knob beyond summation order
  * (P11, split invariance). */

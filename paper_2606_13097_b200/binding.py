@@ -96,6 +96,9 @@ SYMBOLS = {
     "fcg_patch_rope": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
     "fcg_patch_batch": (_I, [_P, _PI, _PI, _I, _I, _I, _P, _P, _P, _PI, _P, _P]),
     "fcg_patch_batch_host": (_I, [_P, _PI, _PI, _I, _I, _I, _P, _P, _P, _PI, _P, _P]),
+    "fcg_patch_plan_create": (_I, [_P, _PI, _PI, _I, _PI, _I, _P, C.POINTER(_P)]),
+    "fcg_patch_planned": (_I, [_P, _P, _I, _I, _P, _P, _P, _P, _P]),
+    "fcg_patch_plan_destroy": (_I, [_P, _P]),
     "fcg_task_page_table": (_I, [_P, _I, C.POINTER(_P), _PI, _PI]),
     "fcg_task_page_table_host": (_I, [_P, _I, _PI, _I, _PI]),
     "fcg_task_release": (_I, [_P, _I]),
@@ -275,6 +278,23 @@ def fcg_patch_batch_host(handle, task_ids, n_per_task, layer_begin, n_layers, q,
     _check(load().fcg_patch_batch_host(handle, ids.ctypes.data_as(_PI), npt.ctypes.data_as(_PI), int(ids.size),
                                        int(layer_begin), int(n_layers), _ptr(q), _ptr(k), _ptr(v),
                                        pos.ctypes.data_as(_PI), _ptr(out), _stream(stream)))
+
+
+def fcg_patch_plan_create(handle, task_ids, n_per_task, positions, layers_per_call, stream=None) -> int:
+    ids, npt, pos = _i32(task_ids), _i32(n_per_task), _i32(positions)
+    h = _P()
+    _check(load().fcg_patch_plan_create(handle, ids.ctypes.data_as(_PI), npt.ctypes.data_as(_PI), int(ids.size),
+                                        pos.ctypes.data_as(_PI), int(layers_per_call), _stream(stream), C.byref(h)))
+    return h.value
+
+
+def fcg_patch_planned(handle, plan, layer_begin, n_layers, q, k, v, out, stream=None) -> None:
+    _check(load().fcg_patch_planned(handle, plan, int(layer_begin), int(n_layers), _ptr(q), _ptr(k), _ptr(v), _ptr(out),
+                                    _stream(stream)))
+
+
+def fcg_patch_plan_destroy(handle, plan) -> None:
+    _check(load().fcg_patch_plan_destroy(handle, plan))
 
 
 def fcg_task_page_table(handle, task_id):
@@ -486,6 +506,16 @@ class FcgLibrary:
         assert not q.is_cuda and q.is_contiguous() and k.is_contiguous() and v.is_contiguous() and out.is_contiguous()
         fcg_patch_batch_host(self.handle, task_ids, n_per_task, layer_begin, q.shape[0], q, k, v, positions, out, stream)
         return out
+
+    def patch_plan_create(self, task_ids, n_per_task, positions, layers_per_call, stream=None) -> int:
+        return fcg_patch_plan_create(self.handle, task_ids, n_per_task, positions, layers_per_call, stream)
+
+    def patch_planned(self, plan, layer_begin, q, k, v, out, stream=None) -> torch.Tensor:
+        fcg_patch_planned(self.handle, plan, layer_begin, q.shape[0], q, k, v, out, stream)
+        return out
+
+    def patch_plan_destroy(self, plan) -> None:
+        fcg_patch_plan_destroy(self.handle, plan)
 
     def task_page_table(self, task_id):
         return fcg_task_page_table(self.handle, task_id)

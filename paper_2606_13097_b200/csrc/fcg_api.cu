@@ -40,7 +40,6 @@ constexpr uint64_t ALIGN = 256;
 constexpr int BLOB_SLOTS = 16;
 constexpr uint64_t BLOB_BYTES = 1ull << 20;
 constexpr int KV_TILE = 64;          // tokens per attention tile (fcg_attn_split.cu BN)
-constexpr int N_SMS = 148;
 
 uint64_t align_up(uint64_t x, uint64_t a = ALIGN) { return (x + a - 1) / a * a; }
 
@@ -53,6 +52,7 @@ struct SegmentRec {
 
 struct TaskRec {
   bool live = false;
+  uint32_t gen = 0;                 // bumped when the task is stitched or released (validates patch plans)
   std::vector<int32_t> pages;
   int32_t capacity = 0, n_tokens = 0;
   std::vector<uint8_t> filled;
@@ -93,13 +93,23 @@ struct fcg_library {
   // (the staging area belongs to patch calls only), so they overlap a stitch enqueued just before on the caller's stream
   cudaStream_t copy_stream = nullptr, d2h_stream = nullptr;
   static constexpr int HOST_GROUPS = 4;          // layer groups of a host call: copy in / attend / copy out pipelined
-  cudaEvent_t last_patch_ev = nullptr, h2d_ev[HOST_GROUPS] = {}, attn_ev[HOST_GROUPS] = {}, d2h_ev = nullptr;
-  bool have_last_patch = false;
+  cudaEvent_t h2d_ev[HOST_GROUPS] = {}, attn_ev[HOST_GROUPS] = {}, d2h_ev = nullptr;
+  // DESIGN.md R29: scratch area, plan blobs and recycled pages are library-wide, so a call issued on another stream than
+  // the previous call first waits for that call's device work (last_ev, recorded at the end of every enqueueing call)
+  cudaEvent_t last_ev = nullptr;
+  cudaStream_t last_stream = nullptr;
+  bool have_last = false;
+  int n_sms = 148;                               // SMs of cfg.device (split selection)
+  uint32_t task_gen = 0;
   // the plan blob of the last patch call: a call that produces the same bytes (the same patch issued for the next layer)
   // reuses the copy that is already on the device instead of uploading it again
   std::vector<unsigned char> patch_blob_copy;
   int patch_blob_slot = -1;
   uint64_t patch_blob_gen = 0;
+  cudaStream_t patch_blob_stream = nullptr;      // the stream that uploaded it (reuse only on the same stream)
+  cudaEvent_t staging_ev = nullptr;              // last use of the host-call staging area
+  bool have_staging_ev = false;
+  int n_plans_live = 0;
   int next_slot = 0;
   fcg_stats_t stats;
   int n_segments_live = 0, n_tasks_live = 0;
@@ -175,6 +185,68 @@ fcg_status_t make_pool_tensor_map(const fcg_config_t &c, void *pool, fcg::TmaDes
   if (r != CUDA_SUCCESS) return fail(FCG_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
   return FCG_OK;
 }
+
+// Every API call runs with the library's device current and puts the caller's device back on return.
+struct DeviceGuard {
+  int prev = -1;
+  bool changed = false;
+  cudaError_t err;
+  explicit DeviceGuard(int dev) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != dev) {
+      err = cudaSetDevice(dev);
+      changed = err == cudaSuccess;
+    }
+  }
+  ~DeviceGuard() {
+    if (changed) cudaSetDevice(prev);
+  }
+};
+#define FCG_DEVICE(lib)                \
+  DeviceGuard dg__((lib)->cfg.device); \
+  if (dg__.err != cudaSuccess) return fail(FCG_ERR_CUDA, "cudaSetDevice(%d): %s", (lib)->cfg.device, cudaGetErrorString(dg__.err))
+
+// R29: order this call after the previous call's device work when the stream changes.  A capturing stream takes
+// no part in it (events recorded inside a capture cannot be waited for outside): only fcg_patch_planned may be
+// captured, and the caller orders the graph against other work on the library.
+fcg_status_t order_after_previous(fcg_library *lib, cudaStream_t stream, bool *capturing) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess) {
+    cudaGetLastError();
+    cs = cudaStreamCaptureStatusNone;
+  }
+  *capturing = cs != cudaStreamCaptureStatusNone;
+  if (!*capturing && lib->have_last && stream != lib->last_stream) FCG_CUDA(cudaStreamWaitEvent(stream, lib->last_ev, 0));
+  return FCG_OK;
+}
+fcg_status_t mark_last(fcg_library *lib, cudaStream_t stream) {
+  FCG_CUDA(cudaEventRecord(lib->last_ev, stream));
+  lib->last_stream = stream;
+  lib->have_last = true;
+  return FCG_OK;
+}
+// calls that upload a plan blob from pinned host memory cannot be captured into a CUDA graph (a replay would re-read
+// host memory that has been reused since)
+#define FCG_ORDER(lib, stream)                                                                                          \
+  do {                                                                                                                  \
+    bool cap__ = false;                                                                                                 \
+    fcg_status_t st__ = order_after_previous((lib), (stream), &cap__);                                                  \
+    if (st__ != FCG_OK) return st__;                                                                                    \
+    if (cap__)                                                                                                          \
+      return fail(FCG_ERR_INVALID_ARG, "this call cannot be captured into a CUDA graph (it uploads a plan blob): use "   \
+                                       "fcg_patch_plan_create + fcg_patch_planned");                                    \
+  } while (0)
+
+// A blob slot in use by one call: whatever path the call leaves by, once anything that reads the slot has been
+// enqueued the slot's event is recorded, so the pinned blob is not rewritten under a copy in flight.
+struct SlotUse {
+  BlobSlot *slot = nullptr;
+  cudaStream_t stream = nullptr;
+  bool enqueued = false;
+  ~SlotUse() {
+    if (slot && enqueued && cudaEventRecord(slot->ev, stream) == cudaSuccess) slot->in_flight = true;
+  }
+};
 
 // acquire a blob slot whose previous consumer kernels have finished
 fcg_status_t acquire_slot(fcg_library *lib, BlobSlot **out) {
@@ -329,19 +401,22 @@ struct GatherBuilder {
 };
 
 struct GatherBlob {
+  SlotUse use;
   BlobSlot *slot = nullptr;
   uint64_t off_pages = 0;
 };
 
-// pack the builder into a blob slot, ship it, launch the kernel; page ids sit at out.off_pages of the slot
+// pack the builder into a blob slot, ship it, launch the kernel; page ids sit at out.off_pages of the slot.  The
+// slot's event is recorded when `out` goes out of scope (SlotUse), after whatever else the caller enqueues from it.
 fcg_status_t enqueue_gather(fcg_library *lib, const GatherBuilder &gb, cudaStream_t stream, GatherBlob &out) {
   const fcg_config_t &c = lib->cfg;
   if (gb.blob_bytes() > BLOB_BYTES) return fail(FCG_ERR_OUT_OF_ARENA, "plan blob of %llu bytes exceeds %llu", (unsigned long long)gb.blob_bytes(), (unsigned long long)BLOB_BYTES);
   if ((uint64_t)c.n_pages * c.n_kv_heads * c.page_size > 0x7fffffffull) return fail(FCG_ERR_INVALID_ARG, "pool too large for 32-bit row offsets");
-  FCG_CUDA(cudaSetDevice(c.device));
   BlobSlot *slot = nullptr;
   fcg_status_t st = acquire_slot(lib, &slot);
   if (st != FCG_OK) return st;
+  out.use.slot = slot;
+  out.use.stream = stream;
   BlobWriter bw(slot->host, BLOB_BYTES);
   const uint64_t off_entries = bw.reserve(gb.entries.size() * sizeof(fcg::StitchEntryDev));
   const uint64_t off_chunks = bw.reserve(gb.chunks.size() * sizeof(fcg::StitchChunkDev));
@@ -351,7 +426,10 @@ fcg_status_t enqueue_gather(fcg_library *lib, const GatherBuilder &gb, cudaStrea
   if (!gb.chunks.empty()) memcpy(slot->host + off_chunks, gb.chunks.data(), gb.chunks.size() * sizeof(fcg::StitchChunkDev));
   if (!gb.pages.empty()) memcpy(slot->host + off_pages, gb.pages.data(), gb.pages.size() * sizeof(int32_t));
   if (!gb.table.empty()) memcpy(slot->host + off_table, gb.table.data(), gb.table.size() * sizeof(float4));
-  if (bw.used > 0) FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, bw.used, cudaMemcpyHostToDevice, stream));
+  if (bw.used > 0) {
+    FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, bw.used, cudaMemcpyHostToDevice, stream));
+    out.use.enqueued = true;
+  }
   fcg::StitchParams sp;
   sp.entries = reinterpret_cast<const fcg::StitchEntryDev *>(slot->dev + off_entries);
   sp.chunks = reinterpret_cast<const fcg::StitchChunkDev *>(slot->dev + off_chunks);
@@ -366,12 +444,6 @@ fcg_status_t enqueue_gather(fcg_library *lib, const GatherBuilder &gb, cudaStrea
   }
   out.slot = slot;
   out.off_pages = off_pages;
-  return FCG_OK;
-}
-
-fcg_status_t finish_gather(GatherBlob &gbl, cudaStream_t stream) {
-  FCG_CUDA(cudaEventRecord(gbl.slot->ev, stream));
-  gbl.slot->in_flight = true;
   return FCG_OK;
 }
 
@@ -406,10 +478,15 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
   int n_dev = 0;
   FCG_CUDA(cudaGetDeviceCount(&n_dev));
   if (cfg->device < 0 || cfg->device >= n_dev) return fail(FCG_ERR_INVALID_ARG, "device %d out of range", cfg->device);
-  FCG_CUDA(cudaSetDevice(cfg->device));
+  DeviceGuard dg(cfg->device);
+  if (dg.err != cudaSuccess) return fail(FCG_ERR_CUDA, "cudaSetDevice(%d): %s", cfg->device, cudaGetErrorString(dg.err));
 
   fcg_library *lib = new fcg_library();
   lib->cfg = *cfg;
+  if (cudaDeviceGetAttribute(&lib->n_sms, cudaDevAttrMultiProcessorCount, cfg->device) != cudaSuccess || lib->n_sms <= 0) {
+    cudaGetLastError();
+    lib->n_sms = 148;
+  }
   lib->cfg.workspace_bytes = l.ws_bytes;
   const int half = cfg->head_dim / 2;
   lib->inv_freq.resize(half);
@@ -449,7 +526,8 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
   {
     cudaError_t e = cudaStreamCreateWithFlags(&lib->copy_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&lib->d2h_stream, cudaStreamNonBlocking);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->last_patch_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->last_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->staging_ev, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->d2h_ev, cudaEventDisableTiming);
     for (int g = 0; g < fcg_library::HOST_GROUPS && e == cudaSuccess; ++g) {
       e = cudaEventCreateWithFlags(&lib->h2d_ev[g], cudaEventDisableTiming);
@@ -487,7 +565,7 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
 
 fcg_status_t fcg_library_destroy(fcg_library_t *lib) {
   if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
-  cudaSetDevice(lib->cfg.device);
+  DeviceGuard dg(lib->cfg.device);
   cudaDeviceSynchronize();
   for (int i = 0; i < BLOB_SLOTS; ++i) {
     if (lib->slots[i].host) cudaFreeHost(lib->slots[i].host);
@@ -495,7 +573,8 @@ fcg_status_t fcg_library_destroy(fcg_library_t *lib) {
   }
   if (lib->copy_stream) cudaStreamDestroy(lib->copy_stream);
   if (lib->d2h_stream) cudaStreamDestroy(lib->d2h_stream);
-  if (lib->last_patch_ev) cudaEventDestroy(lib->last_patch_ev);
+  if (lib->last_ev) cudaEventDestroy(lib->last_ev);
+  if (lib->staging_ev) cudaEventDestroy(lib->staging_ev);
   if (lib->d2h_ev) cudaEventDestroy(lib->d2h_ev);
   for (int g = 0; g < fcg_library::HOST_GROUPS; ++g) {
     if (lib->h2d_ev[g]) cudaEventDestroy(lib->h2d_ev[g]);
@@ -538,9 +617,14 @@ fcg_status_t fcg_segment_register(fcg_library_t *lib, const void *k, const void 
   rp.n_kv_heads = c.n_kv_heads;
   rp.n_tokens = n_tokens;
   rp.head_dim = c.head_dim;
-  FCG_CUDA(cudaSetDevice(c.device));
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, static_cast<cudaStream_t>(stream));
   FCG_CUDA(fcg::launch_register_copy(rp, static_cast<cudaStream_t>(stream)));
   lib->stats.register_launches++;
+  {
+    fcg_status_t mst = mark_last(lib, static_cast<cudaStream_t>(stream));
+    if (mst != FCG_OK) return mst;
+  }
 
   commit_segment_slot(lib, sl, n_tokens, orig_start);
   *seg_id_out = sid;
@@ -559,9 +643,14 @@ fcg_status_t fcg_segment_offload(fcg_library_t *lib, int32_t seg_id, void *strea
   if (fi == lib->host_free.size())
     return fail(FCG_ERR_OUT_OF_ARENA, "no free host-tier range of %llu bytes for segment %d", (unsigned long long)s.bytes, seg_id);
   const uint64_t hoff = lib->host_free[fi].off;
-  FCG_CUDA(cudaSetDevice(lib->cfg.device));
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, static_cast<cudaStream_t>(stream));
   FCG_CUDA(cudaMemcpyAsync(lib->host_arena + hoff, lib->arena + s.offset, s.bytes, cudaMemcpyDeviceToHost,
                            static_cast<cudaStream_t>(stream)));
+  {
+    fcg_status_t mst = mark_last(lib, static_cast<cudaStream_t>(stream));
+    if (mst != FCG_OK) return mst;
+  }
   range_take(lib->host_free, fi, s.bytes);
   range_give(lib->seg_free, s.offset, s.bytes);
   s.offset = hoff;
@@ -581,9 +670,14 @@ fcg_status_t fcg_segment_prefetch(fcg_library_t *lib, int32_t seg_id, void *stre
   if (fi == lib->seg_free.size())
     return fail(FCG_ERR_OUT_OF_ARENA, "no free arena range of %llu bytes for segment %d", (unsigned long long)s.bytes, seg_id);
   const uint64_t off = lib->seg_free[fi].off;
-  FCG_CUDA(cudaSetDevice(lib->cfg.device));
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, static_cast<cudaStream_t>(stream));
   FCG_CUDA(cudaMemcpyAsync(lib->arena + off, lib->host_arena + s.offset, s.bytes, cudaMemcpyHostToDevice,
                            static_cast<cudaStream_t>(stream)));
+  {
+    fcg_status_t mst = mark_last(lib, static_cast<cudaStream_t>(stream));
+    if (mst != FCG_OK) return mst;
+  }
   range_take(lib->seg_free, fi, s.bytes);
   range_give(lib->host_free, s.offset, s.bytes);
   s.offset = off;
@@ -720,6 +814,8 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
   }
 
   // ---- enqueue: blob, kernel, page tables -----------------------------------------------------
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, stream);
   GatherBlob gbl;
   fcg_status_t st = enqueue_gather(lib, gb, stream, gbl);
   if (st != FCG_OK) return st;
@@ -728,7 +824,7 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
     FCG_CUDA(cudaMemcpyAsync(dst, gbl.slot->dev + gbl.off_pages + plan_page_base[i] * sizeof(int32_t),
                              (size_t)checked[i].n_pages * sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
   }
-  st = finish_gather(gbl, stream);
+  st = mark_last(lib, stream);
   if (st != FCG_OK) return st;
   const int32_t *pages = gb.pages.data();
 
@@ -737,6 +833,7 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
   for (int i = 0; i < n_plans; ++i) {
     TaskRec &t = lib->tasks[plans[i].task_id];
     t.live = true;
+    t.gen = ++lib->task_gen;
     t.capacity = checked[i].capacity;
     t.n_tokens = checked[i].T;
     t.pages.assign(pages + plan_page_base[i], pages + plan_page_base[i] + checked[i].n_pages);
@@ -759,9 +856,9 @@ namespace {
 
 // choose the number of KV splits for `base` CTAs per split so that waves on the GPU are well filled
 // without paying much for fp32 partials.
-int choose_splits(int64_t base_ctas, int tiles, int rows, int head_dim, int ctas_per_sm) {
+int choose_splits(int64_t base_ctas, int tiles, int rows, int head_dim, int ctas_per_sm, int n_sms) {
   if (tiles <= 1) return 1;
-  const double slots = (double)N_SMS * ctas_per_sm;
+  const double slots = (double)n_sms * ctas_per_sm;
   // everything in bytes streamed by one SM (an SM's share of HBM is ~44 GB/s: 10 us ~ 440 KB)
   const double kFixedPerCta = 6000.0;            // launch + prologue + epilogue of a CTA
   const double kCombineLaunch = 400000.0;        // the extra combine kernel: launch gap + its own ramp
@@ -777,7 +874,7 @@ int choose_splits(int64_t base_ctas, int tiles, int rows, int head_dim, int ctas
     // time ~ waves * (one CTA's K/V stream + its fp32 partial rows), plus what the combine kernel reads and writes
     const double kv_bytes = (double)tiles_per * KV_TILE * head_dim * 4.0;
     const double part_bytes = s > 1 ? (double)rows * (head_dim + 2) * 4.0 : 0.0;
-    const double combine = s > 1 ? kCombineLaunch + ctas * part_bytes / N_SMS : 0.0;
+    const double combine = s > 1 ? kCombineLaunch + ctas * part_bytes / n_sms : 0.0;
     const double cost = waves * (kv_bytes + part_bytes + kFixedPerCta) + combine;
     if (s == 1) cost_1 = cost;
     if (cost < best_cost * 0.999) {
@@ -790,89 +887,166 @@ int choose_splits(int64_t base_ctas, int tiles, int rows, int head_dim, int ctas
   return best_cost < 0.85 * cost_1 ? best : 1;
 }
 
-struct PatchCall {
+// What a patch is, independent of the tensors it is run on: the tasks, their position lists and the layer count per call.
+struct PatchSpec {
   const int32_t *task_ids;
   const int32_t *n_per_task;
   int32_t n_tasks;
+  const int32_t *positions;
+  int32_t n_layers;           // layers per call (split selection, partial sizing)
+};
+
+// the tensors and the layer range of one call
+struct PatchIO {
   int32_t layer_begin, n_layers;
   const void *q, *k, *v;
-  const int32_t *positions;
   void *out;
   cudaStream_t stream;
 };
 
-fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
-  const fcg_config_t &c = lib->cfg;
-  if (!pc.q || !pc.k || !pc.v || !pc.out || !pc.positions || !pc.task_ids || !pc.n_per_task || pc.n_tasks <= 0)
-    return fail(FCG_ERR_INVALID_ARG, "NULL / empty argument");
-  if (pc.layer_begin < 0 || pc.n_layers <= 0 || pc.layer_begin + pc.n_layers > c.n_layers)
-    return fail(FCG_ERR_INVALID_ARG, "layer range [%d, %d) outside [0, %d)", pc.layer_begin, pc.layer_begin + pc.n_layers, c.n_layers);
-  // ---- validate every task before touching anything ------------------------------------------
+struct PatchCheck {
   int64_t n_total = 0;
-  for (int t = 0; t < pc.n_tasks; ++t) {
-    const int32_t id = pc.task_ids[t];
+  std::vector<int32_t> new_capacity;   // per task: capacity after this patch (R25: appends grow the task)
+  std::vector<int32_t> new_pages;      // per task: pages to add
+  int64_t pages_needed = 0;
+};
+
+// Host-side validation of a patch; touches nothing (fcg.h conventions: a failing call leaves the library unchanged and
+// launches nothing).  R6: every position a query sees is filled by earlier work or by this call.  R25: positions at or
+// beyond the capacity append -- the task grows to positions[n-1] + 1 <= max_task_tokens, pages come on demand.
+fcg_status_t validate_patch(fcg_library *lib, const PatchSpec &ps, PatchCheck &ck) {
+  const fcg_config_t &c = lib->cfg;
+  if (!ps.positions || !ps.task_ids || !ps.n_per_task || ps.n_tasks <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty argument");
+  ck.n_total = 0;
+  ck.pages_needed = 0;
+  ck.new_capacity.assign(ps.n_tasks, 0);
+  ck.new_pages.assign(ps.n_tasks, 0);
+  const int P = c.page_size;
+  for (int t = 0; t < ps.n_tasks; ++t) {
+    const int32_t id = ps.task_ids[t];
     if (id < 0 || id >= c.max_tasks || !lib->tasks[id].live) return fail(FCG_ERR_BAD_TASK, "unknown task %d", id);
     for (int u = 0; u < t; ++u)
-      if (pc.task_ids[u] == id) return fail(FCG_ERR_BAD_TASK, "task %d repeated in the batch", id);
-    const int32_t n = pc.n_per_task[t];
+      if (ps.task_ids[u] == id) return fail(FCG_ERR_BAD_TASK, "task %d repeated in the batch", id);
+    const int32_t n = ps.n_per_task[t];
     if (n <= 0) return fail(FCG_ERR_INVALID_ARG, "task %d: n must be > 0", id);
-    const int32_t *pos = pc.positions + n_total;
+    const int32_t *pos = ps.positions + ck.n_total;
     for (int i = 1; i < n; ++i)
       if (pos[i] <= pos[i - 1]) return fail(FCG_ERR_INVALID_ARG, "task %d: positions must be strictly increasing", id);
     const TaskRec &tr = lib->tasks[id];
-    if (pos[0] < 0 || pos[n - 1] >= tr.capacity) return fail(FCG_ERR_RANGE, "task %d: position outside capacity %d", id, tr.capacity);
-    // every x <= pos[n-1] must be filled by earlier work or by this call
+    if (pos[0] < 0 || pos[n - 1] >= c.max_task_tokens)
+      return fail(FCG_ERR_RANGE, "task %d: position outside [0, max_task_tokens = %d)", id, c.max_task_tokens);
+    // every x <= pos[n-1] must be filled by earlier work or by this call (positions beyond the capacity are unfilled)
     int pi = 0;
     for (int32_t x = tr.filled_prefix; x <= pos[n - 1]; ++x) {
       while (pi < n && pos[pi] < x) ++pi;
-      if (!tr.filled[x] && !(pi < n && pos[pi] == x))
+      const bool was = x < tr.capacity && tr.filled[x];
+      if (!was && !(pi < n && pos[pi] == x))
         return fail(FCG_ERR_UNFILLED, "task %d: position %d is visible to a patch query but was never filled", id, x);
     }
-    n_total += n;
+    ck.new_capacity[t] = std::max(tr.capacity, pos[n - 1] + 1);
+    ck.new_pages[t] = std::max<int32_t>(0, (ck.new_capacity[t] + P - 1) / P - (int32_t)tr.pages.size());
+    ck.pages_needed += ck.new_pages[t];
+    ck.n_total += n;
   }
-  if (n_total > (1 << 20)) return fail(FCG_ERR_INVALID_ARG, "too many patch tokens in one call");
+  if (ck.n_total > (1 << 20)) return fail(FCG_ERR_INVALID_ARG, "too many patch tokens in one call");
+  if (ck.pages_needed > (int64_t)lib->page_stack.size())
+    return fail(FCG_ERR_OUT_OF_PAGES, "need %lld pages to grow, %zu free", (long long)ck.pages_needed, lib->page_stack.size());
+  return FCG_OK;
+}
 
-  // ---- blob: positions, per-token table offsets / split counts, task descriptors --------------
-  FCG_CUDA(cudaSetDevice(c.device));
-  BlobSlot *slot = nullptr;
-  fcg_status_t st = acquire_slot(lib, &slot);
-  if (st != FCG_OK) return st;
-  BlobWriter bw(slot->host, BLOB_BYTES);
-  const uint64_t off_pos = bw.reserve(n_total * 4), off_toff = bw.reserve(n_total * 4), off_tspl = bw.reserve(n_total * 4);
-  const uint64_t off_tasks = bw.reserve((uint64_t)pc.n_tasks * sizeof(fcg::AttnTaskDev));
-  const uint64_t off_tasks2 = bw.reserve((uint64_t)pc.n_tasks * sizeof(fcg::AttnTaskDev));   // tcgen05 path: tasks by Q-tile class
-  if (off_pos == UINT64_MAX || off_toff == UINT64_MAX || off_tspl == UINT64_MAX || off_tasks == UINT64_MAX || off_tasks2 == UINT64_MAX)
-    return fail(FCG_ERR_OUT_OF_ARENA, "patch blob exceeds %llu bytes", (unsigned long long)BLOB_BYTES);
-  auto *h_pos = reinterpret_cast<int32_t *>(slot->host + off_pos);
-  auto *h_toff = reinterpret_cast<int32_t *>(slot->host + off_toff);
-  auto *h_tspl = reinterpret_cast<int32_t *>(slot->host + off_tspl);
-  auto *h_tasks = reinterpret_cast<fcg::AttnTaskDev *>(slot->host + off_tasks);
-  memcpy(h_pos, pc.positions, (size_t)n_total * 4);
+fcg_status_t validate_io(fcg_library *lib, const PatchIO &io) {
+  const fcg_config_t &c = lib->cfg;
+  if (!io.q || !io.k || !io.v || !io.out) return fail(FCG_ERR_INVALID_ARG, "NULL / empty argument");
+  if (io.layer_begin < 0 || io.n_layers <= 0 || io.layer_begin + io.n_layers > c.n_layers)
+    return fail(FCG_ERR_INVALID_ARG, "layer range [%d, %d) outside [0, %d)", io.layer_begin, io.layer_begin + io.n_layers, c.n_layers);
+  return FCG_OK;
+}
+
+// Everything the kernels need besides the tensors, as offsets into one blob (positions, per-token table offsets and
+// split counts, task descriptors in call order and grouped by CTA class, page ids of growing tasks) plus the launch
+// shape.  The blob lives in a transient slot (fcg_patch) or in a plan's own device range (fcg_patch_plan_create).
+struct PatchLayout {
+  int64_t n_total = 0;
+  int32_t n_tasks = 0;
+  uint64_t off_pos = 0, off_toff = 0, off_tspl = 0, off_tasks = 0, off_tasks2 = 0, off_grow = 0, used = 0;
+  bool use_tc = false;
+  int max_splits = 1, max_rows = 0, rows_per_cta_split = 64, max_row_groups = 1;
+  int n_cls[3] = {0, 0, 0}, cls_begin[3] = {0, 0, 0}, cls_rgs[3] = {1, 1, 1};
+  struct Grow {
+    int32_t task_id, first_lp, count;
+    int64_t index;            // first page id of this task inside the off_grow region
+  };
+  std::vector<Grow> grows;
+  std::vector<int32_t> grow_pages;
+};
+
+// fills `host` (capacity `cap` bytes) and `lay`; page ids for growth are taken from the top of a COPY of the stack
+fcg_status_t build_patch_blob(fcg_library *lib, const PatchSpec &ps, const PatchCheck &ck, unsigned char *host, uint64_t cap,
+                              PatchLayout &lay) {
+  const fcg_config_t &c = lib->cfg;
+  const int64_t n_total = ck.n_total;
+  BlobWriter bw(host, cap);
+  lay.n_total = n_total;
+  lay.n_tasks = ps.n_tasks;
+  lay.off_pos = bw.reserve(n_total * 4);
+  lay.off_toff = bw.reserve(n_total * 4);
+  lay.off_tspl = bw.reserve(n_total * 4);
+  lay.off_tasks = bw.reserve((uint64_t)ps.n_tasks * sizeof(fcg::AttnTaskDev));
+  lay.off_tasks2 = bw.reserve((uint64_t)ps.n_tasks * sizeof(fcg::AttnTaskDev));   // tcgen05 path: tasks by Q-tile class
+  lay.off_grow = bw.reserve((uint64_t)std::max<int64_t>(ck.pages_needed, 1) * 4);
+  if (lay.off_pos == UINT64_MAX || lay.off_toff == UINT64_MAX || lay.off_tspl == UINT64_MAX || lay.off_tasks == UINT64_MAX ||
+      lay.off_tasks2 == UINT64_MAX || lay.off_grow == UINT64_MAX)
+    return fail(FCG_ERR_OUT_OF_ARENA, "patch blob exceeds %llu bytes", (unsigned long long)cap);
+  lay.used = bw.used;
+  auto *h_pos = reinterpret_cast<int32_t *>(host + lay.off_pos);
+  auto *h_toff = reinterpret_cast<int32_t *>(host + lay.off_toff);
+  auto *h_tspl = reinterpret_cast<int32_t *>(host + lay.off_tspl);
+  auto *h_tasks = reinterpret_cast<fcg::AttnTaskDev *>(host + lay.off_tasks);
+  auto *h_grow = reinterpret_cast<int32_t *>(host + lay.off_grow);
+  memcpy(h_pos, ps.positions, (size_t)n_total * 4);
+  h_grow[0] = 0;
+
+  // R25: page ids of the growing tasks, tasks in array order, ascending logical order
+  lay.grows.clear();
+  lay.grow_pages.clear();
+  {
+    size_t top = lib->page_stack.size();
+    for (int t = 0; t < ps.n_tasks; ++t) {
+      if (ck.new_pages[t] == 0) continue;
+      PatchLayout::Grow g{ps.task_ids[t], (int32_t)lib->tasks[ps.task_ids[t]].pages.size(), ck.new_pages[t], (int64_t)lay.grow_pages.size()};
+      for (int k = 0; k < g.count; ++k) lay.grow_pages.push_back(lib->page_stack[--top]);
+      lay.grows.push_back(g);
+    }
+    if (!lay.grow_pages.empty()) memcpy(h_grow, lay.grow_pages.data(), lay.grow_pages.size() * 4);
+  }
 
   const int G = c.n_q_heads / c.n_kv_heads;
   int max_rows = 0;
-  for (int t = 0; t < pc.n_tasks; ++t) max_rows = std::max(max_rows, pc.n_per_task[t] * G);
+  for (int t = 0; t < ps.n_tasks; ++t) max_rows = std::max(max_rows, ps.n_per_task[t] * G);
+  lay.max_rows = max_rows;
   const bool use_tc = lib->have_tma && max_rows >= lib->tc_min_rows;
+  lay.use_tc = use_tc;
   // tcgen05 path: a task with <= 128 rows per kv head runs CTAs with one 128-row Q tile (deep K/V rings: the
   // HBM-bound regime), a task with more rows CTAs with two (K/V read once per 256 rows).  A batch that mixes
   // both is launched as two grids, one per class.
-  auto rows_per_cta_of = [&](int rows) { return use_tc ? (rows > 128 ? 256 : 128) : (max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64)); };
+  lay.rows_per_cta_split = max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64);
+  auto rows_per_cta_of = [&](int rows) { return use_tc ? (rows > 128 ? 256 : 128) : lay.rows_per_cta_split; };
   const int ctas_per_sm = use_tc ? 1 : fcg::attn_split_ctas_per_sm(c.head_dim);
   int max_splits = 1;
   int64_t tok_off = 0;
-  for (int t = 0; t < pc.n_tasks; ++t) {
-    const int32_t n = pc.n_per_task[t];
-    const int32_t kv_len = pc.positions[tok_off + n - 1] + 1;
+  for (int t = 0; t < ps.n_tasks; ++t) {
+    const int32_t n = ps.n_per_task[t];
+    const int32_t kv_len = ps.positions[tok_off + n - 1] + 1;
     const int tiles = (kv_len + KV_TILE - 1) / KV_TILE;
     const int rows_per_cta = rows_per_cta_of(n * G);
     const int rg = (n * G + rows_per_cta - 1) / rows_per_cta;
-    const int64_t base = (int64_t)rg * c.n_kv_heads * pc.n_layers * pc.n_tasks;
+    const int64_t base = (int64_t)rg * c.n_kv_heads * ps.n_layers * ps.n_tasks;
     int ns = lib->force_splits > 0 ? std::min(lib->force_splits, tiles)
-                                   : choose_splits(base, tiles, std::min(n * G, rows_per_cta), c.head_dim, ctas_per_sm);
+                                   : choose_splits(base, tiles, std::min(n * G, rows_per_cta), c.head_dim, ctas_per_sm, lib->n_sms);
     const int tiles_per = (tiles + ns - 1) / ns;
     ns = (tiles + tiles_per - 1) / tiles_per;      // no empty trailing split
     fcg::AttnTaskDev &d = h_tasks[t];
-    d.table_off = pc.task_ids[t] * lib->pages_per_task;
+    d.table_off = ps.task_ids[t] * lib->pages_per_task;
     d.n = n;
     d.tok_off = (int32_t)tok_off;
     d.kv_len = kv_len;
@@ -886,146 +1060,314 @@ fcg_status_t patch_common(fcg_library *lib, const PatchCall &pc) {
     }
     tok_off += n;
   }
+  lay.max_splits = max_splits;
+  lay.max_row_groups = (max_rows + rows_per_cta_of(max_rows) - 1) / rows_per_cta_of(max_rows);
   // tcgen05 path: the same descriptors again, grouped by CTA class (rows per kv head <= 64 | <= 128 | more)
-  auto *h_tasks2 = reinterpret_cast<fcg::AttnTaskDev *>(slot->host + off_tasks2);
+  auto *h_tasks2 = reinterpret_cast<fcg::AttnTaskDev *>(host + lay.off_tasks2);
   auto class_of = [&](int rows) { return rows <= 64 ? 0 : (rows <= 128 ? 1 : 2); };
-  int n_cls[3] = {0, 0, 0}, cls_begin[3] = {0, 0, 0};
-  for (int t = 0; t < pc.n_tasks; ++t) n_cls[class_of(h_tasks[t].n * G)]++;
-  cls_begin[1] = n_cls[0];
-  cls_begin[2] = n_cls[0] + n_cls[1];
+  for (int cl = 0; cl < 3; ++cl) lay.n_cls[cl] = 0, lay.cls_rgs[cl] = 1;
+  for (int t = 0; t < ps.n_tasks; ++t) lay.n_cls[class_of(h_tasks[t].n * G)]++;
+  lay.cls_begin[0] = 0;
+  lay.cls_begin[1] = lay.n_cls[0];
+  lay.cls_begin[2] = lay.n_cls[0] + lay.n_cls[1];
   {
     int fill[3] = {0, 0, 0};
-    for (int t = 0; t < pc.n_tasks; ++t) {
+    for (int t = 0; t < ps.n_tasks; ++t) {
       const int cl = class_of(h_tasks[t].n * G);
-      h_tasks2[cls_begin[cl] + fill[cl]++] = h_tasks[t];
+      h_tasks2[lay.cls_begin[cl] + fill[cl]++] = h_tasks[t];
+      const int q_tiles = cl == 2 ? 2 : 1;
+      lay.cls_rgs[cl] = std::max(lay.cls_rgs[cl], (h_tasks[t].n * G + 128 * q_tiles - 1) / (128 * q_tiles));
     }
   }
-  // partials live at the start of the scratch area
-  const uint64_t part_rows = (uint64_t)pc.n_layers * max_splits * n_total * c.n_q_heads;
-  const uint64_t part_o_bytes = max_splits > 1 ? align_up(part_rows * c.head_dim * 4) : 0;
-  const uint64_t part_ml_bytes = max_splits > 1 ? align_up(part_rows * 2 * 4) : 0;
+  return FCG_OK;
+}
+
+// bytes of split-KV partials one call of `n_layers` layers needs
+void partial_bytes(const fcg_library *lib, const PatchLayout &lay, int n_layers, uint64_t &part_o_bytes, uint64_t &part_ml_bytes) {
+  const fcg_config_t &c = lib->cfg;
+  const uint64_t part_rows = (uint64_t)n_layers * lay.max_splits * lay.n_total * c.n_q_heads;
+  part_o_bytes = lay.max_splits > 1 ? align_up(part_rows * c.head_dim * 4) : 0;
+  part_ml_bytes = lay.max_splits > 1 ? align_up(part_rows * 2 * 4) : 0;
+}
+
+// R25: page ids of the growing tasks -> their device page tables (before the scatter reads them)
+fcg_status_t enqueue_growth(fcg_library *lib, const PatchLayout &lay, const unsigned char *dev_blob, cudaStream_t stream) {
+  for (const auto &g : lay.grows)
+    FCG_CUDA(cudaMemcpyAsync(lib->tables() + (int64_t)g.task_id * lib->pages_per_task + g.first_lp,
+                             dev_blob + lay.off_grow + (uint64_t)g.index * 4, (size_t)g.count * 4, cudaMemcpyDeviceToDevice, stream));
+  return FCG_OK;
+}
+
+// scatter -> attention (-> combine): kernel launches only
+fcg_status_t launch_patch(fcg_library *lib, const PatchLayout &lay, const unsigned char *dev_blob, const PatchIO &io) {
+  const fcg_config_t &c = lib->cfg;
+  uint64_t part_o_bytes, part_ml_bytes;
+  partial_bytes(lib, lay, io.n_layers, part_o_bytes, part_ml_bytes);
   if (part_o_bytes + part_ml_bytes > lib->scratch_bytes)
-    return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for %d-way split partials (%llu bytes)", max_splits,
+    return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for %d-way split partials (%llu bytes)", lay.max_splits,
                 (unsigned long long)(part_o_bytes + part_ml_bytes));
-
-  {
-    const int cached = lib->patch_blob_slot;
-    if (cached >= 0 && lib->slots[cached].gen == lib->patch_blob_gen && lib->patch_blob_copy.size() == bw.used &&
-        memcmp(lib->patch_blob_copy.data(), slot->host, bw.used) == 0) {
-      // same bytes as the previous patch call and its device copy is intact: hand the fresh slot back, use that one
-      lib->next_slot = (lib->next_slot + BLOB_SLOTS - 1) % BLOB_SLOTS;
-      slot->gen--;
-      slot = &lib->slots[cached];
-    } else {
-      FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, bw.used, cudaMemcpyHostToDevice, pc.stream));
-      lib->patch_blob_copy.assign(slot->host, slot->host + bw.used);
-      lib->patch_blob_slot = (int)(slot - lib->slots);
-      lib->patch_blob_gen = slot->gen;
-    }
-  }
-
+  const int G = c.n_q_heads / c.n_kv_heads;
   fcg::ScatterParams sp;
-  sp.k_new = static_cast<const uint16_t *>(pc.k);
-  sp.v_new = static_cast<const uint16_t *>(pc.v);
+  sp.k_new = static_cast<const uint16_t *>(io.k);
+  sp.v_new = static_cast<const uint16_t *>(io.v);
   sp.k_pool = lib->k_pool();
   sp.v_pool = lib->v_pool();
   sp.tables = lib->tables();
-  sp.positions = reinterpret_cast<const int32_t *>(slot->dev + off_pos);
-  sp.tok_table_off = reinterpret_cast<const int32_t *>(slot->dev + off_toff);
-  sp.n_layers = pc.n_layers;
-  sp.layer_begin = pc.layer_begin;
-  sp.n_total = (int32_t)n_total;
+  sp.positions = reinterpret_cast<const int32_t *>(dev_blob + lay.off_pos);
+  sp.tok_table_off = reinterpret_cast<const int32_t *>(dev_blob + lay.off_toff);
+  sp.n_layers = io.n_layers;
+  sp.layer_begin = io.layer_begin;
+  sp.n_total = (int32_t)lay.n_total;
   sp.n_kv_heads = c.n_kv_heads;
   sp.head_dim = c.head_dim;
   sp.page_size = c.page_size;
   sp.n_pages = c.n_pages;
-  FCG_CUDA(fcg::launch_scatter(sp, pc.stream));
+  FCG_CUDA(fcg::launch_scatter(sp, io.stream));
   lib->stats.scatter_launches++;
 
   fcg::AttnParams ap;
-  ap.q = static_cast<const uint16_t *>(pc.q);
-  ap.out = static_cast<uint16_t *>(pc.out);
+  ap.q = static_cast<const uint16_t *>(io.q);
+  ap.out = static_cast<uint16_t *>(io.out);
   ap.k_pool = lib->k_pool();
   ap.v_pool = lib->v_pool();
   ap.tables = lib->tables();
   ap.positions = sp.positions;
-  ap.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(slot->dev + off_tasks);
-  ap.tok_splits = reinterpret_cast<const int32_t *>(slot->dev + off_tspl);
+  ap.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(dev_blob + lay.off_tasks);
+  ap.tok_splits = reinterpret_cast<const int32_t *>(dev_blob + lay.off_tspl);
   ap.part_o = reinterpret_cast<float *>(lib->arena + lib->scratch_off);
   ap.part_ml = reinterpret_cast<float *>(lib->arena + lib->scratch_off + part_o_bytes);
-  ap.n_total = (int32_t)n_total;
-  ap.n_layers = pc.n_layers;
-  ap.layer_begin = pc.layer_begin;
+  ap.n_total = (int32_t)lay.n_total;
+  ap.n_layers = io.n_layers;
+  ap.layer_begin = io.layer_begin;
   ap.n_q_heads = c.n_q_heads;
   ap.n_kv_heads = c.n_kv_heads;
   ap.group = G;
   ap.page_size = c.page_size;
-  ap.n_tasks = pc.n_tasks;
-  ap.max_splits = max_splits;
-  ap.max_row_groups = (max_rows + rows_per_cta_of(max_rows) - 1) / rows_per_cta_of(max_rows);
+  ap.n_tasks = lay.n_tasks;
+  ap.max_splits = lay.max_splits;
+  ap.max_row_groups = lay.max_row_groups;
   ap.n_pages = c.n_pages;
   ap.scale_log2 = (float)(1.4426950408889634 / sqrt((double)c.head_dim));
-  if (use_tc) {
+  if (lay.use_tc) {
     // class 0: rows replicated 2x / 4x in one softmax warpgroup (HBM-bound; the deep K/V rings matter most);
     // class 1: two tile-parity softmax warpgroups; class 2: two Q tiles per CTA
     // launched longest-CTA class first, so that the tail of the batch is made of the short CTAs
     for (int cl = 2; cl >= 0; --cl) {
-      if (n_cls[cl] == 0) continue;
+      if (lay.n_cls[cl] == 0) continue;
       const int q_tiles = cl == 2 ? 2 : 1, parity_streams = cl == 1 ? 2 : 1;
-      const fcg::AttnTaskDev *cls = h_tasks2 + cls_begin[cl];
-      int rgs = 1;
-      for (int t = 0; t < n_cls[cl]; ++t) rgs = std::max(rgs, (cls[t].n * G + 128 * q_tiles - 1) / (128 * q_tiles));
       fcg::AttnParams apc = ap;
-      apc.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(slot->dev + off_tasks2) + cls_begin[cl];
-      apc.n_tasks = n_cls[cl];
-      apc.max_row_groups = rgs;
-      FCG_CUDA(fcg::launch_attn_tc(apc, c.head_dim, q_tiles, parity_streams, &lib->tm_k, &lib->tm_v, pc.stream));
+      apc.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(dev_blob + lay.off_tasks2) + lay.cls_begin[cl];
+      apc.n_tasks = lay.n_cls[cl];
+      apc.max_row_groups = lay.cls_rgs[cl];
+      FCG_CUDA(fcg::launch_attn_tc(apc, c.head_dim, q_tiles, parity_streams, &lib->tm_k, &lib->tm_v, io.stream));
       lib->stats.attn_tc_launches++;
     }
     lib->stats.last_attn_path = 2;
   } else {
-    FCG_CUDA(fcg::launch_attn_split(ap, c.head_dim, rows_per_cta_of(max_rows), pc.stream));
+    FCG_CUDA(fcg::launch_attn_split(ap, c.head_dim, lay.rows_per_cta_split, io.stream));
     lib->stats.attn_split_launches++;
     lib->stats.last_attn_path = 1;
   }
-  lib->stats.last_attn_splits = max_splits;
-  if (max_splits > 1) {
-    FCG_CUDA(fcg::launch_attn_combine(ap, c.head_dim, pc.stream));
+  lib->stats.last_attn_splits = lay.max_splits;
+  if (lay.max_splits > 1) {
+    FCG_CUDA(fcg::launch_attn_combine(ap, c.head_dim, io.stream));
     lib->stats.attn_combine_launches++;
   }
-  FCG_CUDA(cudaEventRecord(slot->ev, pc.stream));
-  slot->in_flight = true;
-  FCG_CUDA(cudaEventRecord(lib->last_patch_ev, pc.stream));
-  lib->have_last_patch = true;
+  return FCG_OK;
+}
 
-  // ---- commit fill state ---------------------------------------------------------------------
-  tok_off = 0;
-  for (int t = 0; t < pc.n_tasks; ++t) {
-    TaskRec &tr = lib->tasks[pc.task_ids[t]];
-    const int32_t n = pc.n_per_task[t];
-    for (int i = 0; i < n; ++i) tr.filled[pc.positions[tok_off + i]] = 1;
+// fill state, capacity and page tables of the patched tasks (after everything has been enqueued)
+void commit_patch(fcg_library *lib, const PatchSpec &ps, const PatchCheck &ck, const PatchLayout &lay) {
+  for (const auto &g : lay.grows) {
+    TaskRec &tr = lib->tasks[g.task_id];
+    for (int k = 0; k < g.count; ++k) {
+      tr.pages.push_back(lay.grow_pages[g.index + k]);
+      lib->page_stack.pop_back();
+    }
+  }
+  int64_t tok_off = 0;
+  for (int t = 0; t < ps.n_tasks; ++t) {
+    TaskRec &tr = lib->tasks[ps.task_ids[t]];
+    const int32_t n = ps.n_per_task[t];
+    if (ck.new_capacity[t] > tr.capacity) {
+      tr.capacity = ck.new_capacity[t];
+      tr.filled.resize(tr.capacity, 0);
+    }
+    for (int i = 0; i < n; ++i) tr.filled[ps.positions[tok_off + i]] = 1;
     while (tr.filled_prefix < tr.capacity && tr.filled[tr.filled_prefix]) tr.filled_prefix++;
-    tr.n_tokens = std::max(tr.n_tokens, pc.positions[tok_off + n - 1] + 1);
+    tr.n_tokens = std::max(tr.n_tokens, ps.positions[tok_off + n - 1] + 1);
     tok_off += n;
   }
+}
+
+// One patch call on device tensors: validate -> blob (uploaded, or the previous call's copy reused) -> growth -> kernels
+// -> commit.  `prechecked`: the caller has validated (host / rope variants validate before their own enqueues).
+fcg_status_t patch_common(fcg_library *lib, const PatchSpec &ps, const PatchIO &io, const PatchCheck *prechecked = nullptr) {
+  fcg_status_t st = validate_io(lib, io);
+  if (st != FCG_OK) return st;
+  PatchCheck local;
+  if (!prechecked) {
+    st = validate_patch(lib, ps, local);
+    if (st != FCG_OK) return st;
+  }
+  const PatchCheck &ck = prechecked ? *prechecked : local;
+
+  BlobSlot *slot = nullptr;
+  st = acquire_slot(lib, &slot);
+  if (st != FCG_OK) return st;
+  PatchLayout lay;
+  st = build_patch_blob(lib, ps, ck, slot->host, BLOB_BYTES, lay);
+  if (st != FCG_OK) return st;
+  uint64_t po, pm;
+  partial_bytes(lib, lay, io.n_layers, po, pm);
+  if (po + pm > lib->scratch_bytes)
+    return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for %d-way split partials (%llu bytes)", lay.max_splits, (unsigned long long)(po + pm));
+
+  SlotUse use;
+  use.stream = io.stream;
+  {
+    const int cached = lib->patch_blob_slot;
+    if (cached >= 0 && lib->slots[cached].gen == lib->patch_blob_gen && lib->patch_blob_stream == io.stream &&
+        lib->patch_blob_copy.size() == lay.used && memcmp(lib->patch_blob_copy.data(), slot->host, lay.used) == 0) {
+      // same bytes as the previous patch call on this stream and its device copy is intact: hand the fresh slot back
+      lib->next_slot = (lib->next_slot + BLOB_SLOTS - 1) % BLOB_SLOTS;
+      slot->gen--;
+      slot = &lib->slots[cached];
+      use.slot = slot;
+    } else {
+      use.slot = slot;
+      FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, lay.used, cudaMemcpyHostToDevice, io.stream));
+      use.enqueued = true;
+      lib->patch_blob_copy.assign(slot->host, slot->host + lay.used);
+      lib->patch_blob_slot = (int)(slot - lib->slots);
+      lib->patch_blob_gen = slot->gen;
+      lib->patch_blob_stream = io.stream;
+    }
+  }
+  st = enqueue_growth(lib, lay, slot->dev, io.stream);
+  if (st != FCG_OK) return st;
+  use.enqueued = true;
+  st = launch_patch(lib, lay, slot->dev, io);
+  if (st != FCG_OK) return st;
+  commit_patch(lib, ps, ck, lay);
   return FCG_OK;
 }
 
 }  // namespace
 
+struct fcg_patch_plan {
+  fcg_library *lib = nullptr;
+  PatchLayout lay;
+  uint64_t dev_off = 0, dev_bytes = 0;          // the plan's blob inside the arena (segment allocator)
+  std::vector<int32_t> task_ids;
+  std::vector<uint32_t> task_gens;
+};
+
 fcg_status_t fcg_patch(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers, const void *q,
                        const void *k, const void *v, const int32_t *positions, int32_t n, void *out, void *stream) {
   if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
-  PatchCall pc{&task_id, &n, 1, layer_begin, n_layers, q, k, v, positions, out, static_cast<cudaStream_t>(stream)};
-  return patch_common(lib, pc);
+  PatchSpec ps{&task_id, &n, 1, positions, n_layers};
+  PatchIO io{layer_begin, n_layers, q, k, v, out, static_cast<cudaStream_t>(stream)};
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, io.stream);
+  fcg_status_t st = patch_common(lib, ps, io);
+  return st != FCG_OK ? st : mark_last(lib, io.stream);
 }
 
 fcg_status_t fcg_patch_batch(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task, int32_t n_tasks,
                              int32_t layer_begin, int32_t n_layers, const void *q, const void *k, const void *v,
                              const int32_t *positions, void *out, void *stream) {
   if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
-  PatchCall pc{task_ids, n_per_task, n_tasks, layer_begin, n_layers, q, k, v, positions, out, static_cast<cudaStream_t>(stream)};
-  return patch_common(lib, pc);
+  PatchSpec ps{task_ids, n_per_task, n_tasks, positions, n_layers};
+  PatchIO io{layer_begin, n_layers, q, k, v, out, static_cast<cudaStream_t>(stream)};
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, io.stream);
+  fcg_status_t st = patch_common(lib, ps, io);
+  return st != FCG_OK ? st : mark_last(lib, io.stream);
+}
+
+// ------------------------------------------------------------------ patch plans (graph-capturable patching)
+fcg_status_t fcg_patch_plan_create(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task, int32_t n_tasks,
+                                   const int32_t *positions, int32_t layers_per_call, void *stream_, fcg_patch_plan_t **out) {
+  if (!lib || !out) return fail(FCG_ERR_INVALID_ARG, "NULL argument");
+  *out = nullptr;
+  if (layers_per_call <= 0 || layers_per_call > lib->cfg.n_layers) return fail(FCG_ERR_INVALID_ARG, "layers_per_call must be in [1, n_layers]");
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  PatchSpec ps{task_ids, n_per_task, n_tasks, positions, layers_per_call};
+  PatchCheck ck;
+  fcg_status_t st = validate_patch(lib, ps, ck);
+  if (st != FCG_OK) return st;
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, stream);
+  BlobSlot *slot = nullptr;
+  st = acquire_slot(lib, &slot);
+  if (st != FCG_OK) return st;
+  fcg_patch_plan *pl = new fcg_patch_plan();
+  pl->lib = lib;
+  st = build_patch_blob(lib, ps, ck, slot->host, BLOB_BYTES, pl->lay);
+  if (st != FCG_OK) {
+    delete pl;
+    return st;
+  }
+  pl->dev_bytes = align_up(pl->lay.used);
+  const size_t fi = range_find(lib->seg_free, pl->dev_bytes);
+  if (fi == lib->seg_free.size()) {
+    delete pl;
+    return fail(FCG_ERR_OUT_OF_ARENA, "no free arena range of %llu bytes for a patch plan", (unsigned long long)pl->dev_bytes);
+  }
+  pl->dev_off = lib->seg_free[fi].off;
+  SlotUse use;
+  use.slot = slot;
+  use.stream = stream;
+  cudaError_t e = cudaMemcpyAsync(lib->arena + pl->dev_off, slot->host, pl->lay.used, cudaMemcpyHostToDevice, stream);
+  if (e != cudaSuccess) {
+    delete pl;
+    return fail(FCG_ERR_CUDA, "plan upload: %s", cudaGetErrorString(e));
+  }
+  use.enqueued = true;
+  st = enqueue_growth(lib, pl->lay, lib->arena + pl->dev_off, stream);
+  if (st == FCG_OK) st = mark_last(lib, stream);
+  if (st != FCG_OK) {
+    delete pl;
+    return st;
+  }
+  range_take(lib->seg_free, fi, pl->dev_bytes);
+  commit_patch(lib, ps, ck, pl->lay);
+  for (int t = 0; t < n_tasks; ++t) {
+    pl->task_ids.push_back(task_ids[t]);
+    pl->task_gens.push_back(lib->tasks[task_ids[t]].gen);
+  }
+  lib->n_plans_live++;
+  *out = pl;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_patch_planned(fcg_library_t *lib, fcg_patch_plan_t *plan, int32_t layer_begin, int32_t n_layers, const void *q,
+                               const void *k, const void *v, void *out, void *stream_) {
+  if (!lib || !plan || plan->lib != lib) return fail(FCG_ERR_INVALID_ARG, "NULL plan / plan of another library");
+  for (size_t t = 0; t < plan->task_ids.size(); ++t) {
+    const TaskRec &tr = lib->tasks[plan->task_ids[t]];
+    if (!tr.live || tr.gen != plan->task_gens[t])
+      return fail(FCG_ERR_BAD_TASK, "task %d was released or re-stitched after the plan was made", plan->task_ids[t]);
+  }
+  PatchIO io{layer_begin, n_layers, q, k, v, out, static_cast<cudaStream_t>(stream_)};
+  fcg_status_t st = validate_io(lib, io);
+  if (st != FCG_OK) return st;
+  FCG_DEVICE(lib);
+  bool capturing = false;
+  st = order_after_previous(lib, io.stream, &capturing);
+  if (st != FCG_OK) return st;
+  st = launch_patch(lib, plan->lay, lib->arena + plan->dev_off, io);
+  if (st != FCG_OK) return st;
+  return capturing ? FCG_OK : mark_last(lib, io.stream);
+}
+
+fcg_status_t fcg_patch_plan_destroy(fcg_library_t *lib, fcg_patch_plan_t *plan) {
+  if (!lib || !plan || plan->lib != lib) return fail(FCG_ERR_INVALID_ARG, "NULL plan / plan of another library");
+  range_give(lib->seg_free, plan->dev_off, plan->dev_bytes);
+  lib->n_plans_live--;
+  delete plan;
+  return FCG_OK;
 }
 
 // NEXT-4 (R13 variant): q and k arrive before position encoding; rotate them to positions[i], then patch
@@ -1034,11 +1376,15 @@ fcg_status_t fcg_patch_rope(fcg_library_t *lib, int32_t task_id, int32_t layer_b
   if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
   const fcg_config_t &c = lib->cfg;
   if (c.rope_mode == FCG_ROPE_NONE) return fcg_patch(lib, task_id, layer_begin, n_layers, q, k, v, positions, n, out, stream_);
-  if (!q || !k || !v || !out || !positions || n <= 0 || n_layers <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty argument");
-  for (int i = 0; i < n; ++i)
-    if (positions[i] < 0 || (i > 0 && positions[i] <= positions[i - 1]))
-      return fail(FCG_ERR_INVALID_ARG, "positions must be non-negative and strictly increasing");
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  // every host-side check first: nothing is enqueued for a call that fails (fcg.h conventions)
+  PatchSpec ps{&task_id, &n, 1, positions, n_layers};
+  PatchIO io0{layer_begin, n_layers, q, k, v, out, stream};
+  fcg_status_t st = validate_io(lib, io0);
+  if (st != FCG_OK) return st;
+  PatchCheck ck;
+  st = validate_patch(lib, ps, ck);
+  if (st != FCG_OK) return st;
   const int half = c.head_dim / 2;
   const uint64_t q_bytes = (uint64_t)n_layers * n * c.n_q_heads * c.head_dim * 2;
   const uint64_t kv_bytes = (uint64_t)n_layers * n * c.n_kv_heads * c.head_dim * 2;
@@ -1049,10 +1395,14 @@ fcg_status_t fcg_patch_rope(fcg_library_t *lib, int32_t task_id, int32_t layer_b
   // rotated copies at the END of the scratch area (where fcg_patch_host stages too); split partials grow from its start
   unsigned char *dq = lib->arena + lib->scratch_off + lib->scratch_bytes - need, *dk = dq + align_up(q_bytes);
 
-  FCG_CUDA(cudaSetDevice(c.device));
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, stream);
   BlobSlot *slot = nullptr;
-  fcg_status_t st = acquire_slot(lib, &slot);
+  st = acquire_slot(lib, &slot);
   if (st != FCG_OK) return st;
+  SlotUse use;
+  use.slot = slot;
+  use.stream = stream;
   // cos / sin of p_i * theta_j in fp64: exact evaluation at the start of every run of consecutive positions (and every
   // 32 tokens), angle addition by theta_j in between (error ~1e-16 per step), then the hi / lo split of the stitch table
   float4 *tab = reinterpret_cast<float4 *>(slot->host);
@@ -1089,6 +1439,7 @@ fcg_status_t fcg_patch_rope(fcg_library_t *lib, int32_t task_id, int32_t layer_b
     run = anchor ? 0 : run + 1;
   }
   FCG_CUDA(cudaMemcpyAsync(slot->dev, slot->host, tab_bytes, cudaMemcpyHostToDevice, stream));
+  use.enqueued = true;
   fcg::RopeQkParams rp;
   rp.q = static_cast<const uint16_t *>(q);
   rp.k = static_cast<const uint16_t *>(k);
@@ -1102,14 +1453,14 @@ fcg_status_t fcg_patch_rope(fcg_library_t *lib, int32_t task_id, int32_t layer_b
   rp.interleaved = c.rope_mode == FCG_ROPE_INTERLEAVED ? 1 : 0;
   FCG_CUDA(fcg::launch_rope_qk(rp, c.head_dim, stream));
   lib->stats.rope_qk_launches++;
-  FCG_CUDA(cudaEventRecord(slot->ev, stream));
-  slot->in_flight = true;
   const uint64_t saved = lib->scratch_bytes;
   lib->scratch_bytes = saved - need;
-  PatchCall pc{&task_id, &n, 1, layer_begin, n_layers, dq, dk, v, positions, out, stream};
-  st = patch_common(lib, pc);
+  PatchIO io{layer_begin, n_layers, dq, dk, v, out, stream};
+  st = patch_common(lib, ps, io, &ck);
   lib->scratch_bytes = saved;
-  return st;
+  if (cudaEventRecord(lib->staging_ev, stream) == cudaSuccess) lib->have_staging_ev = true;   // dq / dk are in use until here
+  fcg_status_t mst = mark_last(lib, stream);
+  return st != FCG_OK ? st : mst;
 }
 
 }  // extern "C"
@@ -1118,10 +1469,18 @@ namespace {
 // host-buffer patch of one task or of a batch: n = total patch tokens over the tasks
 fcg_status_t patch_host_common(fcg_library *lib, const int32_t *task_ids, const int32_t *n_per_task, int32_t n_tasks,
                                int32_t layer_begin, int32_t n_layers, const void *q, const void *k, const void *v,
-                               const int32_t *positions, int32_t n, void *out, void *stream_) {
-  if (!q || !k || !v || !out || n <= 0 || n_layers <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty argument");
+                               const int32_t *positions, void *out, void *stream_) {
   const fcg_config_t &c = lib->cfg;
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  // every host-side check first: nothing is copied or launched for a call that fails (fcg.h conventions)
+  PatchIO io0{layer_begin, n_layers, q, k, v, out, stream};
+  fcg_status_t st = validate_io(lib, io0);
+  if (st != FCG_OK) return st;
+  PatchSpec ps0{task_ids, n_per_task, n_tasks, positions, n_layers};
+  PatchCheck ck;
+  st = validate_patch(lib, ps0, ck);
+  if (st != FCG_OK) return st;
+  const int64_t n = ck.n_total;
   const uint64_t q_bytes = (uint64_t)n_layers * n * c.n_q_heads * c.head_dim * 2;
   const uint64_t kv_bytes = (uint64_t)n_layers * n * c.n_kv_heads * c.head_dim * 2;
   const uint64_t need = 2 * align_up(q_bytes) + 2 * align_up(kv_bytes);
@@ -1129,15 +1488,16 @@ fcg_status_t patch_host_common(fcg_library *lib, const int32_t *task_ids, const 
   if (need > lib->scratch_bytes / 2) return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small to stage %llu bytes", (unsigned long long)need);
   unsigned char *base = lib->arena + lib->scratch_off + lib->scratch_bytes - need;
   unsigned char *dq = base, *dk = dq + align_up(q_bytes), *dv = dk + align_up(kv_bytes), *dout = dv + align_up(kv_bytes);
-  FCG_CUDA(cudaSetDevice(c.device));
-  // Copies in on the library's copy stream: after the last user of the staging / partial area, but NOT after a
-  // stitch the caller has just enqueued on `stream` (stitch never touches the scratch area).  Large calls are cut
-  // into layer groups: group g attends while group g+1 is still arriving and group g-1 is leaving (second copy
-  // stream), all joined back into `stream` at the end.
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, stream);
+  // Copies in on the library's copy stream: after the last user of the staging area (staging_ev: host and rope calls),
+  // but NOT after a stitch the caller has just enqueued on `stream` (stitch never touches the scratch area), so the
+  // host->device copies overlap it.  Large calls are cut into layer groups: group g attends while group g+1 is still
+  // arriving and group g-1 is leaving (second copy stream), all joined back into `stream` at the end.
   const int groups = (q_bytes >= (8ull << 20) && n_layers >= fcg_library::HOST_GROUPS) ? fcg_library::HOST_GROUPS : 1;
   const uint64_t q_layer = q_bytes / n_layers, kv_layer = kv_bytes / n_layers;
   auto group_begin = [&](int g) { return (int)((int64_t)n_layers * g / groups); };
-  if (lib->have_last_patch) FCG_CUDA(cudaStreamWaitEvent(lib->copy_stream, lib->last_patch_ev, 0));
+  if (lib->have_staging_ev) FCG_CUDA(cudaStreamWaitEvent(lib->copy_stream, lib->staging_ev, 0));
   for (int g = 0; g < groups; ++g) {
     const int lb = group_begin(g), nl = group_begin(g + 1) - lb;
     FCG_CUDA(cudaMemcpyAsync(dq + lb * q_layer, (const char *)q + lb * q_layer, nl * q_layer, cudaMemcpyHostToDevice, lib->copy_stream));
@@ -1148,7 +1508,6 @@ fcg_status_t patch_host_common(fcg_library *lib, const int32_t *task_ids, const 
   // partials must not collide with the staging area: temporarily shrink the scratch
   const uint64_t saved = lib->scratch_bytes;
   lib->scratch_bytes = saved - need;
-  fcg_status_t st = FCG_OK;
   for (int g = 0; g < groups && st == FCG_OK; ++g) {
     const int lb = group_begin(g), nl = group_begin(g + 1) - lb;
     cudaError_t e = cudaStreamWaitEvent(stream, lib->h2d_ev[g], 0);
@@ -1156,9 +1515,10 @@ fcg_status_t patch_host_common(fcg_library *lib, const int32_t *task_ids, const 
       st = fail(FCG_ERR_CUDA, "cudaStreamWaitEvent: %s", cudaGetErrorString(e));
       break;
     }
-    PatchCall pc{task_ids, n_per_task, n_tasks, layer_begin + lb, nl, dq + lb * q_layer, dk + lb * kv_layer, dv + lb * kv_layer,
-                 positions, dout + lb * q_layer, stream};
-    st = patch_common(lib, pc);
+    PatchSpec ps{task_ids, n_per_task, n_tasks, positions, nl};
+    PatchIO io{layer_begin + lb, nl, dq + lb * q_layer, dk + lb * kv_layer, dv + lb * kv_layer, dout + lb * q_layer, stream};
+    // group 0 carries the growth (if any) and commits the fill state; the later groups re-validate against it (cheap)
+    st = patch_common(lib, ps, io, g == 0 ? &ck : nullptr);
     if (st != FCG_OK) break;
     if (groups > 1) {
       e = cudaEventRecord(lib->attn_ev[g], stream);
@@ -1169,15 +1529,22 @@ fcg_status_t patch_host_common(fcg_library *lib, const int32_t *task_ids, const 
     }
   }
   lib->scratch_bytes = saved;
-  if (st != FCG_OK) return st;
-  if (groups > 1) {
-    FCG_CUDA(cudaEventRecord(lib->d2h_ev, lib->d2h_stream));
-    FCG_CUDA(cudaStreamWaitEvent(stream, lib->d2h_ev, 0));
-  } else {
-    FCG_CUDA(cudaMemcpyAsync(out, dout, q_bytes, cudaMemcpyDeviceToHost, stream));
+  if (st == FCG_OK) {
+    cudaError_t e = cudaSuccess;
+    if (groups > 1) {
+      e = cudaEventRecord(lib->d2h_ev, lib->d2h_stream);
+      if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, lib->d2h_ev, 0);
+    } else {
+      e = cudaMemcpyAsync(out, dout, q_bytes, cudaMemcpyDeviceToHost, stream);
+    }
+    if (e != cudaSuccess) st = fail(FCG_ERR_CUDA, "copy out: %s", cudaGetErrorString(e));
   }
-  FCG_CUDA(cudaEventRecord(lib->last_patch_ev, stream));   // the staged output is in use until these copies are done
-  return FCG_OK;
+  // the copy streams have work in flight whatever happened above: `stream` joins them, and the next user of the staging
+  // area waits for this point
+  cudaStreamWaitEvent(stream, lib->h2d_ev[groups - 1], 0);
+  if (cudaEventRecord(lib->staging_ev, stream) == cudaSuccess) lib->have_staging_ev = true;
+  fcg_status_t mst = mark_last(lib, stream);
+  return st != FCG_OK ? st : mst;
 }
 }  // namespace
 
@@ -1186,21 +1553,14 @@ extern "C" {
 fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers, const void *q,
                             const void *k, const void *v, const int32_t *positions, int32_t n, void *out, void *stream) {
   if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
-  return patch_host_common(lib, &task_id, &n, 1, layer_begin, n_layers, q, k, v, positions, n, out, stream);
+  return patch_host_common(lib, &task_id, &n, 1, layer_begin, n_layers, q, k, v, positions, out, stream);
 }
 
 fcg_status_t fcg_patch_batch_host(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task, int32_t n_tasks,
                                   int32_t layer_begin, int32_t n_layers, const void *q, const void *k, const void *v,
                                   const int32_t *positions, void *out, void *stream) {
   if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
-  if (!task_ids || !n_per_task || n_tasks <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty task list");
-  int64_t n = 0;
-  for (int32_t t = 0; t < n_tasks; ++t) {
-    if (n_per_task[t] <= 0) return fail(FCG_ERR_INVALID_ARG, "task %d: n must be > 0", task_ids[t]);
-    n += n_per_task[t];
-  }
-  if (n > (1 << 20)) return fail(FCG_ERR_INVALID_ARG, "too many patch tokens in one call");
-  return patch_host_common(lib, task_ids, n_per_task, n_tasks, layer_begin, n_layers, q, k, v, positions, (int32_t)n, out, stream);
+  return patch_host_common(lib, task_ids, n_per_task, n_tasks, layer_begin, n_layers, q, k, v, positions, out, stream);
 }
 
 // ------------------------------------------------------------------------------- task utilities
@@ -1246,6 +1606,7 @@ fcg_status_t fcg_task_release(fcg_library_t *lib, int32_t task_id) {
   TaskRec &t = lib->tasks[task_id];
   for (auto it = t.pages.rbegin(); it != t.pages.rend(); ++it) lib->page_stack.push_back(*it);
   t = TaskRec();
+  t.gen = ++lib->task_gen;
   lib->n_tasks_live--;
   return FCG_OK;
 }
@@ -1258,8 +1619,9 @@ fcg_status_t fcg_task_shift(fcg_library_t *lib, int32_t task_id, int32_t src_beg
   if (task_id < 0 || task_id >= c.max_tasks || !lib->tasks[task_id].live) return fail(FCG_ERR_BAD_TASK, "unknown task %d", task_id);
   TaskRec &t = lib->tasks[task_id];
   if (n_tokens <= 0 || src_begin < 0 || dst_begin < 0 || (int64_t)src_begin + n_tokens > t.capacity ||
-      (int64_t)dst_begin + n_tokens > t.capacity)
-    return fail(FCG_ERR_RANGE, "shift range outside the capacity %d of task %d", t.capacity, task_id);
+      (int64_t)dst_begin + n_tokens > c.max_task_tokens)
+    return fail(FCG_ERR_RANGE, "shift source outside the capacity %d of task %d, or destination outside max_task_tokens %d", t.capacity,
+                task_id, c.max_task_tokens);
   for (int32_t x = src_begin; x < src_begin + n_tokens; ++x)
     if (!t.filled[x]) return fail(FCG_ERR_UNFILLED, "task %d: shift source position %d was never filled", task_id, x);
   const int32_t delta = dst_begin - src_begin;
@@ -1267,9 +1629,13 @@ fcg_status_t fcg_task_shift(fcg_library_t *lib, int32_t task_id, int32_t src_beg
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   const int P = c.page_size;
   const int32_t dst_end = dst_begin + n_tokens;
-  const int32_t lp0 = dst_begin / P, lp1 = (dst_end - 1) / P, n_new = lp1 - lp0 + 1;
+  const int32_t n_old = (int32_t)t.pages.size();
+  // R25: every logical page that receives a new physical page -- gap pages between the end of the table and the
+  // destination (a destination beyond the capacity appends), then the destination's pages -- ascending logical order
+  const int32_t lp0 = dst_begin / P, lp1 = (dst_end - 1) / P, first_new = std::min(lp0, n_old), n_new = lp1 - first_new + 1;
   if ((size_t)n_new > lib->page_stack.size())
     return fail(FCG_ERR_OUT_OF_PAGES, "need %d pages, %zu free", n_new, lib->page_stack.size());
+  const int32_t new_cap = std::max(t.capacity, dst_end);
 
   // copy-on-shift: destination pages are fresh, so no page is read and written by the same launch
   GatherBuilder gb;
@@ -1289,7 +1655,7 @@ fcg_status_t fcg_task_shift(fcg_library_t *lib, int32_t task_id, int32_t src_beg
   auto add_chunk = [&](int32_t entry, int32_t dst_pos, int32_t src_pos, int32_t n) {
     fcg::StitchChunkDev dc;
     dc.entry = entry;
-    dc.dst_tok = gb.pool_tok(lib, gb.pages[dst_pos / P - lp0], dst_pos % P);
+    dc.dst_tok = gb.pool_tok(lib, gb.pages[dst_pos / P - first_new], dst_pos % P);
     dc.src_tok = gb.pool_tok(lib, t.pages[src_pos / P], src_pos % P);
     dc.ntok = n;
     gb.chunks.push_back(dc);
@@ -1300,22 +1666,31 @@ fcg_status_t fcg_task_shift(fcg_library_t *lib, int32_t task_id, int32_t src_beg
     add_chunk(0, d, sp, n);
     done += n;
   }
-  if (dst_begin > lp0 * P) add_chunk(1, lp0 * P, lp0 * P, dst_begin - lp0 * P);
-  const int32_t page_end = std::min((lp1 + 1) * P, t.capacity);
+  // slots of re-paged pages outside the destination keep their contents -- as far as the old table held them
+  const int32_t old_end = std::min(n_old * P, t.capacity);
+  if (dst_begin > lp0 * P && lp0 * P < old_end) add_chunk(1, lp0 * P, lp0 * P, std::min(dst_begin, old_end) - lp0 * P);
+  const int32_t page_end = std::min((lp1 + 1) * P, old_end);
   if (dst_end < page_end) add_chunk(1, dst_end, dst_end, page_end - dst_end);
 
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, stream);
   GatherBlob gbl;
   fcg_status_t st = enqueue_gather(lib, gb, stream, gbl);
   if (st != FCG_OK) return st;
-  FCG_CUDA(cudaMemcpyAsync(lib->tables() + (int64_t)task_id * lib->pages_per_task + lp0, gbl.slot->dev + gbl.off_pages,
+  FCG_CUDA(cudaMemcpyAsync(lib->tables() + (int64_t)task_id * lib->pages_per_task + first_new, gbl.slot->dev + gbl.off_pages,
                            (size_t)n_new * sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
-  st = finish_gather(gbl, stream);
+  st = mark_last(lib, stream);
   if (st != FCG_OK) return st;
 
   // ---- commit: new pages in, replaced pages back to the pool (re-issued in ascending logical order) ----
   lib->page_stack.swap(stack);
-  for (int32_t lp = lp1; lp >= lp0; --lp) lib->page_stack.push_back(t.pages[lp]);
-  for (int32_t lp = lp0; lp <= lp1; ++lp) t.pages[lp] = gb.pages[lp - lp0];
+  for (int32_t lp = std::min(lp1, n_old - 1); lp >= lp0; --lp) lib->page_stack.push_back(t.pages[lp]);
+  if ((int32_t)t.pages.size() < lp1 + 1) t.pages.resize(lp1 + 1);
+  for (int32_t lp = first_new; lp <= lp1; ++lp) t.pages[lp] = gb.pages[lp - first_new];
+  if (new_cap > t.capacity) {
+    t.capacity = new_cap;
+    t.filled.resize(new_cap, 0);
+  }
   std::fill(t.filled.begin() + src_begin, t.filled.begin() + src_begin + n_tokens, (uint8_t)0);
   std::fill(t.filled.begin() + dst_begin, t.filled.begin() + dst_end, (uint8_t)1);
   t.filled_prefix = 0;
@@ -1360,10 +1735,12 @@ fcg_status_t fcg_segment_extract(fcg_library_t *lib, int32_t task_id, int32_t be
     gb.chunks.push_back(dc);
     done += n;
   }
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, stream);
   GatherBlob gbl;
   st = enqueue_gather(lib, gb, stream, gbl);
   if (st != FCG_OK) return st;
-  st = finish_gather(gbl, stream);
+  st = mark_last(lib, stream);
   if (st != FCG_OK) return st;
   commit_segment_slot(lib, sl, n_tokens, new_orig_start);
   *seg_id_out = sl.sid;
@@ -1391,10 +1768,11 @@ fcg_status_t fcg_task_read(fcg_library_t *lib, int32_t task_id, int32_t layer, i
   rp.head_dim = c.head_dim;
   rp.page_size = c.page_size;
   rp.n_pages = c.n_pages;
-  FCG_CUDA(cudaSetDevice(c.device));
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, static_cast<cudaStream_t>(stream));
   FCG_CUDA(fcg::launch_task_read(rp, static_cast<cudaStream_t>(stream)));
   lib->stats.read_launches++;
-  return FCG_OK;
+  return mark_last(lib, static_cast<cudaStream_t>(stream));
 }
 
 fcg_status_t fcg_pool_info(fcg_library_t *lib, fcg_pool_info_t *out) {

@@ -381,11 +381,14 @@ template <int D, int MB>
 cudaError_t launch_split_t(const AttnParams &p, cudaStream_t stream) {
   constexpr int SMEM = STAGES * 2 * BN * D * 2;
   static_assert(SMEM >= (4 * 16 * (D + 8) + 2 * 4 * 16) * 4, "merge buffer must fit in the ring");
-  static bool configured = false;
-  if (!configured) {
+  // the attribute is per device (fcg_config_t.device allows libraries on several GPUs in one process)
+  static bool configured[64] = {};
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
+  if (dev < 0 || dev >= 64 || !configured[dev]) {
     cudaError_t e = cudaFuncSetAttribute(attn_split_kernel<D, MB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
     if (e != cudaSuccess) return e;
-    configured = true;
+    if (dev >= 0 && dev < 64) configured[dev] = true;
   }
   dim3 grid((unsigned)(p.max_splits * p.max_row_groups), (unsigned)p.n_kv_heads, (unsigned)(p.n_layers * p.n_tasks));
   attn_split_kernel<D, MB><<<grid, NTHREADS, SMEM, stream>>>(p);

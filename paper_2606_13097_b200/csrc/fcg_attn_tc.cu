@@ -779,11 +779,14 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
 template <int NQ, int PS_>
 cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv, cudaStream_t stream) {
   using C = Cfg<NQ, PS_>;
-  static bool configured = false;
-  if (!configured) {
+  // the attribute is per device (fcg_config_t.device allows libraries on several GPUs in one process)
+  static bool configured[64] = {};
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
+  if (dev < 0 || dev >= 64 || !configured[dev]) {
     cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, PS_>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    configured = true;
+    if (dev >= 0 && dev < 64) configured[dev] = true;
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(p.max_splits * p.max_row_groups), (unsigned)p.n_kv_heads, (unsigned)(p.n_layers * p.n_tasks));

@@ -56,6 +56,14 @@ __device__ __forceinline__ void rot_pair(float a, float b, const float4 &t, floa
   const float yr = __fmaf_rn(b, t.y, __fmul_rn(a, t.w));
   x = __fadd_rn(x0, xr);
   y = __fadd_rn(y0, yr);
+  // IEEE special values ("+-inf / NaN propagate"): with an infinite input the correction term is
+  // inf * c_lo -- of the wrong sign, or NaN when c_lo == 0 -- and turns the infinity the definition gives into NaN.
+  // A NaN result is therefore recomputed from the unsplit table (never taken for finite inputs; NaN stays NaN).
+  if (__builtin_expect(x != x || y != y, 0)) {
+    const float c = __fadd_rn(t.x, t.y), sn = __fadd_rn(t.z, t.w);
+    x = __fmaf_rn(a, c, -__fmul_rn(b, sn));
+    y = __fmaf_rn(b, c, __fmul_rn(a, sn));
+  }
 }
 
 __device__ __forceinline__ void rot_word(uint32_t wa, uint32_t wb, const float4 &t0, const float4 &t1, uint32_t &oa,

@@ -49,11 +49,11 @@ def plans_of(wl: synth.Workload, seg_ids):
 
 
 def make_pair(cfg: synth.GraftConfig, wl: synth.Workload, seed: int, *, n_pages=None, max_tasks=None,
-              workspace_bytes=0, only_segments=None, rope_mode=1, inv_freq=None, host_tier_tokens=0):
+              workspace_bytes=0, only_segments=None, rope_mode=1, inv_freq=None, host_tier_tokens=0, max_task_tokens=None):
     """Create oracle + CUDA library holding the same segment bits.  Returns (orc, lib, seg_ids)."""
     from paper_2606_13097_b200.binding import FcgLibrary
     used = sorted({s for t in wl.tasks for (s, _, _, _) in t.entries}) if only_segments is None else only_segments
-    cap_tokens = max(t.capacity for t in wl.tasks)
+    cap_tokens = max_task_tokens or max(t.capacity for t in wl.tasks)
     total_pages = sum(-(-t.capacity // cfg.page_size) for t in wl.tasks)
     n_pages = n_pages or total_pages + 8
     seg_tokens = int(sum(int(wl.seg_lens[s]) for s in used))

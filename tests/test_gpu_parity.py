@@ -321,7 +321,9 @@ def test_p14_rejections_match_oracle_and_leave_state_unchanged():
     assert len(set(ids)) == len(ids) and max(ids) < 8
     # patch argument errors
     q, k, v = [x.cuda() for x in synth.patch_qkv(cfg, 2, 2, 1)]
-    for pos, status in (([11, 10], bnd.FCG_ERR_INVALID_ARG), ([10, 24], bnd.FCG_ERR_RANGE), ([12, 13], bnd.FCG_ERR_UNFILLED)):
+    # (capacity of task 2 is 24: position 24 would append (R25) but 11..23 are unfilled; RANGE starts at max_task_tokens = 64)
+    for pos, status in (([11, 10], bnd.FCG_ERR_INVALID_ARG), ([10, 64], bnd.FCG_ERR_RANGE), ([10, 24], bnd.FCG_ERR_UNFILLED),
+                        ([12, 13], bnd.FCG_ERR_UNFILLED)):
         with pytest.raises(bnd.FcgError) as eg:
             lib.patch(2, 0, q, k, v, pos)
         assert eg.value.status == status

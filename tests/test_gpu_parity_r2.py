@@ -1,0 +1,293 @@
+"""Round-2 parity reach ("What's weak" 1):
+
+* EVERY stitched K and V element of C2 and C3 (all layers, all kv heads) against the oracle, ulp histogram printed;
+* >= 16 (layer, kv head) slices of C4 and of C5 over layout seeds 1, 2, 3;
+* IEEE special values (+-0, bf16 subnormals, near-max magnitudes, +-inf, NaN) through stitch, scatter and attention;
+* peaked softmax inputs (a few keys dominate, among them the last visible key and the first key of KV tiles and
+  splits) with a tolerance that a dropped key cannot hide under.
+"""
+import numpy as np
+import pytest
+import torch
+
+import bench
+import fcg_testlib as T
+from oracle import fcg_oracle as O
+from paper_2606_13097_b200 import synth
+from test_gpu_fullsize import run_fullsize
+
+pytestmark = pytest.mark.gpu
+
+
+def _full_stitch_check(name, seed):
+    """the timed stitch of bench.py, then layer by layer: oracle with L = 1 holding that layer of every used segment
+    (the path is independent per layer), all kv heads, every filled position."""
+    cfg = synth.CONFIGS[name]
+    wl = synth.make_workload(cfg, seed)
+    used = sorted({s for t in wl.tasks for (s, _, _, _) in t.entries})
+    kept = {}
+
+    def keep(s, k, v):
+        if s in used:
+            kept[s] = (synth.to_bits(k), synth.to_bits(v))          # host copies of the device-generated bits
+
+    lib = bench.build_library(cfg, wl, seed, 0, on_segment=keep)
+    try:
+        lib.stitch(bench.plans_for(wl))
+        torch.cuda.synchronize()
+        hist = np.zeros(4, np.int64)
+        n_v = 0
+        for layer in range(cfg.n_layers):
+            orc = O.OracleLibrary(1, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, page_size=cfg.page_size, rope_base=cfg.rope_base,
+                                  n_pages=sum(-(-t.capacity // cfg.page_size) for t in wl.tasks) + 16)
+            sid = {s: orc.segment_register(kept[s][0][layer:layer + 1], kept[s][1][layer:layer + 1], int(wl.orig_starts[s])) for s in used}
+            orc.stitch([O.Plan(t.task_id, [O.PlanEntry(sid[s], b, n, d) for (s, b, n, d) in t.entries],
+                               [O.Hole(*h) for h in t.holes], t.capacity) for t in wl.tasks])
+            for t in wl.tasks:
+                ot = orc.tasks[t.task_id]
+                if layer == 0:
+                    assert np.array_equal(lib.task_page_table_host(t.task_id), np.asarray(ot.page_table, np.int32))
+                kg, vg = lib.task_read(t.task_id, layer, 0, t.capacity)
+                kb, vb = synth.to_bits(kg), synth.to_bits(vg)
+                f = ot.filled
+                assert np.array_equal(vb[:, f], ot.v[0][:, f]), f"{name}: V gather not bit-exact (task {t.task_id}, layer {layer})"
+                n_v += int(vb[:, f].size)
+                hist += T.assert_k_within_1ulp(kb[:, f], ot.k[0][:, f], f"{name} task {t.task_id} layer {layer}")
+        total = wl.stitched_tokens * cfg.n_layers * cfg.n_kv_heads * cfg.head_dim
+        assert hist.sum() == total == n_v, "not every stitched element was compared"
+        print(f"{name} seed {seed}: ALL {total} stitched K elements compared, ulp histogram [0,1,2,>=3] = {hist.tolist()} "
+              f"({hist[1] / total:.2e} off by one), all {n_v} V elements bit-exact")
+    finally:
+        lib.close()
+
+
+def test_c2_every_stitched_element():
+    _full_stitch_check("C2", 1)
+
+
+def test_c3_every_stitched_element():
+    _full_stitch_check("C3", 1)
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_c4_six_slices_per_layout_seed(seed):
+    run_fullsize("C4", seed, 6, 1)
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_c5_six_slices_per_layout_seed(seed):
+    run_fullsize("C5", seed, 6, 1)
+
+
+@pytest.mark.parametrize("seed", [2, 3])
+def test_c2_c3_sampled_slices_other_layout_seeds(seed):
+    run_fullsize("C2", seed, 4, 2)
+    run_fullsize("C3", seed, 4, 1)
+
+
+# ------------------------------------------------------------------------------------------------
+# IEEE special values ("No flush-to-zero; +-inf / NaN propagate"; R30)
+# ------------------------------------------------------------------------------------------------
+SPECIALS = np.asarray([0x0000, 0x8000,                    # +-0
+                       0x0001, 0x8001, 0x007F, 0x0040,    # bf16 subnormals (smallest, largest, middle)
+                       0x0080, 0x8080,                    # smallest normals
+                       0x7F7F, 0xFF7F, 0x7F00, 0x7E80,    # near +-3.39e38
+                       0x7F80, 0xFF80,                    # +-inf
+                       0x7FC0, 0xFFC1, 0x7F81], np.uint16)  # NaNs (quiet, negative with payload, signalling pattern)
+
+
+def _classes(bits):
+    """0 finite, 1 +inf, 2 -inf, 3 NaN"""
+    b = np.asarray(bits, np.uint16)
+    mag = b & 0x7FFF
+    return np.where(mag < 0x7F80, 0, np.where(mag > 0x7F80, 3, np.where(b == 0x7F80, 1, 2)))
+
+
+@pytest.mark.parametrize("D,rope_mode", [(128, 1), (64, 1), (128, 2), (128, 0)])
+def test_special_values_through_stitch_and_scatter(D, rope_mode):
+    L, Hq, Hkv, P = 2, 4, 2, 16
+    rng = np.random.default_rng(D + rope_mode)
+    n = 96
+    kb = O.f64_to_bf16(rng.standard_normal((L, Hkv, n, D)))
+    vb = O.f64_to_bf16(rng.standard_normal((L, Hkv, n, D)))
+    # specials at known places: every special value meets a normal partner, a special partner and itself, in both halves
+    half = D // 2
+    for i, sv in enumerate(SPECIALS):
+        kb[:, :, 2 * i, 3] = sv                                   # low half (or even slot), normal partner
+        kb[:, :, 2 * i + 1, half + 5] = sv                        # high half, normal partner
+        kb[:, :, 40 + i, 7] = sv                                  # both elements of a half-split pair special
+        kb[:, :, 40 + i, half + 7] = SPECIALS[(i + 3) % len(SPECIALS)]
+        kb[:, :, 60 + i, 10:12] = sv                              # both elements of an interleaved pair
+        vb[:, :, i, i % D] = sv
+    kb[:, :, 80] = 0x0003                                         # whole rows of subnormals / near-max values
+    kb[:, :, 81] = 0x7F7F
+    kb[:, :, 82] = 0x8000
+    from paper_2606_13097_b200.binding import FcgLibrary
+    lib = FcgLibrary(n_layers=L, n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, page_size=P, rope_mode=rope_mode, rope_base=1e4,
+                     max_segments=2, max_tasks=2, max_task_tokens=512, n_pages=64, segment_tokens=2 * n + 8)
+    orc = O.OracleLibrary(L, Hq, Hkv, D, page_size=P, rope_mode=rope_mode, rope_base=1e4, n_pages=64, max_task_tokens=512)
+    sid = lib.segment_register(synth.from_bits(kb, "cuda"), synth.from_bits(vb, "cuda"), 1000)
+    assert sid == orc.segment_register(kb, vb, 1000)
+    # a second copy of the segment with another orig_start, so that the four entries get the deltas
+    # -1000 (large angle), -900, 0 (bit copy) and +100
+    sid2 = lib.segment_register(synth.from_bits(kb, "cuda"), synth.from_bits(vb, "cuda"), 200)
+    assert sid2 == orc.segment_register(kb, vb, 200)
+    plan = {"task_id": 0, "entries": [(sid, 0, n, 0), (sid, 0, n, 100), (sid2, 0, n, 200), (sid2, 0, n, 300)],
+            "holes": [(396, 4)], "capacity_tokens": 400}
+    orc.stitch([O.Plan(0, [O.PlanEntry(*e) for e in plan["entries"]], [O.Hole(396, 4)], 400)])
+    lib.stitch([plan])
+    assert orc.tasks[0].deltas == [-1000, -900, 0, 100]
+    hist = np.zeros(4, np.int64)
+    for layer in range(L):
+        kg, vg = lib.task_read(0, layer, 0, 400)
+        gk, gv = synth.to_bits(kg), synth.to_bits(vg)
+        f = orc.tasks[0].filled
+        ok, ov = orc.tasks[0].k[layer], orc.tasks[0].v[layer]
+        assert np.array_equal(gv[:, f], ov[:, f]), "V (incl. NaN payloads, -0, subnormals) must be a bit copy"
+        cg, co = _classes(gk[:, f]), _classes(ok[:, f])
+        assert np.array_equal(cg, co), f"inf / NaN pattern differs in {int((cg != co).sum())} K elements (layer {layer})"
+        fin = co == 0
+        hist += T.assert_k_within_1ulp(gk[:, f][fin], ok[:, f][fin], f"finite K elements, layer {layer}")
+        # delta 0 is a bit copy of everything, specials included
+        assert np.array_equal(gk[:, 200:200 + n], kb[layer])
+        # no flush-to-zero: a rotated subnormal row stays non-zero wherever the oracle's is
+        z_o, z_g = (ok[:, f] & 0x7FFF) == 0, (gk[:, f] & 0x7FFF) == 0
+        assert int((z_g & ~z_o).sum()) <= int(hist[1]), "subnormal results flushed to zero"
+    assert (co != 0).sum() > 50 and hist[0] > 0
+    # scatter: patch K / V rows full of specials land bit-exact
+    pos = np.asarray([396, 397, 398, 399], np.int32)
+    pk = np.tile(SPECIALS, 2 * 4 * Hkv * D // len(SPECIALS) + 1)[: L * 4 * Hkv * D].reshape(L, 4, Hkv, D).copy()
+    q = O.f64_to_bf16(rng.standard_normal((L, 4, Hq, D)))
+    lib.patch(0, 0, synth.from_bits(q, "cuda"), synth.from_bits(pk, "cuda"), synth.from_bits(pk[::-1].copy(), "cuda"), pos)
+    torch.cuda.synchronize()
+    for layer in range(L):
+        kg, vg = lib.task_read(0, layer, 396, 4)
+        assert np.array_equal(synth.to_bits(kg), np.transpose(pk[layer], (1, 0, 2)))
+        assert np.array_equal(synth.to_bits(vg), np.transpose(pk[::-1][layer], (1, 0, 2)))
+    lib.close()
+
+
+@pytest.mark.parametrize("D,tc_min_rows", [(128, 1), (128, 2 ** 31 - 1), (64, 1)])
+def test_attention_rows_that_see_no_special_value_are_unaffected(D, tc_min_rows):
+    """Two tasks and two kv heads share the pool.  Special values (inf, NaN, near-max, subnormal, +-0) sit (a) in the
+    OTHER task's cache, (b) in the OTHER kv head, (c) in this task at positions beyond the last patch position, (d) in
+    pool pages nobody owns.  Harmless ones (+-0, subnormals) also sit where the queries do see them.  The outputs must
+    match the oracle within the usual tolerance and be free of NaN / inf.  (R30 states what is NOT promised:
+    a non-finite V at a position <= positions[n-1] of the same task and kv head.)"""
+    L, Hq, Hkv, P = 2, 8, 2, 16
+    rng = np.random.default_rng(D)
+    n = 700
+    kb = O.f64_to_bf16(rng.standard_normal((L, Hkv, n, D)))
+    vb = O.f64_to_bf16(rng.standard_normal((L, Hkv, n, D)))
+    bad = np.asarray([0x7F80, 0xFF80, 0x7FC0, 0x7F7F, 0xFF7F], np.uint16)
+    kb2, vb2 = kb.copy(), vb.copy()
+    kb2[:, :, ::3, ::5] = bad[rng.integers(0, len(bad), kb2[:, :, ::3, ::5].shape)]      # segment 1: poisoned everywhere
+    vb2[:, :, ::2, ::7] = bad[rng.integers(0, len(bad), vb2[:, :, ::2, ::7].shape)]
+    kb1, vb1 = kb.copy(), vb.copy()
+    kb1[:, 1, ::4, ::3] = bad[rng.integers(0, len(bad), kb1[:, 1, ::4, ::3].shape)]      # segment 0: kv head 1 poisoned
+    vb1[:, 1, ::5, ::2] = bad[rng.integers(0, len(bad), vb1[:, 1, ::5, ::2].shape)]
+    kb1[:, 0, 600:, :] = 0x7FC0                                                           # head 0: only its tail (c)
+    vb1[:, 0, 600:, :] = 0x7F80
+    harmless = np.asarray([0x0000, 0x8000, 0x0001, 0x807F, 0x0040], np.uint16)
+    kb1[:, 0, :600:7, ::4] = harmless[rng.integers(0, 5, kb1[:, 0, :600:7, ::4].shape)]
+    vb1[:, 0, :600:9, ::3] = harmless[rng.integers(0, 5, vb1[:, 0, :600:9, ::3].shape)]
+    from paper_2606_13097_b200.binding import FcgLibrary
+    lib = FcgLibrary(n_layers=L, n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, page_size=P, rope_mode=0, max_segments=2, max_tasks=2,
+                     max_task_tokens=1024, n_pages=128, segment_tokens=2 * n)
+    # (d) poison the whole pool first: pages that the tasks never write keep NaN bits
+    info = lib.pool_info()
+    lib.arena[info["k_pool_offset"]: info["k_pool_offset"] + 2 * info["pool_bytes"]].view(torch.int16).fill_(0x7FC1)
+    orc = O.OracleLibrary(L, Hq, Hkv, D, page_size=P, rope_mode=0, n_pages=128, max_task_tokens=1024)
+    for kk, vv in ((kb1, vb1), (kb2, vb2)):
+        assert lib.segment_register(synth.from_bits(kk, "cuda"), synth.from_bits(vv, "cuda"), 0) == orc.segment_register(kk, vv, 0)
+    # task 0: segment 0 with a 20-token hole at 500 (patched below; kv_len = 520 < 600), task 1: the poisoned segment
+    plans = [{"task_id": 0, "entries": [(0, 0, 500, 0), (0, 520, 180, 520)], "holes": [(500, 20)], "capacity_tokens": 700},
+             {"task_id": 1, "entries": [(1, 0, 700, 0)], "holes": [], "capacity_tokens": 700}]
+    lib.stitch(plans)
+    orc.stitch([O.Plan(0, [O.PlanEntry(0, 0, 500, 0), O.PlanEntry(0, 520, 180, 520)], [O.Hole(500, 20)], 700),
+                O.Plan(1, [O.PlanEntry(1, 0, 700, 0)], [], 700)])
+    lib.set_attn_policy(tc_min_rows, 0)
+    pos = np.arange(500, 520, dtype=np.int32)
+    q = O.f64_to_bf16(rng.standard_normal((L, 20, Hq, D)))
+    pk = O.f64_to_bf16(rng.standard_normal((L, 20, Hkv, D)))
+    pv = O.f64_to_bf16(rng.standard_normal((L, 20, Hkv, D)))
+    pk[:, :, 1] = 0x7F80                                            # the patch's own rows of kv head 1 are poisoned too
+    pv[:, :, 1] = 0x7FC0
+    pk[:, 3, 0, ::2] = 0x8000                                       # harmless values in head 0's fresh rows
+    for splits in (1, 3):
+        lib.set_attn_policy(tc_min_rows, splits)
+        out = lib.patch(0, 0, synth.from_bits(q, "cuda"), synth.from_bits(pk, "cuda"), synth.from_bits(pv, "cuda"), pos)
+        torch.cuda.synchronize()
+        ref = orc.patch(0, 0, q, pk, pv, pos)
+        G = Hq // Hkv
+        got0 = out[:, :, :G]                                        # q heads of kv head 0
+        assert torch.isfinite(got0.float()).all(), "special values leaked into rows that cannot see them"
+        T.assert_attn_close(got0, ref[:, :, :G], f"kv head 0, {splits} split(s)")
+        assert not np.isfinite(ref[:, :, G:]).all()                 # the oracle's kv head 1 is poisoned, as constructed
+    lib.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# peaked softmax: a dropped or mis-masked key must show
+# ------------------------------------------------------------------------------------------------
+PEAK_ATOL, PEAK_RTOL = 4e-3, 1e-2       # bf16 output rounding is 2^-9 relative, bf16 P another 2^-9: ~4x the observed error
+
+
+@pytest.mark.parametrize("n,Hq,Hkv,D,ctx,tc_min_rows,splits", [
+    (16, 4, 4, 128, 4096, 1, 0), (16, 4, 4, 128, 4096, 1, 4), (48, 8, 2, 128, 2000, 1, 3), (130, 2, 1, 128, 2600, 1, 2),
+    (300, 2, 2, 128, 1500, 1, 0), (16, 4, 4, 128, 4096, 2 ** 31 - 1, 4), (32, 8, 4, 64, 3000, 1, 3), (5, 32, 4, 128, 1000, 1, 0)])
+def test_peaked_softmax_dominant_keys_at_tile_and_split_boundaries(n, Hq, Hkv, D, ctx, tc_min_rows, splits):
+    """Each query row gets ONE dominant key (score ~ +25 above the rest): the last visible key (its own fresh row), the
+    first key of a 64-token KV tile, the first / last key of a KV split, key 0, or a key inside the patch that the row
+    must NOT see (then masked: the row's dominant key is elsewhere).  The output of a row is then essentially the V row
+    of its dominant key, so a dropped tile, an off-by-one mask or a wrong split weight is an O(1) error; tolerance
+    4e-3 + 1e-2 |o| instead of north_star's 1e-2 + 2e-2 |o|."""
+    L, P = 2, 16
+    rng = np.random.default_rng(n + ctx)
+    G = Hq // Hkv
+    kb = O.f64_to_bf16(rng.standard_normal((L, Hkv, ctx, D)) * 0.25)
+    vb = O.f64_to_bf16(rng.standard_normal((L, Hkv, ctx, D)))
+    q = O.f64_to_bf16(rng.standard_normal((L, n, Hq, D)))
+    pk = O.f64_to_bf16(rng.standard_normal((L, n, Hkv, D)) * 0.25)
+    pv = O.f64_to_bf16(rng.standard_normal((L, n, Hkv, D)))
+    pos = np.arange(ctx, ctx + n, dtype=np.int32)
+    kv_len = ctx + n
+    tiles = -(-kv_len // 64)
+    per = -(-tiles // max(splits, 1)) * 64
+    targets = [0, 63, 64, 65, per - 1, per, per + 1, 2 * per, kv_len - 65, (kv_len - 1) // 64 * 64, ctx - 1]
+    targets = [t for t in targets if 0 <= t < ctx]
+    qf = O.bf16_to_f64(q)
+    for i in range(n):
+        for h in range(Hq):
+            g = h // G
+            if h % G:                                              # one dominant key per (row, kv head): set it for the group's first head
+                continue
+            kind = (i + g) % (len(targets) + 2)
+            u = qf[:, i, h] / np.sum(qf[:, i, h] ** 2, axis=-1, keepdims=True) * 30.0 * np.sqrt(D)   # q . u / sqrt(D) = 30
+            if kind < len(targets):
+                kb[:, g, targets[kind]] = O.f64_to_bf16(u)
+            elif kind == len(targets):
+                pk[:, i, g] = O.f64_to_bf16(u)                      # the row's own key: the last one it sees
+            elif i + 1 < n:
+                pk[:, i + 1, g] = O.f64_to_bf16(u)                  # a FUTURE key: must be masked for row i
+    from paper_2606_13097_b200.binding import FcgLibrary
+    lib = FcgLibrary(n_layers=L, n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, page_size=P, rope_mode=0, max_segments=1, max_tasks=1,
+                     max_task_tokens=kv_len, n_pages=-(-kv_len // P) + 2, segment_tokens=ctx, workspace_bytes=128 << 20)
+    orc = O.OracleLibrary(L, Hq, Hkv, D, page_size=P, rope_mode=0, n_pages=-(-kv_len // P) + 2)
+    lib.segment_register(synth.from_bits(kb, "cuda"), synth.from_bits(vb, "cuda"), 0)
+    orc.segment_register(kb, vb, 0)
+    lib.stitch([{"task_id": 0, "entries": [(0, 0, ctx, 0)], "holes": [(ctx, n)], "capacity_tokens": kv_len}])
+    orc.stitch([O.Plan(0, [O.PlanEntry(0, 0, ctx, 0)], [O.Hole(ctx, n)], kv_len)])
+    lib.set_attn_policy(tc_min_rows, splits)
+    out = lib.patch(0, 0, synth.from_bits(q, "cuda"), synth.from_bits(pk, "cuda"), synth.from_bits(pv, "cuda"), pos)
+    torch.cuda.synchronize()
+    ref = orc.patch(0, 0, q, pk, pv, pos)
+    got = out.float().cpu().numpy().astype(np.float64)
+    err = np.abs(got - ref)
+    tol = PEAK_ATOL + PEAK_RTOL * np.abs(ref)
+    assert np.abs(ref).max() > 1.0, "the inputs are not peaked"
+    assert (err <= tol).all(), (f"{int((err > tol).sum())} of {err.size} outputs out of the tight tolerance; max abs err {err.max():.4g}, "
+                                f"worst ratio {(err / tol).max():.3g}; path {lib.stats()['last_attn_path']} splits {lib.stats()['last_attn_splits']}")
+    if splits:
+        assert lib.stats()["last_attn_splits"] == min(splits, tiles)
+    lib.close()
