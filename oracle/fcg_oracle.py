@@ -129,22 +129,31 @@ def rope_rotate_f64(x: np.ndarray, delta, inv_freq: np.ndarray, rope_mode: int =
     phi = np.asarray(delta, dtype=np.float64)[..., None] * inv_freq     # scalar delta -> [D/2]; per-row -> [..., D/2]
     c, s = np.cos(phi), np.sin(phi)
     out = np.empty_like(x)
-    if rope_mode == ROPE_HALF_SPLIT:
-        a, b = x[..., :half], x[..., half:]
-        out[..., :half] = a * c - b * s
-        out[..., half:] = b * c + a * s
-    elif rope_mode == ROPE_INTERLEAVED:
-        a, b = x[..., 0::2], x[..., 1::2]
-        out[..., 0::2] = a * c - b * s
-        out[..., 1::2] = b * c + a * s
-    else:
-        raise OracleError(FCG_ERR_INVALID_ARG, "rope_mode must be half-split (1) or interleaved (2) to rotate")
+    with np.errstate(invalid="ignore"):            # inf - inf, inf * 0 are NaN, quietly (IEEE special values propagate)
+        if rope_mode == ROPE_HALF_SPLIT:
+            a, b = x[..., :half], x[..., half:]
+            out[..., :half] = a * c - b * s
+            out[..., half:] = b * c + a * s
+        elif rope_mode == ROPE_INTERLEAVED:
+            a, b = x[..., 0::2], x[..., 1::2]
+            out[..., 0::2] = a * c - b * s
+            out[..., 1::2] = b * c + a * s
+        else:
+            raise OracleError(FCG_ERR_INVALID_ARG, "rope_mode must be half-split (1) or interleaved (2) to rotate")
     return out
 
 
 def rope_shift_bf16(k_bits: np.ndarray, delta, inv_freq: np.ndarray, rope_mode: int = ROPE_HALF_SPLIT) -> np.ndarray:
-    """bf16 keys -> bf16 keys rotated by ``delta``: fp64 arithmetic, one RNE."""
-    return f64_to_bf16(rope_rotate_f64(bf16_to_f64(k_bits), delta, inv_freq, rope_mode))
+    """bf16 keys -> bf16 keys rotated by ``delta``: fp64 arithmetic, one RNE.
+
+    delta == 0 is the identity ON THE BITS (SURVEY 8(c) P2: "grafted with delta 0 -> K bit-identical to the source";
+    8(c).1: "+-inf / NaN propagate"): evaluating a cos 0 - b sin 0 literally would turn an infinite a or b into NaN
+    through inf * 0 and would canonicalise NaN payloads, which a rotation by nothing must not do.
+    """
+    k_bits = np.asarray(k_bits, dtype=np.uint16)
+    out = f64_to_bf16(rope_rotate_f64(bf16_to_f64(k_bits), delta, inv_freq, rope_mode))
+    same = np.broadcast_to(np.asarray(delta)[..., None] == 0, k_bits.shape)
+    return np.where(same, k_bits, out)
 
 
 # ----------------------------------------------------------------------------

@@ -145,7 +145,11 @@ def test_special_values_through_stitch_and_scatter(D, rope_mode):
         ok, ov = orc.tasks[0].k[layer], orc.tasks[0].v[layer]
         assert np.array_equal(gv[:, f], ov[:, f]), "V (incl. NaN payloads, -0, subnormals) must be a bit copy"
         cg, co = _classes(gk[:, f]), _classes(ok[:, f])
-        assert np.array_equal(cg, co), f"inf / NaN pattern differs in {int((cg != co).sum())} K elements (layer {layer})"
+        if not np.array_equal(cg, co):
+            pos_f = np.flatnonzero(f)
+            bad = np.argwhere(cg != co)
+            lines = [f"head {h} pos {pos_f[t]} el {e}: gpu {gk[h, pos_f[t], e]:#06x} oracle {ok[h, pos_f[t], e]:#06x}" for h, t, e in bad[:16]]
+            raise AssertionError(f"inf / NaN pattern differs in {len(bad)} K elements (layer {layer}):\n" + "\n".join(lines))
         fin = co == 0
         hist += T.assert_k_within_1ulp(gk[:, f][fin], ok[:, f][fin], f"finite K elements, layer {layer}")
         # delta 0 is a bit copy of everything, specials included

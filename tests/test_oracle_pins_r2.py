@@ -278,3 +278,24 @@ def test_fp8_deep_subnormal_rows_round_once():
     lib.stitch([O.Plan(0, [O.PlanEntry(s, 0, 1, 0)])])
     assert np.array_equal(lib.tasks[0].v[0, 0], O.f64_to_bf16(dq))
     assert np.array_equal(lib.tasks[0].k[0, 0], O.f64_to_bf16(dq))       # delta 0: cos 0 = 1, sin 0 = 0 exactly
+
+
+def test_rotation_by_zero_is_the_identity_on_every_bit_pattern():
+    """P2 / 8(c).1: delta = 0 leaves every bf16 pattern alone -- infinities, NaN payloads, -0, subnormals -- for a
+    scalar delta and for the rows of a per-row delta array that are 0; the other rows are rotated."""
+    th = O.rope_inv_freq(16, 1e4)
+    allbits = np.arange(65536, dtype=np.uint16).reshape(-1, 16)
+    for mode in (O.ROPE_HALF_SPLIT, O.ROPE_INTERLEAVED):
+        assert np.array_equal(O.rope_shift_bf16(allbits, 0, th, mode), allbits)
+        deltas = np.where(np.arange(allbits.shape[0]) % 2 == 0, 0, 5)
+        got = O.rope_shift_bf16(allbits, deltas, th, mode)
+        assert np.array_equal(got[0::2], allbits[0::2])
+        assert np.array_equal(got[1::2], O.rope_shift_bf16(allbits[1::2], 5, th, mode))
+    # and a non-zero rotation propagates specials as IEEE arithmetic does: inf stays inf (sign by the cos / sin), NaN stays NaN
+    row = np.zeros((1, 16), np.uint16)
+    row[0, 2] = 0x7F80                                   # +inf in the low half, partner (element 10) = 0
+    out = O.bf16_to_f64(O.rope_shift_bf16(row, 3, th))
+    c, s = np.cos(3 * th[2]), np.sin(3 * th[2])
+    assert out[0, 2] == np.copysign(np.inf, c) and out[0, 10] == np.copysign(np.inf, s)
+    row[0, 10] = 0x7FC0
+    assert np.isnan(O.bf16_to_f64(O.rope_shift_bf16(row, 3, th))[0, [2, 10]]).all()
