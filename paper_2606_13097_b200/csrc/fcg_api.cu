@@ -113,8 +113,8 @@ struct fcg_library {
   int next_slot = 0;
   fcg_stats_t stats;
   int n_segments_live = 0, n_tasks_live = 0;
-  int32_t tc_min_rows = 1;                       // rows per kv head from which the tcgen05 path is used (head_dim 128)
-  fcg::TmaDesc tm_k, tm_v;                       // K / V pool tensor maps for the tcgen05 path (head_dim 128)
+  int32_t tc_min_rows = 1;                       // rows per kv head from which the tcgen05 path is used
+  fcg::TmaDesc tm_k, tm_v;                       // K / V pool tensor maps for the tcgen05 path
   bool have_tma = false;
   int32_t force_splits = 0;                      // > 0: KV splits per task (clamped to its tile count); 0 = choose_splits
 
@@ -550,7 +550,7 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
     lib->host_dev = static_cast<unsigned char *>(attr.devicePointer);
     lib->host_free.push_back({0, cfg->host_arena_bytes / ALIGN * ALIGN});
   }
-  if (cfg->head_dim == 128) {
+  {
     fcg_status_t st = make_pool_tensor_map(lib->cfg, lib->k_pool(), &lib->tm_k);
     if (st == FCG_OK) st = make_pool_tensor_map(lib->cfg, lib->v_pool(), &lib->tm_v);
     if (st != FCG_OK) {

@@ -1,6 +1,6 @@
 // S6: tensor-core patch attention on tcgen05 / TMEM (cache-patching, Eq. 6, PAPER.md:118-123, 718;
-// DESIGN.md "Kernel S6").  Default attention path for head_dim 128: short patches and decode steps (HBM-bound)
-// as well as long patches (tensor-bound).
+// DESIGN.md "Kernel S6").  Default attention path for both head dims (128: two 64-column operand halves per tile;
+// 64: one): short patches and decode steps (HBM-bound) as well as long patches (tensor-bound).
 //
 //   CTA   = (KV split x row group of NQ*128 rows, kv head, layer x task), 1 CTA / SM, template <NQ, PS>:
 //             <1,1>  one 128-row Q tile; R <= 64 rows are held 2x / 4x ("row streams": stream s owns the columns
@@ -33,7 +33,6 @@ namespace {
 
 constexpr int BM = 128;        // query rows per Q tile (UMMA M)
 constexpr int BN = 64;         // cache tokens per K/V tile
-constexpr int D = 128;
 constexpr float RESCALE_TAU = 8.0f;   // log2 units: keep a stale row max while the new one is < 2^8 larger
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -210,19 +209,21 @@ __device__ __forceinline__ float ex2_approx(float x) {
 }
 
 // ---- shared memory map -------------------------------------------------------------------------
-constexpr int Q_TILE_B = BM * D * 2;          // two 64-column halves of [128][128 B]
-constexpr int KV_TILE_B = BN * D * 2;         // two halves of [64][128 B]
-
-template <int NQ, int PS_>
+// D = head_dim (128 or 64): a tile is D / 64 halves of 64 columns, each [rows][128 B] with the 128B swizzle
+template <int NQ, int PS_, int D_>
 struct Cfg {
+  static constexpr int D = D_;
+  static constexpr int CPR = D / 8;                     // 16-byte chunks per row
+  static constexpr int Q_TILE_B = BM * D * 2;
+  static constexpr int KV_TILE_B = BN * D * 2;
   // separate rings: a K stage is free again as soon as Q K^T of its tile has completed, a V stage only after P V
   // P (the A operand of P V) lives in TMEM: the softmax threads write it with tcgen05.st and the MMA reads it from
   // there, so it never crosses shared memory (whose bandwidth -- Q, K, P, V operand reads plus the TMA and P writes,
   // 224 KB per 64-token step with two Q tiles -- was the limiter of the tensor-bound class).  One Q tile: own
   // columns; two Q tiles: P overwrites the first half of its S tile in place (S is then freed by P V, not by s_free).
   static constexpr bool P_ALIAS = NQ == 2;
-  static constexpr int K_STAGES = NQ == 1 ? 6 : 5;
-  static constexpr int V_STAGES = NQ == 1 ? 6 : 5;
+  static constexpr int K_STAGES = (NQ == 1 ? 6 : 5) * (128 / D);      // the same bytes in flight for either head_dim
+  static constexpr int V_STAGES = (NQ == 1 ? 6 : 5) * (128 / D);
   // Tile-parity streams (NQ == 1 only): two softmax warpgroups, group w owns the KV tiles j = w (mod 2), its own
   // S / P buffer and its own O accumulator, with its own running (m, l); the streams are merged by log-sum-exp in
   // the epilogue like the row streams.  Two softmax warps per SM sub-partition hide each other's latencies.
@@ -233,7 +234,7 @@ struct Cfg {
   static constexpr int KLOAD_WARP = N_SOFTMAX / 32, VLOAD_WARP = KLOAD_WARP + 1, MMA_WARP = KLOAD_WARP + 2;
   static constexpr int TMEM_COLS = 512;                 // S: 2*NQ x 64 columns, O: NQ*PS x 128 columns
   static constexpr int TMEM_O = NQ * 128;               // first O column
-  static constexpr int Q_ITERS = NQ * BM * 16 / N_SOFTMAX;
+  static constexpr int Q_ITERS = NQ * BM * CPR / N_SOFTMAX;
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + NQ * Q_TILE_B;                // K stage s at +s*KV_TILE_B
   static constexpr int OFF_V = OFF_K + K_STAGES * KV_TILE_B;         // V stage s at +s*KV_TILE_B
@@ -247,11 +248,12 @@ struct Cfg {
   static_assert((K_STAGES + V_STAGES) * KV_TILE_B >= PS * BM * MROW * 4 + PS * BM * 8, "merge buffer must fit in the idle rings");
 };
 
-template <int NQ, int PS_>
-__global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
+template <int NQ, int PS_, int D>
+__global__ void __launch_bounds__(Cfg<NQ, PS_, D>::NTHREADS, 1)
     attn_tc_kernel(const AttnParams p, const __grid_constant__ TmaDesc tm_k, const __grid_constant__ TmaDesc tm_v) {
-  using C = Cfg<NQ, PS_>;
+  using C = Cfg<NQ, PS_, D>;
   constexpr int SK = C::K_STAGES, SV = C::V_STAGES, PS = C::PS;
+  constexpr int Q_TILE_B = C::Q_TILE_B, KV_TILE_B = C::KV_TILE_B, CPR = C::CPR;
   extern __shared__ unsigned char smem_raw[];
   // 1024-byte alignment for the 128B-swizzle atoms
   unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -378,7 +380,7 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
         for (int i = 0; i < n_ok; ++i) {
           const int pg = __shfl_sync(0xffffffffu, page, i);
           tma_load_5d(dst + i * P * 128, tm, bar, 0, 0, g, pg, layer);
-          tma_load_5d(dst + i * P * 128 + BN * 128, tm, bar, 64, 0, g, pg, layer);
+          if (D == 128) tma_load_5d(dst + i * P * 128 + BN * 128, tm, bar, 64, 0, g, pg, layer);
         }
         page = page_next;
         if (++st == NS) {
@@ -445,8 +447,8 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
           // ragged last tile: zero the V rows that hold no token of this split (whole warp)
           const int r0 = t_end - ts;
           unsigned char *vt = smem + C::OFF_V + sv * KV_TILE_B;
-          for (int i = lane; i < (BN - r0) * 16; i += 32) {
-            const int row = r0 + (i >> 4), c = i & 15;
+          for (int i = lane; i < (BN - r0) * CPR; i += 32) {
+            const int row = r0 + i / CPR, c = i % CPR;
             *reinterpret_cast<uint4 *>(vt + (c >> 3) * (BN * 128) + row * 128 + ((c & 7) << 4)) = make_uint4(0, 0, 0, 0);
           }
           fence_proxy_async();
@@ -503,7 +505,7 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
 #pragma unroll
       for (int i = 0; i < C::Q_ITERS; ++i) {
         const int ci = tid + C::N_SOFTMAX * i;
-        const int row = ci >> 4, c = ci & 15;
+        const int row = ci / CPR, c = ci % CPR;
         const int rt = row & (BM - 1), tq = row >> 7;
         const int rl = rt & (rps - 1);
         qv[i] = make_uint4(0, 0, 0, 0);
@@ -516,7 +518,7 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
 #pragma unroll
       for (int i = 0; i < C::Q_ITERS; ++i) {
         const int ci = tid + C::N_SOFTMAX * i;
-        const int row = ci >> 4, c = ci & 15;
+        const int row = ci / CPR, c = ci % CPR;
         const int rt = row & (BM - 1), tq = row >> 7;
         const uint32_t dst = C::OFF_Q + tq * Q_TILE_B + (c >> 3) * (BM * 128) + rt * 128 + (((c & 7) ^ (rt & 7)) << 4);
         *reinterpret_cast<uint4 *>(smem + dst) = qv[i];
@@ -776,15 +778,15 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_>::NTHREADS, 1)
   }
 }
 
-template <int NQ, int PS_>
+template <int NQ, int PS_, int D>
 cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv, cudaStream_t stream) {
-  using C = Cfg<NQ, PS_>;
+  using C = Cfg<NQ, PS_, D>;
   // the attribute is per device (fcg_config_t.device allows libraries on several GPUs in one process)
   static bool configured[64] = {};
   int dev = -1;
   if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
   if (dev < 0 || dev >= 64 || !configured[dev]) {
-    cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, PS_>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, PS_, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     if (dev >= 0 && dev < 64) configured[dev] = true;
   }
@@ -798,7 +800,7 @@ cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv,
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, attn_tc_kernel<NQ, PS_>, p, tk, tv);
+  return cudaLaunchKernelEx(&cfg, attn_tc_kernel<NQ, PS_, D>, p, tk, tv);
 }
 
 }  // namespace
@@ -807,10 +809,16 @@ cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv,
 // parity_streams (q_tiles == 1 only): 2 = two softmax warpgroups on alternating KV tiles, 1 = one warpgroup.
 cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, int parity_streams, const TmaDesc *tm_k,
                            const TmaDesc *tm_v, cudaStream_t stream) {
-  if (head_dim != 128 || !tm_k || !tm_v) return cudaErrorNotSupported;
-  if (q_tiles == 1 && parity_streams == 2) return launch_nq<1, 2>(p, *tm_k, *tm_v, stream);
-  if (q_tiles == 1) return launch_nq<1, 1>(p, *tm_k, *tm_v, stream);
-  if (q_tiles == 2) return launch_nq<2, 1>(p, *tm_k, *tm_v, stream);
+  if ((head_dim != 128 && head_dim != 64) || !tm_k || !tm_v) return cudaErrorNotSupported;
+  if (head_dim == 128) {
+    if (q_tiles == 1 && parity_streams == 2) return launch_nq<1, 2, 128>(p, *tm_k, *tm_v, stream);
+    if (q_tiles == 1) return launch_nq<1, 1, 128>(p, *tm_k, *tm_v, stream);
+    if (q_tiles == 2) return launch_nq<2, 1, 128>(p, *tm_k, *tm_v, stream);
+  } else {
+    if (q_tiles == 1 && parity_streams == 2) return launch_nq<1, 2, 64>(p, *tm_k, *tm_v, stream);
+    if (q_tiles == 1) return launch_nq<1, 1, 64>(p, *tm_k, *tm_v, stream);
+    if (q_tiles == 2) return launch_nq<2, 1, 64>(p, *tm_k, *tm_v, stream);
+  }
   return cudaErrorInvalidValue;
 }
 

@@ -128,18 +128,18 @@ def test_special_values_through_stitch_and_scatter(D, rope_mode):
     orc = O.OracleLibrary(L, Hq, Hkv, D, page_size=P, rope_mode=rope_mode, rope_base=1e4, n_pages=64, max_task_tokens=512)
     sid = lib.segment_register(synth.from_bits(kb, "cuda"), synth.from_bits(vb, "cuda"), 1000)
     assert sid == orc.segment_register(kb, vb, 1000)
-    # a second copy of the segment with another orig_start, so that the four entries get the deltas
-    # -1000 (large angle), -900, 0 (bit copy) and +100
-    sid2 = lib.segment_register(synth.from_bits(kb, "cuda"), synth.from_bits(vb, "cuda"), 200)
-    assert sid2 == orc.segment_register(kb, vb, 200)
-    plan = {"task_id": 0, "entries": [(sid, 0, n, 0), (sid, 0, n, 100), (sid2, 0, n, 200), (sid2, 0, n, 300)],
-            "holes": [(396, 4)], "capacity_tokens": 400}
-    orc.stitch([O.Plan(0, [O.PlanEntry(*e) for e in plan["entries"]], [O.Hole(396, 4)], 400)])
+    # a second copy of the segment with another orig_start, so that the four back-to-back entries get the deltas
+    # -1000 (large angle), -904, 0 (bit copy) and +96
+    sid2 = lib.segment_register(synth.from_bits(kb, "cuda"), synth.from_bits(vb, "cuda"), 192)
+    assert sid2 == orc.segment_register(kb, vb, 192)
+    plan = {"task_id": 0, "entries": [(sid, 0, n, 0), (sid, 0, n, 96), (sid2, 0, n, 192), (sid2, 0, n, 288)],
+            "holes": [(384, 4)], "capacity_tokens": 388}
+    orc.stitch([O.Plan(0, [O.PlanEntry(*e) for e in plan["entries"]], [O.Hole(384, 4)], 388)])
     lib.stitch([plan])
-    assert orc.tasks[0].deltas == [-1000, -900, 0, 100]
+    assert orc.tasks[0].deltas == [-1000, -904, 0, 96]
     hist = np.zeros(4, np.int64)
     for layer in range(L):
-        kg, vg = lib.task_read(0, layer, 0, 400)
+        kg, vg = lib.task_read(0, layer, 0, 388)
         gk, gv = synth.to_bits(kg), synth.to_bits(vg)
         f = orc.tasks[0].filled
         ok, ov = orc.tasks[0].k[layer], orc.tasks[0].v[layer]
@@ -153,19 +153,19 @@ def test_special_values_through_stitch_and_scatter(D, rope_mode):
         fin = co == 0
         hist += T.assert_k_within_1ulp(gk[:, f][fin], ok[:, f][fin], f"finite K elements, layer {layer}")
         # delta 0 is a bit copy of everything, specials included
-        assert np.array_equal(gk[:, 200:200 + n], kb[layer])
+        assert np.array_equal(gk[:, 192:192 + n], kb[layer])
         # no flush-to-zero: a rotated subnormal row stays non-zero wherever the oracle's is
         z_o, z_g = (ok[:, f] & 0x7FFF) == 0, (gk[:, f] & 0x7FFF) == 0
         assert int((z_g & ~z_o).sum()) <= int(hist[1]), "subnormal results flushed to zero"
     assert (co != 0).sum() > 50 and hist[0] > 0
     # scatter: patch K / V rows full of specials land bit-exact
-    pos = np.asarray([396, 397, 398, 399], np.int32)
+    pos = np.asarray([384, 385, 386, 387], np.int32)
     pk = np.tile(SPECIALS, 2 * 4 * Hkv * D // len(SPECIALS) + 1)[: L * 4 * Hkv * D].reshape(L, 4, Hkv, D).copy()
     q = O.f64_to_bf16(rng.standard_normal((L, 4, Hq, D)))
     lib.patch(0, 0, synth.from_bits(q, "cuda"), synth.from_bits(pk, "cuda"), synth.from_bits(pk[::-1].copy(), "cuda"), pos)
     torch.cuda.synchronize()
     for layer in range(L):
-        kg, vg = lib.task_read(0, layer, 396, 4)
+        kg, vg = lib.task_read(0, layer, 384, 4)
         assert np.array_equal(synth.to_bits(kg), np.transpose(pk[layer], (1, 0, 2)))
         assert np.array_equal(synth.to_bits(vg), np.transpose(pk[::-1][layer], (1, 0, 2)))
     lib.close()
