@@ -45,6 +45,10 @@ FALLBACK_BF16_SUSTAINED = 1400.0
 HEADLINE = "C4"
 ALL_CONFIGS = ("C4", "C2", "C3", "C5")
 EXTRACT_TOKENS = 1024
+# not a BASELINE.json configuration: the head_dim-64 geometry of C1 at a size that streams from HBM (4k tokens, a
+# 16-token patch at the end; the decode step is in its next_rows) -- the short-patch path of north_star at head_dim 64
+D64 = synth.GraftConfig("D64-4k", 32, 32, 32, 64, 16, 1e4, 64, 128, 1024, 8192, 1, 6, 6, 4096, holes=((-1, 16),))
+BENCH_CONFIGS = dict(synth.CONFIGS, D64=D64)
 
 
 def _peaks_file():
@@ -218,15 +222,18 @@ def build_library(cfg, wl, seed, device_index, on_segment=None, kv_heads=None, t
     tasks = wl.tasks if tasks is None else tasks
     total_pages = sum(-(-t.capacity // cfg.page_size) for t in tasks)
     seg_tokens = int(wl.seg_lens.sum())
+    n_fp8 = 0
     if extra:
         # + EXTRACT_TOKENS of arena and + half a task of pages: room for the NEXT-row measurements (segment extraction,
-        # copy-on-shift); neither changes what the graft step itself touches
-        seg_tokens += EXTRACT_TOKENS
+        # copy-on-shift, fp8 copies of task 0's segments); none changes what the graft step itself touches
+        used0 = sorted({s for (s, _, _, _) in tasks[0].entries})
+        n_fp8 = len(used0)
+        seg_tokens += EXTRACT_TOKENS + int(sum(int(wl.seg_lens[s]) for s in used0)) * 5 // 8 + 16 * n_fp8
         total_pages += max(-(-t.capacity // cfg.page_size) for t in tasks) // 2 + 8
     full = wl.cfg
     lib = binding.FcgLibrary(n_layers=cfg.n_layers, n_q_heads=cfg.n_q_heads, n_kv_heads=cfg.n_kv_heads,
                              head_dim=cfg.head_dim, page_size=cfg.page_size, rope_base=cfg.rope_base,
-                             max_segments=full.n_segments + 1, max_tasks=max(max(t.task_id for t in tasks) + 1, 1),
+                             max_segments=full.n_segments + 1 + n_fp8, max_tasks=max(max(t.task_id for t in tasks) + 1, 1),
                              max_task_tokens=max(t.capacity for t in tasks), n_pages=total_pages + 16,
                              workspace_bytes=2 << 30, segment_tokens=seg_tokens, device=device_index,
                              host_tier_tokens=(int(wl.seg_lens[tasks[0].entries[0][0]]) + 16) if extra else 0)
@@ -415,7 +422,7 @@ def describe(cfg, name, wl, tasks, seed):
 def measure_config(args, name, seed, D: Dist, sampler, traffic, steps, *, full, shard_mode="none"):
     """One configuration on this rank's shard: build the library, time `steps` graft steps; `full` adds the end-to-end
     leg and (rank 0) the NEXT rows.  Returns the per-config record (rank 0 decides what to print)."""
-    cfg_full = synth.CONFIGS[name]
+    cfg_full = BENCH_CONFIGS[name]
     if args.page_size:
         cfg_full = synth.scaled(cfg_full, page_size=args.page_size)
     kv_heads = q_heads = None
@@ -579,6 +586,25 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
         res["patch_one_call_per_layer_graph"] = {"ms": ms, "host_enqueue_ms": host, "calls": 1,
                                                  "note": f"the {cfg.n_layers} planned per-layer calls captured into one CUDA graph, one replay per step"}
         del g
+        # layers are independent: inside the capture the per-layer calls are forked over 4 streams (their split-KV
+        # partials live in per-layer slots), so the launch latencies of one layer hide behind the kernels of the others
+        lanes = [side] + [torch.cuda.Stream(device=dev) for _ in range(3)]
+        g4 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g4, stream=side):
+            fork = torch.cuda.Event()
+            fork.record(side)
+            for st_ in lanes[1:]:
+                st_.wait_event(fork)
+            for l, (a_, b_, c_, d_) in enumerate(views):
+                lib.patch_planned(plan, l, a_, b_, c_, d_, stream=lanes[l % 4])
+            for st_ in lanes[1:]:
+                ev = torch.cuda.Event()
+                ev.record(st_)
+                side.wait_event(ev)
+        ms, host = timed_loop(g4.replay)
+        res["patch_one_call_per_layer_graph_4_lanes"] = {"ms": ms, "host_enqueue_ms": host, "calls": 1,
+                                                         "note": "the same graph with the layers forked round-robin over 4 captured streams"}
+        del g4
         lib.patch_plan_destroy(plan)
         del qp, kp, vp, op, views
     except Exception as e:
@@ -619,12 +645,70 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
         host_ms = timed(lambda: lib.stitch(plan), before=lambda: lib.pool_info()["n_tasks_live"] and lib.task_release(t.task_id))
         lib.task_release(t.task_id)
         lib.segment_prefetch(seg)
+        # NEXT-3 overlap: task 0's real plan with its first segment in the host tier -- read in place (fcg_stitch) vs
+        # copied back by the copy engine while the resident entries are stitched (fcg_stitch_prefetch)
+        try:
+            plan0 = [{"task_id": t.task_id, "entries": t.entries, "holes": t.holes, "capacity_tokens": t.capacity}]
+            rel = lambda: lib.pool_info()["n_tasks_live"] and lib.task_release(t.task_id)
+
+            def before():
+                rel()
+                lib.segment_offload(seg)
+
+            inplace_ms = timed(lambda: lib.stitch(plan0), before=before)
+            overlap_ms = timed(lambda: lib.stitch_prefetch(plan0), before=before)
+            rel()
+            res["stitch_prefetch_overlap"] = {"ms": overlap_ms, "in_place_ms": inplace_ms, "offloaded_bytes": int(seg_bytes),
+                                              "offloaded_GBps": seg_bytes / (overlap_ms * 1e-3) / 1e9,
+                                              "note": f"task 0's plan ({sum(n for (_, _, n, _) in t.entries)} tokens) with one {n_seg}-token segment offloaded: "
+                                                      "fcg_stitch_prefetch (copy engine + overlapped stitch of the resident entries; the segment ends up "
+                                                      "resident) vs fcg_stitch reading it in place over the host link"}
+        except Exception as e:
+            res["stitch_prefetch_overlap"] = {"error": repr(e)}
         res["segment_offload"] = {"ms": off_ms, "GBps": seg_bytes / (off_ms * 1e-3) / 1e9, "bytes": int(seg_bytes)}
         res["segment_prefetch"] = {"ms": pre_ms, "GBps": seg_bytes / (pre_ms * 1e-3) / 1e9, "bytes": int(seg_bytes)}
         res["stitch_from_host_tier"] = {"ms": host_ms, "GBps": seg_bytes / (host_ms * 1e-3) / 1e9, "bytes": int(seg_bytes),
                                         "note": f"{n_seg}-token segment read in place from pinned host memory (bytes = one-way)"}
     except Exception as e:
         res["two_tier"] = {"error": repr(e)}
+    # NEXT-4 fp8 library storage (R26): task 0's segments once more as fp8 segments, the same plan stitched from them;
+    # algorithmic bytes per stitched token = L * Hkv * (2 D + 2 read + 4 D written) instead of L * Hkv * 8 D
+    try:
+        used0 = sorted({s for (s, _, _, _) in t.entries})
+        gen_cfg = synth.scaled(wl.cfg, page_size=cfg.page_size)
+        fp8_id = {}
+        for s_ in used0:
+            k8, v8 = synth.segment_kv(gen_cfg, s_, int(wl.seg_lens[s_]), seed, dev)
+            if k8.shape[1] != cfg.n_kv_heads:
+                raise RuntimeError("head-sharded library: fp8 row skipped")
+            fp8_id[s_] = lib.segment_register_fp8(k8, v8, int(wl.orig_starts[s_]))
+            del k8, v8
+        n_st = int(sum(n for (_, _, n, _) in t.entries))
+        plan16 = [{"task_id": t.task_id, "entries": t.entries, "holes": t.holes, "capacity_tokens": t.capacity}]
+        plan8 = [{"task_id": t.task_id, "entries": [(fp8_id[s_], b_, n_, d_) for (s_, b_, n_, d_) in t.entries], "holes": t.holes,
+                  "capacity_tokens": t.capacity}]
+
+        def restitch(pl_):
+            def f():
+                if lib.pool_info()["n_tasks_live"]:
+                    lib.task_release(t.task_id)
+                lib.stitch(pl_)
+            return f
+
+        ms16, _ = timed_loop(restitch(plan16))
+        ms8, _ = timed_loop(restitch(plan8))
+        lib.task_release(t.task_id)
+        b16 = n_st * cfg.n_layers * cfg.n_kv_heads * cfg.head_dim * 8
+        b8 = n_st * cfg.n_layers * cfg.n_kv_heads * (cfg.head_dim * 6 + 2)
+        fmt, nb8 = lib.segment_storage(fp8_id[used0[0]])
+        _, nb16 = lib.segment_storage(used0[0])
+        res["stitch_fp8"] = {"ms": ms8, "GBps": b8 / (ms8 * 1e-3) / 1e9, "bytes": int(b8), "bf16_same_plan_ms": ms16,
+                             "bf16_same_plan_GBps": b16 / (ms16 * 1e-3) / 1e9, "stored_bytes_ratio": nb8 / nb16,
+                             "note": f"task 0 ({n_st} tokens) stitched from e4m3 segments (de-quantise -> rotate -> bf16 pages) vs from bf16 segments"}
+        for s_ in used0:
+            lib.segment_release(fp8_id[s_])
+    except Exception as e:
+        res["stitch_fp8"] = {"error": repr(e)}
     res["task_shift"]["note"] = f"two moves of {n_shift} tokens (-16, +16) per iteration"
     res["segment_extract"]["note"] = f"{n_ext} tokens un-rotated to orig_start 0"
     res["segment_register"]["note"] = f"S1: {n_ext} tokens copied into the library (read + write)"
@@ -721,10 +805,10 @@ def run_cuda(args):
     single = args.config != "all"
     head_name = args.config if single else HEADLINE
     if D.world > 1:
-        mode = args.shard if args.shard != "auto" else ("weak" if synth.CONFIGS[head_name].n_tasks > 1 else "head")
+        mode = args.shard if args.shard != "auto" else ("weak" if BENCH_CONFIGS[head_name].n_tasks > 1 else "head")
     else:
         mode = "none"
-    if mode == "head" and synth.CONFIGS[head_name].n_kv_heads % D.world:
+    if mode == "head" and BENCH_CONFIGS[head_name].n_kv_heads % D.world:
         mode = "replica"
     seeds = [int(s) for s in args.seeds.split(",") if s]
     configs = {}
@@ -761,7 +845,7 @@ def run_cuda(args):
 
     def region_steps(name):
         # sub-configurations: at least 20 steps and a region of >= ~0.12 s, so that the clock samples fall inside it
-        est = {"C2": 1.0, "C3": 0.75, "C4": 8.0, "C5": 13.5}.get(name, 5.0)
+        est = {"C2": 1.0, "C3": 0.75, "C4": 8.0, "C5": 13.5, "D64": 0.5}.get(name, 5.0)
         return int(max(20, args.steps, math.ceil(120.0 / est)))
 
     def other_seeds(name, mode_):
@@ -808,6 +892,15 @@ def run_cuda(args):
                 configs["C1"] = c1_latency(args, D, args.seed)
             except Exception as e:
                 configs["C1"] = {"error": repr(e)}
+        if D.world == 1:
+            try:
+                r, l, _ = measure_config(args, "D64", args.seed, D, sampler, traffic, 120, full=True, shard_mode="none")
+                l.close()
+                del l
+                torch.cuda.empty_cache()
+                configs["D64"] = {k: v for k, v in r.items() if not k.startswith("_")}
+            except Exception as e:
+                configs["D64"] = {"error": repr(e)}
     res["configs"] = configs
     if sampler:
         sampler.stop()
@@ -882,7 +975,7 @@ def run_reference(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return None
     name = args.config if args.config != "all" else HEADLINE
-    cfg = synth.CONFIGS[name]
+    cfg = BENCH_CONFIGS[name]
     wl = synth.make_workload(cfg, args.seed)
     seed = args.seed
     cache = {}
@@ -928,7 +1021,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="all", choices=["all"] + sorted(synth.CONFIGS),
+    ap.add_argument("--config", default="all", choices=["all"] + sorted(BENCH_CONFIGS),
                     help="all (default): headline C4 plus C2, C3, C5 and C1 in the `configs` key; or one configuration only")
     ap.add_argument("--seed", type=int, default=1, help="layout seed of the headline numbers")
     ap.add_argument("--seeds", default="1,2,3", help="layout seeds reported per configuration (the paper's seeds)")

@@ -62,6 +62,7 @@ enum {
 };
 
 enum { FCG_ROPE_NONE = 0, FCG_ROPE_HALF_SPLIT = 1, FCG_ROPE_INTERLEAVED = 2 };
+enum { FCG_STORE_BF16 = 0, FCG_STORE_FP8_E4M3 = 1 };   /* storage format of a library segment */
 
 /* Geometry and capacities, fixed at create time.
  * Arena layout (all offsets 256-byte aligned, reported by fcg_pool_info):
@@ -112,6 +113,24 @@ fcg_status_t fcg_library_destroy(fcg_library_t *lib);
 fcg_status_t fcg_segment_register(fcg_library_t *lib, const void *k, const void *v, int32_t n_tokens,
                                   int32_t orig_start, const int64_t *strides, void *stream,
                                   int32_t *seg_id_out);
+/* S1 with fp8 storage (memory pressure of the code cache: PAPER.md:81-87; R26).
+ * Same arguments as fcg_segment_register; the bf16 rows are quantised once, here: every stored row (the head_dim
+ * elements of one (layer, kv head, token)) keeps OCP E4M3 codes (1 byte per element) and one power-of-two scale
+ * 2^e (1 byte, e + 127): e = the smallest integer with max|x| <= 448 * 2^e over the row's finite elements, clamped
+ * to [-127, 127], 0 for an all-zero row; code = RNE_e4m3(x * 2^-e); +-inf and NaN have no E4M3 value and become the
+ * NaN code.  The segment takes (head_dim + 1) / (2 head_dim) of the bf16 bytes.  Plans, offload / prefetch and
+ * release treat it like any segment; fcg_stitch de-quantises (exactly) BEFORE the rotation, so a shifted key is one
+ * rounding away from the exact rotation of the stored value, and values are the de-quantised values rounded to
+ * bf16 (exact outside bf16's subnormal range).  The paged cache itself stays bf16. */
+fcg_status_t fcg_segment_register_fp8(fcg_library_t *lib, const void *k, const void *v, int32_t n_tokens,
+                                      int32_t orig_start, const int64_t *strides, void *stream, int32_t *seg_id_out);
+/* Storage format (FCG_STORE_*) and bytes a segment occupies in its tier; either output may be NULL. */
+fcg_status_t fcg_segment_storage(fcg_library_t *lib, int32_t seg_id, int32_t *format, uint64_t *bytes);
+/* Copies the stored representation of a segment out (tests, inspection): k_out, v_out [n_layers][n_kv_heads][n][head_dim]
+ * -- bf16, or uint8 E4M3 codes for an fp8 segment, whose scale bytes (e + 127) go to k_exp_out, v_exp_out
+ * [n_layers][n_kv_heads][n] (required then, ignored otherwise).  Device or host destinations.  Asynchronous on `stream`. */
+fcg_status_t fcg_segment_read(fcg_library_t *lib, int32_t seg_id, void *k_out, void *v_out, void *k_exp_out,
+                              void *v_exp_out, void *stream);
 /* The caller guarantees no enqueued stitch still reads the segment. */
 fcg_status_t fcg_segment_release(fcg_library_t *lib, int32_t seg_id);
 
@@ -138,6 +157,15 @@ typedef struct {
  * Entries with delta 0 (and rope_mode NONE) are bit copies.  Any failing plan fails the whole batch
  * with nothing changed.  Unused tail slots of the last page are never written nor read (R10). */
 fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_plans, void *stream);
+
+/* fcg_stitch with overlapped prefetch (Table 19: CPU -> GPU reloads "only
+ * when a required function cache is not resident").  Same arguments, same result, same page tables.  Segments of
+ * the host tier that the plans name are first copied back to the device tier -- one host->device copy each, on a
+ * stream of the library's own, into a first-fit arena range (a segment that finds no room stays offloaded and is read
+ * in place, as fcg_stitch does) -- WHILE the entries of the resident segments are being stitched on `stream`; the
+ * entries of the prefetched segments are stitched by a second launch on `stream` once their copies have landed.  On
+ * return (status OK) those segments are resident, as after fcg_segment_prefetch. */
+fcg_status_t fcg_stitch_prefetch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_plans, void *stream);
 
 /* S4 + S5/S6 (Eq. 6).  q [n_layers][n][n_q_heads][head_dim], k, v [n_layers][n][n_kv_heads][head_dim],
  * out [n_layers][n][n_q_heads][head_dim]: device bf16, contiguous, for cache layers
@@ -199,7 +227,10 @@ fcg_status_t fcg_patch_batch_host(fcg_library_t *lib, const int32_t *task_ids, c
  * n_layers) with q, k, v, out as in fcg_patch_batch; it may be called any number of times, with any tensors, and
  * may be captured into a CUDA graph (it makes no copies and touches no host state besides launch statistics; while
  * the stream is capturing, the stream-ordering rule above is skipped and the caller orders the graph against other
- * work on the library).  BAD_TASK if a task of the plan was released or re-stitched since.  Destroy returns the
+ * work on the library).  Planned calls for DISJOINT layer ranges touch disjoint memory (their split-KV partials live
+ * in per-layer slots of the workspace; OUT_OF_ARENA at plan creation if those do not fit), so inside a capture they
+ * may be forked over several streams and run concurrently.  BAD_TASK if a task of the plan was released or
+ * re-stitched since.  Destroy returns the
  * device range; the caller guarantees no enqueued work still reads it. */
 typedef struct fcg_patch_plan fcg_patch_plan_t;
 fcg_status_t fcg_patch_plan_create(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task, int32_t n_tasks,

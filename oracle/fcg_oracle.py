@@ -411,8 +411,12 @@ class OracleLibrary:
         return capacity, T, deltas
 
     # -- S2 + S3 -------------------------------------------------------------
-    def stitch(self, plans: list) -> None:
+    def stitch(self, plans: list, prefetch: bool = False) -> None:
         """Build page tables and gather + RoPE-shift (Eq. 4).
+
+        ``prefetch`` (reloads "only when a required function cache is not
+        resident"): offloaded segments named by the plans come back to the device tier as part of the call; the
+        stitched cache is the same either way -- only the residency flags differ afterwards.
 
         All plans are validated and all pages reserved before any state
         changes (allocate-then-commit): a failing batch leaves the library as
@@ -431,6 +435,10 @@ class OracleLibrary:
             checked.append((plan, cap, T, deltas, n_pg))
         if need > self.pool.available():
             raise OracleError(FCG_ERR_OUT_OF_PAGES, f"need {need} pages, {self.pool.available()} free")
+        if prefetch:
+            for plan, *_ in checked:
+                for e in plan.entries:
+                    self.segments[e.seg_id].resident = True
         for plan, cap, T, deltas, n_pg in checked:
             table = self.pool.allocate(n_pg)           # plans in array order, pages in ascending logical order
             kc = np.zeros((self.L, self.Hkv, cap, self.D), np.uint16)
@@ -444,7 +452,7 @@ class OracleLibrary:
                     # R26: de-quantise (exact), rotate in fp64, ONE rounding to bf16; V: de-quantise, round to bf16
                     # (exact whenever code * 2^e is a bf16 value, i.e. everywhere but the deepest subnormals)
                     kf = fp8_dequantize_rows(seg.k[:, :, src], seg.k_exp[:, :, src])
-                    if self.rope_mode != 0:
+                    if self.rope_mode != 0 and delta != 0:         # delta 0 is the identity (P2), also for a NaN partner
                         kf = rope_rotate_f64(kf, delta, self.inv_freq, self.rope_mode)
                     kc[:, :, dst] = f64_to_bf16(kf)
                     vc[:, :, dst] = f64_to_bf16(fp8_dequantize_rows(seg.v[:, :, src], seg.v_exp[:, :, src]))

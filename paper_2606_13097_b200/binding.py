@@ -31,6 +31,8 @@ FCG_ERR_BAD_TASK = -9
 FCG_ROPE_NONE = 0
 FCG_ROPE_HALF_SPLIT = 1
 FCG_ROPE_INTERLEAVED = 2
+FCG_STORE_BF16 = 0
+FCG_STORE_FP8_E4M3 = 1
 
 
 class FcgError(RuntimeError):
@@ -86,11 +88,15 @@ SYMBOLS = {
     "fcg_library_create": (_I, [C.POINTER(fcg_config_t), C.POINTER(_P)]),
     "fcg_library_destroy": (_I, [_P]),
     "fcg_segment_register": (_I, [_P, _P, _P, _I, _I, C.POINTER(C.c_int64), _P, _PI]),
+    "fcg_segment_register_fp8": (_I, [_P, _P, _P, _I, _I, C.POINTER(C.c_int64), _P, _PI]),
+    "fcg_segment_storage": (_I, [_P, _I, _PI, C.POINTER(C.c_uint64)]),
+    "fcg_segment_read": (_I, [_P, _I, _P, _P, _P, _P, _P]),
     "fcg_segment_release": (_I, [_P, _I]),
     "fcg_segment_offload": (_I, [_P, _I, _P]),
     "fcg_segment_prefetch": (_I, [_P, _I, _P]),
     "fcg_segment_info": (_I, [_P, _I, _PI, _PI, _PI]),
     "fcg_stitch": (_I, [_P, C.POINTER(fcg_plan_t), _I, _P]),
+    "fcg_stitch_prefetch": (_I, [_P, C.POINTER(fcg_plan_t), _I, _P]),
     "fcg_patch": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
     "fcg_patch_host": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
     "fcg_patch_rope": (_I, [_P, _I, _I, _I, _P, _P, _P, _PI, _I, _P, _P]),
@@ -220,6 +226,27 @@ def fcg_segment_register(handle, k, v, n_tokens, orig_start, strides=None, strea
     return sid.value
 
 
+def fcg_segment_register_fp8(handle, k, v, n_tokens, orig_start, strides=None, stream=None) -> int:
+    sid = C.c_int32(-1)
+    st = None
+    if strides is not None:
+        st = (C.c_int64 * 4)(*[int(s) for s in strides])
+    _check(load().fcg_segment_register_fp8(handle, _ptr(k), _ptr(v), int(n_tokens), int(orig_start), st,
+                                           _stream(stream), C.byref(sid)))
+    return sid.value
+
+
+def fcg_segment_storage(handle, seg_id):
+    """-> (format, bytes)"""
+    fmt, nbytes = C.c_int32(), C.c_uint64()
+    _check(load().fcg_segment_storage(handle, int(seg_id), C.byref(fmt), C.byref(nbytes)))
+    return fmt.value, nbytes.value
+
+
+def fcg_segment_read(handle, seg_id, k_out, v_out, k_exp_out=None, v_exp_out=None, stream=None) -> None:
+    _check(load().fcg_segment_read(handle, int(seg_id), _ptr(k_out), _ptr(v_out), _ptr(k_exp_out), _ptr(v_exp_out), _stream(stream)))
+
+
 def fcg_segment_release(handle, seg_id) -> None:
     _check(load().fcg_segment_release(handle, int(seg_id)))
 
@@ -246,6 +273,11 @@ def _marshal_plans(plans):
 def fcg_stitch(handle, plans, stream=None) -> None:
     arr, _keep = _marshal_plans(list(plans))
     _check(load().fcg_stitch(handle, arr, len(arr), _stream(stream)))
+
+
+def fcg_stitch_prefetch(handle, plans, stream=None) -> None:
+    arr, _keep = _marshal_plans(list(plans))
+    _check(load().fcg_stitch_prefetch(handle, arr, len(arr), _stream(stream)))
 
 
 def fcg_patch(handle, task_id, layer_begin, n_layers, q, k, v, positions, out, stream=None) -> None:
@@ -462,6 +494,28 @@ class FcgLibrary:
         assert k.shape == v.shape and k.stride() == v.stride()
         return fcg_segment_register(self.handle, k, v, k.shape[2], orig_start, k.stride(), stream)
 
+    def segment_register_fp8(self, k: torch.Tensor, v: torch.Tensor, orig_start: int, stream=None) -> int:
+        assert k.dtype == torch.bfloat16 and v.dtype == torch.bfloat16 and k.is_cuda and v.is_cuda
+        assert k.shape == v.shape and k.stride() == v.stride()
+        return fcg_segment_register_fp8(self.handle, k, v, k.shape[2], orig_start, k.stride(), stream)
+
+    def segment_storage(self, seg_id):
+        return fcg_segment_storage(self.handle, seg_id)
+
+    def segment_read(self, seg_id, stream=None):
+        """the stored representation: (k, v) bf16 tensors, or (k codes, v codes, k scale bytes, v scale bytes) uint8"""
+        n, _, _ = fcg_segment_info(self.handle, seg_id)
+        fmt, _ = fcg_segment_storage(self.handle, seg_id)
+        shape = (self.n_layers, self.n_kv_heads, n, self.head_dim)
+        if fmt == FCG_STORE_FP8_E4M3:
+            k, v = torch.empty(shape, dtype=torch.uint8, device=self.device), torch.empty(shape, dtype=torch.uint8, device=self.device)
+            ke, ve = torch.empty(shape[:3], dtype=torch.uint8, device=self.device), torch.empty(shape[:3], dtype=torch.uint8, device=self.device)
+            fcg_segment_read(self.handle, seg_id, k, v, ke, ve, stream)
+            return k, v, ke, ve
+        k, v = torch.empty(shape, dtype=torch.bfloat16, device=self.device), torch.empty(shape, dtype=torch.bfloat16, device=self.device)
+        fcg_segment_read(self.handle, seg_id, k, v, None, None, stream)
+        return k, v
+
     def segment_release(self, seg_id):
         fcg_segment_release(self.handle, seg_id)
 
@@ -476,6 +530,9 @@ class FcgLibrary:
 
     def stitch(self, plans, stream=None):
         fcg_stitch(self.handle, plans, stream)
+
+    def stitch_prefetch(self, plans, stream=None):
+        fcg_stitch_prefetch(self.handle, plans, stream)
 
     def patch(self, task_id, layer_begin, q, k, v, positions, out=None, stream=None) -> torch.Tensor:
         assert q.is_cuda and q.is_contiguous() and k.is_contiguous() and v.is_contiguous()

@@ -48,6 +48,7 @@ struct SegmentRec {
   uint64_t offset = 0, bytes = 0;   // in the arena (resident) or in the host tier (offloaded); K then V
   bool resident = true;
   int32_t n_tokens = 0, orig_start = 0;
+  int32_t fmt = FCG_STORE_BF16;     // FCG_STORE_FP8_E4M3: K codes, K scale bytes, V codes, V scale bytes (R26)
 };
 
 struct TaskRec {
@@ -107,6 +108,7 @@ struct fcg_library {
   int patch_blob_slot = -1;
   uint64_t patch_blob_gen = 0;
   cudaStream_t patch_blob_stream = nullptr;      // the stream that uploaded it (reuse only on the same stream)
+  cudaEvent_t prefetch_ev = nullptr;             // fcg_stitch_prefetch: the host->device copies of one call have landed
   cudaEvent_t staging_ev = nullptr;              // last use of the host-call staging area
   bool have_staging_ev = false;
   int n_plans_live = 0;
@@ -122,9 +124,12 @@ struct fcg_library {
   uint16_t *v_pool() const { return reinterpret_cast<uint16_t *>(arena + v_pool_off); }
   int32_t *tables() const { return reinterpret_cast<int32_t *>(arena + table_off); }
   uint64_t kv_row_bytes() const { return (uint64_t)cfg.head_dim * 2; }
-  uint64_t seg_bytes_for(int64_t n) const {
-    return 2 * align_up((uint64_t)cfg.n_layers * cfg.n_kv_heads * (uint64_t)n * kv_row_bytes());
+  uint64_t seg_bytes_for(int64_t n, int32_t fmt = FCG_STORE_BF16) const {
+    const uint64_t rows = (uint64_t)cfg.n_layers * cfg.n_kv_heads * (uint64_t)n;
+    if (fmt == FCG_STORE_FP8_E4M3) return 2 * (fp8_code_bytes(n) + align_up(rows));
+    return 2 * align_up(rows * kv_row_bytes());
   }
+  uint64_t fp8_code_bytes(int64_t n) const { return align_up((uint64_t)cfg.n_layers * cfg.n_kv_heads * (uint64_t)n * cfg.head_dim); }
 };
 
 namespace {
@@ -310,7 +315,7 @@ struct SegmentSlot {
   uint64_t off = 0, bytes = 0;
 };
 
-fcg_status_t find_segment_slot(fcg_library *lib, int32_t n_tokens, SegmentSlot &sl) {
+fcg_status_t find_segment_slot(fcg_library *lib, int32_t n_tokens, SegmentSlot &sl, int32_t fmt = FCG_STORE_BF16) {
   const fcg_config_t &c = lib->cfg;
   sl.sid = -1;
   for (int32_t i = 0; i < c.max_segments; ++i)
@@ -319,7 +324,7 @@ fcg_status_t find_segment_slot(fcg_library *lib, int32_t n_tokens, SegmentSlot &
       break;
     }
   if (sl.sid < 0) return fail(FCG_ERR_OUT_OF_ARENA, "segment table full (%d)", c.max_segments);
-  sl.bytes = lib->seg_bytes_for(n_tokens);
+  sl.bytes = lib->seg_bytes_for(n_tokens, fmt);
   sl.fi = range_find(lib->seg_free, sl.bytes);
   if (sl.fi == lib->seg_free.size())
     return fail(FCG_ERR_OUT_OF_ARENA, "no free arena range of %llu bytes for a %d-token segment", (unsigned long long)sl.bytes, n_tokens);
@@ -327,10 +332,11 @@ fcg_status_t find_segment_slot(fcg_library *lib, int32_t n_tokens, SegmentSlot &
   return FCG_OK;
 }
 
-void commit_segment_slot(fcg_library *lib, const SegmentSlot &sl, int32_t n_tokens, int32_t orig_start) {
+void commit_segment_slot(fcg_library *lib, const SegmentSlot &sl, int32_t n_tokens, int32_t orig_start, int32_t fmt = FCG_STORE_BF16) {
   range_take(lib->seg_free, sl.fi, sl.bytes);
   SegmentRec &s = lib->segments[sl.sid];
   s.live = true;
+  s.fmt = fmt;
   s.offset = sl.off;
   s.bytes = sl.bytes;
   s.n_tokens = n_tokens;
@@ -347,6 +353,7 @@ struct GatherBuilder {
   std::vector<float4> table;
   std::vector<int32_t> pages;                    // page ids, copied device-to-device into page tables after the H2D
   std::map<int32_t, int32_t> table_of_delta;
+  bool any_fp8 = false;
 
   // first float4 of the table of `delta`, or -1 for a bit copy
   int32_t table_for(const fcg_library *lib, int32_t delta) {
@@ -391,6 +398,18 @@ struct GatherBuilder {
     layer_stride = (int64_t)lib->cfg.n_kv_heads * n;
     head_stride = n;
   }
+  // source side of an entry that reads a library segment (either tier, either storage format)
+  void source_segment(const fcg_library *lib, const SegmentRec &s, fcg::StitchEntryDev &de) {
+    segment_side(lib, s.resident ? lib->arena : lib->host_dev, s.offset, s.bytes, s.n_tokens, de.k_src, de.v_src, de.src_layer_stride,
+                 de.src_head_stride);
+    de.src_fp8 = s.fmt == FCG_STORE_FP8_E4M3 ? 1 : 0;
+    de.k_exp = de.v_exp = 0;
+    if (de.src_fp8) {
+      de.k_exp = de.k_src + lib->fp8_code_bytes(s.n_tokens);
+      de.v_exp = de.v_src + lib->fp8_code_bytes(s.n_tokens);
+      any_fp8 = true;
+    }
+  }
   int32_t pool_tok(const fcg_library *lib, int32_t page, int32_t slot) const {
     return page * lib->cfg.n_kv_heads * lib->cfg.page_size + slot;
   }
@@ -434,6 +453,7 @@ fcg_status_t enqueue_gather(fcg_library *lib, const GatherBuilder &gb, cudaStrea
   sp.entries = reinterpret_cast<const fcg::StitchEntryDev *>(slot->dev + off_entries);
   sp.chunks = reinterpret_cast<const fcg::StitchChunkDev *>(slot->dev + off_chunks);
   sp.table = reinterpret_cast<const float4 *>(slot->dev + off_table);
+  sp.any_fp8 = gb.any_fp8 ? 1 : 0;
   sp.n_chunks = (int32_t)gb.chunks.size();
   sp.n_layers = c.n_layers;
   sp.n_kv_heads = c.n_kv_heads;
@@ -528,6 +548,7 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&lib->d2h_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->last_ev, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->staging_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->prefetch_ev, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lib->d2h_ev, cudaEventDisableTiming);
     for (int g = 0; g < fcg_library::HOST_GROUPS && e == cudaSuccess; ++g) {
       e = cudaEventCreateWithFlags(&lib->h2d_ev[g], cudaEventDisableTiming);
@@ -575,6 +596,7 @@ fcg_status_t fcg_library_destroy(fcg_library_t *lib) {
   if (lib->d2h_stream) cudaStreamDestroy(lib->d2h_stream);
   if (lib->last_ev) cudaEventDestroy(lib->last_ev);
   if (lib->staging_ev) cudaEventDestroy(lib->staging_ev);
+  if (lib->prefetch_ev) cudaEventDestroy(lib->prefetch_ev);
   if (lib->d2h_ev) cudaEventDestroy(lib->d2h_ev);
   for (int g = 0; g < fcg_library::HOST_GROUPS; ++g) {
     if (lib->h2d_ev[g]) cudaEventDestroy(lib->h2d_ev[g]);
@@ -629,6 +651,86 @@ fcg_status_t fcg_segment_register(fcg_library_t *lib, const void *k, const void 
   commit_segment_slot(lib, sl, n_tokens, orig_start);
   *seg_id_out = sid;
   return FCG_OK;
+}
+
+// ------------------------------------------------------------------ NEXT-4: fp8 (e4m3) segment storage (R26)
+fcg_status_t fcg_segment_register_fp8(fcg_library_t *lib, const void *k, const void *v, int32_t n_tokens, int32_t orig_start,
+                                      const int64_t *strides, void *stream, int32_t *seg_id_out) {
+  if (!lib || !k || !v || !seg_id_out) return fail(FCG_ERR_INVALID_ARG, "NULL argument");
+  if (n_tokens <= 0 || orig_start < 0) return fail(FCG_ERR_INVALID_ARG, "n_tokens must be > 0 and orig_start >= 0");
+  const fcg_config_t &c = lib->cfg;
+  int64_t st[4] = {(int64_t)c.n_kv_heads * n_tokens * c.head_dim, (int64_t)n_tokens * c.head_dim, c.head_dim, 1};
+  if (strides) {
+    if (strides[3] != 1) return fail(FCG_ERR_INVALID_ARG, "strides[3] must be 1 (contiguous head_dim)");
+    for (int i = 0; i < 3; ++i) {
+      if (strides[i] % 8) return fail(FCG_ERR_INVALID_ARG, "strides must be multiples of 8 elements (16-byte rows)");
+      st[i] = strides[i];
+    }
+  }
+  if (((uintptr_t)k % 16) || ((uintptr_t)v % 16)) return fail(FCG_ERR_INVALID_ARG, "k and v must be 16-byte aligned");
+  SegmentSlot sl;
+  fcg_status_t sst = find_segment_slot(lib, n_tokens, sl, FCG_STORE_FP8_E4M3);
+  if (sst != FCG_OK) return sst;
+  const uint64_t codes = lib->fp8_code_bytes(n_tokens), half = sl.bytes / 2;
+  fcg::RegisterFp8Params rp;
+  rp.k_src = static_cast<const uint16_t *>(k);
+  rp.v_src = static_cast<const uint16_t *>(v);
+  rp.k_dst = lib->arena + sl.off;
+  rp.k_exp = lib->arena + sl.off + codes;
+  rp.v_dst = lib->arena + sl.off + half;
+  rp.v_exp = lib->arena + sl.off + half + codes;
+  rp.s_layer = st[0];
+  rp.s_head = st[1];
+  rp.s_tok = st[2];
+  rp.n_layers = c.n_layers;
+  rp.n_kv_heads = c.n_kv_heads;
+  rp.n_tokens = n_tokens;
+  rp.head_dim = c.head_dim;
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, static_cast<cudaStream_t>(stream));
+  FCG_CUDA(fcg::launch_register_fp8(rp, static_cast<cudaStream_t>(stream)));
+  lib->stats.register_launches++;
+  {
+    fcg_status_t mst = mark_last(lib, static_cast<cudaStream_t>(stream));
+    if (mst != FCG_OK) return mst;
+  }
+  commit_segment_slot(lib, sl, n_tokens, orig_start, FCG_STORE_FP8_E4M3);
+  *seg_id_out = sl.sid;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_segment_storage(fcg_library_t *lib, int32_t seg_id, int32_t *format, uint64_t *bytes) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  if (seg_id < 0 || seg_id >= lib->cfg.max_segments || !lib->segments[seg_id].live)
+    return fail(FCG_ERR_BAD_SEGMENT, "unknown segment %d", seg_id);
+  if (format) *format = lib->segments[seg_id].fmt;
+  if (bytes) *bytes = lib->segments[seg_id].bytes;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_segment_read(fcg_library_t *lib, int32_t seg_id, void *k_out, void *v_out, void *k_exp_out, void *v_exp_out,
+                              void *stream_) {
+  if (!lib || !k_out || !v_out) return fail(FCG_ERR_INVALID_ARG, "NULL argument");
+  if (seg_id < 0 || seg_id >= lib->cfg.max_segments || !lib->segments[seg_id].live)
+    return fail(FCG_ERR_BAD_SEGMENT, "unknown segment %d", seg_id);
+  const SegmentRec &s = lib->segments[seg_id];
+  const fcg_config_t &c = lib->cfg;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  const unsigned char *base = (s.resident ? lib->arena : lib->host_arena) + s.offset;
+  const uint64_t rows = (uint64_t)c.n_layers * c.n_kv_heads * (uint64_t)s.n_tokens;
+  const bool fp8 = s.fmt == FCG_STORE_FP8_E4M3;
+  if (fp8 && (!k_exp_out || !v_exp_out)) return fail(FCG_ERR_INVALID_ARG, "an fp8 segment needs k_exp_out and v_exp_out");
+  const uint64_t payload = rows * (fp8 ? (uint64_t)c.head_dim : lib->kv_row_bytes());
+  FCG_DEVICE(lib);
+  FCG_ORDER(lib, stream);
+  FCG_CUDA(cudaMemcpyAsync(k_out, base, payload, cudaMemcpyDefault, stream));
+  FCG_CUDA(cudaMemcpyAsync(v_out, base + s.bytes / 2, payload, cudaMemcpyDefault, stream));
+  if (fp8) {
+    const uint64_t codes = lib->fp8_code_bytes(s.n_tokens);
+    FCG_CUDA(cudaMemcpyAsync(k_exp_out, base + codes, rows, cudaMemcpyDefault, stream));
+    FCG_CUDA(cudaMemcpyAsync(v_exp_out, base + s.bytes / 2 + codes, rows, cudaMemcpyDefault, stream));
+  }
+  return mark_last(lib, stream);
 }
 
 // ------------------------------------------------------------------ NEXT-3: two-tier residency
@@ -756,10 +858,15 @@ fcg_status_t validate_plan(fcg_library *lib, const fcg_plan_t &pl, CheckedPlan &
 }
 }  // namespace
 
-fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_plans, void *stream_) {
-  if (!lib || !plans || n_plans <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty plan array");
+}  // extern "C"
+
+namespace {
+// fcg_stitch / fcg_stitch_prefetch.  `prefetch`: offloaded segments named by the plans are first copied back to the
+// device tier on the library's copy stream (first-fit arena range; a segment that finds no room stays where it is and
+// is read in place) while the entries of the resident segments are stitched on `stream`; the entries of the prefetched
+// segments follow in a second launch once the copies have landed.  Page allocation does not depend on the mode.
+fcg_status_t stitch_impl(fcg_library *lib, const fcg_plan_t *plans, int32_t n_plans, cudaStream_t stream, bool prefetch) {
   const fcg_config_t &c = lib->cfg;
-  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   std::vector<CheckedPlan> checked(n_plans);
   int64_t need_pages = 0;
   for (int i = 0; i < n_plans; ++i) {
@@ -772,9 +879,38 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
   if (need_pages > (int64_t)lib->page_stack.size())
     return fail(FCG_ERR_OUT_OF_PAGES, "need %lld pages, %zu free", (long long)need_pages, lib->page_stack.size());
 
-  // ---- build the launch (host) ----------------------------------------------------------------
+  // ---- prefetch planning: arena ranges for the offloaded segments the plans name (nothing committed yet) ----
+  struct Move {
+    int32_t seg;
+    uint64_t dev_off, host_off, bytes;
+  };
+  std::vector<Move> moves;
+  std::vector<FreeRange> seg_free = lib->seg_free;              // a copy: committed at the end
+  if (prefetch && lib->host_arena) {
+    for (int i = 0; i < n_plans; ++i)
+      for (int e = 0; e < plans[i].n_entries; ++e) {
+        const int32_t sid = plans[i].entries[e].seg_id;
+        const SegmentRec &s = lib->segments[sid];
+        if (s.resident) continue;
+        bool seen = false;
+        for (auto &m : moves) seen |= m.seg == sid;
+        if (seen) continue;
+        const size_t fi = range_find(seg_free, s.bytes);
+        if (fi == seg_free.size()) continue;                      // no room: this one is read in place
+        moves.push_back({sid, seg_free[fi].off, s.offset, s.bytes});
+        range_take(seg_free, fi, s.bytes);
+      }
+  }
+  auto move_of = [&](int32_t sid) -> const Move * {
+    for (auto &m : moves)
+      if (m.seg == sid) return &m;
+    return nullptr;
+  };
+
+  // ---- build the launches (host): gb = entries of resident (or in-place) segments + all page ids, gb2 = entries of
+  // the segments being prefetched ----------------------------------------------------------------------------------
   const int P = c.page_size;
-  GatherBuilder gb;
+  GatherBuilder gb, gb2;
   // page ids are taken from a COPY of the stack; committed only when everything has been enqueued
   std::vector<int32_t> stack = lib->page_stack;
   std::vector<int64_t> plan_page_base(n_plans);
@@ -787,15 +923,23 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
     for (int e = 0; e < plans[i].n_entries; ++e) {
       const fcg_plan_entry_t &pe = plans[i].entries[e];
       const SegmentRec &s = lib->segments[pe.seg_id];
+      const Move *mv = move_of(pe.seg_id);
+      GatherBuilder &g = mv ? gb2 : gb;
       fcg::StitchEntryDev de;
-      // an offloaded segment is read in place from the pinned host tier
-      gb.segment_side(lib, s.resident ? lib->arena : lib->host_dev, s.offset, s.bytes, s.n_tokens, de.k_src, de.v_src,
-                      de.src_layer_stride, de.src_head_stride);
-      gb.pool_side(lib, de.k_dst, de.v_dst, de.dst_layer_stride, de.dst_head_stride);
-      de.table_off = gb.table_for(lib, checked[i].deltas[e]);
-      de.pad0 = 0;
-      const int32_t ei = (int32_t)gb.entries.size();
-      gb.entries.push_back(de);
+      // an offloaded segment is read in place from the pinned host tier (or from the arena range it is being
+      // prefetched into); an fp8 segment is de-quantised on the way
+      if (mv) {
+        SegmentRec moved = s;
+        moved.offset = mv->dev_off;
+        moved.resident = true;
+        g.source_segment(lib, moved, de);
+      } else {
+        g.source_segment(lib, s, de);
+      }
+      g.pool_side(lib, de.k_dst, de.v_dst, de.dst_layer_stride, de.dst_head_stride);
+      de.table_off = g.table_for(lib, checked[i].deltas[e]);
+      const int32_t ei = (int32_t)g.entries.size();
+      g.entries.push_back(de);
       // chunks: one per destination page touched
       int32_t done = 0;
       while (done < pe.n_tokens) {
@@ -804,18 +948,25 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
         const int32_t n = std::min(P - slot0, pe.n_tokens - done);
         fcg::StitchChunkDev dc;
         dc.entry = ei;
-        dc.dst_tok = gb.pool_tok(lib, gb.pages[plan_page_base[i] + dst / P], slot0);
+        dc.dst_tok = g.pool_tok(lib, gb.pages[plan_page_base[i] + dst / P], slot0);
         dc.src_tok = pe.src_begin + done;
         dc.ntok = n;
-        gb.chunks.push_back(dc);
+        g.chunks.push_back(dc);
         done += n;
       }
     }
   }
 
-  // ---- enqueue: blob, kernel, page tables -----------------------------------------------------
+  // ---- enqueue: copies, blob, kernel, page tables -----------------------------------------------
   FCG_DEVICE(lib);
   FCG_ORDER(lib, stream);
+  if (!moves.empty()) {
+    // the copy stream starts after whatever used the library last (the arena ranges it writes may have just been freed)
+    if (lib->have_last) FCG_CUDA(cudaStreamWaitEvent(lib->copy_stream, lib->last_ev, 0));
+    for (auto &m : moves)
+      FCG_CUDA(cudaMemcpyAsync(lib->arena + m.dev_off, lib->host_arena + m.host_off, m.bytes, cudaMemcpyHostToDevice, lib->copy_stream));
+    FCG_CUDA(cudaEventRecord(lib->prefetch_ev, lib->copy_stream));
+  }
   GatherBlob gbl;
   fcg_status_t st = enqueue_gather(lib, gb, stream, gbl);
   if (st != FCG_OK) return st;
@@ -824,12 +975,28 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
     FCG_CUDA(cudaMemcpyAsync(dst, gbl.slot->dev + gbl.off_pages + plan_page_base[i] * sizeof(int32_t),
                              (size_t)checked[i].n_pages * sizeof(int32_t), cudaMemcpyDeviceToDevice, stream));
   }
+  GatherBlob gbl2;
+  if (!moves.empty()) {
+    FCG_CUDA(cudaStreamWaitEvent(stream, lib->prefetch_ev, 0));
+    st = enqueue_gather(lib, gb2, stream, gbl2);
+    if (st != FCG_OK) return st;
+  }
   st = mark_last(lib, stream);
   if (st != FCG_OK) return st;
   const int32_t *pages = gb.pages.data();
 
   // ---- commit ------------------------------------------------------------------------------------
   lib->page_stack.swap(stack);
+  if (!moves.empty()) {
+    lib->seg_free.swap(seg_free);
+    for (auto &m : moves) {
+      SegmentRec &s = lib->segments[m.seg];
+      range_give(lib->host_free, m.host_off, m.bytes);
+      s.offset = m.dev_off;
+      s.resident = true;
+      lib->stats.prefetch_copies++;
+    }
+  }
   for (int i = 0; i < n_plans; ++i) {
     TaskRec &t = lib->tasks[plans[i].task_id];
     t.live = true;
@@ -849,6 +1016,19 @@ fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_p
     lib->n_tasks_live++;
   }
   return FCG_OK;
+}
+}  // namespace
+
+extern "C" {
+
+fcg_status_t fcg_stitch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_plans, void *stream) {
+  if (!lib || !plans || n_plans <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty plan array");
+  return stitch_impl(lib, plans, n_plans, static_cast<cudaStream_t>(stream), false);
+}
+
+fcg_status_t fcg_stitch_prefetch(fcg_library_t *lib, const fcg_plan_t *plans, int32_t n_plans, void *stream) {
+  if (!lib || !plans || n_plans <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty plan array");
+  return stitch_impl(lib, plans, n_plans, static_cast<cudaStream_t>(stream), true);
 }
 
 // ------------------------------------------------------------------------------------ S4 + S5/S6
@@ -1098,11 +1278,25 @@ fcg_status_t enqueue_growth(fcg_library *lib, const PatchLayout &lay, const unsi
   return FCG_OK;
 }
 
-// scatter -> attention (-> combine): kernel launches only
-fcg_status_t launch_patch(fcg_library *lib, const PatchLayout &lay, const unsigned char *dev_blob, const PatchIO &io) {
+// scatter -> attention (-> combine): kernel launches only.  `layer_slots`: the split-KV partials of layer l live in a slot
+// of their own (planned calls: calls for different layers may then run concurrently, e.g. on the forked streams of a
+// captured graph); otherwise they sit at the start of the scratch area (calls are ordered by R29).
+fcg_status_t launch_patch(fcg_library *lib, const PatchLayout &lay, const unsigned char *dev_blob, const PatchIO &io, bool layer_slots = false) {
   const fcg_config_t &c = lib->cfg;
   uint64_t part_o_bytes, part_ml_bytes;
   partial_bytes(lib, lay, io.n_layers, part_o_bytes, part_ml_bytes);
+  uint64_t part_o_off = 0, part_ml_off = part_o_bytes;
+  if (layer_slots && lay.max_splits > 1) {
+    uint64_t o1, ml1, o_all, ml_all;
+    partial_bytes(lib, lay, 1, o1, ml1);
+    partial_bytes(lib, lay, c.n_layers, o_all, ml_all);
+    // two arrays indexed by the absolute layer: [n_layers][splits][rows][D] and [n_layers][splits][rows][2]
+    const uint64_t rows1 = (uint64_t)lay.max_splits * lay.n_total * c.n_q_heads;
+    part_o_off = (uint64_t)io.layer_begin * rows1 * c.head_dim * 4;
+    part_ml_off = o_all + (uint64_t)io.layer_begin * rows1 * 2 * 4;
+    part_o_bytes = o_all;
+    part_ml_bytes = ml_all;
+  }
   if (part_o_bytes + part_ml_bytes > lib->scratch_bytes)
     return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for %d-way split partials (%llu bytes)", lay.max_splits,
                 (unsigned long long)(part_o_bytes + part_ml_bytes));
@@ -1134,8 +1328,8 @@ fcg_status_t launch_patch(fcg_library *lib, const PatchLayout &lay, const unsign
   ap.positions = sp.positions;
   ap.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(dev_blob + lay.off_tasks);
   ap.tok_splits = reinterpret_cast<const int32_t *>(dev_blob + lay.off_tspl);
-  ap.part_o = reinterpret_cast<float *>(lib->arena + lib->scratch_off);
-  ap.part_ml = reinterpret_cast<float *>(lib->arena + lib->scratch_off + part_o_bytes);
+  ap.part_o = reinterpret_cast<float *>(lib->arena + lib->scratch_off + part_o_off);
+  ap.part_ml = reinterpret_cast<float *>(lib->arena + lib->scratch_off + part_ml_off);
   ap.n_total = (int32_t)lay.n_total;
   ap.n_layers = io.n_layers;
   ap.layer_begin = io.layer_begin;
@@ -1309,6 +1503,16 @@ fcg_status_t fcg_patch_plan_create(fcg_library_t *lib, const int32_t *task_ids, 
     delete pl;
     return st;
   }
+  {
+    uint64_t o_all, ml_all;
+    partial_bytes(lib, pl->lay, lib->cfg.n_layers, o_all, ml_all);
+    if (o_all + ml_all > lib->scratch_bytes) {
+      const int ns = pl->lay.max_splits;
+      delete pl;
+      return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for the per-layer partial slots of a %d-way split plan (%llu bytes)", ns,
+                  (unsigned long long)(o_all + ml_all));
+    }
+  }
   pl->dev_bytes = align_up(pl->lay.used);
   const size_t fi = range_find(lib->seg_free, pl->dev_bytes);
   if (fi == lib->seg_free.size()) {
@@ -1357,7 +1561,7 @@ fcg_status_t fcg_patch_planned(fcg_library_t *lib, fcg_patch_plan_t *plan, int32
   bool capturing = false;
   st = order_after_previous(lib, io.stream, &capturing);
   if (st != FCG_OK) return st;
-  st = launch_patch(lib, plan->lay, lib->arena + plan->dev_off, io);
+  st = launch_patch(lib, plan->lay, lib->arena + plan->dev_off, io, /*layer_slots=*/true);
   if (st != FCG_OK) return st;
   return capturing ? FCG_OK : mark_last(lib, io.stream);
 }
@@ -1647,7 +1851,8 @@ fcg_status_t fcg_task_shift(fcg_library_t *lib, int32_t task_id, int32_t src_beg
   fcg::StitchEntryDev de;
   gb.pool_side(lib, de.k_src, de.v_src, de.src_layer_stride, de.src_head_stride);
   gb.pool_side(lib, de.k_dst, de.v_dst, de.dst_layer_stride, de.dst_head_stride);
-  de.pad0 = 0;
+  de.src_fp8 = 0;
+  de.k_exp = de.v_exp = 0;
   de.table_off = gb.table_for(lib, delta);
   gb.entries.push_back(de);          // entry 0: the moved range, rotated by delta
   de.table_off = -1;
@@ -1722,7 +1927,8 @@ fcg_status_t fcg_segment_extract(fcg_library_t *lib, int32_t task_id, int32_t be
   gb.pool_side(lib, de.k_src, de.v_src, de.src_layer_stride, de.src_head_stride);
   gb.segment_side(lib, lib->arena, sl.off, sl.bytes, n_tokens, de.k_dst, de.v_dst, de.dst_layer_stride, de.dst_head_stride);
   de.table_off = gb.table_for(lib, new_orig_start - begin);
-  de.pad0 = 0;
+  de.src_fp8 = 0;
+  de.k_exp = de.v_exp = 0;
   gb.entries.push_back(de);
   for (int32_t done = 0; done < n_tokens;) {          // one chunk per source page
     const int32_t sp = begin + done;

@@ -16,15 +16,16 @@ namespace fcg {
 //   segment [L][Hkv][n][D]:          layer_stride = Hkv * n,           head_stride = n, tok = index in the segment
 //   pool    [L][n_pages][Hkv][P][D]: layer_stride = n_pages * Hkv * P, head_stride = P, tok = page * Hkv * P + slot
 // ---------------------------------------------------------------------------------------------
-struct StitchEntryDev {  // 64 B
-  uint64_t k_src, v_src;         // device addresses of the source K / V
+struct StitchEntryDev {  // 80 B
+  uint64_t k_src, v_src;         // device addresses of the source K / V (bf16 rows, or e4m3 code rows: src_fp8)
   uint64_t k_dst, v_dst;         // device addresses of the destination K / V
   int64_t src_layer_stride;      // in token rows
   int64_t dst_layer_stride;
   int32_t src_head_stride;
   int32_t dst_head_stride;
   int32_t table_off;             // first float4 of this entry's rope table; -1 -> bit copy (delta 0 / rope off)
-  int32_t pad0;
+  int32_t src_fp8;               // 1: the source is an fp8 segment (R26): D code bytes per row + one scale byte per row
+  uint64_t k_exp, v_exp;         // fp8 source: device addresses of the per-row scale exponents (one byte e + 127 per row)
 };
 
 struct StitchChunkDev {  // 16 B
@@ -35,6 +36,7 @@ struct StitchChunkDev {  // 16 B
 };
 
 struct StitchParams {
+  int32_t any_fp8;       // some entry reads an fp8 segment: launch the kernel variant that can de-quantise
   const StitchEntryDev *entries;
   const StitchChunkDev *chunks;
   const float4 *table;   // per (entry, j): {c_hi, c_lo, s_hi, s_lo}; c_hi/s_hi have <= 16 significant bits
@@ -64,6 +66,15 @@ struct RegisterParams {
   int32_t n_layers, n_kv_heads, n_tokens, head_dim;
 };
 cudaError_t launch_register_copy(const RegisterParams &p, cudaStream_t stream);
+// S1 with fp8 storage (R26): quantise the caller's bf16 rows to e4m3 codes + one power-of-two scale exponent per row.
+// k_dst / v_dst: [L][Hkv][n][D] bytes; k_exp / v_exp: [L][Hkv][n] bytes (e + 127)
+struct RegisterFp8Params {
+  const uint16_t *k_src, *v_src;
+  uint8_t *k_dst, *v_dst, *k_exp, *v_exp;
+  int64_t s_layer, s_head, s_tok;  // source strides in elements
+  int32_t n_layers, n_kv_heads, n_tokens, head_dim;
+};
+cudaError_t launch_register_fp8(const RegisterFp8Params &p, cudaStream_t stream);
 
 struct ScatterParams {
   const uint16_t *k_new, *v_new;  // [n_layers][n_total][Hkv][D]

@@ -2,6 +2,8 @@
 // S4 patch K/V scatter (Eq. 6: the recomputed span is written into the cache),
 // and the dense read-back of a task's cache through its page table.  All are 16-byte vectorised
 // row copies; none does arithmetic on the payload.
+#include <cuda_fp8.h>
+
 #include "fcg_internal.h"
 
 namespace fcg {
@@ -25,6 +27,63 @@ __global__ void __launch_bounds__(256) register_copy_kernel(const RegisterParams
     const size_t dst = idx * 8;
     st16(p.k_dst + dst, ld16(p.k_src + src));
     st16(p.v_dst + dst, ld16(p.v_src + src));
+  }
+}
+
+// S1, fp8 storage (R26): one warp per row of D bf16 elements.  e = the smallest integer with amax <= 448 * 2^e
+// (amax over the finite elements; integer arithmetic on the exponent field: 448 = 1.75 * 2^8), clamped to [-127, 127],
+// 0 for an all-zero row; code = RNE_e4m3(x * 2^-e) (the scaling is exact), non-finite elements -> the NaN code 0x7F.
+template <int D>
+__global__ void __launch_bounds__(256) register_fp8_kernel(const RegisterFp8Params p) {
+  constexpr int EPL = D / 32;                         // elements per lane: 4 (D = 128) or 2 (D = 64)
+  const size_t n_rows = (size_t)p.n_layers * p.n_kv_heads * p.n_tokens;
+  const int lane = threadIdx.x & 31;
+  for (size_t row = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); row < 2 * n_rows;
+       row += (size_t)gridDim.x * (blockDim.x >> 5)) {
+    const bool is_v = row >= n_rows;
+    const size_t r = is_v ? row - n_rows : row;
+    const int t = (int)(r % p.n_tokens);
+    const size_t lh = r / p.n_tokens;
+    const int h = (int)(lh % p.n_kv_heads), l = (int)(lh / p.n_kv_heads);
+    const uint16_t *src = (is_v ? p.v_src : p.k_src) + (size_t)((int64_t)l * p.s_layer + (int64_t)h * p.s_head + (int64_t)t * p.s_tok) + lane * EPL;
+    float x[EPL];
+    if (EPL == 4) {
+      const uint2 w = *reinterpret_cast<const uint2 *>(src);
+      x[0] = __uint_as_float(w.x << 16), x[1] = __uint_as_float(w.x & 0xffff0000u);
+      x[EPL - 2] = __uint_as_float(w.y << 16), x[EPL - 1] = __uint_as_float(w.y & 0xffff0000u);
+    } else {
+      const uint32_t w = *reinterpret_cast<const uint32_t *>(src);
+      x[0] = __uint_as_float(w << 16), x[1] = __uint_as_float(w & 0xffff0000u);
+    }
+    uint32_t amax = 0;                                // |x| as bits: ordered like the values for non-negative floats
+#pragma unroll
+    for (int i = 0; i < EPL; ++i) {
+      const uint32_t a = __float_as_uint(x[i]) & 0x7fffffffu;
+      if (a < 0x7f800000u) amax = max(amax, a);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) amax = max(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    int e = 0;
+    if (amax != 0) {
+      const int be = (int)(amax >> 23);               // biased exponent; 0 = subnormal: far below 448 * 2^-127 -> clamps
+      e = be == 0 ? -127 : (be - 127) - ((amax & 0x7fffffu) <= 0x600000u ? 8 : 7);
+      e = max(-127, min(127, e));
+    }
+    uint32_t packed = 0;
+#pragma unroll
+    for (int i = 0; i < EPL; i += 2) {
+      const float a = scalbnf(x[i], -e), b = scalbnf(x[i + 1], -e);
+      uint32_t c2 = (uint32_t)__nv_cvt_float2_to_fp8x2(make_float2(a, b), __NV_SATFINITE, __NV_E4M3);
+      if ((__float_as_uint(x[i]) & 0x7fffffffu) >= 0x7f800000u) c2 = (c2 & 0xff00u) | 0x7fu;
+      if ((__float_as_uint(x[i + 1]) & 0x7fffffffu) >= 0x7f800000u) c2 = (c2 & 0x00ffu) | 0x7f00u;
+      packed |= c2 << (8 * i);
+    }
+    uint8_t *dst = (is_v ? p.v_dst : p.k_dst) + r * D + lane * EPL;
+    if (EPL == 4)
+      *reinterpret_cast<uint32_t *>(dst) = packed;
+    else
+      *reinterpret_cast<uint16_t *>(dst) = (uint16_t)packed;
+    if (lane == 0) (is_v ? p.v_exp : p.k_exp)[r] = (uint8_t)(e + 127);
   }
 }
 
@@ -82,6 +141,18 @@ inline unsigned grid_for(size_t total_threads) {
 cudaError_t launch_register_copy(const RegisterParams &p, cudaStream_t stream) {
   const size_t total = (size_t)p.n_layers * p.n_kv_heads * p.n_tokens * (p.head_dim >> 3);
   register_copy_kernel<<<grid_for(total), 256, 0, stream>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_register_fp8(const RegisterFp8Params &p, cudaStream_t stream) {
+  const size_t rows = 2 * (size_t)p.n_layers * p.n_kv_heads * p.n_tokens;
+  const unsigned grid = grid_for(rows * 32);
+  if (p.head_dim == 128)
+    register_fp8_kernel<128><<<grid, 256, 0, stream>>>(p);
+  else if (p.head_dim == 64)
+    register_fp8_kernel<64><<<grid, 256, 0, stream>>>(p);
+  else
+    return cudaErrorInvalidValue;
   return cudaGetLastError();
 }
 

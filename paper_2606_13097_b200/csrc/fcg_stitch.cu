@@ -17,6 +17,7 @@
 //   and likewise y = b cos + a sin.  The fp32 result is within ~2^-23 relative of the exact value;
 //   RNE to bf16 then differs from the fp64 oracle by at most 1 bf16 ulp (double rounding only).
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 
 #include "fcg_internal.h"
 
@@ -82,8 +83,116 @@ __device__ __forceinline__ uint32_t rot_word_il(uint32_t w, const float4 &t) {
   return pack_bf16(x, y);
 }
 
+// ---- fp8 (e4m3) source rows, R26 ---------------------------------------------------------
+__device__ __forceinline__ uint2 ldg_stream8(const void *p) {
+  uint2 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "l"(p));
+  return r;
+}
+// two e4m3 codes -> two floats (exact: e4m3 is a subset of fp16)
+__device__ __forceinline__ float2 e4m3x2_to_float2(uint32_t two_codes) {
+  uint32_t h2;
+  asm("{cvt.rn.f16x2.e4m3x2 %0, %1;}" : "=r"(h2) : "h"((unsigned short)two_codes));
+  return __half22float2(*reinterpret_cast<__half2 *>(&h2));
+}
+// 2^(eb - 127) for a scale byte eb in [0, 254] (0 -> the subnormal 2^-127)
+__device__ __forceinline__ float scale_of(uint32_t eb) { return __uint_as_float(eb ? (eb << 23) : 0x00400000u); }
+// 8 codes (two 32-bit words) -> 8 de-quantised floats: value(code) * 2^e, exact in fp32
+__device__ __forceinline__ void dequant8(const uint2 &c, float sc, float *out) {
+  const float2 a = e4m3x2_to_float2(c.x & 0xffffu), b = e4m3x2_to_float2(c.x >> 16);
+  const float2 d = e4m3x2_to_float2(c.y & 0xffffu), e = e4m3x2_to_float2(c.y >> 16);
+  out[0] = a.x * sc, out[1] = a.y * sc, out[2] = b.x * sc, out[3] = b.y * sc;
+  out[4] = d.x * sc, out[5] = d.y * sc, out[6] = e.x * sc, out[7] = e.y * sc;
+}
+__device__ __forceinline__ uint4 pack8(const float *x) {
+  return make_uint4(pack_bf16(x[0], x[1]), pack_bf16(x[2], x[3]), pack_bf16(x[4], x[5]), pack_bf16(x[6], x[7]));
+}
+
+// The body of one entry whose source is an fp8 segment: same work split as the bf16 path (a lane owns the 8 low-half and
+// the 8 matching high-half elements of a row), rows are D code bytes + one scale byte.  K: de-quantise, rotate with the
+// compensated fp32 scheme (a de-quantised element has <= 4 significant bits, so its products with c_hi / s_hi are exact
+// as for bf16 inputs), ONE rounding to bf16.  V: de-quantise, round to bf16 (exact outside the deepest subnormals).
 template <int D>
-__global__ void __launch_bounds__(128, 4) stitch_kernel(const StitchParams p) {
+__device__ __forceinline__ void stitch_fp8_rows(const StitchEntryDev &en, const StitchChunkDev &ch, int layer, int Hkv, int warp,
+                                                int col, int tl, bool rotate, bool il, const float4 *tab) {
+  constexpr int LPT = D / 16, TPS = 32 / LPT, STEPS = 4, HEADS = 2;
+  const int ntok = ch.ntok;
+  // a code row is half a bf16 row: two kv heads per pass keep as many bytes in flight per lane as the bf16 path has
+  for (int g0 = warp; g0 < Hkv; g0 += 4 * HEADS) {
+    for (int t0 = 0; t0 < ntok; t0 += TPS * STEPS) {
+      uint2 klo[HEADS][STEPS], khi[HEADS][STEPS], vlo[HEADS][STEPS], vhi[HEADS][STEPS];
+      uint32_t ke[HEADS][STEPS], ve[HEADS][STEPS];
+#pragma unroll
+      for (int h = 0; h < HEADS; ++h) {
+        const int g = g0 + 4 * h;
+        if (g < Hkv) {
+          const size_t src_row = (size_t)layer * (size_t)en.src_layer_stride + (size_t)g * (size_t)en.src_head_stride + (size_t)ch.src_tok;
+          const char *ksrc = reinterpret_cast<const char *>(en.k_src) + src_row * D + col * 8;
+          const char *vsrc = reinterpret_cast<const char *>(en.v_src) + src_row * D + col * 8;
+          const uint8_t *kexp = reinterpret_cast<const uint8_t *>(en.k_exp) + src_row;
+          const uint8_t *vexp = reinterpret_cast<const uint8_t *>(en.v_exp) + src_row;
+#pragma unroll
+          for (int s = 0; s < STEPS; ++s) {
+            const int t = t0 + s * TPS + tl;
+            if (t < ntok) {
+              const size_t off = (size_t)t * D;
+              klo[h][s] = ldg_stream8(ksrc + off);
+              khi[h][s] = ldg_stream8(ksrc + off + D / 2);
+              vlo[h][s] = ldg_stream8(vsrc + off);
+              vhi[h][s] = ldg_stream8(vsrc + off + D / 2);
+              ke[h][s] = __ldg(kexp + t);
+              ve[h][s] = __ldg(vexp + t);
+            }
+          }
+        }
+      }
+#pragma unroll
+      for (int h = 0; h < HEADS; ++h) {
+        const int g = g0 + 4 * h;
+        if (g < Hkv) {
+          const size_t dst_row = (size_t)layer * (size_t)en.dst_layer_stride + (size_t)g * (size_t)en.dst_head_stride + (size_t)ch.dst_tok;
+          char *kdst = reinterpret_cast<char *>(en.k_dst) + dst_row * (D * 2) + col * 16;
+          char *vdst = reinterpret_cast<char *>(en.v_dst) + dst_row * (D * 2) + col * 16;
+#pragma unroll
+          for (int s = 0; s < STEPS; ++s) {
+            const int t = t0 + s * TPS + tl;
+            if (t < ntok) {
+              const size_t off = (size_t)t * (D * 2);
+              float a[8], b[8];
+              dequant8(klo[h][s], scale_of(ke[h][s]), a);
+              dequant8(khi[h][s], scale_of(ke[h][s]), b);
+              if (rotate) {
+                float x[8], y[8];
+                if (!il) {
+#pragma unroll
+                  for (int i = 0; i < 8; ++i) rot_pair(a[i], b[i], tab[i], x[i], y[i]);
+                } else {
+#pragma unroll
+                  for (int i = 0; i < 4; ++i) {
+                    rot_pair(a[2 * i], a[2 * i + 1], tab[i], x[2 * i], x[2 * i + 1]);
+                    rot_pair(b[2 * i], b[2 * i + 1], tab[4 + i], y[2 * i], y[2 * i + 1]);
+                  }
+                }
+                stg_16(kdst + off, pack8(x));
+                stg_16(kdst + off + D, pack8(y));
+              } else {
+                stg_16(kdst + off, pack8(a));
+                stg_16(kdst + off + D, pack8(b));
+              }
+              dequant8(vlo[h][s], scale_of(ve[h][s]), a);
+              dequant8(vhi[h][s], scale_of(ve[h][s]), b);
+              stg_16(vdst + off, pack8(a));
+              stg_16(vdst + off + D, pack8(b));
+            }
+          }
+        }
+      }
+    }
+  }
+}
+
+template <int D, bool FP8>
+__global__ void __launch_bounds__(128, FP8 ? 3 : 4) stitch_kernel(const StitchParams p) {
   constexpr int LPT = D / 16;      // lanes per token: one 16-byte column of each half per lane
   constexpr int TPS = 32 / LPT;    // tokens per warp step
   constexpr int STEPS = 4;         // steps in flight per batch (4 x 64 B per lane)
@@ -113,6 +222,10 @@ __global__ void __launch_bounds__(128, 4) stitch_kernel(const StitchParams p) {
   }
 
   const int Hkv = p.n_kv_heads;
+  if (FP8 && en.src_fp8) {           // (the bf16 instantiation carries no fp8 code: its registers and SASS stay as they were)
+    stitch_fp8_rows<D>(en, ch, layer, Hkv, warp, col, tl, rotate, il, tab);
+    return;
+  }
   for (int g = warp; g < Hkv; g += 4) {
     const size_t src_row = (size_t)layer * (size_t)en.src_layer_stride + (size_t)g * (size_t)en.src_head_stride + (size_t)ch.src_tok;
     const size_t dst_row = (size_t)layer * (size_t)en.dst_layer_stride + (size_t)g * (size_t)en.dst_head_stride + (size_t)ch.dst_tok;
@@ -228,12 +341,19 @@ cudaError_t launch_stitch(const StitchParams &p, int head_dim, cudaStream_t stre
   if (p.n_chunks <= 0) return cudaSuccess;
   dim3 grid((unsigned)p.n_chunks, (unsigned)p.n_layers, 1);
   dim3 block(128, 1, 1);
-  if (head_dim == 128)
-    stitch_kernel<128><<<grid, block, 0, stream>>>(p);
-  else if (head_dim == 64)
-    stitch_kernel<64><<<grid, block, 0, stream>>>(p);
-  else
+  if (head_dim == 128) {
+    if (p.any_fp8)
+      stitch_kernel<128, true><<<grid, block, 0, stream>>>(p);
+    else
+      stitch_kernel<128, false><<<grid, block, 0, stream>>>(p);
+  } else if (head_dim == 64) {
+    if (p.any_fp8)
+      stitch_kernel<64, true><<<grid, block, 0, stream>>>(p);
+    else
+      stitch_kernel<64, false><<<grid, block, 0, stream>>>(p);
+  } else {
     return cudaErrorInvalidValue;
+  }
   return cudaGetLastError();
 }
 

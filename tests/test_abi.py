@@ -15,7 +15,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def _declared():
     text = open(os.path.join(ROOT, "include", "fcg.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return set(re.findall(r"\b(fcg_[a-z_]+)\s*\(", text))
+    return set(re.findall(r"\b(fcg_[a-z0-9_]+)\s*\(", text))
 
 
 def test_library_is_built_and_exports_every_declared_symbol():

@@ -300,3 +300,58 @@ def test_host_and_rope_variants_validate_before_enqueueing():
     torch.cuda.synchronize()
     T.assert_attn_close(oh, ref, "host patch after the rejections")
     lib.close()
+
+
+def test_stitch_prefetch_overlaps_and_matches_the_oracle():
+    """NEXT-3: offloaded segments (one of them fp8) named by a plan come back through the copy engine while the resident
+    entries are stitched; same cache, same page tables, the segments end up resident.  Then the no-room case: a segment
+    that finds no arena range stays offloaded and is read in place."""
+    L, Hq, Hkv, D, P = 4, 4, 2, 128, 16
+    from paper_2606_13097_b200.binding import FcgLibrary
+    rng = np.random.default_rng(21)
+    lens = [400, 250, 600, 130]
+    lib = FcgLibrary(n_layers=L, n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, page_size=P, rope_base=1e4, max_segments=6, max_tasks=3,
+                     max_task_tokens=2048, n_pages=300, segment_tokens=sum(lens) + 40, host_tier_tokens=1200)
+    orc = O.OracleLibrary(L, Hq, Hkv, D, page_size=P, rope_base=1e4, n_pages=300, max_task_tokens=2048)
+    for i, n in enumerate(lens):
+        k, kb = _bits(rng, (L, Hkv, n, D))
+        v, vb = _bits(rng, (L, Hkv, n, D))
+        if i == 2:
+            assert lib.segment_register_fp8(k.cuda(), v.cuda(), 100 * i) == orc.segment_register_fp8(kb, vb, 100 * i) == i
+        else:
+            assert lib.segment_register(k.cuda(), v.cuda(), 100 * i) == orc.segment_register(kb, vb, 100 * i) == i
+    for sid in (0, 2):
+        lib.segment_offload(sid)
+        orc.segment_offload(sid)
+    entries = [(0, 10, 380, 0), (1, 0, 250, 380), (2, 0, 600, 630), (3, 5, 100, 1230), (0, 0, 64, 1330)]
+    plan = {"task_id": 0, "entries": entries, "holes": [], "capacity_tokens": 0}
+    lib.stitch_prefetch([plan])
+    orc.stitch([O.Plan(0, [O.PlanEntry(*e) for e in entries])], prefetch=True)
+    torch.cuda.synchronize()
+
+    def check(tid, what):
+        ot = orc.tasks[tid]
+        assert np.array_equal(lib.task_page_table_host(tid), np.asarray(ot.page_table, np.int32)), what
+        for layer in range(L):
+            kg, vg = lib.task_read(tid, layer, 0, ot.capacity)
+            f = ot.filled
+            assert np.array_equal(synth.to_bits(vg)[:, f], ot.v[layer][:, f]), what
+            T.assert_k_within_1ulp(synth.to_bits(kg)[:, f], ot.k[layer][:, f], what)
+
+    check(0, "stitch_prefetch")
+    assert [lib.segment_info(i)[2] for i in range(4)] == [orc.segment_info(i)[2] for i in range(4)] == [True] * 4
+    assert lib.stats()["prefetch_copies"] == 2
+    # no room on the device tier: fill the arena, offload one segment, and ask for it again -- it is read in place
+    lib.segment_offload(1)
+    orc.segment_offload(1)
+    n_fill = lib.pool_info()["segments_bytes_free"] // (L * Hkv * D * 4) - 100       # leaves room for ~100 tokens < the 250 needed
+    filler, _ = _bits(rng, (L, Hkv, n_fill, D))
+    fid = lib.segment_register(filler.cuda(), filler.cuda(), 0)
+    orc.segment_register(synth.to_bits(filler), synth.to_bits(filler), 0)
+    lib.stitch_prefetch([{"task_id": 1, "entries": [(1, 0, 250, 0), (3, 0, 130, 250)], "holes": [], "capacity_tokens": 0}])
+    orc.stitch([O.Plan(1, [O.PlanEntry(1, 0, 250, 0), O.PlanEntry(3, 0, 130, 250)])])
+    torch.cuda.synchronize()
+    check(1, "stitch_prefetch without room")
+    assert lib.segment_info(1)[2] is False and lib.stats()["prefetch_copies"] == 2
+    lib.segment_release(fid)
+    lib.close()

@@ -245,6 +245,7 @@ def test_fp8_stitch_equals_bf16_stitch_of_the_dequantised_segment(rope_mode):
     bf16 path (closed forms, complex multiplication, group law ...)."""
     L, Hq, Hkv, D, P = 2, 4, 2, 32, 4
     k, v = _rand_bf16((L, Hkv, 21, D), 1), _rand_bf16((L, Hkv, 21, D), 2, scale=3.0)
+    k[0, 0, 6, 3] = 0x7F80                       # no e4m3 value: stored as the NaN code; its rotation partner must survive delta 0
     a = O.OracleLibrary(L, Hq, Hkv, D, page_size=P, rope_mode=rope_mode, rope_base=1e4, n_pages=128)
     b = O.OracleLibrary(L, Hq, Hkv, D, page_size=P, rope_mode=rope_mode, rope_base=1e4, n_pages=128)
     sa = a.segment_register_fp8(k, v, 300)
@@ -252,14 +253,19 @@ def test_fp8_stitch_equals_bf16_stitch_of_the_dequantised_segment(rope_mode):
     assert sg.fmt == O.FMT_FP8_E4M3 and sg.k.dtype == np.uint8 and sg.k.shape == k.shape and sg.k_exp.shape == k.shape[:3]
     kd = O.f64_to_bf16(O.fp8_dequantize_rows(sg.k, sg.k_exp))
     vd = O.f64_to_bf16(O.fp8_dequantize_rows(sg.v, sg.v_exp))
-    assert np.array_equal(O.bf16_to_f64(kd), O.fp8_dequantize_rows(sg.k, sg.k_exp))      # exact, not merely close
+    dq = O.fp8_dequantize_rows(sg.k, sg.k_exp)
+    assert np.array_equal(np.isnan(dq), np.isnan(O.bf16_to_f64(kd))) and np.isnan(dq).sum() == 1
+    assert np.array_equal(O.bf16_to_f64(kd)[~np.isnan(dq)], dq[~np.isnan(dq)])           # exact, not merely close
     sb = b.segment_register(kd, vd, 300)
     plan = lambda s: [O.Plan(0, [O.PlanEntry(s, 2, 9, 0), O.PlanEntry(s, 0, 21, 12), O.PlanEntry(s, 5, 4, 302 + 3)], [O.Hole(9, 3)], 0)]
     a.stitch(plan(sa))
     b.stitch(plan(sb))
     ta, tb = a.tasks[0], b.tasks[0]
     assert ta.deltas == tb.deltas and 0 in [ta.deltas[2]]                # the third entry is an identity graft (delta 0)
-    assert np.array_equal(ta.k, tb.k) and np.array_equal(ta.v, tb.v) and np.array_equal(ta.filled, tb.filled)
+    nan = (tb.k & 0x7FFF) > 0x7F80
+    assert np.array_equal(nan, (ta.k & 0x7FFF) > 0x7F80) and nan.sum() >= 3
+    assert np.array_equal(ta.k[~nan], tb.k[~nan]) and np.array_equal(ta.v, tb.v) and np.array_equal(ta.filled, tb.filled)
+    assert (nan[:, :, 305:309].sum() == 1) or rope_mode == 0    # the identity graft keeps the NaN to itself
     # and the stored bytes are half of bf16's (+ one exponent per row)
     assert sg.k.nbytes * 2 == k.nbytes
 
@@ -299,3 +305,21 @@ def test_rotation_by_zero_is_the_identity_on_every_bit_pattern():
     assert out[0, 2] == np.copysign(np.inf, c) and out[0, 10] == np.copysign(np.inf, s)
     row[0, 10] = 0x7FC0
     assert np.isnan(O.bf16_to_f64(O.rope_shift_bf16(row, 3, th))[0, [2, 10]]).all()
+
+
+def test_stitch_with_prefetch_changes_residency_only():
+    L, Hq, Hkv, D = 1, 2, 1, 16
+    libs = []
+    for prefetch in (False, True):
+        lib = O.OracleLibrary(L, Hq, Hkv, D, page_size=4, n_pages=32)
+        for i in range(3):
+            lib.segment_register(_rand_bf16((L, Hkv, 9, D), i), _rand_bf16((L, Hkv, 9, D), 10 + i), 5 * i)
+        lib.segment_offload(0)
+        lib.segment_offload(2)
+        lib.stitch([O.Plan(0, [O.PlanEntry(0, 0, 9, 0), O.PlanEntry(1, 2, 5, 9)])], prefetch=prefetch)
+        libs.append(lib)
+    a, b = libs
+    assert np.array_equal(a.tasks[0].k, b.tasks[0].k) and np.array_equal(a.tasks[0].v, b.tasks[0].v)
+    assert a.tasks[0].page_table == b.tasks[0].page_table
+    assert [a.segment_info(i)[2] for i in range(3)] == [False, True, False]
+    assert [b.segment_info(i)[2] for i in range(3)] == [True, True, False]      # only the segments the plan names come back
