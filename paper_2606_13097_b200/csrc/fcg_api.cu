@@ -1211,7 +1211,8 @@ fcg_status_t build_patch_blob(fcg_library *lib, const PatchSpec &ps, const Patch
   // both is launched as two grids, one per class.
   lay.rows_per_cta_split = max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64);
   auto rows_per_cta_of = [&](int rows) { return use_tc ? (rows > 128 ? 256 : 128) : lay.rows_per_cta_split; };
-  const int ctas_per_sm = use_tc ? 1 : fcg::attn_split_ctas_per_sm(c.head_dim);
+  const int ctas_per_sm = use_tc ? fcg::attn_tc_ctas_per_sm(c.head_dim, max_rows > 128 ? 2 : 1, (max_rows > 64 && max_rows <= 128) ? 2 : 1)
+                                 : fcg::attn_split_ctas_per_sm(c.head_dim);
   int max_splits = 1;
   int64_t tok_off = 0;
   for (int t = 0; t < ps.n_tasks; ++t) {

@@ -222,8 +222,13 @@ struct Cfg {
   // 224 KB per 64-token step with two Q tiles -- was the limiter of the tensor-bound class).  One Q tile: own
   // columns; two Q tiles: P overwrites the first half of its S tile in place (S is then freed by P V, not by s_free).
   static constexpr bool P_ALIAS = NQ == 2;
-  static constexpr int K_STAGES = (NQ == 1 ? 6 : 5) * (128 / D);      // the same bytes in flight for either head_dim
-  static constexpr int V_STAGES = (NQ == 1 ? 6 : 5) * (128 / D);
+  // head_dim 64, one Q tile, one softmax warpgroup (the short-patch / decode class): TWO CTAs per SM -- a 64-token tile
+  // is only 16 KB there, so the per-tile latency chain (S ready -> softmax -> P ready -> P V) of a single CTA cannot
+  // keep the SM's share of HBM busy; two independent CTAs hide each other's.  Each takes half the shared memory
+  // (6 + 5 stages of 8 KB) and 256 TMEM columns (S 2 x 64, O 64, P 2 x 32).
+  static constexpr int CTAS_PER_SM = (D == 64 && NQ == 1 && PS_ == 1) ? 2 : 1;
+  static constexpr int K_STAGES = CTAS_PER_SM == 2 ? 6 : (NQ == 1 ? 6 : 5) * (128 / D);      // else the same bytes in flight for either head_dim
+  static constexpr int V_STAGES = CTAS_PER_SM == 2 ? 5 : (NQ == 1 ? 6 : 5) * (128 / D);
   // Tile-parity streams (NQ == 1 only): two softmax warpgroups, group w owns the KV tiles j = w (mod 2), its own
   // S / P buffer and its own O accumulator, with its own running (m, l); the streams are merged by log-sum-exp in
   // the epilogue like the row streams.  Two softmax warps per SM sub-partition hide each other's latencies.
@@ -232,14 +237,14 @@ struct Cfg {
   static constexpr int N_SOFTMAX = 128 * NQ * PS;       // (Q tile | parity stream) x 4 lane quarters x 32 rows
   static constexpr int NTHREADS = N_SOFTMAX + 96;
   static constexpr int KLOAD_WARP = N_SOFTMAX / 32, VLOAD_WARP = KLOAD_WARP + 1, MMA_WARP = KLOAD_WARP + 2;
-  static constexpr int TMEM_COLS = 512;                 // S: 2*NQ x 64 columns, O: NQ*PS x 128 columns
+  static constexpr int TMEM_COLS = CTAS_PER_SM == 2 ? 256 : 512;   // S: 2*NQ x 64 columns, O: NQ*PS x 128 columns
   static constexpr int TMEM_O = NQ * 128;               // first O column
   static constexpr int Q_ITERS = NQ * BM * CPR / N_SOFTMAX;
   static constexpr int OFF_Q = 0;
   static constexpr int OFF_K = OFF_Q + NQ * Q_TILE_B;                // K stage s at +s*KV_TILE_B
   static constexpr int OFF_V = OFF_K + K_STAGES * KV_TILE_B;         // V stage s at +s*KV_TILE_B
   static constexpr int OFF_BAR = OFF_V + V_STAGES * KV_TILE_B;
-  static constexpr int TMEM_P = 384;                    // one Q tile: P[b] at TMEM_P + b*32 (S 0..127, O 128..383)
+  static constexpr int TMEM_P = CTAS_PER_SM == 2 ? 192 : 384;   // one Q tile: P[b] at TMEM_P + b*32 (S 0..127, O from 128)
   // k_full[SK], k_empty[SK], v_full[SV], v_empty[SV], s_full[NQ][2], p_full[NQ][2], pv_done[NQ][2], s_free[NQ][2],
   // q_full, all_done
   static constexpr int N_BARS = 2 * K_STAGES + 2 * V_STAGES + 8 * NQ + 2;
@@ -249,7 +254,7 @@ struct Cfg {
 };
 
 template <int NQ, int PS_, int D>
-__global__ void __launch_bounds__(Cfg<NQ, PS_, D>::NTHREADS, 1)
+__global__ void __launch_bounds__(Cfg<NQ, PS_, D>::NTHREADS, Cfg<NQ, PS_, D>::CTAS_PER_SM)
     attn_tc_kernel(const AttnParams p, const __grid_constant__ TmaDesc tm_k, const __grid_constant__ TmaDesc tm_v) {
   using C = Cfg<NQ, PS_, D>;
   constexpr int SK = C::K_STAGES, SV = C::V_STAGES, PS = C::PS;
@@ -804,6 +809,10 @@ cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv,
 }
 
 }  // namespace
+
+int attn_tc_ctas_per_sm(int head_dim, int q_tiles, int parity_streams) {
+  return (head_dim == 64 && q_tiles == 1 && parity_streams == 1) ? 2 : 1;
+}
 
 // q_tiles = 128-row Q tiles per CTA (1 or 2); p.max_row_groups counts groups of q_tiles*128 rows.
 // parity_streams (q_tiles == 1 only): 2 = two softmax warpgroups on alternating KV tiles, 1 = one warpgroup.

@@ -140,5 +140,6 @@ struct alignas(64) TmaDesc {
 // with box (64, P, 1, 1, 1) and 128B swizzle (make_pool_tensor_map).
 cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, int parity_streams, const TmaDesc *tm_k,
                            const TmaDesc *tm_v, cudaStream_t stream);
+int attn_tc_ctas_per_sm(int head_dim, int q_tiles, int parity_streams);
 
 }  // namespace fcg

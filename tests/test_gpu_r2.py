@@ -310,7 +310,7 @@ def test_stitch_prefetch_overlaps_and_matches_the_oracle():
     from paper_2606_13097_b200.binding import FcgLibrary
     rng = np.random.default_rng(21)
     lens = [400, 250, 600, 130]
-    lib = FcgLibrary(n_layers=L, n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, page_size=P, rope_base=1e4, max_segments=6, max_tasks=3,
+    lib = FcgLibrary(n_layers=L, n_q_heads=Hq, n_kv_heads=Hkv, head_dim=D, page_size=P, rope_base=1e4, max_segments=12, max_tasks=3,
                      max_task_tokens=2048, n_pages=300, segment_tokens=sum(lens) + 40, host_tier_tokens=1200)
     orc = O.OracleLibrary(L, Hq, Hkv, D, page_size=P, rope_base=1e4, n_pages=300, max_task_tokens=2048)
     for i, n in enumerate(lens):
@@ -344,14 +344,23 @@ def test_stitch_prefetch_overlaps_and_matches_the_oracle():
     # no room on the device tier: fill the arena, offload one segment, and ask for it again -- it is read in place
     lib.segment_offload(1)
     orc.segment_offload(1)
-    n_fill = lib.pool_info()["segments_bytes_free"] // (L * Hkv * D * 4) - 100       # leaves room for ~100 tokens < the 250 needed
-    filler, _ = _bits(rng, (L, Hkv, n_fill, D))
-    fid = lib.segment_register(filler.cuda(), filler.cuda(), 0)
-    orc.segment_register(synth.to_bits(filler), synth.to_bits(filler), 0)
+    filler, _ = _bits(rng, (L, Hkv, 100, D))
+    B = _B()
+    fillers = []
+    while True:                                       # 100-token fillers until none fits: no free range of 250 tokens is left
+        try:
+            fillers.append(lib.segment_register(filler.cuda(), filler.cuda(), 0))
+        except B.FcgError as e:
+            assert e.status == B.FCG_ERR_OUT_OF_ARENA
+            break
+    assert 1 <= len(fillers) <= 6
+    for _ in fillers:
+        orc.segment_register(synth.to_bits(filler), synth.to_bits(filler), 0)
     lib.stitch_prefetch([{"task_id": 1, "entries": [(1, 0, 250, 0), (3, 0, 130, 250)], "holes": [], "capacity_tokens": 0}])
     orc.stitch([O.Plan(1, [O.PlanEntry(1, 0, 250, 0), O.PlanEntry(3, 0, 130, 250)])])
     torch.cuda.synchronize()
     check(1, "stitch_prefetch without room")
     assert lib.segment_info(1)[2] is False and lib.stats()["prefetch_copies"] == 2
-    lib.segment_release(fid)
+    for fid in fillers:
+        lib.segment_release(fid)
     lib.close()
