@@ -320,6 +320,11 @@ fcg_status_t fcg_pool_info(fcg_library_t *lib, fcg_pool_info_t *out);
  * 0 = the library's wave-filling choice.  The result does not depend on either knob beyond summation order
  * (P11, split invariance). */
 fcg_status_t fcg_set_attn_policy(fcg_library_t *lib, int32_t tc_min_rows, int32_t force_splits);
+/* Tasks with more than 128 query rows per kv head (head_dim 128) run on single CTAs holding two Q tiles (default,
+ * enable == 0) or on CTA pairs -- clusters of two CTAs sharing every K / V tile through tcgen05 cta_group::2
+ * (enable != 0; measured: equal on the power-capped C5, 10-15 % slower on C3 / C4).  Same
+ * results up to summation order. */
+fcg_status_t fcg_set_attn_pairs(fcg_library_t *lib, int32_t enable);
 
 /* Launch statistics since create (kernels launched by this library; bench.py reports them). */
 typedef struct {

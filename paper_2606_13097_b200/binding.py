@@ -114,6 +114,7 @@ SYMBOLS = {
     "fcg_task_read": (_I, [_P, _I, _I, _I, _I, _P, _P, _P]),
     "fcg_pool_info": (_I, [_P, C.POINTER(fcg_pool_info_t)]),
     "fcg_set_attn_policy": (_I, [_P, _I, _I]),
+    "fcg_set_attn_pairs": (_I, [_P, _I]),
     "fcg_stats": (_I, [_P, C.POINTER(fcg_stats_t)]),
     "fcg_scorer_create": (_I, [C.POINTER(_P)]),
     "fcg_scorer_destroy": (_I, [_P]),
@@ -396,6 +397,10 @@ def fcg_set_attn_policy(handle, tc_min_rows: int, force_splits: int = 0) -> None
     _check(load().fcg_set_attn_policy(handle, int(tc_min_rows), int(force_splits)))
 
 
+def fcg_set_attn_pairs(handle, enable: bool) -> None:
+    _check(load().fcg_set_attn_pairs(handle, 1 if enable else 0))
+
+
 def fcg_stats(handle) -> dict:
     st = fcg_stats_t()
     _check(load().fcg_stats(handle, C.byref(st)))
@@ -606,3 +611,6 @@ class FcgLibrary:
 
     def set_attn_policy(self, tc_min_rows: int, force_splits: int = 0) -> None:
         fcg_set_attn_policy(self.handle, tc_min_rows, force_splits)
+
+    def set_attn_pairs(self, enable: bool) -> None:
+        fcg_set_attn_pairs(self.handle, enable)

@@ -119,6 +119,7 @@ struct fcg_library {
   fcg::TmaDesc tm_k, tm_v;                       // K / V pool tensor maps for the tcgen05 path
   bool have_tma = false;
   int32_t force_splits = 0;                      // > 0: KV splits per task (clamped to its tile count); 0 = choose_splits
+  bool use_pairs = false;                        // > 128 rows per kv head at head_dim 128: CTA pairs (cta_group::2) instead of two Q tiles per CTA
 
   uint16_t *k_pool() const { return reinterpret_cast<uint16_t *>(arena + k_pool_off); }
   uint16_t *v_pool() const { return reinterpret_cast<uint16_t *>(arena + v_pool_off); }
@@ -1245,6 +1246,7 @@ fcg_status_t build_patch_blob(fcg_library *lib, const PatchSpec &ps, const Patch
   lay.max_row_groups = (max_rows + rows_per_cta_of(max_rows) - 1) / rows_per_cta_of(max_rows);
   // tcgen05 path: the same descriptors again, grouped by CTA class (rows per kv head <= 64 | <= 128 | more)
   auto *h_tasks2 = reinterpret_cast<fcg::AttnTaskDev *>(host + lay.off_tasks2);
+  // (two 128-row CTAs instead of one two-Q-tile CTA for 129..256 rows was measured slower: C4 patch 3.24 vs 3.13 ms)
   auto class_of = [&](int rows) { return rows <= 64 ? 0 : (rows <= 128 ? 1 : 2); };
   for (int cl = 0; cl < 3; ++cl) lay.n_cls[cl] = 0, lay.cls_rgs[cl] = 1;
   for (int t = 0; t < ps.n_tasks; ++t) lay.n_cls[class_of(h_tasks[t].n * G)]++;
@@ -1354,7 +1356,10 @@ fcg_status_t launch_patch(fcg_library *lib, const PatchLayout &lay, const unsign
       apc.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(dev_blob + lay.off_tasks2) + lay.cls_begin[cl];
       apc.n_tasks = lay.n_cls[cl];
       apc.max_row_groups = lay.cls_rgs[cl];
-      FCG_CUDA(fcg::launch_attn_tc(apc, c.head_dim, q_tiles, parity_streams, &lib->tm_k, &lib->tm_v, io.stream));
+      if (cl == 2 && c.head_dim == 128 && lib->use_pairs)
+        FCG_CUDA(fcg::launch_attn_pair(apc, &lib->tm_k, &lib->tm_v, io.stream));
+      else
+        FCG_CUDA(fcg::launch_attn_tc(apc, c.head_dim, q_tiles, parity_streams, &lib->tm_k, &lib->tm_v, io.stream));
       lib->stats.attn_tc_launches++;
     }
     lib->stats.last_attn_path = 2;
@@ -2004,6 +2009,12 @@ fcg_status_t fcg_set_attn_policy(fcg_library_t *lib, int32_t tc_min_rows, int32_
   if (!lib || tc_min_rows < 0 || force_splits < 0) return fail(FCG_ERR_INVALID_ARG, "NULL library or negative threshold / split count");
   lib->tc_min_rows = tc_min_rows;
   lib->force_splits = force_splits;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_set_attn_pairs(fcg_library_t *lib, int32_t enable) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  lib->use_pairs = enable != 0;
   return FCG_OK;
 }
 

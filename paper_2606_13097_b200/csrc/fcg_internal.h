@@ -141,5 +141,8 @@ struct alignas(64) TmaDesc {
 cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, int parity_streams, const TmaDesc *tm_k,
                            const TmaDesc *tm_v, cudaStream_t stream);
 int attn_tc_ctas_per_sm(int head_dim, int q_tiles, int parity_streams);
+// CTA-pair variant (tcgen05 cta_group::2, clusters of 2) for the > 128-rows class at head_dim 128; same parameters,
+// p.max_row_groups counts groups of 256 rows (fcg_attn_pair.cu)
+cudaError_t launch_attn_pair(const AttnParams &p, const TmaDesc *tm_k, const TmaDesc *tm_v, cudaStream_t stream);
 
 }  // namespace fcg

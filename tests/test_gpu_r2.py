@@ -364,3 +364,37 @@ def test_stitch_prefetch_overlaps_and_matches_the_oracle():
     for fid in fillers:
         lib.segment_release(fid)
     lib.close()
+
+
+@pytest.mark.parametrize("n,Hq,Hkv,ctx,P,splits", [(130, 2, 1, 2600, 16, 0), (260, 2, 2, 1500, 8, 2), (45, 8, 2, 1000, 64, 0), (300, 2, 2, 777, 16, 3),
+                                                  (64, 16, 4, 4096, 32, 0), (200, 4, 4, 100, 16, 0)])
+def test_cta_pair_kernel_matches_the_oracle(n, Hq, Hkv, ctx, P, splits):
+    """the cta_group::2 variant of the > 128-rows class (fcg_set_attn_pairs): page sizes, ragged last tiles, a trailing row
+    group whose second CTA holds no row, KV splits + combine, a mid hole and an appended patch -- all against the oracle,
+    pool poisoned with NaN."""
+    L, D = 2, 128
+    cfg = synth.GraftConfig("pair", L, Hq, Hkv, D, P, 1e4, 2, ctx, ctx, 1000, 1, 1, 1, 0, holes=((-1, n),))
+    wl = synth.make_workload(cfg, n + ctx)
+    orc, lib, seg_ids = T.make_pair(cfg, wl, 3, n_pages=-(-(ctx + 2 * n + 8) // P) + 4, max_task_tokens=ctx + 2 * n + 8, workspace_bytes=128 << 20)
+    info = lib.pool_info()
+    lib.arena[info["k_pool_offset"]: info["k_pool_offset"] + 2 * info["pool_bytes"]].view(torch.int16).fill_(0x7FC1)
+    c_plans, o_plans = T.plans_of(wl, seg_ids)
+    orc.stitch(o_plans)
+    lib.stitch(c_plans)
+    lib.set_attn_pairs(True)
+    lib.set_attn_policy(1, splits)
+    task = wl.tasks[0]
+    out, ref = T.run_patch_both(orc, lib, cfg, task, 5)
+    assert lib.stats()["last_attn_path"] == 2
+    T.assert_attn_close(out, ref, "pair kernel, patch at the end")
+    T.compare_cache_bits(orc, lib, 0, task.positions)
+    # a second, appended patch (grows the task): queries see the first patch too
+    pos = np.arange(task.capacity, task.capacity + n, dtype=np.int32)
+    out, ref = T.run_patch_both(orc, lib, cfg, task, 6, positions=pos)
+    T.assert_attn_close(out, ref, "pair kernel, appended patch")
+    # and the single-CTA kernel gives the same answer within the tolerance of both
+    lib.set_attn_pairs(False)
+    out2, ref2 = T.run_patch_both(orc, lib, cfg, task, 6, positions=pos)
+    T.assert_attn_close(out2, ref2, "single-CTA kernel, same patch")
+    assert float((out.float() - out2.float()).abs().max()) < 2e-2
+    lib.close()
