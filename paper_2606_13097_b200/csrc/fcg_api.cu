@@ -1261,6 +1261,11 @@ fcg_status_t build_patch_blob(fcg_library *lib, const PatchSpec &ps, const Patch
       const int q_tiles = cl == 2 ? 2 : 1;
       lay.cls_rgs[cl] = std::max(lay.cls_rgs[cl], (h_tasks[t].n * G + 128 * q_tiles - 1) / (128 * q_tiles));
     }
+    // longest first inside a class: the grid's z index runs over (layer, task), so every layer ends with the shortest
+    // CTAs of the class and the tail of the launch is short (block dispatch is greedy in index order)
+    for (int cl = 0; cl < 3; ++cl)
+      std::stable_sort(h_tasks2 + lay.cls_begin[cl], h_tasks2 + lay.cls_begin[cl] + lay.n_cls[cl],
+                       [](const fcg::AttnTaskDev &a, const fcg::AttnTaskDev &b) { return a.kv_len > b.kv_len; });
   }
   return FCG_OK;
 }
