@@ -383,7 +383,9 @@ def time_e2e(lib, plans, ids, npt, pos, q, k, v, out, steps, warmup, D: Dist):
     b.record()
     D.barrier()
     ms = D.max(a.elapsed_time(b) / steps)
-    assert torch.equal(oh, out.cpu()), "host-buffer call and device call disagree"
+    # the host call patches in layer groups, so its KV-split choice (and with it the summation order) may differ from
+    # the one-call device step: same result within the attention tolerance, not necessarily the same bits
+    assert torch.allclose(oh.float(), out.cpu().float(), rtol=2e-2, atol=1e-2), "host-buffer call and device call disagree"
     return ms, int(qh.numel() + kh.numel() + vh.numel()) * 2, int(oh.numel()) * 2
 
 
@@ -398,15 +400,18 @@ def rooflines(cfg, wl, tasks, timing, traffic, name):
     stitch = {"kernel": "stitch_kernel (fused gather + RoPE-shift)", "bound": "hbm", "achieved": sb / st_s / 1e9, "peak": peak,
               "unit": "GB/s", "frac": sb / st_s / 1e9 / peak, "peak_source": peak_src, "frac_of_8TBps": sb / st_s / 1e9 / 8000.0,
               "traffic": tr.get("stitch")}
-    if rows >= 250:
+    # intensity of the whole call in flop per K/V byte (= R for a single task; a mixed batch like C4 averages its tasks):
+    # tensor-bound from ~250 flop/B (sustained bf16 peak / measured HBM peak), HBM-bound below
+    if af / max(ab, 1) >= 250:
         tpeak, tsrc = tensor_peak()
         attn = {"kernel": "attn_tc_kernel (tcgen05 / TMEM)", "bound": "tensor", "achieved": af / at_s / 1e12, "peak": tpeak, "unit": "TFLOP/s",
-                "frac": af / at_s / 1e12 / tpeak, "peak_source": tsrc, "rows_per_kv_head": rows, "hbm_GBps": ab / at_s / 1e9,
-                "hbm_frac": ab / at_s / 1e9 / peak}
+                "frac": af / at_s / 1e12 / tpeak, "peak_source": tsrc, "rows_per_kv_head": rows, "flop_per_byte": af / max(ab, 1),
+                "hbm_GBps": ab / at_s / 1e9, "hbm_frac": ab / at_s / 1e9 / peak}
     else:
         attn = {"kernel": "attn_tc_kernel (tcgen05 / TMEM)" if timing["stats"]["last_attn_path"] == 2 else "attn_split_kernel (mma.sync split-KV)",
                 "bound": "hbm", "achieved": ab / at_s / 1e9, "peak": peak, "unit": "GB/s", "frac": ab / at_s / 1e9 / peak,
-                "frac_of_8TBps": ab / at_s / 1e9 / 8000.0, "rows_per_kv_head": rows, "TFLOPs": af / at_s / 1e12}
+                "frac_of_8TBps": ab / at_s / 1e9 / 8000.0, "rows_per_kv_head": rows, "flop_per_byte": af / max(ab, 1),
+                "TFLOPs": af / at_s / 1e12}
     attn["traffic"] = tr.get("attn")
     attn["note"] = "timed as scatter + attention (+ combine); scatter is ~1 % of it"
     return stitch, attn, sb, ab, af
@@ -554,6 +559,13 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
         torch.cuda.synchronize(dev)
         return a.elapsed_time(b) / n, (t1 - t0) * 1e3 / n
 
+    def release0():
+        """task 0 goes away if it is live (other tasks of a batched workload stay)"""
+        try:
+            lib.task_release(t.task_id)
+        except Exception:
+            pass
+
     res = {}
     # the call pattern of a model that patches layer by layer: L calls of one layer each (task 0's own patch tokens)
     try:
@@ -622,7 +634,7 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
     n_seg = int(wl.seg_lens[seg])
     seg_bytes = n_seg * per_tok
     try:
-        lib.task_release(t.task_id)
+        release0()
         plan = [{"task_id": t.task_id, "entries": [(seg, 0, n_seg, 0)], "holes": [], "capacity_tokens": n_seg}]
 
         def timed(fn, before=None, n=3):
@@ -642,22 +654,20 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
         off_ms = timed(lambda: lib.segment_offload(seg), before=lambda: lib.segment_prefetch(seg))
         pre_ms = timed(lambda: lib.segment_prefetch(seg), before=lambda: lib.segment_offload(seg))
         lib.segment_offload(seg)
-        host_ms = timed(lambda: lib.stitch(plan), before=lambda: lib.pool_info()["n_tasks_live"] and lib.task_release(t.task_id))
-        lib.task_release(t.task_id)
+        host_ms = timed(lambda: lib.stitch(plan), before=release0)
+        release0()
         lib.segment_prefetch(seg)
         # NEXT-3 overlap: task 0's real plan with its first segment in the host tier -- read in place (fcg_stitch) vs
         # copied back by the copy engine while the resident entries are stitched (fcg_stitch_prefetch)
         try:
             plan0 = [{"task_id": t.task_id, "entries": t.entries, "holes": t.holes, "capacity_tokens": t.capacity}]
-            rel = lambda: lib.pool_info()["n_tasks_live"] and lib.task_release(t.task_id)
-
             def before():
-                rel()
+                release0()
                 lib.segment_offload(seg)
 
             inplace_ms = timed(lambda: lib.stitch(plan0), before=before)
             overlap_ms = timed(lambda: lib.stitch_prefetch(plan0), before=before)
-            rel()
+            release0()
             res["stitch_prefetch_overlap"] = {"ms": overlap_ms, "in_place_ms": inplace_ms, "offloaded_bytes": int(seg_bytes),
                                               "offloaded_GBps": seg_bytes / (overlap_ms * 1e-3) / 1e9,
                                               "note": f"task 0's plan ({sum(n for (_, _, n, _) in t.entries)} tokens) with one {n_seg}-token segment offloaded: "
@@ -690,14 +700,13 @@ def time_next_rows(lib, cfg, wl, seed, dev, iters=5):
 
         def restitch(pl_):
             def f():
-                if lib.pool_info()["n_tasks_live"]:
-                    lib.task_release(t.task_id)
+                release0()
                 lib.stitch(pl_)
             return f
 
         ms16, _ = timed_loop(restitch(plan16))
         ms8, _ = timed_loop(restitch(plan8))
-        lib.task_release(t.task_id)
+        release0()
         b16 = n_st * cfg.n_layers * cfg.n_kv_heads * cfg.head_dim * 8
         b8 = n_st * cfg.n_layers * cfg.n_kv_heads * (cfg.head_dim * 6 + 2)
         fmt, nb8 = lib.segment_storage(fp8_id[used0[0]])
