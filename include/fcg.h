@@ -220,7 +220,8 @@ fcg_status_t fcg_patch_batch_host(fcg_library_t *lib, const int32_t *task_ids, c
 
 /* Patch plans: the per-layer call pattern of a real model without per-call host work, and CUDA-graph capture.
  * fcg_patch_plan_create does everything of fcg_patch_batch that does not depend on the tensors -- validation (R6),
- * growth (R25), split selection for calls of `layers_per_call` layers, the upload of positions / descriptors into a
+ * growth (R25), split selection for `layers_per_call` layers on the GPU at a time (the layers of one call, or -- for
+ * per-layer calls forked over several streams -- the number of calls in flight), the upload of positions / descriptors into a
  * device range of the plan's own (taken from the segment arena; OUT_OF_ARENA), and the COMMIT of the fill state:
  * the positions count as filled from here on, the caller runs the plan for every layer before relying on them.
  * fcg_patch_planned then only launches scatter -> attention (-> combine) for layers [layer_begin, layer_begin +
