@@ -200,7 +200,8 @@ fcg_status_t fcg_patch_rope(fcg_library_t *lib, int32_t task_id, int32_t layer_b
  * once `stream` has been synchronised.  The host->device copies run on a stream of the library's own, ordered
  * after the previous patch call and joined into `stream` before the kernels, so they overlap whatever else the
  * caller has enqueued on `stream` just before (typically the fcg_stitch of the same graft); calls of 8 MiB of q or
- * more are pipelined in layer groups (copy in, attend, copy out overlap).  Staging comes from the workspace
+ * more are pipelined in four layer groups (copy in, attend, copy out overlap; the plan blob is uploaded ahead of
+ * the big copies on the copy stream, so the first group's kernels do not queue behind them).  Staging comes from the workspace
  * (OUT_OF_ARENA if it does not fit). */
 fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_begin, int32_t n_layers,
                             const void *q, const void *k, const void *v, const int32_t *positions, int32_t n,
