@@ -327,6 +327,10 @@ fcg_status_t fcg_set_attn_policy(fcg_library_t *lib, int32_t tc_min_rows, int32_
  * (enable != 0; measured: equal on the power-capped C5, 10-15 % slower on C3 / C4).  Same
  * results up to summation order. */
 fcg_status_t fcg_set_attn_pairs(fcg_library_t *lib, int32_t enable);
+/* A batch whose tasks fall into several CTA classes (<= 64, 65..128, > 128 query rows per kv head; head_dim 128) runs as
+ * one launch per class, longest class first (default, enable == 0), or as ONE launch with the classes interleaved
+ * (enable != 0; measured equal on C4: the classes do not speed each other up). */
+fcg_status_t fcg_set_attn_mixed(fcg_library_t *lib, int32_t enable);
 
 /* Launch statistics since create (kernels launched by this library; bench.py reports them). */
 typedef struct {

@@ -115,6 +115,7 @@ SYMBOLS = {
     "fcg_pool_info": (_I, [_P, C.POINTER(fcg_pool_info_t)]),
     "fcg_set_attn_policy": (_I, [_P, _I, _I]),
     "fcg_set_attn_pairs": (_I, [_P, _I]),
+    "fcg_set_attn_mixed": (_I, [_P, _I]),
     "fcg_stats": (_I, [_P, C.POINTER(fcg_stats_t)]),
     "fcg_scorer_create": (_I, [C.POINTER(_P)]),
     "fcg_scorer_destroy": (_I, [_P]),
@@ -401,6 +402,10 @@ def fcg_set_attn_pairs(handle, enable: bool) -> None:
     _check(load().fcg_set_attn_pairs(handle, 1 if enable else 0))
 
 
+def fcg_set_attn_mixed(handle, enable: bool) -> None:
+    _check(load().fcg_set_attn_mixed(handle, 1 if enable else 0))
+
+
 def fcg_stats(handle) -> dict:
     st = fcg_stats_t()
     _check(load().fcg_stats(handle, C.byref(st)))
@@ -614,3 +619,6 @@ class FcgLibrary:
 
     def set_attn_pairs(self, enable: bool) -> None:
         fcg_set_attn_pairs(self.handle, enable)
+
+    def set_attn_mixed(self, enable: bool) -> None:
+        fcg_set_attn_mixed(self.handle, enable)

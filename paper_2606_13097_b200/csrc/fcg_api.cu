@@ -119,6 +119,7 @@ struct fcg_library {
   fcg::TmaDesc tm_k, tm_v;                       // K / V pool tensor maps for the tcgen05 path
   bool have_tma = false;
   int32_t force_splits = 0;                      // > 0: KV splits per task (clamped to its tile count); 0 = choose_splits
+  bool mix_classes = false;                      // a batch with several CTA classes as ONE interleaved launch (head_dim 128) instead of one per class
   bool use_pairs = false;                        // > 128 rows per kv head at head_dim 128: CTA pairs (cta_group::2) instead of two Q tiles per CTA
 
   uint16_t *k_pool() const { return reinterpret_cast<uint16_t *>(arena + k_pool_off); }
@@ -1153,6 +1154,8 @@ struct PatchLayout {
   bool use_tc = false;
   int max_splits = 1, max_rows = 0, rows_per_cta_split = 64, max_row_groups = 1;
   int n_cls[3] = {0, 0, 0}, cls_begin[3] = {0, 0, 0}, cls_rgs[3] = {1, 1, 1};
+  uint64_t off_items = 0;     // mixed-class launch: int4 {class, task index in the class-grouped list, row group, split}
+  int32_t n_items = 0;
   struct Grow {
     int32_t task_id, first_lp, count;
     int64_t index;            // first page id of this task inside the off_grow region
@@ -1178,7 +1181,6 @@ fcg_status_t build_patch_blob(fcg_library *lib, const PatchSpec &ps, const Patch
   if (lay.off_pos == UINT64_MAX || lay.off_toff == UINT64_MAX || lay.off_tspl == UINT64_MAX || lay.off_tasks == UINT64_MAX ||
       lay.off_tasks2 == UINT64_MAX || lay.off_grow == UINT64_MAX)
     return fail(FCG_ERR_OUT_OF_ARENA, "patch blob exceeds %llu bytes", (unsigned long long)cap);
-  lay.used = bw.used;
   auto *h_pos = reinterpret_cast<int32_t *>(host + lay.off_pos);
   auto *h_toff = reinterpret_cast<int32_t *>(host + lay.off_toff);
   auto *h_tspl = reinterpret_cast<int32_t *>(host + lay.off_tspl);
@@ -1267,6 +1269,45 @@ fcg_status_t build_patch_blob(fcg_library *lib, const PatchSpec &ps, const Patch
       std::stable_sort(h_tasks2 + lay.cls_begin[cl], h_tasks2 + lay.cls_begin[cl] + lay.n_cls[cl],
                        [](const fcg::AttnTaskDev &a, const fcg::AttnTaskDev &b) { return a.kv_len > b.kv_len; });
   }
+  // Work items of a mixed-class batch (one launch for all classes, fcg_attn_tc.cu attn_tc_mixed_kernel): every (task, row
+  // group, split), the classes interleaved proportionally -- item i of the n_c items of class c sits at (i + 0.5) / n_c --
+  // so that HBM-bound and compute-bound CTAs are resident side by side throughout the launch.
+  lay.n_items = 0;
+  lay.off_items = 0;
+  const int n_classes = (lay.n_cls[0] > 0) + (lay.n_cls[1] > 0) + (lay.n_cls[2] > 0);
+  if (use_tc && c.head_dim == 128 && n_classes >= 2 && !lib->use_pairs && lib->mix_classes) {
+    struct Item {
+      double key;
+      int32_t cls, task, rg, split;
+    };
+    std::vector<Item> items;
+    for (int cl = 0; cl < 3; ++cl) {
+      std::vector<Item> mine;
+      for (int t = 0; t < lay.n_cls[cl]; ++t) {
+        const fcg::AttnTaskDev &d = h_tasks2[lay.cls_begin[cl] + t];
+        const int rows_per_cta = cl == 2 ? 256 : 128;
+        const int rgs = (d.n * G + rows_per_cta - 1) / rows_per_cta;
+        for (int rg = 0; rg < rgs; ++rg)
+          for (int sp = 0; sp < d.n_splits; ++sp) mine.push_back({0.0, cl, lay.cls_begin[cl] + t, rg, sp});
+      }
+      for (size_t i = 0; i < mine.size(); ++i) {
+        mine[i].key = ((double)i + 0.5) / (double)mine.size();
+        items.push_back(mine[i]);
+      }
+    }
+    std::stable_sort(items.begin(), items.end(), [](const Item &a, const Item &b) { return a.key < b.key; });
+    lay.off_items = bw.reserve(items.size() * 16);
+    if (lay.off_items == UINT64_MAX) return fail(FCG_ERR_OUT_OF_ARENA, "patch blob exceeds %llu bytes", (unsigned long long)cap);
+    auto *h_items = reinterpret_cast<int32_t *>(host + lay.off_items);
+    for (size_t i = 0; i < items.size(); ++i) {
+      h_items[4 * i + 0] = items[i].cls;
+      h_items[4 * i + 1] = items[i].task;
+      h_items[4 * i + 2] = items[i].rg;
+      h_items[4 * i + 3] = items[i].split;
+    }
+    lay.n_items = (int32_t)items.size();
+  }
+  lay.used = bw.used;
   return FCG_OK;
 }
 
@@ -1350,7 +1391,18 @@ fcg_status_t launch_patch(fcg_library *lib, const PatchLayout &lay, const unsign
   ap.max_row_groups = lay.max_row_groups;
   ap.n_pages = c.n_pages;
   ap.scale_log2 = (float)(1.4426950408889634 / sqrt((double)c.head_dim));
-  if (lay.use_tc) {
+  ap.items = nullptr;
+  ap.n_items = 0;
+  if (lay.use_tc && lay.n_items > 0) {
+    // all classes in one launch, interleaved (see build_patch_blob)
+    fcg::AttnParams apm = ap;
+    apm.tasks = reinterpret_cast<const fcg::AttnTaskDev *>(dev_blob + lay.off_tasks2);
+    apm.items = reinterpret_cast<const int4 *>(dev_blob + lay.off_items);
+    apm.n_items = lay.n_items;
+    FCG_CUDA(fcg::launch_attn_tc_mixed(apm, &lib->tm_k, &lib->tm_v, io.stream));
+    lib->stats.attn_tc_launches++;
+    lib->stats.last_attn_path = 2;
+  } else if (lay.use_tc) {
     // class 0: rows replicated 2x / 4x in one softmax warpgroup (HBM-bound; the deep K/V rings matter most);
     // class 1: two tile-parity softmax warpgroups; class 2: two Q tiles per CTA
     // launched longest-CTA class first, so that the tail of the batch is made of the short CTAs
@@ -2045,6 +2097,12 @@ fcg_status_t fcg_set_attn_policy(fcg_library_t *lib, int32_t tc_min_rows, int32_
   if (!lib || tc_min_rows < 0 || force_splits < 0) return fail(FCG_ERR_INVALID_ARG, "NULL library or negative threshold / split count");
   lib->tc_min_rows = tc_min_rows;
   lib->force_splits = force_splits;
+  return FCG_OK;
+}
+
+fcg_status_t fcg_set_attn_mixed(fcg_library_t *lib, int32_t enable) {
+  if (!lib) return fail(FCG_ERR_INVALID_ARG, "lib is NULL");
+  lib->mix_classes = enable != 0;
   return FCG_OK;
 }
 

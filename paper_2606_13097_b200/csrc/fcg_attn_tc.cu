@@ -81,27 +81,24 @@ struct Cfg {
   static_assert((K_STAGES + V_STAGES) * KV_TILE_B >= PS * BM * MROW * 4 + PS * BM * 8, "merge buffer must fit in the idle rings");
 };
 
+// The whole CTA program for one work item (task, layer index, kv head, KV split, row group).  Called by the per-class
+// kernels below (indices from the 3-D grid) and by attn_tc_mixed_kernel (indices from an item table); a CTA may have
+// more warps than this class uses (mixed kernel): those take no role and only meet the two CTA-wide barriers.
 template <int NQ, int PS_, int D>
-__global__ void __launch_bounds__(Cfg<NQ, PS_, D>::NTHREADS, Cfg<NQ, PS_, D>::CTAS_PER_SM)
-    attn_tc_kernel(const AttnParams p, const __grid_constant__ TmaDesc tm_k, const __grid_constant__ TmaDesc tm_v) {
+__device__ __forceinline__ void attn_tc_body(const AttnParams &p, const TmaDesc &tm_k, const TmaDesc &tm_v, unsigned char *smem_raw,
+                                             const int task_i, const int li, const int g, const int split, const int rg) {
   using C = Cfg<NQ, PS_, D>;
   constexpr int SK = C::K_STAGES, SV = C::V_STAGES, PS = C::PS;
   constexpr int Q_TILE_B = C::Q_TILE_B, KV_TILE_B = C::KV_TILE_B, CPR = C::CPR;
-  extern __shared__ unsigned char smem_raw[];
   // 1024-byte alignment for the 128B-swizzle atoms
   unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   const uint32_t sbase = smem_u32(smem);
 
-  const int task_i = blockIdx.z % p.n_tasks;
-  const int li = blockIdx.z / p.n_tasks;
   const AttnTaskDev tk = p.tasks[task_i];
-  const int split = blockIdx.x % p.max_splits;
-  const int rg = blockIdx.x / p.max_splits;
   const int G = p.group;
   const int R = tk.n * G;
   const int row0 = rg * (NQ * BM);                 // first query row of this CTA
   if (split >= tk.n_splits || row0 >= R) return;
-  const int g = blockIdx.y;
   const int layer = p.layer_begin + li;
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // tells the compiler that the warp index is warp-uniform
@@ -326,7 +323,7 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_, D>::NTHREADS, Cfg<NQ, PS_, D>::CT
       for (int j = max(0, n_tiles - LAG); j < n_tiles; ++j) issue_pv(j);
       umma_commit(all_done);
     }
-  } else {
+  } else if (warp < C::N_SOFTMAX / 32) {
     // ======================================= softmax ========================================
     // Q tiles: MMA row m of tile t holds query row  row0 + t*BM + (m % rps)  -> (token, head-in-group); with
     // dup > 1 the same query rows are replicated `dup` times (one copy per stream); rows past the valid ones
@@ -612,6 +609,41 @@ __global__ void __launch_bounds__(Cfg<NQ, PS_, D>::NTHREADS, Cfg<NQ, PS_, D>::CT
 }
 
 template <int NQ, int PS_, int D>
+__global__ void __launch_bounds__(Cfg<NQ, PS_, D>::NTHREADS, Cfg<NQ, PS_, D>::CTAS_PER_SM)
+    attn_tc_kernel(const AttnParams p, const __grid_constant__ TmaDesc tm_k, const __grid_constant__ TmaDesc tm_v) {
+  extern __shared__ unsigned char smem_raw[];
+  attn_tc_body<NQ, PS_, D>(p, tm_k, tm_v, smem_raw, blockIdx.z % p.n_tasks, blockIdx.z / p.n_tasks, blockIdx.y, blockIdx.x % p.max_splits,
+                           blockIdx.x / p.max_splits);
+}
+
+// A batch that mixes the three CTA classes (C4: 8..64-token patches with G = 4 give 32..256 rows per kv head) in ONE
+// launch: block b = hl * n_items + k runs item k (class, task, row group, split; p.items, interleaved proportionally
+// over the classes by the host, longest task first inside a class) for (layer, kv head) hl.  One launch per class ran
+// the classes back to back -- the HBM-bound ones (<= 128 rows) at the memory roofline with the tensor pipe half idle,
+// then the compute-bound one (two Q tiles) with HBM half idle, each with its own tail; interleaved, CTAs of both kinds
+// are resident at any time and share the machine.  head_dim 128 only (the head_dim-64 short-patch class lives on two
+// CTAs per SM, which a kernel sized for the largest class cannot offer).
+constexpr int MIXED_THREADS = Cfg<2, 1, 128>::NTHREADS;
+static_assert(Cfg<1, 2, 128>::NTHREADS == MIXED_THREADS && Cfg<1, 1, 128>::NTHREADS <= MIXED_THREADS, "the mixed kernel is sized for the largest class");
+constexpr int MIXED_SMEM = Cfg<2, 1, 128>::SMEM_BYTES > Cfg<1, 2, 128>::SMEM_BYTES
+                               ? (Cfg<2, 1, 128>::SMEM_BYTES > Cfg<1, 1, 128>::SMEM_BYTES ? Cfg<2, 1, 128>::SMEM_BYTES : Cfg<1, 1, 128>::SMEM_BYTES)
+                               : (Cfg<1, 2, 128>::SMEM_BYTES > Cfg<1, 1, 128>::SMEM_BYTES ? Cfg<1, 2, 128>::SMEM_BYTES : Cfg<1, 1, 128>::SMEM_BYTES);
+
+__global__ void __launch_bounds__(MIXED_THREADS, 1)
+    attn_tc_mixed_kernel(const AttnParams p, const __grid_constant__ TmaDesc tm_k, const __grid_constant__ TmaDesc tm_v) {
+  extern __shared__ unsigned char smem_raw[];
+  const int hl = blockIdx.x / p.n_items;
+  const int4 it = __ldg(p.items + (blockIdx.x - hl * p.n_items));      // {class, task index, row group, split}
+  const int g = hl % p.n_kv_heads, li = hl / p.n_kv_heads;
+  if (it.x == 2)
+    attn_tc_body<2, 1, 128>(p, tm_k, tm_v, smem_raw, it.y, li, g, it.w, it.z);
+  else if (it.x == 1)
+    attn_tc_body<1, 2, 128>(p, tm_k, tm_v, smem_raw, it.y, li, g, it.w, it.z);
+  else
+    attn_tc_body<1, 1, 128>(p, tm_k, tm_v, smem_raw, it.y, li, g, it.w, it.z);
+}
+
+template <int NQ, int PS_, int D>
 cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv, cudaStream_t stream) {
   using C = Cfg<NQ, PS_, D>;
   // the attribute is per device (fcg_config_t.device allows libraries on several GPUs in one process)
@@ -637,6 +669,30 @@ cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv,
 }
 
 }  // namespace
+
+// all CTA classes of a batch in one launch (head_dim 128): p.items / p.n_items list the work items, p.tasks all tasks
+cudaError_t launch_attn_tc_mixed(const AttnParams &p, const TmaDesc *tm_k, const TmaDesc *tm_v, cudaStream_t stream) {
+  if (!tm_k || !tm_v || !p.items || p.n_items <= 0) return cudaErrorInvalidValue;
+  static bool configured[64] = {};
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
+  if (dev < 0 || dev >= 64 || !configured[dev]) {
+    cudaError_t e = cudaFuncSetAttribute(attn_tc_mixed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MIXED_SMEM);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < 64) configured[dev] = true;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)((size_t)p.n_items * p.n_kv_heads * p.n_layers), 1, 1);
+  cfg.blockDim = dim3(MIXED_THREADS, 1, 1);
+  cfg.dynamicSmemBytes = MIXED_SMEM;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, attn_tc_mixed_kernel, p, *tm_k, *tm_v);
+}
 
 int attn_tc_ctas_per_sm(int head_dim, int q_tiles, int parity_streams) {
   return (head_dim == 64 && q_tiles == 1 && parity_streams == 1) ? 2 : 1;

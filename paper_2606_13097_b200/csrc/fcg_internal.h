@@ -123,6 +123,8 @@ struct AttnParams {
   int32_t max_splits, max_row_groups;
   uint32_t n_pages;
   float scale_log2;          // log2(e) / sqrt(D)
+  const int4 *items;         // mixed-class launch: {class, task index, row group, split} per work item (else NULL)
+  int32_t n_items;
 };
 
 // split-KV warp-MMA (mma.sync m16n8k16) path; rows_per_cta in {16, 32, 64}
@@ -141,6 +143,7 @@ struct alignas(64) TmaDesc {
 cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, int parity_streams, const TmaDesc *tm_k,
                            const TmaDesc *tm_v, cudaStream_t stream);
 int attn_tc_ctas_per_sm(int head_dim, int q_tiles, int parity_streams);
+cudaError_t launch_attn_tc_mixed(const AttnParams &p, const TmaDesc *tm_k, const TmaDesc *tm_v, cudaStream_t stream);
 // CTA-pair variant (tcgen05 cta_group::2, clusters of 2) for the > 128-rows class at head_dim 128; same parameters,
 // p.max_row_groups counts groups of 256 rows (fcg_attn_pair.cu)
 cudaError_t launch_attn_pair(const AttnParams &p, const TmaDesc *tm_k, const TmaDesc *tm_v, cudaStream_t stream);

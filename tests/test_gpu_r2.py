@@ -398,3 +398,41 @@ def test_cta_pair_kernel_matches_the_oracle(n, Hq, Hkv, ctx, P, splits):
     T.assert_attn_close(out2, ref2, "single-CTA kernel, same patch")
     assert float((out.float() - out2.float()).abs().max()) < 2e-2
     lib.close()
+
+
+def test_mixed_class_batch_in_one_launch_matches_the_per_class_launches_and_the_oracle():
+    """fcg_set_attn_mixed: a batch whose tasks fall into all three CTA classes (16, 30 and 50 tokens at G = 4: 64, 120 and
+    200 rows per kv head) as ONE interleaved launch; with and without KV splits; against the oracle and against the default
+    one-launch-per-class path (bit-identical: the same CTA program runs either way)."""
+    L, Hq, Hkv, D, P = 3, 8, 2, 128, 16
+    cfg = synth.GraftConfig("mixed", L, Hq, Hkv, D, P, 1e4, 4, 300, 900, 3000, 5, 2, 3, 0, total_min=500, total_max=2500,
+                            distinct_segments=False, holes=((-1, 0),), patch_min=10, patch_max=60)
+    wl = synth.make_workload(cfg, 8)
+    for t, n in zip(wl.tasks, (16, 30, 50, 8, 64)):              # pin the patch sizes: rows 64, 120, 200, 32, 256
+        b = t.holes[-1][0]
+        t.holes[-1] = (b, n)
+        t.capacity = b + n
+        t.positions = np.arange(b, b + n, dtype=np.int32)
+    orc, lib, seg_ids = T.make_pair(cfg, wl, 8, workspace_bytes=128 << 20)
+    c_plans, o_plans = T.plans_of(wl, seg_ids)
+    orc.stitch(o_plans)
+    lib.stitch(c_plans)
+    ids = [t.task_id for t in wl.tasks]
+    npt = [len(t.positions) for t in wl.tasks]
+    pos = np.concatenate([t.positions for t in wl.tasks]).astype(np.int32)
+    qs = [synth.patch_qkv(cfg, t.task_id, len(t.positions), 3) for t in wl.tasks]
+    q, k, v = [torch.cat([x[j] for x in qs], dim=1).contiguous() for j in range(3)]
+    ref = np.concatenate([orc.patch(t.task_id, 0, synth.to_bits(x[0]), synth.to_bits(x[1]), synth.to_bits(x[2]), t.positions)
+                          for t, x in zip(wl.tasks, qs)], axis=1)
+    for splits in (0, 2):
+        outs = []
+        for mixed in (True, False):
+            lib.set_attn_mixed(mixed)
+            lib.set_attn_policy(1, splits)
+            s0 = lib.stats()["attn_tc_launches"]
+            outs.append(lib.patch_batch(ids, npt, 0, q.cuda(), k.cuda(), v.cuda(), pos))
+            torch.cuda.synchronize()
+            assert lib.stats()["attn_tc_launches"] - s0 == (1 if mixed else 3)
+            T.assert_attn_close(outs[-1], ref, f"mixed={mixed} splits={splits}")
+        assert torch.equal(outs[0], outs[1])
+    lib.close()
