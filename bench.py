@@ -48,7 +48,10 @@ EXTRACT_TOKENS = 1024
 # not a BASELINE.json configuration: the head_dim-64 geometry of C1 at a size that streams from HBM (4k tokens, a
 # 16-token patch at the end; the decode step is in its next_rows) -- the short-patch path of north_star at head_dim 64
 D64 = synth.GraftConfig("D64-4k", 32, 32, 32, 64, 16, 1e4, 64, 128, 1024, 8192, 1, 6, 6, 4096, holes=((-1, 16),))
-BENCH_CONFIGS = dict(synth.CONFIGS, D64=D64)
+# likewise for head_dim 256 (R27; Gemma-2-9B geometry: 42 layers, 16 q / 8 kv heads): 4k tokens,
+# a 16-token hole mid-cache and 48 tokens at the end in one call (R = 128 rows per kv head)
+D256 = synth.GraftConfig("D256-4k", 42, 16, 8, 256, 16, 1e4, 64, 128, 1024, 8192, 1, 6, 6, 4096, holes=((2, 16), (-1, 48)))
+BENCH_CONFIGS = dict(synth.CONFIGS, D64=D64, D256=D256)
 
 
 def _peaks_file():
@@ -858,7 +861,7 @@ def run_cuda(args):
 
     def region_steps(name):
         # sub-configurations: at least 20 steps and a region of >= ~0.12 s, so that the clock samples fall inside it
-        est = {"C2": 1.0, "C3": 0.75, "C4": 8.0, "C5": 13.5, "D64": 0.5}.get(name, 5.0)
+        est = {"C2": 1.0, "C3": 0.75, "C4": 8.0, "C5": 13.5, "D64": 0.5, "D256": 0.4}.get(name, 5.0)
         return int(max(20, args.steps, math.ceil(120.0 / est)))
 
     def other_seeds(name, mode_):
@@ -905,15 +908,15 @@ def run_cuda(args):
                 configs["C1"] = c1_latency(args, D, args.seed)
             except Exception as e:
                 configs["C1"] = {"error": repr(e)}
-        if D.world == 1:
+        for extra in (("D64", "D256") if D.world == 1 else ()):
             try:
-                r, l, _ = measure_config(args, "D64", args.seed, D, sampler, traffic, 120, full=True, shard_mode="none")
+                r, l, _ = measure_config(args, extra, args.seed, D, sampler, traffic, region_steps(extra), full=True, shard_mode="none")
                 l.close()
                 del l
                 torch.cuda.empty_cache()
-                configs["D64"] = {k: v for k, v in r.items() if not k.startswith("_")}
+                configs[extra] = {k: v for k, v in r.items() if not k.startswith("_")}
             except Exception as e:
-                configs["D64"] = {"error": repr(e)}
+                configs[extra] = {"error": repr(e)}
     res["configs"] = configs
     if sampler:
         sampler.stop()

@@ -139,7 +139,7 @@ namespace {
 bool geometry_ok(const fcg_config_t *c) {
   if (!c) return false;
   if (c->n_layers <= 0 || c->n_kv_heads <= 0 || c->n_q_heads <= 0 || c->n_q_heads % c->n_kv_heads) return false;
-  if (c->head_dim != 64 && c->head_dim != 128) return false;
+  if (c->head_dim != 64 && c->head_dim != 128 && c->head_dim != 256) return false;
   if (c->page_size != 8 && c->page_size != 16 && c->page_size != 32 && c->page_size != 64) return false;
   if (c->rope_mode != FCG_ROPE_NONE && c->rope_mode != FCG_ROPE_HALF_SPLIT && c->rope_mode != FCG_ROPE_INTERLEAVED) return false;
   if (c->rope_mode != FCG_ROPE_NONE && !c->inv_freq && !(c->rope_base > 0.0)) return false;
@@ -488,7 +488,7 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
   *out = nullptr;
   if (!geometry_ok(cfg))
     return fail(FCG_ERR_INVALID_ARG,
-                "bad configuration (head_dim must be 64/128, page_size 8/16/32/64, n_q_heads %% n_kv_heads == 0, "
+                "bad configuration (head_dim must be 64/128/256, page_size 8/16/32/64, n_q_heads %% n_kv_heads == 0, "
                 "capacities > 0)");
   if (!cfg->arena || ((uintptr_t)cfg->arena % ALIGN)) return fail(FCG_ERR_INVALID_ARG, "arena must be a 256-byte aligned device pointer");
   Layout l = layout_of(cfg);
@@ -1042,7 +1042,9 @@ int choose_splits(int64_t base_ctas, int tiles, int rows, int head_dim, int ctas
   if (tiles <= 1) return 1;
   const double slots = (double)n_sms * ctas_per_sm;
   // everything in bytes streamed by one SM (an SM's share of HBM is ~44 GB/s: 10 us ~ 440 KB)
-  const double kFixedPerCta = 6000.0;            // launch + prologue + epilogue of a CTA
+  // launch + prologue + epilogue of a CTA.  head_dim 256: a 64 KB Q tile to fill and a 5-stage ring to ramp -- measured on
+  // the 4k-token decode step (336 CTAs unsplit: 0.26 ms; 4 / 8 / 16 splits: 0.29 / 0.34 / 0.50 ms), ~6 us per extra CTA
+  const double kFixedPerCta = head_dim == 256 ? 250000.0 : 6000.0;
   const double kCombineLaunch = 400000.0;        // the extra combine kernel: launch gap + its own ramp
   double best_cost = 1e30, cost_1 = 1e30;
   int best = 1;
@@ -1207,14 +1209,17 @@ fcg_status_t build_patch_blob(fcg_library *lib, const PatchSpec &ps, const Patch
   int max_rows = 0;
   for (int t = 0; t < ps.n_tasks; ++t) max_rows = std::max(max_rows, ps.n_per_task[t] * G);
   lay.max_rows = max_rows;
-  const bool use_tc = lib->have_tma && max_rows >= lib->tc_min_rows;
+  // head_dim 256 has the tcgen05 kernel only (one CTA class: a 128-row Q tile, more rows run as more row groups)
+  const bool d256 = c.head_dim == 256;
+  if (d256 && !lib->have_tma) return fail(FCG_ERR_CUDA, "head_dim 256 needs the tcgen05 / TMA attention path, which is unavailable on this device");
+  const bool use_tc = lib->have_tma && (max_rows >= lib->tc_min_rows || d256);
   lay.use_tc = use_tc;
   // tcgen05 path: a task with <= 128 rows per kv head runs CTAs with one 128-row Q tile (deep K/V rings: the
   // HBM-bound regime), a task with more rows CTAs with two (K/V read once per 256 rows).  A batch that mixes
   // both is launched as two grids, one per class.
   lay.rows_per_cta_split = max_rows <= 16 ? 16 : (max_rows <= 32 ? 32 : 64);
-  auto rows_per_cta_of = [&](int rows) { return use_tc ? (rows > 128 ? 256 : 128) : lay.rows_per_cta_split; };
-  const int ctas_per_sm = use_tc ? fcg::attn_tc_ctas_per_sm(c.head_dim, max_rows > 128 ? 2 : 1, (max_rows > 64 && max_rows <= 128) ? 2 : 1)
+  auto rows_per_cta_of = [&](int rows) { return use_tc ? ((rows > 128 && !d256) ? 256 : 128) : lay.rows_per_cta_split; };
+  const int ctas_per_sm = use_tc ? fcg::attn_tc_ctas_per_sm(c.head_dim, (max_rows > 128 && !d256) ? 2 : 1, (max_rows > 64 && max_rows <= 128 && !d256) ? 2 : 1)
                                  : fcg::attn_split_ctas_per_sm(c.head_dim);
   int max_splits = 1;
   int64_t tok_off = 0;
@@ -1249,7 +1254,7 @@ fcg_status_t build_patch_blob(fcg_library *lib, const PatchSpec &ps, const Patch
   // tcgen05 path: the same descriptors again, grouped by CTA class (rows per kv head <= 64 | <= 128 | more)
   auto *h_tasks2 = reinterpret_cast<fcg::AttnTaskDev *>(host + lay.off_tasks2);
   // (two 128-row CTAs instead of one two-Q-tile CTA for 129..256 rows was measured slower: C4 patch 3.24 vs 3.13 ms)
-  auto class_of = [&](int rows) { return rows <= 64 ? 0 : (rows <= 128 ? 1 : 2); };
+  auto class_of = [&](int rows) { return (rows <= 64 || d256) ? 0 : (rows <= 128 ? 1 : 2); };
   for (int cl = 0; cl < 3; ++cl) lay.n_cls[cl] = 0, lay.cls_rgs[cl] = 1;
   for (int t = 0; t < ps.n_tasks; ++t) lay.n_cls[class_of(h_tasks[t].n * G)]++;
   lay.cls_begin[0] = 0;

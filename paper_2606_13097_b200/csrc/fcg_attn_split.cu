@@ -426,6 +426,7 @@ cudaError_t launch_attn_combine(const AttnParams &p, int head_dim, cudaStream_t 
   cfg.numAttrs = 1;
   if (head_dim == 128) return cudaLaunchKernelEx(&cfg, attn_combine_kernel<128>, p);
   if (head_dim == 64) return cudaLaunchKernelEx(&cfg, attn_combine_kernel<64>, p);
+  if (head_dim == 256) return cudaLaunchKernelEx(&cfg, attn_combine_kernel<256>, p);
   return cudaErrorInvalidValue;
 }
 

@@ -37,7 +37,7 @@ constexpr int BN = 64;         // cache tokens per K/V tile
 constexpr float RESCALE_TAU = 8.0f;   // log2 units: keep a stale row max while the new one is < 2^8 larger
 
 // ---- shared memory map -------------------------------------------------------------------------
-// D = head_dim (128 or 64): a tile is D / 64 halves of 64 columns, each [rows][128 B] with the 128B swizzle
+// D = head_dim (64, 128 or 256): a tile is D / 64 halves of 64 columns, each [rows][128 B] with the 128B swizzle
 template <int NQ, int PS_, int D_>
 struct Cfg {
   static constexpr int D = D_;
@@ -55,8 +55,10 @@ struct Cfg {
   // keep the SM's share of HBM busy; two independent CTAs hide each other's.  Each takes half the shared memory
   // (6 + 5 stages of 8 KB) and 256 TMEM columns (S 2 x 64, O 64, P 2 x 32).
   static constexpr int CTAS_PER_SM = (D == 64 && NQ == 1 && PS_ == 1) ? 2 : 1;
-  static constexpr int K_STAGES = CTAS_PER_SM == 2 ? 6 : (NQ == 1 ? 6 : 5) * (128 / D);      // else the same bytes in flight for either head_dim
-  static constexpr int V_STAGES = CTAS_PER_SM == 2 ? 5 : (NQ == 1 ? 6 : 5) * (128 / D);
+  // head_dim 256 (one Q tile only: O alone takes 256 TMEM columns): Q 64 KB + 3 K stages + 2 V stages of 32 KB
+  static constexpr int K_STAGES = D == 256 ? 3 : (CTAS_PER_SM == 2 ? 6 : (NQ == 1 ? 6 : 5) * (128 / D));   // else the same bytes in flight for either head_dim
+  static constexpr int V_STAGES = D == 256 ? 2 : (CTAS_PER_SM == 2 ? 5 : (NQ == 1 ? 6 : 5) * (128 / D));
+  static_assert(D != 256 || (NQ == 1 && PS_ == 1), "head_dim 256: S 2 x 64 + O 256 + P 2 x 32 TMEM columns leave room for one Q tile and one stream set");
   // Tile-parity streams (NQ == 1 only): two softmax warpgroups, group w owns the KV tiles j = w (mod 2), its own
   // S / P buffer and its own O accumulator, with its own running (m, l); the streams are merged by log-sum-exp in
   // the epilogue like the row streams.  Two softmax warps per SM sub-partition hide each other's latencies.
@@ -209,8 +211,8 @@ __device__ __forceinline__ void attn_tc_body(const AttnParams &p, const TmaDesc 
 #pragma unroll 1
         for (int i = 0; i < n_ok; ++i) {
           const int pg = __shfl_sync(0xffffffffu, page, i);
-          tma_load_5d(dst + i * P * 128, tm, bar, 0, 0, g, pg, layer);
-          if (D == 128) tma_load_5d(dst + i * P * 128 + BN * 128, tm, bar, 64, 0, g, pg, layer);
+#pragma unroll
+          for (int h = 0; h < D / 64; ++h) tma_load_5d(dst + i * P * 128 + h * (BN * 128), tm, bar, 64 * h, 0, g, pg, layer);
         }
         page = page_next;
         if (++st == NS) {
@@ -330,11 +332,13 @@ __device__ __forceinline__ void attn_tc_body(const AttnParams &p, const TmaDesc 
     // are zero.  All softmax threads copy cooperatively (coalesced 16-B chunks), then hand Q to the MMA thread.
     // All 16 loads of a thread are issued before the first store: one global-memory round trip per CTA
     // instead of sixteen (the round-1 capture had 16 % of a softmax warp's life in this prologue).
-    {
-      uint4 qv[C::Q_ITERS];
+    constexpr int Q_BATCH = C::Q_ITERS > 16 ? 16 : C::Q_ITERS;    // head_dim 256: two batches of 16 loads (64 registers each)
 #pragma unroll
-      for (int i = 0; i < C::Q_ITERS; ++i) {
-        const int ci = tid + C::N_SOFTMAX * i;
+    for (int i0 = 0; i0 < C::Q_ITERS; i0 += Q_BATCH) {
+      uint4 qv[Q_BATCH];
+#pragma unroll
+      for (int i = 0; i < Q_BATCH; ++i) {
+        const int ci = tid + C::N_SOFTMAX * (i0 + i);
         const int row = ci / CPR, c = ci % CPR;
         const int rt = row & (BM - 1), tq = row >> 7;
         const int rl = rt & (rps - 1);
@@ -346,8 +350,8 @@ __device__ __forceinline__ void attn_tc_body(const AttnParams &p, const TmaDesc 
         }
       }
 #pragma unroll
-      for (int i = 0; i < C::Q_ITERS; ++i) {
-        const int ci = tid + C::N_SOFTMAX * i;
+      for (int i = 0; i < Q_BATCH; ++i) {
+        const int ci = tid + C::N_SOFTMAX * (i0 + i);
         const int row = ci / CPR, c = ci % CPR;
         const int rt = row & (BM - 1), tq = row >> 7;
         const uint32_t dst = C::OFF_Q + tq * Q_TILE_B + (c >> 3) * (BM * 128) + rt * 128 + (((c & 7) ^ (rt & 7)) << 4);
@@ -702,8 +706,11 @@ int attn_tc_ctas_per_sm(int head_dim, int q_tiles, int parity_streams) {
 // parity_streams (q_tiles == 1 only): 2 = two softmax warpgroups on alternating KV tiles, 1 = one warpgroup.
 cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, int parity_streams, const TmaDesc *tm_k,
                            const TmaDesc *tm_v, cudaStream_t stream) {
-  if ((head_dim != 128 && head_dim != 64) || !tm_k || !tm_v) return cudaErrorNotSupported;
-  if (head_dim == 128) {
+  if ((head_dim != 128 && head_dim != 64 && head_dim != 256) || !tm_k || !tm_v) return cudaErrorNotSupported;
+  if (head_dim == 256) {
+    // one CTA class: a 128-row Q tile per CTA, more rows per kv head run as more row groups
+    if (q_tiles == 1 && parity_streams == 1) return launch_nq<1, 1, 256>(p, *tm_k, *tm_v, stream);
+  } else if (head_dim == 128) {
     if (q_tiles == 1 && parity_streams == 2) return launch_nq<1, 2, 128>(p, *tm_k, *tm_v, stream);
     if (q_tiles == 1) return launch_nq<1, 1, 128>(p, *tm_k, *tm_v, stream);
     if (q_tiles == 2) return launch_nq<2, 1, 128>(p, *tm_k, *tm_v, stream);

@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(256) register_copy_kernel(const RegisterParams
 // 0 for an all-zero row; code = RNE_e4m3(x * 2^-e) (the scaling is exact), non-finite elements -> the NaN code 0x7F.
 template <int D>
 __global__ void __launch_bounds__(256) register_fp8_kernel(const RegisterFp8Params p) {
-  constexpr int EPL = D / 32;                         // elements per lane: 4 (D = 128) or 2 (D = 64)
+  constexpr int EPL = D / 32;                         // elements per lane: 8 (D = 256), 4 (D = 128) or 2 (D = 64)
   const size_t n_rows = (size_t)p.n_layers * p.n_kv_heads * p.n_tokens;
   const int lane = threadIdx.x & 31;
   for (size_t row = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); row < 2 * n_rows;
@@ -47,13 +47,19 @@ __global__ void __launch_bounds__(256) register_fp8_kernel(const RegisterFp8Para
     const int h = (int)(lh % p.n_kv_heads), l = (int)(lh / p.n_kv_heads);
     const uint16_t *src = (is_v ? p.v_src : p.k_src) + (size_t)((int64_t)l * p.s_layer + (int64_t)h * p.s_head + (int64_t)t * p.s_tok) + lane * EPL;
     float x[EPL];
-    if (EPL == 4) {
-      const uint2 w = *reinterpret_cast<const uint2 *>(src);
-      x[0] = __uint_as_float(w.x << 16), x[1] = __uint_as_float(w.x & 0xffff0000u);
-      x[EPL - 2] = __uint_as_float(w.y << 16), x[EPL - 1] = __uint_as_float(w.y & 0xffff0000u);
-    } else {
-      const uint32_t w = *reinterpret_cast<const uint32_t *>(src);
-      x[0] = __uint_as_float(w << 16), x[1] = __uint_as_float(w & 0xffff0000u);
+    {
+      uint32_t w[EPL / 2];
+      if (EPL == 8) {
+        const uint4 v = *reinterpret_cast<const uint4 *>(src);
+        w[0] = v.x, w[EPL / 2 > 1 ? 1 : 0] = v.y, w[EPL / 2 > 2 ? 2 : 0] = v.z, w[EPL / 2 > 3 ? 3 : 0] = v.w;
+      } else if (EPL == 4) {
+        const uint2 v = *reinterpret_cast<const uint2 *>(src);
+        w[0] = v.x, w[EPL / 2 > 1 ? 1 : 0] = v.y;
+      } else {
+        w[0] = *reinterpret_cast<const uint32_t *>(src);
+      }
+#pragma unroll
+      for (int i = 0; i < EPL / 2; ++i) x[2 * i] = __uint_as_float(w[i] << 16), x[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
     }
     uint32_t amax = 0;                                // |x| as bits: ordered like the values for non-negative floats
 #pragma unroll
@@ -69,18 +75,20 @@ __global__ void __launch_bounds__(256) register_fp8_kernel(const RegisterFp8Para
       e = be == 0 ? -127 : (be - 127) - ((amax & 0x7fffffu) <= 0x600000u ? 8 : 7);
       e = max(-127, min(127, e));
     }
-    uint32_t packed = 0;
+    uint64_t packed = 0;
 #pragma unroll
     for (int i = 0; i < EPL; i += 2) {
       const float a = scalbnf(x[i], -e), b = scalbnf(x[i + 1], -e);
       uint32_t c2 = (uint32_t)__nv_cvt_float2_to_fp8x2(make_float2(a, b), __NV_SATFINITE, __NV_E4M3);
       if ((__float_as_uint(x[i]) & 0x7fffffffu) >= 0x7f800000u) c2 = (c2 & 0xff00u) | 0x7fu;
       if ((__float_as_uint(x[i + 1]) & 0x7fffffffu) >= 0x7f800000u) c2 = (c2 & 0x00ffu) | 0x7f00u;
-      packed |= c2 << (8 * i);
+      packed |= (uint64_t)c2 << (8 * i);
     }
     uint8_t *dst = (is_v ? p.v_dst : p.k_dst) + r * D + lane * EPL;
-    if (EPL == 4)
-      *reinterpret_cast<uint32_t *>(dst) = packed;
+    if (EPL == 8)
+      *reinterpret_cast<uint2 *>(dst) = make_uint2((uint32_t)packed, (uint32_t)(packed >> 32));
+    else if (EPL == 4)
+      *reinterpret_cast<uint32_t *>(dst) = (uint32_t)packed;
     else
       *reinterpret_cast<uint16_t *>(dst) = (uint16_t)packed;
     if (lane == 0) (is_v ? p.v_exp : p.k_exp)[r] = (uint8_t)(e + 127);
@@ -151,6 +159,8 @@ cudaError_t launch_register_fp8(const RegisterFp8Params &p, cudaStream_t stream)
     register_fp8_kernel<128><<<grid, 256, 0, stream>>>(p);
   else if (p.head_dim == 64)
     register_fp8_kernel<64><<<grid, 256, 0, stream>>>(p);
+  else if (p.head_dim == 256)
+    register_fp8_kernel<256><<<grid, 256, 0, stream>>>(p);
   else
     return cudaErrorInvalidValue;
   return cudaGetLastError();

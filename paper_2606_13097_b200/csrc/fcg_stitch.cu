@@ -332,6 +332,8 @@ cudaError_t launch_rope_qk(const RopeQkParams &p, int head_dim, cudaStream_t str
     rope_qk_kernel<128><<<grid, 128, 0, stream>>>(p);
   else if (head_dim == 64)
     rope_qk_kernel<64><<<grid, 128, 0, stream>>>(p);
+  else if (head_dim == 256)
+    rope_qk_kernel<256><<<grid, 128, 0, stream>>>(p);
   else
     return cudaErrorInvalidValue;
   return cudaGetLastError();
@@ -351,6 +353,11 @@ cudaError_t launch_stitch(const StitchParams &p, int head_dim, cudaStream_t stre
       stitch_kernel<64, true><<<grid, block, 0, stream>>>(p);
     else
       stitch_kernel<64, false><<<grid, block, 0, stream>>>(p);
+  } else if (head_dim == 256) {
+    if (p.any_fp8)
+      stitch_kernel<256, true><<<grid, block, 0, stream>>>(p);
+    else
+      stitch_kernel<256, false><<<grid, block, 0, stream>>>(p);
   } else {
     return cudaErrorInvalidValue;
   }

@@ -37,7 +37,7 @@ def sample_slices(cfg, n_samples, seed):
 
 
 def run_fullsize(name, seed, n_samples, n_attn_samples):
-    cfg = synth.CONFIGS[name]
+    cfg = bench.BENCH_CONFIGS[name]
     wl = synth.make_workload(cfg, seed)
     G = cfg.n_q_heads // cfg.n_kv_heads
     dev = torch.device("cuda", 0)
@@ -117,6 +117,15 @@ def test_c4_full_size_sampled_slices():
 
 def test_c5_full_size_sampled_slices():
     run_fullsize("C5", 1, 2, 1)
+
+
+def test_d64_full_size_sampled_slices():
+    run_fullsize("D64", 1, 3, 3)
+
+
+def test_d256_full_size_sampled_slices():
+    """head_dim 256 (R27) in bench.py's launch shape: 42 layers, 16 q / 8 kv heads, 4k tokens, 64-token patch."""
+    run_fullsize("D256", 1, 3, 3)
 
 
 def test_c2_full_size_next_rows():

@@ -81,6 +81,10 @@ GEOMS = [
     (1, 8, 1, 128, 64, 1e6),
     (3, 6, 3, 64, 8, 1e4),
     (1, 16, 2, 64, 32, 1e4),
+    # head_dim 256 (Gemma-style heads, R27): one CTA class on the tcgen05 path, stitch_kernel<256>
+    (2, 8, 2, 256, 16, 1e4),
+    (1, 4, 4, 256, 64, 5e5),
+    (1, 6, 3, 256, 8, 1e6),
 ]
 
 
