@@ -28,6 +28,20 @@ def assert_k_within_1ulp(gpu_bits, ref_bits, what=""):
     return hist
 
 
+def k_pair_close(a_bits, b_bits, c, rope_mode=1):
+    """|a - b| <= c * 2^-9 * |rotation pair| per component: the bar for keys that went through MORE than one rotation
+    generation (each side rounds once per generation, from inputs that may already differ by a rounding), where a ulp
+    count is meaningless for the small component of a pair."""
+    a, b = O.bf16_to_f64(np.asarray(a_bits)), O.bf16_to_f64(np.asarray(b_bits))
+    if rope_mode == 2:
+        norm = np.repeat(np.sqrt(b[..., 0::2] ** 2 + b[..., 1::2] ** 2), 2, axis=-1)
+    else:
+        half = b.shape[-1] // 2
+        n = np.sqrt(b[..., :half] ** 2 + b[..., half:] ** 2)
+        norm = np.concatenate([n, n], axis=-1)
+    return bool(np.all(np.abs(a - b) <= c * 2.0 ** -9 * norm + 1e-30))
+
+
 def assert_attn_close(gpu_out: torch.Tensor, ref: np.ndarray, what=""):
     got = gpu_out.detach().float().cpu().numpy().astype(np.float64)
     err = np.abs(got - ref)
