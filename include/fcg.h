@@ -75,7 +75,9 @@ typedef struct {
   int32_t n_layers;
   int32_t n_q_heads;       /* multiple of n_kv_heads */
   int32_t n_kv_heads;
-  int32_t head_dim;        /* 64, 128 or 256 (R27); 256: patch attention has the tcgen05/TMEM kernel only */
+  int32_t head_dim;        /* a multiple of 16 in [16, 256] (R27).  64, 128 and 256 have kernels of their own; the others run
+                              the gather with head_dim as a run-time value and the tcgen05 attention at the next of those
+                              widths with zero-padded columns.  Only 64 and 128 also have the split-KV warp-MMA kernel */
   int32_t page_size;       /* tokens per page: 8, 16, 32 or 64 */
   int32_t rope_mode;       /* FCG_ROPE_NONE: stitch is a pure gather; FCG_ROPE_HALF_SPLIT: pairs (j, j + head_dim/2) (R2);
                               FCG_ROPE_INTERLEAVED: pairs (2j, 2j + 1) */
@@ -317,8 +319,8 @@ fcg_status_t fcg_pool_info(fcg_library_t *lib, fcg_pool_info_t *out);
 /* Kernel selection for patch attention: calls whose largest task has R = n * G >= tc_min_rows query rows per
  * kv head use the tcgen05/TMEM kernel, others the split-KV warp-MMA kernel.  Default 1: tcgen05 for every R
  * (measured faster than the split-KV kernel down to a decode step, DESIGN.md section 6 -- north_star expected the
- * opposite for short patches); INT32_MAX = never.  head_dim 256 always runs the tcgen05 kernel (it has no split-KV
- * warp-MMA instantiation): tc_min_rows is ignored there, force_splits applies.
+ * opposite for short patches); INT32_MAX = never.  Every head_dim other than 64 and 128 always runs the tcgen05 kernel (no
+ * split-KV warp-MMA instantiation): tc_min_rows is ignored there, force_splits applies.
  * force_splits > 0 fixes the number of KV splits per task (clamped to the task's 64-token tile count);
  * 0 = the library's wave-filling choice.  The result does not depend on either knob beyond summation order
  * (P11, split invariance). */

@@ -139,7 +139,7 @@ namespace {
 bool geometry_ok(const fcg_config_t *c) {
   if (!c) return false;
   if (c->n_layers <= 0 || c->n_kv_heads <= 0 || c->n_q_heads <= 0 || c->n_q_heads % c->n_kv_heads) return false;
-  if (c->head_dim != 64 && c->head_dim != 128 && c->head_dim != 256) return false;
+  if (c->head_dim < 16 || c->head_dim > 256 || c->head_dim % 16) return false;      // R27
   if (c->page_size != 8 && c->page_size != 16 && c->page_size != 32 && c->page_size != 64) return false;
   if (c->rope_mode != FCG_ROPE_NONE && c->rope_mode != FCG_ROPE_HALF_SPLIT && c->rope_mode != FCG_ROPE_INTERLEAVED) return false;
   if (c->rope_mode != FCG_ROPE_NONE && !c->inv_freq && !(c->rope_base > 0.0)) return false;
@@ -460,6 +460,7 @@ fcg_status_t enqueue_gather(fcg_library *lib, const GatherBuilder &gb, cudaStrea
   sp.n_layers = c.n_layers;
   sp.n_kv_heads = c.n_kv_heads;
   sp.interleaved = c.rope_mode == FCG_ROPE_INTERLEAVED ? 1 : 0;
+  sp.head_dim = c.head_dim;
   if (!gb.chunks.empty()) {
     FCG_CUDA(fcg::launch_stitch(sp, c.head_dim, stream));
     lib->stats.stitch_launches++;
@@ -488,7 +489,7 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
   *out = nullptr;
   if (!geometry_ok(cfg))
     return fail(FCG_ERR_INVALID_ARG,
-                "bad configuration (head_dim must be 64/128/256, page_size 8/16/32/64, n_q_heads %% n_kv_heads == 0, "
+                "bad configuration (head_dim must be a multiple of 16 in [16, 256], page_size 8/16/32/64, n_q_heads %% n_kv_heads == 0, "
                 "capacities > 0)");
   if (!cfg->arena || ((uintptr_t)cfg->arena % ALIGN)) return fail(FCG_ERR_INVALID_ARG, "arena must be a 256-byte aligned device pointer");
   Layout l = layout_of(cfg);
@@ -1044,7 +1045,7 @@ int choose_splits(int64_t base_ctas, int tiles, int rows, int head_dim, int ctas
   // everything in bytes streamed by one SM (an SM's share of HBM is ~44 GB/s: 10 us ~ 440 KB)
   // launch + prologue + epilogue of a CTA.  head_dim 256: a 64 KB Q tile to fill and a 5-stage ring to ramp -- measured on
   // the 4k-token decode step (336 CTAs unsplit: 0.26 ms; 4 / 8 / 16 splits: 0.29 / 0.34 / 0.50 ms), ~6 us per extra CTA
-  const double kFixedPerCta = head_dim == 256 ? 250000.0 : 6000.0;
+  const double kFixedPerCta = head_dim > 128 ? 250000.0 : 6000.0;
   const double kCombineLaunch = 400000.0;        // the extra combine kernel: launch gap + its own ramp
   double best_cost = 1e30, cost_1 = 1e30;
   int best = 1;
@@ -1209,10 +1210,12 @@ fcg_status_t build_patch_blob(fcg_library *lib, const PatchSpec &ps, const Patch
   int max_rows = 0;
   for (int t = 0; t < ps.n_tasks; ++t) max_rows = std::max(max_rows, ps.n_per_task[t] * G);
   lay.max_rows = max_rows;
-  // head_dim 256 has the tcgen05 kernel only (one CTA class: a 128-row Q tile, more rows run as more row groups)
-  const bool d256 = c.head_dim == 256;
-  if (d256 && !lib->have_tma) return fail(FCG_ERR_CUDA, "head_dim 256 needs the tcgen05 / TMA attention path, which is unavailable on this device");
-  const bool use_tc = lib->have_tma && (max_rows >= lib->tc_min_rows || d256);
+  // head_dim above 128 has ONE CTA class on the tcgen05 path (a 128-row Q tile, more rows run as more row groups); only
+  // head_dim 64 and 128 have the split-KV mma.sync kernel besides (R27)
+  const bool d256 = c.head_dim > 128;
+  const bool tc_only = c.head_dim != 64 && c.head_dim != 128;
+  if (tc_only && !lib->have_tma) return fail(FCG_ERR_CUDA, "head_dim %d needs the tcgen05 / TMA attention path, which is unavailable on this device", c.head_dim);
+  const bool use_tc = lib->have_tma && (max_rows >= lib->tc_min_rows || tc_only);
   lay.use_tc = use_tc;
   // tcgen05 path: a task with <= 128 rows per kv head runs CTAs with one 128-row Q tile (deep K/V rings: the
   // HBM-bound regime), a task with more rows CTAs with two (K/V read once per 256 rows).  A batch that mixes
@@ -1398,6 +1401,7 @@ fcg_status_t launch_patch(fcg_library *lib, const PatchLayout &lay, const unsign
   ap.scale_log2 = (float)(1.4426950408889634 / sqrt((double)c.head_dim));
   ap.items = nullptr;
   ap.n_items = 0;
+  ap.head_dim = c.head_dim;
   if (lay.use_tc && lay.n_items > 0) {
     // all classes in one launch, interleaved (see build_patch_blob)
     fcg::AttnParams apm = ap;
@@ -1747,6 +1751,7 @@ fcg_status_t fcg_patch_rope(fcg_library_t *lib, int32_t task_id, int32_t layer_b
   rp.n_q_heads = c.n_q_heads;
   rp.n_kv_heads = c.n_kv_heads;
   rp.interleaved = c.rope_mode == FCG_ROPE_INTERLEAVED ? 1 : 0;
+  rp.head_dim = c.head_dim;
   FCG_CUDA(fcg::launch_rope_qk(rp, c.head_dim, stream));
   lib->stats.rope_qk_launches++;
   const uint64_t saved = lib->scratch_bytes;

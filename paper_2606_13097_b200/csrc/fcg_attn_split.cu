@@ -377,6 +377,56 @@ __global__ void __launch_bounds__(256) attn_combine_kernel(const AttnParams p) {
   for (int c = 0; c < CPL; c += 2) *reinterpret_cast<uint32_t *>(dst + c) = pack_bf16(acc[c] * inv, acc[c + 1] * inv);
 }
 
+// the same merge for any head_dim that is a multiple of 16 (p.head_dim; R27): a lane owns the element pairs
+// 2 * lane + 64 * i of the row
+__global__ void __launch_bounds__(256) attn_combine_any_kernel(const AttnParams p) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  const int d = p.head_dim;
+  const size_t n_rows = (size_t)p.n_layers * p.n_total * p.n_q_heads;
+  const size_t rowi = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (rowi >= n_rows) return;
+  const int lane = threadIdx.x & 31;
+  const int h = (int)(rowi % p.n_q_heads);
+  const size_t lt = rowi / p.n_q_heads;
+  const int tok = (int)(lt % p.n_total);
+  const int li = (int)(lt / p.n_total);
+  const int ns = p.tok_splits[tok];
+  if (ns <= 1) return;
+  float M = -INFINITY;
+  for (int s = 0; s < ns; ++s) {
+    const size_t prow = ((size_t)(li * p.max_splits + s) * p.n_total + tok) * p.n_q_heads + h;
+    M = fmaxf(M, p.part_ml[prow * 2]);
+  }
+  const float Mu = M == -INFINITY ? 0.f : M;
+  float acc[8];                                   // up to 4 pairs per lane (d <= 256)
+#pragma unroll
+  for (int c = 0; c < 8; ++c) acc[c] = 0.f;
+  float L = 0.f;
+  for (int s = 0; s < ns; ++s) {
+    const size_t prow = ((size_t)(li * p.max_splits + s) * p.n_total + tok) * p.n_q_heads + h;
+    const float2 ml = *reinterpret_cast<const float2 *>(p.part_ml + prow * 2);
+    const float w = exp2f(ml.x - Mu);
+    L += w * ml.y;
+    const float *src = p.part_o + prow * d;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int c = 2 * lane + 64 * i;
+      if (c < d) {
+        const float2 x = *reinterpret_cast<const float2 *>(src + c);
+        acc[2 * i] += w * x.x;
+        acc[2 * i + 1] += w * x.y;
+      }
+    }
+  }
+  const float inv = L > 0.f ? 1.f / L : 0.f;
+  uint16_t *dst = p.out + rowi * d;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int c = 2 * lane + 64 * i;
+    if (c < d) *reinterpret_cast<uint32_t *>(dst + c) = pack_bf16(acc[2 * i] * inv, acc[2 * i + 1] * inv);
+  }
+}
+
 template <int D, int MB>
 cudaError_t launch_split_t(const AttnParams &p, cudaStream_t stream) {
   constexpr int SMEM = STAGES * 2 * BN * D * 2;
@@ -427,6 +477,7 @@ cudaError_t launch_attn_combine(const AttnParams &p, int head_dim, cudaStream_t 
   if (head_dim == 128) return cudaLaunchKernelEx(&cfg, attn_combine_kernel<128>, p);
   if (head_dim == 64) return cudaLaunchKernelEx(&cfg, attn_combine_kernel<64>, p);
   if (head_dim == 256) return cudaLaunchKernelEx(&cfg, attn_combine_kernel<256>, p);
+  if (head_dim >= 16 && head_dim < 256 && head_dim % 16 == 0 && p.head_dim == head_dim) return cudaLaunchKernelEx(&cfg, attn_combine_any_kernel, p);
   return cudaErrorInvalidValue;
 }
 

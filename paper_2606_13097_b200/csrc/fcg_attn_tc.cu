@@ -86,7 +86,10 @@ struct Cfg {
 // The whole CTA program for one work item (task, layer index, kv head, KV split, row group).  Called by the per-class
 // kernels below (indices from the 3-D grid) and by attn_tc_mixed_kernel (indices from an item table); a CTA may have
 // more warps than this class uses (mixed kernel): those take no role and only meet the two CTA-wide barriers.
-template <int NQ, int PS_, int D>
+// PAD: the real head_dim d = p.head_dim is a multiple of 16 below the instantiated D (R27): Q rows and output rows have d
+// elements, the Q tile's columns [d, D) are zero, and the K / V boxes come from a tensor map whose innermost extent is d, so
+// TMA zero-fills their columns [d, D) -- the MMAs run at D, the zero columns add nothing to S and give zero O columns.
+template <int NQ, int PS_, int D, bool PAD = false>
 __device__ __forceinline__ void attn_tc_body(const AttnParams &p, const TmaDesc &tm_k, const TmaDesc &tm_v, unsigned char *smem_raw,
                                              const int task_i, const int li, const int g, const int split, const int rg) {
   using C = Cfg<NQ, PS_, D>;
@@ -104,6 +107,7 @@ __device__ __forceinline__ void attn_tc_body(const AttnParams &p, const TmaDesc 
   const int layer = p.layer_begin + li;
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // tells the compiler that the warp index is warp-uniform
+  const int d = PAD ? p.head_dim : D;                       // elements per q / out row
 
   // ---- row layout of this CTA (see "Row streams" in the header) ---------------------------------
   const int Rc = min(R - row0, NQ * BM);           // valid query rows of this CTA
@@ -343,9 +347,9 @@ __device__ __forceinline__ void attn_tc_body(const AttnParams &p, const TmaDesc 
         const int rt = row & (BM - 1), tq = row >> 7;
         const int rl = rt & (rps - 1);
         qv[i] = make_uint4(0, 0, 0, 0);
-        if (rl < tile_rows(tq)) {
+        if (rl < tile_rows(tq) && (!PAD || c * 8 < d)) {
           const int r = row0 + tq * BM + rl;
-          const uint16_t *src = p.q + (((size_t)li * p.n_total + tk.tok_off + r / G) * p.n_q_heads + g * G + r % G) * D + c * 8;
+          const uint16_t *src = p.q + (((size_t)li * p.n_total + tk.tok_off + r / G) * p.n_q_heads + g * G + r % G) * d + c * 8;
           qv[i] = __ldg(reinterpret_cast<const uint4 *>(src));
         }
       }
@@ -583,9 +587,10 @@ __device__ __forceinline__ void attn_tc_body(const AttnParams &p, const TmaDesc 
             }
           }
           if (final_out) {
-            uint16_t *dst = p.out + out_row * D + ch * 32;
+            uint16_t *dst = p.out + out_row * d + ch * 32;
 #pragma unroll
             for (int c = 0; c < 32; c += 8) {
+              if (PAD && ch * 32 + c >= d) break;
               uint4 v;
               v.x = pack_bf16(o[c] * inv, o[c + 1] * inv);
               v.y = pack_bf16(o[c + 2] * inv, o[c + 3] * inv);
@@ -594,9 +599,12 @@ __device__ __forceinline__ void attn_tc_body(const AttnParams &p, const TmaDesc 
               *reinterpret_cast<uint4 *>(dst + c) = v;
             }
           } else {
-            float *dst = p.part_o + prow_i * D + ch * 32;
+            float *dst = p.part_o + prow_i * d + ch * 32;
 #pragma unroll
-            for (int c = 0; c < 32; c += 4) *reinterpret_cast<float4 *>(dst + c) = make_float4(o[c], o[c + 1], o[c + 2], o[c + 3]);
+            for (int c = 0; c < 32; c += 4) {
+              if (PAD && ch * 32 + c >= d) break;
+              *reinterpret_cast<float4 *>(dst + c) = make_float4(o[c], o[c + 1], o[c + 2], o[c + 3]);
+            }
           }
         }
       }
@@ -612,11 +620,11 @@ __device__ __forceinline__ void attn_tc_body(const AttnParams &p, const TmaDesc 
   }
 }
 
-template <int NQ, int PS_, int D>
+template <int NQ, int PS_, int D, bool PAD = false>
 __global__ void __launch_bounds__(Cfg<NQ, PS_, D>::NTHREADS, Cfg<NQ, PS_, D>::CTAS_PER_SM)
     attn_tc_kernel(const AttnParams p, const __grid_constant__ TmaDesc tm_k, const __grid_constant__ TmaDesc tm_v) {
   extern __shared__ unsigned char smem_raw[];
-  attn_tc_body<NQ, PS_, D>(p, tm_k, tm_v, smem_raw, blockIdx.z % p.n_tasks, blockIdx.z / p.n_tasks, blockIdx.y, blockIdx.x % p.max_splits,
+  attn_tc_body<NQ, PS_, D, PAD>(p, tm_k, tm_v, smem_raw, blockIdx.z % p.n_tasks, blockIdx.z / p.n_tasks, blockIdx.y, blockIdx.x % p.max_splits,
                            blockIdx.x / p.max_splits);
 }
 
@@ -647,7 +655,7 @@ __global__ void __launch_bounds__(MIXED_THREADS, 1)
     attn_tc_body<1, 1, 128>(p, tm_k, tm_v, smem_raw, it.y, li, g, it.w, it.z);
 }
 
-template <int NQ, int PS_, int D>
+template <int NQ, int PS_, int D, bool PAD = false>
 cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv, cudaStream_t stream) {
   using C = Cfg<NQ, PS_, D>;
   // the attribute is per device (fcg_config_t.device allows libraries on several GPUs in one process)
@@ -655,7 +663,7 @@ cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv,
   int dev = -1;
   if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
   if (dev < 0 || dev >= 64 || !configured[dev]) {
-    cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, PS_, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, PS_, D, PAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     if (dev >= 0 && dev < 64) configured[dev] = true;
   }
@@ -669,7 +677,7 @@ cudaError_t launch_nq(const AttnParams &p, const TmaDesc &tk, const TmaDesc &tv,
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, attn_tc_kernel<NQ, PS_, D>, p, tk, tv);
+  return cudaLaunchKernelEx(&cfg, attn_tc_kernel<NQ, PS_, D, PAD>, p, tk, tv);
 }
 
 }  // namespace
@@ -699,14 +707,14 @@ cudaError_t launch_attn_tc_mixed(const AttnParams &p, const TmaDesc *tm_k, const
 }
 
 int attn_tc_ctas_per_sm(int head_dim, int q_tiles, int parity_streams) {
-  return (head_dim == 64 && q_tiles == 1 && parity_streams == 1) ? 2 : 1;
+  return (head_dim <= 64 && q_tiles == 1 && parity_streams == 1) ? 2 : 1;
 }
 
 // q_tiles = 128-row Q tiles per CTA (1 or 2); p.max_row_groups counts groups of q_tiles*128 rows.
 // parity_streams (q_tiles == 1 only): 2 = two softmax warpgroups on alternating KV tiles, 1 = one warpgroup.
 cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, int parity_streams, const TmaDesc *tm_k,
                            const TmaDesc *tm_v, cudaStream_t stream) {
-  if ((head_dim != 128 && head_dim != 64 && head_dim != 256) || !tm_k || !tm_v) return cudaErrorNotSupported;
+  if (head_dim < 16 || head_dim > 256 || head_dim % 16 || !tm_k || !tm_v || p.head_dim != head_dim) return cudaErrorNotSupported;
   if (head_dim == 256) {
     // one CTA class: a 128-row Q tile per CTA, more rows per kv head run as more row groups
     if (q_tiles == 1 && parity_streams == 1) return launch_nq<1, 1, 256>(p, *tm_k, *tm_v, stream);
@@ -714,10 +722,21 @@ cudaError_t launch_attn_tc(const AttnParams &p, int head_dim, int q_tiles, int p
     if (q_tiles == 1 && parity_streams == 2) return launch_nq<1, 2, 128>(p, *tm_k, *tm_v, stream);
     if (q_tiles == 1) return launch_nq<1, 1, 128>(p, *tm_k, *tm_v, stream);
     if (q_tiles == 2) return launch_nq<2, 1, 128>(p, *tm_k, *tm_v, stream);
-  } else {
+  } else if (head_dim == 64) {
     if (q_tiles == 1 && parity_streams == 2) return launch_nq<1, 2, 64>(p, *tm_k, *tm_v, stream);
     if (q_tiles == 1) return launch_nq<1, 1, 64>(p, *tm_k, *tm_v, stream);
     if (q_tiles == 2) return launch_nq<2, 1, 64>(p, *tm_k, *tm_v, stream);
+  } else if (head_dim > 128) {
+    // other multiples of 16 run the next instantiated width with zero-padded columns (PAD)
+    if (q_tiles == 1 && parity_streams == 1) return launch_nq<1, 1, 256, true>(p, *tm_k, *tm_v, stream);
+  } else if (head_dim > 64) {
+    if (q_tiles == 1 && parity_streams == 2) return launch_nq<1, 2, 128, true>(p, *tm_k, *tm_v, stream);
+    if (q_tiles == 1) return launch_nq<1, 1, 128, true>(p, *tm_k, *tm_v, stream);
+    if (q_tiles == 2) return launch_nq<2, 1, 128, true>(p, *tm_k, *tm_v, stream);
+  } else {
+    if (q_tiles == 1 && parity_streams == 2) return launch_nq<1, 2, 64, true>(p, *tm_k, *tm_v, stream);
+    if (q_tiles == 1) return launch_nq<1, 1, 64, true>(p, *tm_k, *tm_v, stream);
+    if (q_tiles == 2) return launch_nq<2, 1, 64, true>(p, *tm_k, *tm_v, stream);
   }
   return cudaErrorInvalidValue;
 }

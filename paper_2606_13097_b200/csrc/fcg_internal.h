@@ -42,6 +42,7 @@ struct StitchParams {
   const float4 *table;   // per (entry, j): {c_hi, c_lo, s_hi, s_lo}; c_hi/s_hi have <= 16 significant bits
   int32_t n_chunks, n_layers, n_kv_heads;
   int32_t interleaved;   // 0: pairs (j, j + D/2) (half-split); 1: pairs (2j, 2j + 1)
+  int32_t head_dim;      // row length in elements (the run-time-D instantiation reads it)
 };
 
 cudaError_t launch_stitch(const StitchParams &p, int head_dim, cudaStream_t stream);
@@ -53,6 +54,7 @@ struct RopeQkParams {
   uint16_t *q_out, *k_out;   // same shapes
   const float4 *table;       // [n_total][D/2]
   int32_t n_layers, n_total, n_q_heads, n_kv_heads, interleaved;
+  int32_t head_dim;
 };
 cudaError_t launch_rope_qk(const RopeQkParams &p, int head_dim, cudaStream_t stream);
 
@@ -125,6 +127,7 @@ struct AttnParams {
   float scale_log2;          // log2(e) / sqrt(D)
   const int4 *items;         // mixed-class launch: {class, task index, row group, split} per work item (else NULL)
   int32_t n_items;
+  int32_t head_dim;          // the real head_dim (q / out / partial row length); the tcgen05 kernels may run at a padded width
 };
 
 // split-KV warp-MMA (mma.sync m16n8k16) path; rows_per_cta in {16, 32, 64}

@@ -95,6 +95,58 @@ __global__ void __launch_bounds__(256) register_fp8_kernel(const RegisterFp8Para
   }
 }
 
+// the same for any head_dim that is a multiple of 8 (p.head_dim <= 256): lane c owns the elements [8c, 8c + 8) of the row
+__global__ void __launch_bounds__(256) register_fp8_any_kernel(const RegisterFp8Params p) {
+  const int D = p.head_dim;
+  const size_t n_rows = (size_t)p.n_layers * p.n_kv_heads * p.n_tokens;
+  const int lane = threadIdx.x & 31;
+  const bool on = lane * 8 < D;
+  for (size_t row = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); row < 2 * n_rows;
+       row += (size_t)gridDim.x * (blockDim.x >> 5)) {
+    const bool is_v = row >= n_rows;
+    const size_t r = is_v ? row - n_rows : row;
+    const int t = (int)(r % p.n_tokens);
+    const size_t lh = r / p.n_tokens;
+    const int h = (int)(lh % p.n_kv_heads), l = (int)(lh / p.n_kv_heads);
+    const uint16_t *src = (is_v ? p.v_src : p.k_src) + (size_t)((int64_t)l * p.s_layer + (int64_t)h * p.s_head + (int64_t)t * p.s_tok) + lane * 8;
+    float x[8];
+    uint32_t amax = 0;
+    if (on) {
+      const uint4 v = *reinterpret_cast<const uint4 *>(src);
+      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int i = 0; i < 4; ++i) x[2 * i] = __uint_as_float(w[i] << 16), x[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const uint32_t a = __float_as_uint(x[i]) & 0x7fffffffu;
+        if (a < 0x7f800000u) amax = max(amax, a);
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) amax = max(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    int e = 0;
+    if (amax != 0) {
+      const int be = (int)(amax >> 23);
+      e = be == 0 ? -127 : (be - 127) - ((amax & 0x7fffffu) <= 0x600000u ? 8 : 7);
+      e = max(-127, min(127, e));
+    }
+    if (on) {
+      uint64_t packed = 0;
+#pragma unroll
+      for (int i = 0; i < 8; i += 2) {
+        const float a = scalbnf(x[i], -e), b = scalbnf(x[i + 1], -e);
+        uint32_t c2 = (uint32_t)__nv_cvt_float2_to_fp8x2(make_float2(a, b), __NV_SATFINITE, __NV_E4M3);
+        if ((__float_as_uint(x[i]) & 0x7fffffffu) >= 0x7f800000u) c2 = (c2 & 0xff00u) | 0x7fu;
+        if ((__float_as_uint(x[i + 1]) & 0x7fffffffu) >= 0x7f800000u) c2 = (c2 & 0x00ffu) | 0x7f00u;
+        packed |= (uint64_t)c2 << (8 * i);
+      }
+      uint8_t *dst = (is_v ? p.v_dst : p.k_dst) + r * D + lane * 8;
+      *reinterpret_cast<uint2 *>(dst) = make_uint2((uint32_t)packed, (uint32_t)(packed >> 32));
+    }
+    if (lane == 0) (is_v ? p.v_exp : p.k_exp)[r] = (uint8_t)(e + 127);
+  }
+}
+
 __global__ void __launch_bounds__(256) scatter_kernel(const ScatterParams p) {
   // the attention kernel that follows may start its prologue now (it waits for this grid before reading the cache)
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -161,6 +213,8 @@ cudaError_t launch_register_fp8(const RegisterFp8Params &p, cudaStream_t stream)
     register_fp8_kernel<64><<<grid, 256, 0, stream>>>(p);
   else if (p.head_dim == 256)
     register_fp8_kernel<256><<<grid, 256, 0, stream>>>(p);
+  else if (p.head_dim >= 8 && p.head_dim < 256 && p.head_dim % 8 == 0)
+    register_fp8_any_kernel<<<grid, 256, 0, stream>>>(p);
   else
     return cudaErrorInvalidValue;
   return cudaGetLastError();

@@ -112,11 +112,14 @@ __device__ __forceinline__ uint4 pack8(const float *x) {
 // the 8 matching high-half elements of a row), rows are D code bytes + one scale byte.  K: de-quantise, rotate with the
 // compensated fp32 scheme (a de-quantised element has <= 4 significant bits, so its products with c_hi / s_hi are exact
 // as for bf16 inputs), ONE rounding to bf16.  V: de-quantise, round to bf16 (exact outside the deepest subnormals).
-template <int D>
+// DT = 0: head_dim at run time (`Dr`, any multiple of 16 up to 256; lanes beyond TPS * LPT idle)
+template <int DT>
 __device__ __forceinline__ void stitch_fp8_rows(const StitchEntryDev &en, const StitchChunkDev &ch, int layer, int Hkv, int warp,
-                                                int col, int tl, bool rotate, bool il, const float4 *tab) {
-  constexpr int LPT = D / 16, TPS = 32 / LPT, STEPS = 4, HEADS = 2;
-  const int ntok = ch.ntok;
+                                                int col, int tl, bool rotate, bool il, const float4 *tab, int Dr) {
+  const int D = DT ? DT : Dr;
+  const int LPT = D / 16, TPS = 32 / LPT;
+  constexpr int STEPS = 4, HEADS = 2;
+  const int ntok = DT ? ch.ntok : (tl < TPS ? ch.ntok : 0);   // an idle lane sees an empty chunk
   // a code row is half a bf16 row: two kv heads per pass keep as many bytes in flight per lane as the bf16 path has
   for (int g0 = warp; g0 < Hkv; g0 += 4 * HEADS) {
     for (int t0 = 0; t0 < ntok; t0 += TPS * STEPS) {
@@ -191,12 +194,14 @@ __device__ __forceinline__ void stitch_fp8_rows(const StitchEntryDev &en, const 
   }
 }
 
-template <int D, bool FP8>
+template <int DT, bool FP8>
 __global__ void __launch_bounds__(128, FP8 ? 3 : 4) stitch_kernel(const StitchParams p) {
-  constexpr int LPT = D / 16;      // lanes per token: one 16-byte column of each half per lane
-  constexpr int TPS = 32 / LPT;    // tokens per warp step
+  // DT = 0: head_dim at run time (p.head_dim: any multiple of 16 up to 256, R27); the lanes beyond TPS * LPT idle
+  const int D = DT ? DT : p.head_dim;
+  const int LPT = D / 16;          // lanes per token: one 16-byte column of each half per lane
+  const int TPS = 32 / LPT;        // tokens per warp step
   constexpr int STEPS = 4;         // steps in flight per batch (4 x 64 B per lane)
-  constexpr int ROW_BYTES = D * 2;
+  const int ROW_BYTES = D * 2;
 
   const StitchChunkDev ch = p.chunks[blockIdx.x];
   const StitchEntryDev en = p.entries[ch.entry];
@@ -205,7 +210,7 @@ __global__ void __launch_bounds__(128, FP8 ? 3 : 4) stitch_kernel(const StitchPa
   const int warp = threadIdx.x >> 5;
   const int col = lane % LPT;
   const int tl = lane / LPT;
-  const int ntok = ch.ntok;
+  const int ntok = DT ? ch.ntok : (tl < TPS ? ch.ntok : 0);   // an idle lane sees an empty chunk
   const bool rotate = en.table_off >= 0;
   const bool il = p.interleaved != 0;
 
@@ -223,7 +228,7 @@ __global__ void __launch_bounds__(128, FP8 ? 3 : 4) stitch_kernel(const StitchPa
 
   const int Hkv = p.n_kv_heads;
   if (FP8 && en.src_fp8) {           // (the bf16 instantiation carries no fp8 code: its registers and SASS stay as they were)
-    stitch_fp8_rows<D>(en, ch, layer, Hkv, warp, col, tl, rotate, il, tab);
+    stitch_fp8_rows<DT>(en, ch, layer, Hkv, warp, col, tl, rotate, il, tab, D);
     return;
   }
   for (int g = warp; g < Hkv; g += 4) {
@@ -282,9 +287,10 @@ __global__ void __launch_bounds__(128, FP8 ? 3 : 4) stitch_kernel(const StitchPa
 
 // q / k rows of the patch tokens -> rotated to their absolute positions (fcg_patch_rope).  One CTA per (token, layer);
 // a thread owns the two 16-byte vectors [col*8, +8) and [D/2 + col*8, +8) of one head row, as in stitch_kernel.
-template <int D>
+template <int DT>
 __global__ void __launch_bounds__(128) rope_qk_kernel(const RopeQkParams p) {
-  constexpr int LPT = D / 16;
+  const int D = DT ? DT : p.head_dim;      // DT = 0: head_dim at run time
+  const int LPT = D / 16;
   const int tok = blockIdx.x, layer = blockIdx.y;
   const int rows = p.n_q_heads + p.n_kv_heads;
   const bool il = p.interleaved != 0;
@@ -334,6 +340,8 @@ cudaError_t launch_rope_qk(const RopeQkParams &p, int head_dim, cudaStream_t str
     rope_qk_kernel<64><<<grid, 128, 0, stream>>>(p);
   else if (head_dim == 256)
     rope_qk_kernel<256><<<grid, 128, 0, stream>>>(p);
+  else if (head_dim >= 16 && head_dim < 256 && head_dim % 16 == 0 && p.head_dim == head_dim)
+    rope_qk_kernel<0><<<grid, 128, 0, stream>>>(p);
   else
     return cudaErrorInvalidValue;
   return cudaGetLastError();
@@ -358,6 +366,11 @@ cudaError_t launch_stitch(const StitchParams &p, int head_dim, cudaStream_t stre
       stitch_kernel<256, true><<<grid, block, 0, stream>>>(p);
     else
       stitch_kernel<256, false><<<grid, block, 0, stream>>>(p);
+  } else if (head_dim >= 16 && head_dim < 256 && head_dim % 16 == 0 && p.head_dim == head_dim) {
+    if (p.any_fp8)
+      stitch_kernel<0, true><<<grid, block, 0, stream>>>(p);
+    else
+      stitch_kernel<0, false><<<grid, block, 0, stream>>>(p);
   } else {
     return cudaErrorInvalidValue;
   }

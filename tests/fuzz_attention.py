@@ -19,7 +19,7 @@ from paper_2606_13097_b200 import synth  # noqa: E402
 
 
 def one_case(rng):
-    D = int(rng.choice([64, 128, 256]))
+    D = int(rng.choice([64, 128, 256, 16, 32, 48, 80, 96, 112, 144, 160, 176, 192, 208, 224, 240]))
     Hkv = int(rng.choice([1, 2, 4]))
     G = int(rng.choice([1, 2, 4, 8]))
     Hq = Hkv * G

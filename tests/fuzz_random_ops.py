@@ -20,7 +20,7 @@ def main(campaign_seed: int, n: int) -> int:
     fails = 0
     for _ in range(n):
         seed = int(rng.integers(1000, 10 ** 6))
-        D = int(rng.choice([64, 128, 256]))
+        D = int(rng.choice([64, 128, 256, 16, 48, 80, 96, 112, 160, 192, 224]))
         Hq, Hkv = [(4, 2), (4, 4), (8, 2), (2, 1), (6, 2)][int(rng.integers(5))]
         P = int(rng.choice([8, 16, 32, 64]))
         rope_mode = int(rng.integers(3))

@@ -54,7 +54,7 @@ def _guarded_library(L, Hq, Hkv, D, P, rope_mode, seg_tokens, n_pages, max_task_
     return lib, g
 
 
-@pytest.mark.parametrize("D,rope_mode", [(128, 1), (64, 2), (256, 1)])
+@pytest.mark.parametrize("D,rope_mode", [(128, 1), (64, 2), (256, 1), (96, 1), (176, 2)])
 def test_no_kernel_writes_outside_its_buffers_and_nothing_unwritten_is_read(D, rope_mode):
     L, Hq, Hkv, P = 3, 8, 2, 16
     rng = np.random.default_rng(D)

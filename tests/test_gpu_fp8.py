@@ -32,7 +32,7 @@ def _compare_stored(lib, orc, sid):
     assert np.array_equal(vc, sg.v), "V codes"
 
 
-@pytest.mark.parametrize("D", [128, 64, 256])
+@pytest.mark.parametrize("D", [128, 64, 256, 96, 80, 192, 16])
 def test_quantised_codes_and_scales_are_bit_exact(D):
     L, Hq, Hkv, P = 2, 4, 2, 16
     lib, orc = _lib(L, Hq, Hkv, D, P, 1, 4000)
@@ -70,7 +70,7 @@ def test_quantised_codes_and_scales_are_bit_exact(D):
     lib.close()
 
 
-@pytest.mark.parametrize("D,rope_mode,P", [(128, 1, 16), (64, 1, 8), (128, 2, 32), (128, 0, 16), (256, 1, 16), (256, 2, 8)])
+@pytest.mark.parametrize("D,rope_mode,P", [(128, 1, 16), (64, 1, 8), (128, 2, 32), (128, 0, 16), (256, 1, 16), (256, 2, 8), (96, 1, 16), (192, 2, 8), (80, 1, 32)])
 def test_stitch_from_fp8_segments_matches_the_oracle(D, rope_mode, P):
     L, Hq, Hkv = 3, 4, 2
     lib, orc = _lib(L, Hq, Hkv, D, P, rope_mode, 6000, host_tier_tokens=600, base=5e5)

@@ -56,7 +56,7 @@ def _compare_task(orc, lib, task_id, what):
 # ------------------------------------------------------------------------------------------------
 # NEXT-4: interleaved pairs
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("D", [64, 128, 256])
+@pytest.mark.parametrize("D", [64, 128, 256, 96, 192, 48])
 def test_interleaved_rope_stitch(D):
     cfg = synth.GraftConfig("il", 2, 4, 2, D, 16, 1e4, 6, 40, 200, 3000, 1, 4, 4, 0)
     wl, orc, lib, seg_ids = _pair(cfg, seed=2, rope_mode=O.ROPE_INTERLEAVED)
@@ -262,7 +262,7 @@ def test_two_tier_residency_stitch_from_host_and_prefetch():
 # ------------------------------------------------------------------------------------------------
 # NEXT-4: fcg_patch_rope -- q / k given before position encoding
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("rope_mode,D", [(1, 128), (2, 128), (1, 64), (0, 128), (1, 256), (2, 256)])
+@pytest.mark.parametrize("rope_mode,D", [(1, 128), (2, 128), (1, 64), (0, 128), (1, 256), (2, 256), (1, 96), (2, 160), (1, 80)])
 def test_patch_rope_matches_oracle(rope_mode, D):
     cfg = synth.GraftConfig("prope", 2, 8, 2, D, 16, 5e5, 3, 100, 300, 30000, 1, 3, 3, 0, holes=((0, 45), (-1, 50)))
     wl, orc, lib, seg_ids = _pair(cfg, seed=4, rope_mode=rope_mode)

@@ -85,6 +85,16 @@ GEOMS = [
     (2, 8, 2, 256, 16, 1e4),
     (1, 4, 4, 256, 64, 5e5),
     (1, 6, 3, 256, 8, 1e6),
+    # other multiples of 16 (R27): run-time-D gather kernel, tcgen05 attention at the next instantiated width with zero padding
+    (2, 4, 2, 96, 16, 1e4),
+    (1, 8, 2, 80, 32, 5e5),
+    (1, 4, 4, 192, 16, 1e4),
+    (2, 6, 3, 160, 8, 1e4),
+    (1, 2, 2, 32, 16, 1e4),
+    (1, 4, 1, 112, 64, 1e4),
+    (1, 2, 1, 224, 16, 1e6),
+    (1, 4, 2, 16, 16, 1e4),
+    (1, 2, 2, 48, 8, 1e4),
 ]
 
 

@@ -103,7 +103,7 @@ def _classes(bits):
     return np.where(mag < 0x7F80, 0, np.where(mag > 0x7F80, 3, np.where(b == 0x7F80, 1, 2)))
 
 
-@pytest.mark.parametrize("D,rope_mode", [(128, 1), (64, 1), (128, 2), (128, 0), (256, 1)])
+@pytest.mark.parametrize("D,rope_mode", [(128, 1), (64, 1), (128, 2), (128, 0), (256, 1), (96, 1), (160, 2)])
 def test_special_values_through_stitch_and_scatter(D, rope_mode):
     L, Hq, Hkv, P = 2, 4, 2, 16
     rng = np.random.default_rng(D + rope_mode)
@@ -171,7 +171,7 @@ def test_special_values_through_stitch_and_scatter(D, rope_mode):
     lib.close()
 
 
-@pytest.mark.parametrize("D,tc_min_rows", [(128, 1), (128, 2 ** 31 - 1), (64, 1), (256, 1)])
+@pytest.mark.parametrize("D,tc_min_rows", [(128, 1), (128, 2 ** 31 - 1), (64, 1), (256, 1), (96, 1), (192, 1)])
 def test_attention_rows_that_see_no_special_value_are_unaffected(D, tc_min_rows):
     """Two tasks and two kv heads share the pool.  Special values (inf, NaN, near-max, subnormal, +-0) sit (a) in the
     OTHER task's cache, (b) in the OTHER kv head, (c) in this task at positions beyond the last patch position, (d) in
@@ -241,7 +241,9 @@ PEAK_ATOL, PEAK_RTOL = 4e-3, 1e-2       # bf16 output rounding is 2^-9 relative,
     (16, 4, 4, 128, 4096, 1, 0), (16, 4, 4, 128, 4096, 1, 4), (48, 8, 2, 128, 2000, 1, 3), (130, 2, 1, 128, 2600, 1, 2),
     (300, 2, 2, 128, 1500, 1, 0), (16, 4, 4, 128, 4096, 2 ** 31 - 1, 4), (32, 8, 4, 64, 3000, 1, 3), (5, 32, 4, 128, 1000, 1, 0),
     # head_dim 256: row streams x4, x2, a full Q tile, several row groups of one task, with and without KV splits
-    (7, 4, 4, 256, 2100, 1, 0), (16, 4, 1, 256, 4096, 1, 3), (130, 2, 1, 256, 2600, 1, 2), (300, 2, 2, 256, 1500, 1, 0)])
+    (7, 4, 4, 256, 2100, 1, 0), (16, 4, 1, 256, 4096, 1, 3), (130, 2, 1, 256, 2600, 1, 2), (300, 2, 2, 256, 1500, 1, 0),
+    # padded widths: 96 -> 128 (all three CTA classes), 48 -> 64, 176 -> 256
+    (16, 4, 4, 96, 2100, 1, 3), (100, 4, 4, 96, 1500, 1, 0), (300, 2, 2, 96, 1500, 1, 2), (40, 4, 2, 48, 2000, 1, 0), (130, 2, 1, 176, 1300, 1, 2)])
 def test_peaked_softmax_dominant_keys_at_tile_and_split_boundaries(n, Hq, Hkv, D, ctx, tc_min_rows, splits):
     """Each query row gets ONE dominant key (score ~ +25 above the rest): the last visible key (its own fresh row), the
     first key of a 64-token KV tile, the first / last key of a KV split, key 0, or a key inside the patch that the row

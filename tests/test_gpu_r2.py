@@ -63,7 +63,7 @@ def test_growth_script_by_hand_on_the_c_library():
     lib.close()
 
 
-@pytest.mark.parametrize("D,Hq,Hkv", [(128, 8, 2), (64, 4, 4), (256, 4, 2)])
+@pytest.mark.parametrize("D,Hq,Hkv", [(128, 8, 2), (64, 4, 4), (256, 4, 2), (96, 4, 2)])
 def test_decode_130_steps_past_the_stitched_capacity(D, Hq, Hkv):
     """Eq. 6's x_mid is decoded token by token without reserving room for it (R25): stitch with capacity = T exactly,
     then 130 single-token patches, every one an append; 130 tokens at P = 16 cross 8 page boundaries.  A second task

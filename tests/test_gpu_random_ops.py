@@ -44,7 +44,7 @@ def _bits(rng, shape):
 
 
 @pytest.mark.parametrize("seed,D,Hq,Hkv,P,rope_mode", [(11, 128, 4, 2, 16, 1), (12, 64, 4, 4, 8, 1), (13, 128, 8, 2, 32, 2),
-                                                     (14, 128, 2, 1, 16, 0), (15, 128, 6, 2, 64, 1), (16, 256, 4, 2, 16, 1)])
+                                                     (14, 128, 2, 1, 16, 0), (15, 128, 6, 2, 64, 1), (16, 256, 4, 2, 16, 1), (17, 96, 4, 2, 16, 1), (18, 160, 4, 4, 32, 2)])
 def test_random_operation_sequences(seed, D, Hq, Hkv, P, rope_mode):
     from paper_2606_13097_b200.binding import FcgLibrary, FcgError
     rng = np.random.default_rng(seed)
