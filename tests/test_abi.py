@@ -44,8 +44,12 @@ def test_arena_bytes_required_is_host_arithmetic():
     assert binding.fcg_arena_bytes_required(cfg, 1000) - base == 1000 * per_tok
     bad = binding.make_config(n_layers=1, n_q_heads=3, n_kv_heads=2, head_dim=128)
     assert binding.fcg_arena_bytes_required(bad, 0) == 0
-    bad = binding.make_config(n_layers=1, n_q_heads=2, n_kv_heads=2, head_dim=80)
-    assert binding.fcg_arena_bytes_required(bad, 0) == 0
+    for hd in (72, 8, 0, 272, 100):                       # R27: multiples of 16 in [16, 256] only
+        bad = binding.make_config(n_layers=1, n_q_heads=2, n_kv_heads=2, head_dim=hd)
+        assert binding.fcg_arena_bytes_required(bad, 0) == 0, hd
+    for hd in (16, 80, 96, 192, 256):
+        ok = binding.make_config(n_layers=1, n_q_heads=2, n_kv_heads=2, head_dim=hd)
+        assert binding.fcg_arena_bytes_required(ok, 0) > 0, hd
 
 
 def test_create_rejects_bad_config_and_needs_a_device():
