@@ -211,7 +211,8 @@ fcg_status_t fcg_patch_host(fcg_library_t *lib, int32_t task_id, int32_t layer_b
 
 /* Batched patching (independent tasks, one launch): task_ids host int32[n_tasks] (distinct, live);
  * n_per_task host int32[n_tasks]; positions host int32[sum n], the tasks' position lists back to back;
- * q/k/v/out device bf16 [n_layers][sum n][heads][head_dim]. */
+ * q/k/v/out device bf16 [n_layers][sum n][heads][head_dim].  n_layers * n_tasks <= 65535 per call (the attention grid
+ * runs (layer, task) along z; INVALID_ARG otherwise: patch fewer layers or tasks per call). */
 fcg_status_t fcg_patch_batch(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task,
                              int32_t n_tasks, int32_t layer_begin, int32_t n_layers, const void *q,
                              const void *k, const void *v, const int32_t *positions, void *out, void *stream);

@@ -1102,6 +1102,10 @@ struct PatchCheck {
 fcg_status_t validate_patch(fcg_library *lib, const PatchSpec &ps, PatchCheck &ck) {
   const fcg_config_t &c = lib->cfg;
   if (!ps.positions || !ps.task_ids || !ps.n_per_task || ps.n_tasks <= 0) return fail(FCG_ERR_INVALID_ARG, "NULL / empty argument");
+  // the attention grids run (layer, task) along z and kv heads along y: CUDA's limit for both is 65535
+  if ((int64_t)ps.n_layers * ps.n_tasks > 65535 || c.n_kv_heads > 65535)
+    return fail(FCG_ERR_INVALID_ARG, "%d layers x %d tasks in one call exceed the launch limit of 65535: patch fewer layers or tasks per call",
+                ps.n_layers, ps.n_tasks);
   ck.n_total = 0;
   ck.pages_needed = 0;
   ck.new_capacity.assign(ps.n_tasks, 0);
@@ -1650,6 +1654,8 @@ fcg_status_t fcg_patch_planned(fcg_library_t *lib, fcg_patch_plan_t *plan, int32
     if (!tr.live || tr.gen != plan->task_gens[t])
       return fail(FCG_ERR_BAD_TASK, "task %d was released or re-stitched after the plan was made", plan->task_ids[t]);
   }
+  if ((int64_t)n_layers * (int64_t)plan->task_ids.size() > 65535)
+    return fail(FCG_ERR_INVALID_ARG, "%d layers x %zu tasks in one call exceed the launch limit of 65535", n_layers, plan->task_ids.size());
   PatchIO io{layer_begin, n_layers, q, k, v, out, static_cast<cudaStream_t>(stream_)};
   fcg_status_t st = validate_io(lib, io);
   if (st != FCG_OK) return st;

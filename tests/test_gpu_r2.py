@@ -436,3 +436,18 @@ def test_mixed_class_batch_in_one_launch_matches_the_per_class_launches_and_the_
             T.assert_attn_close(outs[-1], ref, f"mixed={mixed} splits={splits}")
         assert torch.equal(outs[0], outs[1])
     lib.close()
+
+
+def test_batches_beyond_the_launch_limit_are_rejected_before_anything_runs():
+    """n_layers x n_tasks > 65535 would not fit the attention grid's z extent: INVALID_ARG, nothing launched (fcg.h)."""
+    B = _B()
+    lib = B.FcgLibrary(n_layers=2, n_q_heads=2, n_kv_heads=2, head_dim=64, page_size=16, rope_base=1e4, max_segments=1, max_tasks=4,
+                       max_task_tokens=64, n_pages=8, segment_tokens=64)
+    n_tasks = 40000
+    q = torch.zeros((2, n_tasks, 2, 64), dtype=torch.bfloat16, device="cuda")
+    before = lib.stats()
+    with pytest.raises(B.FcgError) as e:
+        lib.patch_batch(np.arange(n_tasks, dtype=np.int32), np.ones(n_tasks, np.int32), 0, q, q, q, np.zeros(n_tasks, np.int32))
+    assert e.value.status == B.FCG_ERR_INVALID_ARG
+    assert lib.stats() == before
+    lib.close()
