@@ -139,6 +139,7 @@ namespace {
 bool geometry_ok(const fcg_config_t *c) {
   if (!c) return false;
   if (c->n_layers <= 0 || c->n_kv_heads <= 0 || c->n_q_heads <= 0 || c->n_q_heads % c->n_kv_heads) return false;
+  if (c->n_layers > 65535 || c->n_kv_heads > 65535) return false;      // layers / kv heads run along grid y
   if (c->head_dim < 16 || c->head_dim > 256 || c->head_dim % 16) return false;      // R27
   if (c->page_size != 8 && c->page_size != 16 && c->page_size != 32 && c->page_size != 64) return false;
   if (c->rope_mode != FCG_ROPE_NONE && c->rope_mode != FCG_ROPE_HALF_SPLIT && c->rope_mode != FCG_ROPE_INTERLEAVED) return false;
