@@ -1055,6 +1055,8 @@ int choose_splits(int64_t base_ctas, int tiles, int rows, int head_dim, int ctas
     const int tiles_per = (tiles + s - 1) / s;
     const int s_eff = (tiles + tiles_per - 1) / tiles_per;
     if (s_eff != s) continue;
+    // every (row group, split) CTA counts, also those of a row group that stops early (a hole in the middle of the cache):
+    // counting only the non-empty ones picked 12 splits instead of 9 for one layer of C3 and took 51 us instead of 37
     const double ctas = (double)base_ctas * s;
     const double waves = ceil(ctas / slots);
     // time ~ waves * (one CTA's K/V stream + its fp32 partial rows), plus what the combine kernel reads and writes
@@ -1238,7 +1240,7 @@ fcg_status_t build_patch_blob(fcg_library *lib, const PatchSpec &ps, const Patch
     const int rows_per_cta = rows_per_cta_of(n * G);
     const int rg = (n * G + rows_per_cta - 1) / rows_per_cta;
     const int64_t base = (int64_t)rg * c.n_kv_heads * ps.n_layers * ps.n_tasks;
-    int ns = lib->force_splits > 0 ? std::min(lib->force_splits, tiles)
+    int ns = lib->force_splits > 0 ? std::min(std::min(lib->force_splits, tiles), 64)      // the combine kernel holds a split per lane, twice
                                    : choose_splits(base, tiles, std::min(n * G, rows_per_cta), c.head_dim, ctas_per_sm, lib->n_sms);
     const int tiles_per = (tiles + ns - 1) / ns;
     ns = (tiles + tiles_per - 1) / tiles_per;      // no empty trailing split
