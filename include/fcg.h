@@ -366,6 +366,47 @@ fcg_status_t fcg_scorer_score(fcg_scorer_t *s, int32_t id, double alpha, double 
 fcg_status_t fcg_scorer_rank(fcg_scorer_t *s, const int32_t *ids, int32_t n, double alpha, double beta, double gamma,
                              int32_t *ids_out, double *scores_out);
 
+/* The key re-rotation of cache-stitching (Eq. 4; RoPE group law, R1) for callers that are not
+ * allowed to allocate device memory.
+ *
+ * Who that is: a plug-in inside a serving engine that claimed all of HBM for its own block pool at start-up (a
+ * cudaMalloc there fails, or takes memory the engine believes it owns); code that runs while another thread of the
+ * process records a CUDA graph in global capture mode (the runtime refuses cudaMalloc for everybody until the capture
+ * ends); and latency-critical loops that cannot afford the device-wide synchronisation an allocation or a free may
+ * bring.  Such callers also cannot build an fcg_library_t just for one segment, because a library needs an arena with
+ * a workspace.  This call needs neither: it allocates nothing, on the host or on the device, and uses no handle.
+ *
+ * What it does: reads one dense bf16 segment  k_src, v_src  [n_layers][n_kv_heads][n_tokens][head_dim]  and writes
+ * k_dst, v_dst of the same shape: every key rotated by the angle  delta * theta_j  (theta_j = inv_freq[j] when
+ * inv_freq is given -- head_dim / 2 host doubles read during the call -- else rope_base^(-2j / head_dim)), every
+ * value copied bit for bit.  delta == 0 or FCG_ROPE_NONE copies the keys too.  It is the same kernel with the same
+ * arithmetic as fcg_stitch, so the bits equal those of stitching the segment at distance delta from where it was
+ * encoded.  All four buffers are device memory of the CURRENT device (there is no library whose device could be
+ * made current), 16-byte aligned, owned by the caller; no destination may overlap a source or the other
+ * destination (OVERLAP).  head_dim: a multiple of 16 in [16, 256]; n_layers <= 65535; n_tokens == 0 is a no-op.
+ *
+ * Where the scratch lives: the kernel reads a small plan (entry descriptor, chunk list, the cos / sin table of
+ * delta).  For this call the plan sits in a fixed 67 840-byte array inside the library image, present on every GPU
+ * that loads libfcg.so for as long as the process lives.  Its size is what bounds a call:
+ * n_tokens <= FCG_STATIC_SHIFT_MAX_TOKENS (also returned by fcg_segment_shift_static_max_tokens); a longer segment
+ * is refused with FCG_ERR_RANGE and a message that names the limit -- split it into several calls, or use a library.
+ *
+ * Sharing: there is ONE such array per GPU, and each call first overwrites the part of it that it is going to read
+ * (nothing needs to be zero, nothing of an earlier call is relied upon).  Two calls are therefore only safe when
+ * the GPU runs them one after the other: same stream, or streams ordered by an event.  Calls that may overlap on
+ * the device race on the plan and produce garbage in both destinations; the library does not detect that.
+ *
+ * First call on a device: it looks up the device address of the array (one runtime query, cached per device
+ * ordinal, thread-safe).  Make that first call during start-up, outside any stream capture.
+ *
+ * Asynchronous on `stream`: two kernel launches, no copy.  Errors: INVALID_ARG (shape, alignment, NULL, rope
+ * parameters), RANGE (too many tokens), OVERLAP, CUDA.  Every check happens before anything is enqueued. */
+#define FCG_STATIC_SHIFT_MAX_TOKENS 65536
+fcg_status_t fcg_segment_shift_static(const void *k_src, const void *v_src, void *k_dst, void *v_dst, int32_t n_layers,
+                                      int32_t n_kv_heads, int32_t n_tokens, int32_t head_dim, int32_t rope_mode,
+                                      double rope_base, const double *inv_freq, int32_t delta, void *stream);
+int32_t fcg_segment_shift_static_max_tokens(void);
+
 /* Message for the last non-OK status returned on this thread (never NULL). */
 const char *fcg_last_error(void);
 /* "x.y.z sm_100a" */

@@ -124,6 +124,8 @@ SYMBOLS = {
     "fcg_scorer_forget": (_I, [_P, _I]),
     "fcg_scorer_score": (_I, [_P, _I, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double)]),
     "fcg_scorer_rank": (_I, [_P, _PI, _I, C.c_double, C.c_double, C.c_double, _PI, C.POINTER(C.c_double)]),
+    "fcg_segment_shift_static": (_I, [_P, _P, _P, _P, _I, _I, _I, _I, _I, C.c_double, C.POINTER(C.c_double), _I, _P]),
+    "fcg_segment_shift_static_max_tokens": (_I, []),
     "fcg_last_error": (C.c_char_p, []),
     "fcg_version": (C.c_char_p, []),
 }
@@ -386,6 +388,27 @@ def fcg_segment_extract(handle, task_id, begin, n_tokens, new_orig_start, stream
 def fcg_task_read(handle, task_id, layer, begin, n, k_out, v_out, stream=None) -> None:
     _check(load().fcg_task_read(handle, int(task_id), int(layer), int(begin), int(n), _ptr(k_out), _ptr(v_out),
                                 _stream(stream)))
+
+
+def fcg_segment_shift_static_max_tokens() -> int:
+    return int(load().fcg_segment_shift_static_max_tokens())
+
+
+def fcg_segment_shift_static(k_src, v_src, k_dst, v_dst, n_layers, n_kv_heads, n_tokens, head_dim, delta,
+                             rope_mode=FCG_ROPE_HALF_SPLIT, rope_base=1e4, inv_freq=None, stream=None) -> None:
+    """Re-rotate one dense segment [n_layers][n_kv_heads][n_tokens][head_dim] by `delta` positions (values copied)
+    without allocating anything: for callers inside an engine that owns all device memory, or running while a graph
+    capture forbids cudaMalloc.  The kernel's plan lives in a fixed array inside libfcg.so, one per GPU, so at most
+    fcg_segment_shift_static_max_tokens() tokens per call and never two calls that can overlap on the device (keep them
+    on one stream).  Buffers are on the CURRENT device.  Make the first call per device outside stream capture."""
+    freq = None
+    if inv_freq is not None:
+        freq = np.ascontiguousarray(np.asarray(inv_freq, dtype=np.float64))
+        assert freq.size == head_dim // 2
+    _check(load().fcg_segment_shift_static(_ptr(k_src), _ptr(v_src), _ptr(k_dst), _ptr(v_dst), n_layers, n_kv_heads,
+                                           n_tokens, head_dim, rope_mode, float(rope_base),
+                                           None if freq is None else freq.ctypes.data_as(C.POINTER(C.c_double)),
+                                           int(delta), _stream(stream)))
 
 
 def fcg_pool_info(handle) -> dict:

@@ -75,6 +75,11 @@ struct FreeRange {
 
 }  // namespace
 
+namespace fcg {
+// for the other translation units of the library (fcg_static.cu): the message fcg_last_error() returns on this thread
+void set_last_error(const char *msg) { g_err = msg ? msg : ""; }
+}  // namespace fcg
+
 struct fcg_library {
   fcg_config_t cfg;
   std::vector<double> inv_freq;

@@ -7,6 +7,9 @@
 
 namespace fcg {
 
+// sets the thread-local message behind fcg_last_error() (defined in fcg_api.cu)
+void set_last_error(const char *msg);
+
 // ---------------------------------------------------------------------------------------------
 // S3: fused gather + RoPE-shift.  One kernel moves token rows between any two of {library segment,
 // paged cache}: stitch (segment -> cache), suffix re-graft (cache -> cache, fcg_task_shift) and segment
