@@ -834,7 +834,9 @@ def run_cuda(args):
         "metric": METRIC, "value": rec["value_GBps"], "unit": UNIT, "n_gpus": D.world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": rec["ms_per_step"], "higher_is_better": True, "scaling": rec["scaling"], "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": rec["workload"], "l2": rec["l2"], "stitch_ms": rec["stitch_ms"], "stitch_ms_min": rec["stitch_ms_min"],
+        "config": {"workload": short_workload(head_name, cfg, len(tasks), int(sum(n for t in tasks for (_, _, n, _) in t.entries)),
+                                              int(sum(len(t.positions) for t in tasks)), args.seed),
+                   "workload_long": rec["workload"], "l2": rec["l2"], "stitch_ms": rec["stitch_ms"], "stitch_ms_min": rec["stitch_ms_min"],
                    "stitch_ms_median": rec["stitch_ms_median"], "patch_ms": rec["patch_ms"], "patch_ms_min": rec["patch_ms_min"],
                    "patch_ms_median": rec["patch_ms_median"], "stitch_bytes": rec["stitch_bytes"], "attn_bytes": rec["attn_bytes"],
                    "attn_flops": rec["attn_flops"], "attn_path": rec["attn_path"], "attn_splits": rec["attn_splits"],
@@ -922,6 +924,99 @@ def run_cuda(args):
         sampler.stop()
     D.close()
     return res if D.rank == 0 else None
+
+
+# --------------------------------------------------------------------------------------------------
+# the line the driver reads: compact (< 4 KB), strict JSON, last on stdout.  Everything else goes on a DETAIL line.
+# --------------------------------------------------------------------------------------------------
+HEADLINE_MAX_BYTES = 4096
+
+
+def _sig(x, digits=5):
+    """numbers to `digits` significant digits (non-finite -> None: strict JSON), containers recursively"""
+    if isinstance(x, bool) or x is None or isinstance(x, (int, str)):
+        return x
+    if isinstance(x, (float, np.floating)):
+        x = float(x)
+        if not math.isfinite(x):
+            return None
+        return float(f"{x:.{digits}g}")
+    if isinstance(x, np.integer):
+        return int(x)
+    if isinstance(x, dict):
+        return {k: _sig(v, digits) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_sig(v, digits) for v in x]
+    return str(x)
+
+
+def _pick(d, keys, str_max=80):
+    if not isinstance(d, dict):
+        return None
+    out = {}
+    for k in keys:
+        if k in d:
+            v = d[k]
+            out[k] = v[:str_max] if isinstance(v, str) else v
+    return out
+
+
+def short_workload(name, cfg, n_tasks, stitched, patched, seed):
+    """<= 120 characters (the driver cuts `config.workload` there); the long description is on the DETAIL line"""
+    return (f"{name}: L={cfg.n_layers} Hq={cfg.n_q_heads} Hkv={cfg.n_kv_heads} D={cfg.head_dim} page={cfg.page_size}; "
+            f"{n_tasks} task(s), {stitched} stitched + {patched} patch tokens; seed {seed}")[:120]
+
+
+def headline(res: dict) -> dict:
+    """The compact record: the contract's keys, the dominant kernel's roofline (+ patch attention), cpu_baseline, clocks,
+    e2e, C5's prefill comparison and six numbers per configuration.  `res` is the full record of run_cuda."""
+    roof_keys = ("kernel", "bound", "achieved", "peak", "unit", "frac", "traffic", "frac_of_8TBps")
+    cfg_in = res.get("config") or {}
+    config = _pick(cfg_in, ("workload", "l2", "stitch_ms", "stitch_ms_min", "stitch_ms_median", "patch_ms", "patch_ms_min",
+                            "patch_ms_median", "stitch_bytes", "attn_bytes", "attn_flops", "attn_path", "attn_splits", "parallelism"), 120)
+    if "l2" in config:
+        config["l2"] = config["l2"][:60]
+    out = {k: res.get(k) for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                                   "vs_baseline", "dtype", "data", "gpu_launches")}
+    out["config"] = config
+    roof = res.get("roofline")
+    if isinstance(roof, dict):
+        r = _pick(roof, roof_keys, 60)
+        r["peak_source"] = "MEASURED_PEAKS.json" if "MEASURED_PEAKS" in str(roof.get("peak_source")) else "fallback"
+        pa = roof.get("patch_attention")
+        if isinstance(pa, dict):
+            r["patch_attention"] = _pick(pa, roof_keys + ("rows_per_kv_head", "hbm_GBps"), 60)
+        out["roofline"] = r
+    else:
+        out["roofline"] = None
+    cb = res.get("cpu_baseline")
+    out["cpu_baseline"] = _pick(cb, ("value", "unit", "cores", "kind", "seconds", "sample"), 200) if cb else None
+    out["clocks"] = _pick(res.get("clocks"), ("sm_mhz", "sm_min_mhz", "sm_max_mhz", "power_w_max", "reasons", "samples"))
+    out["e2e"] = _pick(res.get("e2e"), ("value", "unit", "ms_per_step", "h2d_bytes_per_step", "d2h_bytes_per_step"))
+    pc = res.get("prefill_compare")
+    if isinstance(pc, dict):
+        out["prefill_compare"] = _pick(pc, ("tokens", "graft_ms", "own_kernel_ms_all_layers", "torch_sdpa_ms_all_layers", "error"), 80)
+        if pc.get("graft_ms") and pc.get("own_kernel_ms_all_layers"):
+            out["prefill_compare"]["ratio"] = pc["own_kernel_ms_all_layers"] / pc["graft_ms"]
+    summ = {}
+    for name, c in (res.get("configs") or {}).items():
+        if not isinstance(c, dict) or "error" in c:
+            summ[name] = {"error": str((c or {}).get("error"))[:60]}
+            continue
+        roof_c = c.get("roofline") or {}
+        pa_c = roof_c.get("patch_attention") or {}
+        summ[name] = {"step_ms": c.get("ms_per_step"), "stitch_frac": roof_c.get("frac"), "patch_frac": pa_c.get("frac"),
+                      "patch_bound": pa_c.get("bound"), "e2e_ms": (c.get("e2e") or {}).get("ms_per_step"),
+                      "sm_mhz": (c.get("clocks") or {}).get("sm_mhz")}
+    out["configs_summary"] = summ
+    out["detail"] = "the full per-configuration record is the earlier stdout line that starts with DETAIL"
+    out = _sig(out)
+    # never hand the driver an oversized line: drop the optional parts, least important first
+    for victim in ("detail", "configs_summary", "prefill_compare"):
+        if len(json.dumps(out)) < HEADLINE_MAX_BYTES:
+            break
+        out.pop(victim, None)
+    return out
 
 
 # --------------------------------------------------------------------------------------------------
@@ -1063,7 +1158,11 @@ def main():
             sys.exit(spawn_ranks(args))
         res = run_cuda(args)
     if res is not None:
-        print(json.dumps(res))
+        if args.impl == "cuda":
+            # the fat record first (own line, prefixed), the compact headline LAST: the driver parses the last stdout line
+            print("DETAIL " + json.dumps(_sig(res, 7)), flush=True)
+            res = headline(res)
+        print(json.dumps(res, allow_nan=False), flush=True)
 
 
 if __name__ == "__main__":
