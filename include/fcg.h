@@ -233,10 +233,14 @@ fcg_status_t fcg_patch_batch_host(fcg_library_t *lib, const int32_t *task_ids, c
  * may be captured into a CUDA graph (it makes no copies and touches no host state besides launch statistics; while
  * the stream is capturing, the stream-ordering rule above is skipped and the caller orders the graph against other
  * work on the library).  Planned calls for DISJOINT layer ranges touch disjoint memory (their split-KV partials live
- * in per-layer slots of the workspace; OUT_OF_ARENA at plan creation if those do not fit), so inside a capture they
- * may be forked over several streams and run concurrently.  BAD_TASK if a task of the plan was released or
- * re-stitched since.  Destroy returns the
- * device range; the caller guarantees no enqueued work still reads it. */
+ * in per-layer slots in the lower half of the workspace's scratch area -- the upper half is where the host variants
+ * stage; OUT_OF_ARENA at plan creation if the slots do not fit there), so inside a capture they
+ * may be forked over several streams and run concurrently.  BAD_TASK if a task of the plan was released,
+ * re-stitched or moved by fcg_task_shift since (a shift un-fills positions and re-assigns pages: make a new plan).
+ * Destroy returns the device range to the segment arena with no stream ordering: the caller guarantees no enqueued work
+ * still reads it, and a CUDA graph captured from the plan must be destroyed (or never replayed again) BEFORE the plan
+ * is -- a replay after that reads whatever segment was registered into the range next.  Destroying a plan twice is
+ * INVALID_ARG.  fcg_library_destroy frees the plans the caller did not destroy. */
 typedef struct fcg_patch_plan fcg_patch_plan_t;
 fcg_status_t fcg_patch_plan_create(fcg_library_t *lib, const int32_t *task_ids, const int32_t *n_per_task, int32_t n_tasks,
                                    const int32_t *positions, int32_t layers_per_call, void *stream, fcg_patch_plan_t **out);

@@ -80,12 +80,16 @@ namespace fcg {
 void set_last_error(const char *msg) { g_err = msg ? msg : ""; }
 }  // namespace fcg
 
+struct fcg_patch_plan;
+extern "C++" __attribute__((visibility("hidden"))) void free_plans(struct fcg_library *lib);
+
 struct fcg_library {
   fcg_config_t cfg;
   std::vector<double> inv_freq;
   unsigned char *arena = nullptr;
   uint64_t k_pool_off = 0, v_pool_off = 0, pool_bytes = 0, table_off = 0, ws_off = 0, seg_off = 0, seg_bytes = 0;
   uint64_t scratch_off = 0, scratch_bytes = 0;   // workspace after the blob slots
+  uint64_t scratch_total = 0;                    // scratch_bytes as created (the host variants shrink scratch_bytes for the duration of a call)
   int32_t pages_per_task = 0;
   std::vector<int32_t> page_stack;               // LIFO: back() is handed out next
   std::vector<SegmentRec> segments;
@@ -117,6 +121,7 @@ struct fcg_library {
   cudaEvent_t staging_ev = nullptr;              // last use of the host-call staging area
   bool have_staging_ev = false;
   int n_plans_live = 0;
+  std::vector<struct fcg_patch_plan *> plans;    // live patch plans (freed by fcg_library_destroy if the caller did not)
   int next_slot = 0;
   fcg_stats_t stats;
   int n_segments_live = 0, n_tasks_live = 0;
@@ -533,6 +538,7 @@ fcg_status_t fcg_library_create(const fcg_config_t *cfg, fcg_library_t **out) {
   lib->pages_per_task = l.pages_per_task;
   lib->scratch_off = l.ws_off + (uint64_t)BLOB_SLOTS * BLOB_BYTES;
   lib->scratch_bytes = l.ws_bytes - (uint64_t)BLOB_SLOTS * BLOB_BYTES;
+  lib->scratch_total = lib->scratch_bytes;
   lib->page_stack.resize(cfg->n_pages);
   for (uint32_t i = 0; i < cfg->n_pages; ++i) lib->page_stack[i] = (int32_t)(cfg->n_pages - 1 - i);  // back() == 0
   lib->segments.resize(cfg->max_segments);
@@ -601,6 +607,7 @@ fcg_status_t fcg_library_destroy(fcg_library_t *lib) {
     if (lib->slots[i].host) cudaFreeHost(lib->slots[i].host);
     if (lib->slots[i].ev) cudaEventDestroy(lib->slots[i].ev);
   }
+  free_plans(lib);
   if (lib->copy_stream) cudaStreamDestroy(lib->copy_stream);
   if (lib->d2h_stream) cudaStreamDestroy(lib->d2h_stream);
   if (lib->last_ev) cudaEventDestroy(lib->last_ev);
@@ -1450,6 +1457,14 @@ fcg_status_t launch_patch(fcg_library *lib, const PatchLayout &lay, const unsign
   if (lay.max_splits > 1) {
     FCG_CUDA(fcg::launch_attn_combine(ap, c.head_dim, io.stream));
     lib->stats.attn_combine_launches++;
+    // The host variants stage q / k / v in the last <= scratch_total / 2 bytes of the scratch area from the copy stream,
+    // which is ordered after staging_ev only (not after `stream`).  Partials that reach into the upper half may lie where
+    // the next host call stages: they count as a use of the staging area until the combine kernel has read them.
+    // (Planned calls keep their per-layer slots inside the lower half: fcg_patch_plan_create.)
+    if (!layer_slots && part_ml_off + part_ml_bytes > lib->scratch_total / 2) {
+      FCG_CUDA(cudaEventRecord(lib->staging_ev, io.stream));
+      lib->have_staging_ev = true;
+    }
   }
   return FCG_OK;
 }
@@ -1614,10 +1629,12 @@ fcg_status_t fcg_patch_plan_create(fcg_library_t *lib, const int32_t *task_ids, 
   {
     uint64_t o_all, ml_all;
     partial_bytes(lib, pl->lay, lib->cfg.n_layers, o_all, ml_all);
-    if (o_all + ml_all > lib->scratch_bytes) {
+    // the slots stay inside the lower half of the scratch area: the upper half is where the host variants stage from their
+    // copy stream, and a planned call (possibly a graph replay) cannot record the event that would order them
+    if (o_all + ml_all > lib->scratch_total / 2) {
       const int ns = pl->lay.max_splits;
       delete pl;
-      return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for the per-layer partial slots of a %d-way split plan (%llu bytes)", ns,
+      return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for the per-layer partial slots of a %d-way split plan (%llu bytes; a plan may use half of the scratch area)", ns,
                   (unsigned long long)(o_all + ml_all));
     }
   }
@@ -1650,6 +1667,7 @@ fcg_status_t fcg_patch_plan_create(fcg_library_t *lib, const int32_t *task_ids, 
     pl->task_gens.push_back(lib->tasks[task_ids[t]].gen);
   }
   lib->n_plans_live++;
+  lib->plans.push_back(pl);
   *out = pl;
   return FCG_OK;
 }
@@ -1678,10 +1696,20 @@ fcg_status_t fcg_patch_planned(fcg_library_t *lib, fcg_patch_plan_t *plan, int32
 
 fcg_status_t fcg_patch_plan_destroy(fcg_library_t *lib, fcg_patch_plan_t *plan) {
   if (!lib || !plan || plan->lib != lib) return fail(FCG_ERR_INVALID_ARG, "NULL plan / plan of another library");
+  auto it = std::find(lib->plans.begin(), lib->plans.end(), plan);
+  if (it == lib->plans.end()) return fail(FCG_ERR_INVALID_ARG, "unknown (already destroyed?) plan");
+  lib->plans.erase(it);
   range_give(lib->seg_free, plan->dev_off, plan->dev_bytes);
   lib->n_plans_live--;
   delete plan;
   return FCG_OK;
+}
+
+// fcg_library_destroy: plans the caller never destroyed go with the library
+extern "C++" void free_plans(fcg_library *lib) {
+  for (fcg_patch_plan *pl : lib->plans) delete pl;
+  lib->plans.clear();
+  lib->n_plans_live = 0;
 }
 
 // NEXT-4 (R13 variant): q and k arrive before position encoding; rotate them to positions[i], then patch
@@ -2019,6 +2047,9 @@ fcg_status_t fcg_task_shift(fcg_library_t *lib, int32_t task_id, int32_t src_beg
   t.filled_prefix = 0;
   while (t.filled_prefix < t.capacity && t.filled[t.filled_prefix]) t.filled_prefix++;
   t.n_tokens = std::max(t.n_tokens, dst_end);
+  // positions were un-filled and pages re-assigned: a patch plan made before the shift no longer describes this task
+  // (fcg_patch_planned does not re-validate the fill state, it compares generations)
+  t.gen = ++lib->task_gen;
   return FCG_OK;
 }
 
