@@ -120,6 +120,7 @@ struct fcg_library {
   cudaEvent_t prefetch_ev = nullptr;             // fcg_stitch_prefetch: the host->device copies of one call have landed
   cudaEvent_t staging_ev = nullptr;              // last use of the host-call staging area
   bool have_staging_ev = false;
+  std::vector<unsigned char> dry_blob;           // host scratch of dry_check_patch
   int n_plans_live = 0;
   std::vector<struct fcg_patch_plan *> plans;    // live patch plans (freed by fcg_library_destroy if the caller did not)
   int next_slot = 0;
@@ -973,6 +974,12 @@ fcg_status_t stitch_impl(fcg_library *lib, const fcg_plan_t *plans, int32_t n_pl
     }
   }
 
+  // ---- the last host-side checks, BEFORE anything is enqueued (fcg.h conventions; enqueue_gather repeats them) -----
+  if (gb.blob_bytes() > BLOB_BYTES || gb2.blob_bytes() > BLOB_BYTES)
+    return fail(FCG_ERR_OUT_OF_ARENA, "plan blob of %llu bytes exceeds %llu (fewer entries / plans per call)",
+                (unsigned long long)std::max(gb.blob_bytes(), gb2.blob_bytes()), (unsigned long long)BLOB_BYTES);
+  if ((uint64_t)c.n_pages * c.n_kv_heads * c.page_size > 0x7fffffffull) return fail(FCG_ERR_INVALID_ARG, "pool too large for 32-bit row offsets");
+
   // ---- enqueue: copies, blob, kernel, page tables -----------------------------------------------
   FCG_DEVICE(lib);
   FCG_ORDER(lib, stream);
@@ -1517,6 +1524,21 @@ fcg_status_t prime_patch_blob(fcg_library *lib, const PatchSpec &ps, const Patch
   return FCG_OK;
 }
 
+// Host only: would a patch of ps.n_layers layers fit the plan blob and `scratch_limit` bytes of split-KV partials?  The host
+// and rope variants ask BEFORE they enqueue their copies / rotation, so that a call that fails has enqueued nothing.
+fcg_status_t dry_check_patch(fcg_library *lib, const PatchSpec &ps, const PatchCheck &ck, uint64_t scratch_limit) {
+  if (lib->dry_blob.size() < BLOB_BYTES) lib->dry_blob.resize(BLOB_BYTES);
+  PatchLayout lay;
+  fcg_status_t st = build_patch_blob(lib, ps, ck, lib->dry_blob.data(), BLOB_BYTES, lay);
+  if (st != FCG_OK) return st;
+  uint64_t po, pm;
+  partial_bytes(lib, lay, ps.n_layers, po, pm);
+  if (po + pm > scratch_limit)
+    return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for %d-way split partials (%llu bytes) beside the staging area", lay.max_splits,
+                (unsigned long long)(po + pm));
+  return FCG_OK;
+}
+
 // One patch call on device tensors: validate -> blob (uploaded, or the previous call's copy reused) -> growth -> kernels
 // -> commit.  `prechecked`: the caller has validated (host / rope variants validate before their own enqueues).
 fcg_status_t patch_common(fcg_library *lib, const PatchSpec &ps, const PatchIO &io, const PatchCheck *prechecked = nullptr) {
@@ -1736,6 +1758,8 @@ fcg_status_t fcg_patch_rope(fcg_library_t *lib, int32_t task_id, int32_t layer_b
   if (need > lib->scratch_bytes / 2) return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small for %llu bytes of rotated q / k", (unsigned long long)need);
   // rotated copies at the END of the scratch area (where fcg_patch_host stages too); split partials grow from its start
   unsigned char *dq = lib->arena + lib->scratch_off + lib->scratch_bytes - need, *dk = dq + align_up(q_bytes);
+  st = dry_check_patch(lib, ps, ck, lib->scratch_bytes - need);
+  if (st != FCG_OK) return st;
 
   FCG_DEVICE(lib);
   FCG_ORDER(lib, stream);
@@ -1831,6 +1855,15 @@ fcg_status_t patch_host_common(fcg_library *lib, const int32_t *task_ids, const 
   if (need > lib->scratch_bytes / 2) return fail(FCG_ERR_OUT_OF_ARENA, "workspace too small to stage %llu bytes", (unsigned long long)need);
   unsigned char *base = lib->arena + lib->scratch_off + lib->scratch_bytes - need;
   unsigned char *dq = base, *dk = dq + align_up(q_bytes), *dv = dk + align_up(kv_bytes), *dout = dv + align_up(kv_bytes);
+  {
+    // the largest layer group decides (the split choice and the partials grow with the layers of one call)
+    const int groups_ = (q_bytes >= (8ull << 20) && n_layers >= fcg_library::HOST_GROUPS) ? fcg_library::HOST_GROUPS : 1;
+    int max_nl = 0;
+    for (int g = 0; g < groups_; ++g) max_nl = std::max(max_nl, (int)((int64_t)n_layers * (g + 1) / groups_) - (int)((int64_t)n_layers * g / groups_));
+    PatchSpec ps_max{task_ids, n_per_task, n_tasks, positions, max_nl};
+    st = dry_check_patch(lib, ps_max, ck, lib->scratch_bytes - need);
+    if (st != FCG_OK) return st;
+  }
   FCG_DEVICE(lib);
   FCG_ORDER(lib, stream);
   // Copies in on the library's copy stream: after the last user of the staging area (staging_ev: host and rope calls),

@@ -87,3 +87,55 @@ def test_plans_are_invalidated_by_task_shift_and_freed_with_the_library():
     # the second plan is still live when the library goes away: it is freed with it (no crash; the arena is the caller's)
     torch.cuda.synchronize()
     lib.close()
+
+
+def test_failing_calls_enqueue_nothing():
+    """fcg.h: every host-side check of a call happens before any copy or launch.  (a) a stitch whose plan blob would exceed
+    1 MiB (12 000 one-token entries) is refused with the library unchanged and usable; (b) a host patch whose split
+    partials do not fit beside its staging area is refused before its host->device copies: nothing was counted as launched,
+    the output buffer is untouched and the same call succeeds with fewer splits."""
+    from paper_2606_13097_b200 import binding as B
+    # (a)
+    lib = B.FcgLibrary(n_layers=1, n_q_heads=1, n_kv_heads=1, head_dim=16, max_segments=2, max_tasks=2, max_task_tokens=12032,
+                       n_pages=800, segment_tokens=64)
+    k = torch.randn(1, 1, 16, 16).to(torch.bfloat16).cuda()
+    seg = lib.segment_register(k, k.clone(), 0)
+    big = {"task_id": 0, "entries": [(seg, i % 16, 1, i) for i in range(12000)], "holes": [], "capacity_tokens": 12000}
+    before = (lib.pool_info(), lib.stats())
+    with pytest.raises(B.FcgError) as e:
+        lib.stitch([big])
+    assert e.value.status == B.FCG_ERR_OUT_OF_ARENA and "plan blob" in str(e.value)
+    assert (lib.pool_info(), lib.stats()) == before
+    lib.stitch([{"task_id": 0, "entries": [(seg, 0, 16, 0)], "holes": [], "capacity_tokens": 16}])
+    kk, _ = lib.task_read(0, 0, 0, 16)
+    assert torch.equal(kk.view(torch.int16), k[0].view(torch.int16))
+    lib.close()
+    # (b)
+    L, Hq, Hkv, D, P = 6, 8, 2, 128, 16
+    cfg = synth.GraftConfig("dry", L, Hq, Hkv, D, P, 5e5, 2, 1000, 1200, 4000, 1, 2, 2, 0, holes=((-1, 128),))
+    wl = synth.make_workload(cfg, 5)
+    orc, lib, seg_ids = T.make_pair(cfg, wl, 5, workspace_bytes=32 << 20)
+    c_plans, o_plans = T.plans_of(wl, seg_ids)
+    orc.stitch(o_plans)
+    lib.stitch(c_plans)
+    pos = wl.tasks[0].positions
+    q, k, v = synth.patch_qkv(cfg, 0, len(pos), 3, "cpu")
+    ref = orc.patch(0, 0, synth.to_bits(q), synth.to_bits(k), synth.to_bits(v), pos)
+    h = [x.contiguous().pin_memory() for x in (q, k, v)]
+    out = torch.empty_like(h[0]).pin_memory()
+    out.fill_(float("nan"))
+    lib.set_attn_policy(1, 12)            # 128 tokens x 12 splits x 6 layers x 8 heads x 130 fp32 = 38 MB of partials: no room
+    before = lib.stats()
+    with pytest.raises(B.FcgError) as e:
+        lib.patch_host(0, 0, *h, pos, out)
+    assert e.value.status == B.FCG_ERR_OUT_OF_ARENA
+    torch.cuda.synchronize()
+    assert lib.stats() == before and bool(torch.isnan(out.float()).all())
+    with pytest.raises(B.FcgError) as e:  # the rope variant checks before it launches its rotation kernel
+        lib.patch_rope(0, 0, *[x.cuda() for x in (q, k, v)], pos)
+    assert e.value.status == B.FCG_ERR_OUT_OF_ARENA and lib.stats() == before
+    lib.set_attn_policy(1, 1)
+    lib.patch_host(0, 0, *h, pos, out)
+    torch.cuda.synchronize()
+    T.assert_attn_close(out, ref, "host patch after the refused one")
+    lib.close()
