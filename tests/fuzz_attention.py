@@ -1,4 +1,4 @@
-"""Fuzz campaign for patch attention (not collected by pytest): random geometry, patch placement, KV-split count and
+"""Fuzz campaign for patch attention (a campaign driver; tests/test_gpu_fuzz.py runs a bounded, fixed-seed slice of it): random geometry, patch placement, KV-split count and
 kernel policy against the oracle -- the ragged edges of the CTA classes (rows per kv head around 32 / 64 / 128 / 256, a last
 KV tile or split of a few tokens, holes in the middle of the cache, appends that grow the task), NaN-poisoned pool.
 

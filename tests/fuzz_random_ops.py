@@ -1,4 +1,4 @@
-"""Fuzz campaign over tests/test_gpu_random_ops.py (not collected by pytest): N seeded random operation sequences with
+"""Fuzz campaign over tests/test_gpu_random_ops.py (a campaign driver; tests/test_gpu_fuzz.py runs a bounded, fixed-seed slice of it): N seeded random operation sequences with
 random geometry (head_dim 64 / 128 / 256, GQA group, page size, rope mode) on the CUDA library and the oracle side by side.
 
     python tests/fuzz_random_ops.py <campaign seed> <number of sequences>        (needs a GPU)
