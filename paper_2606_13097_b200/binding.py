@@ -15,7 +15,8 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfcg.so")
+# FCG_LIBRARY: another build of the same library (the ASan / UBSan build of `python -m paper_2606_13097_b200.build --sanitize`)
+LIB_PATH = os.environ.get("FCG_LIBRARY") or os.path.join(_HERE, "libfcg.so")
 
 FCG_OK = 0
 FCG_ERR_INVALID_ARG = -1

@@ -41,7 +41,28 @@ def _headers():
     return hs
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+# (nvcc splits -Xcompiler arguments at commas, so one flag per sanitizer)
+SANITIZE_FLAGS = ["-Xcompiler", "-fsanitize=address", "-Xcompiler", "-fsanitize=undefined", "-Xcompiler", "-fno-omit-frame-pointer"]
+
+
+def build(force: bool = False, verbose: bool = False, sanitize: bool = False) -> str:
+    """sanitize=True: the HOST code of the library (planner, arena bookkeeping, blob packing) built with ASan + UBSan into
+    libfcg_asan.so (objects under build_asan/).  Load it with FCG_LIBRARY=<path> and LD_PRELOAD=$(gcc -print-file-name=libasan.so),
+    ASAN_OPTIONS=protect_shadow_gap=0 (CUDA maps memory where ASan keeps its shadow gap); see profiles/r03_sanitizer.md."""
+    global BUILD, LIB
+    if sanitize:
+        saved = (BUILD, LIB)
+        BUILD, LIB = os.path.join(HERE, "build_asan"), os.path.join(HERE, "libfcg_asan.so")
+        NVCC_FLAGS.extend(SANITIZE_FLAGS)
+        try:
+            return _build(force, verbose, SANITIZE_FLAGS)
+        finally:
+            BUILD, LIB = saved
+            del NVCC_FLAGS[-len(SANITIZE_FLAGS):]
+    return _build(force, verbose, [])
+
+
+def _build(force: bool, verbose: bool, link_flags) -> str:
     os.makedirs(BUILD, exist_ok=True)
     nvcc = _nvcc()
     newest_header = max(os.path.getmtime(h) for h in _headers())
@@ -70,7 +91,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with ThreadPoolExecutor(max_workers=max(1, min(8, len(jobs)))) as ex:
         list(ex.map(compile_one, jobs))
     if jobs or force or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
-        cmd = [nvcc, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "static"]
+        cmd = [nvcc, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "static", *link_flags]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
@@ -78,5 +99,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    path = build(force="--force" in sys.argv, verbose="-v" in sys.argv)
+    path = build(force="--force" in sys.argv, verbose="-v" in sys.argv, sanitize="--sanitize" in sys.argv)
     print(path)

@@ -1696,7 +1696,9 @@ fcg_status_t fcg_patch_plan_create(fcg_library_t *lib, const int32_t *task_ids, 
 
 fcg_status_t fcg_patch_planned(fcg_library_t *lib, fcg_patch_plan_t *plan, int32_t layer_begin, int32_t n_layers, const void *q,
                                const void *k, const void *v, void *out, void *stream_) {
-  if (!lib || !plan || plan->lib != lib) return fail(FCG_ERR_INVALID_ARG, "NULL plan / plan of another library");
+  // membership first: a destroyed plan (or one of another library) is recognised without touching its memory
+  if (!lib || !plan || std::find(lib->plans.begin(), lib->plans.end(), plan) == lib->plans.end())
+    return fail(FCG_ERR_INVALID_ARG, "NULL plan, a plan of another library or one that was already destroyed");
   for (size_t t = 0; t < plan->task_ids.size(); ++t) {
     const TaskRec &tr = lib->tasks[plan->task_ids[t]];
     if (!tr.live || tr.gen != plan->task_gens[t])
@@ -1717,9 +1719,9 @@ fcg_status_t fcg_patch_planned(fcg_library_t *lib, fcg_patch_plan_t *plan, int32
 }
 
 fcg_status_t fcg_patch_plan_destroy(fcg_library_t *lib, fcg_patch_plan_t *plan) {
-  if (!lib || !plan || plan->lib != lib) return fail(FCG_ERR_INVALID_ARG, "NULL plan / plan of another library");
-  auto it = std::find(lib->plans.begin(), lib->plans.end(), plan);
-  if (it == lib->plans.end()) return fail(FCG_ERR_INVALID_ARG, "unknown (already destroyed?) plan");
+  if (!lib || !plan) return fail(FCG_ERR_INVALID_ARG, "NULL library / plan");
+  auto it = std::find(lib->plans.begin(), lib->plans.end(), plan);   // before the plan's memory is touched (found by the ASan run)
+  if (it == lib->plans.end()) return fail(FCG_ERR_INVALID_ARG, "a plan of another library or one that was already destroyed");
   lib->plans.erase(it);
   range_give(lib->seg_free, plan->dev_off, plan->dev_bytes);
   lib->n_plans_live--;
