@@ -139,3 +139,23 @@ def test_failing_calls_enqueue_nothing():
     torch.cuda.synchronize()
     T.assert_attn_close(out, ref, "host patch after the refused one")
     lib.close()
+
+
+def test_bench_two_ranks_on_one_gpu_prints_a_compact_last_line():
+    """Readiness for the day the scaling run happens: `bench.py --gpus 2` spawns two ranks (here both on cuda:0 with gloo as
+    the control plane, so the ranks' kernels never wait on one another), shards the workload and has rank 0 print the compact
+    headline as the LAST stdout line, the fat record before it on a DETAIL line."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--devices", "same", "--config", "C2", "--steps", "2",
+                        "--no-seeds", "--no-next", "--no-cpu-baseline"], capture_output=True, text=True, timeout=540, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.strip()]
+    last = lines[-1]
+    assert len(last) < 4096 and any(ln.startswith("DETAIL ") for ln in lines[:-1])
+    rec = json.loads(last)
+    assert rec["n_gpus"] == 2 and rec["steps"] == 2 and rec["value"] > 0 and rec["scaling"] in ("weak", "strong")
+    assert rec["gpu_launches"] > 0 and rec["roofline"]["frac"] > 0 and rec["e2e"]["h2d_bytes_per_step"] > 0
